@@ -1,0 +1,147 @@
+"""Seeded synthetic workloads shaped like BASELINE.json's configs.
+
+This module serves BOTH the CUDA path and the oracle and therefore holds none of the method's arithmetic:
+it only describes grids/species and samples analytic (bi-)Maxwellians at dof coordinates that the caller
+obtained from whichever implementation it is driving.  Random numbers come from a counter-based
+splitmix64 stream: value(seed, counter) -- no hidden state, so any subset of a batch can be regenerated.
+
+Stand-ins: the paper's p4est AMR grids, Simmetrix meshes and PETSc option files are not
+available; these generated grids and Maxwellian states replace them.
+"""
+import math
+
+import numpy as np
+
+SEED_BASE = 0x220903228000
+_M64 = (1 << 64) - 1
+
+
+def splitmix64(seed, counter):
+    """Counter-based 64-bit hash: the `counter`-th output of a splitmix64 stream started at `seed`."""
+    z = (seed + (counter + 1) * 0x9E3779B97F4A7C15) & _M64
+    z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & _M64
+    z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & _M64
+    return z ^ (z >> 31)
+
+
+def uniform01(seed, counter):
+    return (splitmix64(seed, counter) >> 11) * (1.0 / (1 << 53))
+
+
+def normal01(seed, counter):
+    """Box-Muller on two sub-counters of `counter`."""
+    u1 = uniform01(seed, 2 * counter + (1 << 40))
+    u2 = uniform01(seed, 2 * counter + 1 + (1 << 40))
+    return math.sqrt(-2.0 * math.log(1.0 - u1)) * math.cos(2.0 * math.pi * u2)
+
+
+def _grid(kind, extent, nr, nz, levels=0):
+    return dict(kind=kind, r_max=extent, z_min=-extent, z_max=extent, nr=nr, nz=nz, levels=levels)
+
+
+_A = [2, 4, 7, 9, 12, 14, 16, 20, 40]
+_Z = [1, 2, 3, 4, 6, 7, 8, 10, 18]
+
+
+def config(index, batch=None):
+    """Problem description of BASELINE.json configs[index-1] (index 1..5) plus small test-only variants.
+
+    Returns dict(name, grids, species, degree, dt, batch, state) where state in {"maxwellian",
+    "shifted", "bimaxwellian"} selects what `species_state` draws.
+    """
+    if index == 1:
+        return dict(name="cfg1_e_8x16_Q2", index=1, grids=[_grid(0, 5.0, 8, 16)],
+                    species=[dict(mass=1.0, charge=-1.0, grid=0)], degree=2, dt=1.0, batch=batch or 1,
+                    state="maxwellian", alpha=[1.0])
+    if index in (2, 5):
+        n = (8, 16) if index == 2 else (14, 28)
+        md = 3670.0
+        return dict(name="cfg%d_eD_%dx%d_Q3" % (index, n[0], n[1]), index=index,
+                    grids=[_grid(0, 5.0, n[0], n[1]), _grid(0, 5.0 / math.sqrt(md), n[0], n[1])],
+                    species=[dict(mass=1.0, charge=-1.0, grid=0), dict(mass=md, charge=1.0, grid=1)],
+                    degree=3, dt=1.0, batch=batch or (64 if index == 2 else 1024), state="shifted", alpha=[1.0, 1.0])
+    if index == 3:
+        masses = [1.0] + [1836.15 * a for a in _A]
+        charges = [-1.0] + [float(z) for z in _Z]
+        sgrid = [0, 1, 1, 1] + [2] * 6
+        grids = [_grid(0, 5.0, 8, 8), _grid(0, 5.0 / math.sqrt(masses[1]), 8, 8),
+                 _grid(0, 5.0 / math.sqrt(masses[4]), 8, 8)]
+        return dict(name="cfg3_10species_3grids_Q3", index=3, grids=grids,
+                    species=[dict(mass=m, charge=q, grid=g) for m, q, g in zip(masses, charges, sgrid)],
+                    degree=3, dt=1.0, batch=batch or 256, state="maxwellian_nT", alpha=[1.0] * 10)
+    if index == 4:
+        md = 3670.0
+        return dict(name="cfg4_eD_quadtree_Q3", index=4,
+                    grids=[_grid(1, 5.0, 4, 8, 3), _grid(1, 5.0 / math.sqrt(md), 4, 8, 3)],
+                    species=[dict(mass=1.0, charge=-1.0, grid=0), dict(mass=md, charge=1.0, grid=1)],
+                    degree=3, dt=0.1, batch=batch or 256, state="bimaxwellian", alpha=[2.0, 0.5])
+    raise ValueError("unknown config %r" % (index,))
+
+
+def tiny_config(kind="uniform", degree=2, two_species=True, batch=2):
+    """Small problems for fast tests (same recipe, fewer cells)."""
+    if kind == "uniform":
+        grids = [_grid(0, 5.0, 3, 6)] + ([_grid(0, 5.0 / 5.0, 2, 4)] if two_species else [])
+    else:
+        grids = [_grid(1, 5.0, 2, 4, 1)] + ([_grid(1, 5.0 / 5.0, 2, 4, 2)] if two_species else [])
+    species = [dict(mass=1.0, charge=-1.0, grid=0)]
+    if two_species:
+        species.append(dict(mass=25.0, charge=2.0, grid=1))
+    return dict(name="tiny_%s_Q%d" % (kind, degree), index=90 + degree, grids=grids, species=species, degree=degree,
+                dt=0.5, batch=batch, state="shifted", alpha=[1.0] * len(species))
+
+
+def species_state(cfg, batch=None, entries=None):
+    """Seeded (n, T, u, alpha) per (entry, species): arrays [len(entries), S].  Draw order (entry, species, {n,T,u})."""
+    B = batch or cfg["batch"]
+    entries = list(range(B)) if entries is None else list(entries)
+    S = len(cfg["species"])
+    seed = SEED_BASE + cfg["index"]
+    n = np.ones((len(entries), S))
+    T = np.ones((len(entries), S))
+    u = np.zeros((len(entries), S))
+    al = np.tile(np.asarray(cfg["alpha"], dtype=np.float64), (len(entries), 1))
+    st = cfg["state"]
+    for row, b in enumerate(entries):
+        for s in range(S):
+            c = (b * S + s) * 3
+            theta_ref = 1.0 / cfg["species"][s]["mass"]
+            if st in ("shifted", "maxwellian_nT"):
+                n[row, s] = 0.9 + 0.2 * uniform01(seed, c)
+                T[row, s] = 0.8 + 0.4 * uniform01(seed, c + 1)
+                if st == "shifted":
+                    u[row, s] = 0.05 * math.sqrt(theta_ref) * normal01(seed, c + 2)
+            elif st == "bimaxwellian":
+                n[row, s] = 0.9 + 0.2 * uniform01(seed, c)
+                T[row, s] = 0.9 + 0.2 * uniform01(seed, c + 1)
+    return n, T, u, al
+
+
+def sample_state(mass, n, T, u, alpha, rz):
+    """f = (n/alpha)(pi theta)^{-3/2} exp(-((z-u)^2 + r^2/alpha)/theta), theta = T/mass (eq. 6.1, reading A11)."""
+    theta = T / mass
+    r, z = rz[:, 0], rz[:, 1]
+    return (n / alpha) * (math.pi * theta) ** -1.5 * np.exp(-((z - u) ** 2 + r * r / alpha) / theta)
+
+
+def sample_state_grad(mass, n, T, u, alpha, rz):
+    """Analytic (f, df/dr, df/dz) of the same state (used by closed-form pins only)."""
+    theta = T / mass
+    r, z = rz[:, 0], rz[:, 1]
+    f = sample_state(mass, n, T, u, alpha, rz)
+    return f, f * (-2.0 * r / (alpha * theta)), f * (-2.0 * (z - u) / theta)
+
+
+def make_batch_f(cfg, dof_coords, batch=None, entries=None):
+    """Nodal interpolant of the seeded states: array [len(entries), sum_alpha n_dof(g(alpha))].
+
+    dof_coords[g] = [n_dof_g, 2] (r, z) from the implementation being driven.
+    """
+    n, T, u, al = species_state(cfg, batch, entries)
+    out = []
+    for row in range(n.shape[0]):
+        parts = []
+        for s, sp in enumerate(cfg["species"]):
+            parts.append(sample_state(sp["mass"], n[row, s], T[row, s], u[row, s], al[row, s], dof_coords[sp["grid"]]))
+        out.append(np.concatenate(parts))
+    return np.ascontiguousarray(np.stack(out))
