@@ -1,0 +1,175 @@
+/* landau.h -- C ABI of the B200-native batched Landau Jacobian library (liblandau_b200.so).
+ *
+ * One thing is built here: the data-parallel hot path of the fully implicit Landau collision advance of
+ * arxiv 2209.03228 -- for every batch entry (an independent axisymmetric (r,z) velocity-space
+ * problem, sec. 3.1) the O(N^2) inner integral of the Landau tensor (eq. 2.1/2.3),
+ * the per-element finite-element matrices of the weak form (eq. 2.4) and the assembly of the
+ * shifted matrix M/dt - J into one batched CSR per species.
+ *
+ * Conventions common to every entry point
+ *   - plain C: pointers + sizes, no C++/torch types.  "host" / "dev" in a parameter comment says where the
+ *     memory lives.  Device pointers must belong to the CUDA device the context was created on.
+ *   - all floating point is IEEE FP64, all indices int32 (offsets into batched arrays: long long).
+ *   - return value: 0 (LANDAU_OK) or a negative landau_status; nothing throws, nothing aborts.  A message for
+ *     the last failure of a context is kept in landau_last_error(ctx) (ctx == NULL: last create failure).
+ *   - a context is owned by the caller (landau_destroy), is bound to one device, and is not re-entrant:
+ *     calls on one context must be serialised by the caller.  Different contexts are independent.
+ *   - landau_jacobian / landau_apply are asynchronous on `cuda_stream` (a cudaStream_t passed as void*; NULL =
+ *     legacy default stream) and perform no hidden device synchronisation unless their scratch must grow
+ *     (first call with a larger batch: one cudaMalloc).
+ *   - there is no CPU fallback: without a CUDA device landau_create fails with LANDAU_CUDA_ERROR.
+ *
+ * Units and discretisation (readings A3-A17): velocity coordinates of every grid are in the common
+ * unit v0 (electron thermal speed), m0 = electron mass = 1, f in units n0/v0^3; tensor-product Lagrange Qk
+ * elements on k+1 equispaced nodes, (k+1)^2 Gauss-Legendre points per cell, axis-aligned rectangular cells,
+ * hanging nodes of quadtree grids constrained to the coarse edge, natural (zero-flux) boundaries, no
+ * essential boundary conditions; coincident integration points contribute zero to the inner integral.
+ */
+#ifndef LANDAU_B200_H
+#define LANDAU_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  LANDAU_OK = 0,
+  LANDAU_INVALID_ARG = -1,   /* NULL pointer, non-positive size, dt <= 0, species on a missing grid, ...   */
+  LANDAU_UNSUPPORTED = -2,   /* degree not in {2,3}, n_gauss_1d != degree+1, grid kind unknown, chain of
+                                hanging-node constraints (mesh not 2:1 balanced)                           */
+  LANDAU_OUT_OF_MEMORY = -3, /* host or device allocation failed                                           */
+  LANDAU_CUDA_ERROR = -4     /* any other CUDA runtime failure (no device, launch failure, ...)            */
+} landau_status;
+
+typedef struct landau_ctx landau_ctx; /* opaque; owns all device tables and scratch */
+
+/* One velocity-space grid: the half plane r in [0,r_max], z in [z_min,z_max] (sec. 2.3).
+ * kind 0: uniform nr x nz cells.  kind 1: quadtree: base nr x nz cells; for l = 1..levels every
+ * level-(l-1) cell inside the box [0, r_max/2^l] x [zc - zh/2^l, zc + zh/2^l] (zc, zh = centre and half extent
+ * of the z range) is split in four (reading A12). */
+typedef struct {
+  int kind;
+  double r_max, z_min, z_max;
+  int nr, nz;
+  int levels; /* ignored for kind 0 */
+} landau_grid_desc;
+
+/* One species: mass in units of m0 (electron mass), charge in units of e, index of the grid it lives on.
+ * Several species may share a grid (sec. 3). */
+typedef struct {
+  double mass, charge;
+  int grid;
+} landau_species_desc;
+
+/* Element degree k (Qk) and Gauss points per direction (must be k+1; Table 13). */
+typedef struct {
+  int degree;
+  int n_gauss_1d;
+} landau_quadrature_desc;
+
+/* Build a context: meshes, dof numbering (lexicographic by (z,r)), hanging-node constraints, integration
+ * point tables, CSR patterns and gather tables, uploaded once to `cuda_device`.
+ *   grids[n_grids], species[n_species], quadrature : host, read only during the call.
+ *   nu : host, n_species x n_species row-major symmetric collision-frequency matrix nu~_ab of eq. (2.2)
+ *        (PAPER.md:52-57), or NULL for nu_ab = q_a^2 q_b^2 (equal Coulomb logarithms, reading A3).
+ *        A matrix of the form a_a * b_b is detected and takes the fast path that sums the species of all
+ *        grids into one source field per batch entry before the inner integral.
+ *   cuda_device : CUDA device ordinal.  A NEGATIVE value builds a host-only context: the geometry queries
+ *        (landau_sizes, landau_dof_coords, landau_ip_table, landau_csr_pattern_host) work without a GPU, every
+ *        compute entry point returns LANDAU_CUDA_ERROR -- used by the CPU-only test-suite for the host logic.
+ *   out : receives the context; untouched on failure. */
+int landau_create(const landau_grid_desc* grids, int n_grids, const landau_species_desc* species, int n_species,
+                  const landau_quadrature_desc* quadrature, const double* nu, int cuda_device, landau_ctx** out);
+
+/* Frees every host and device resource of the context (synchronises the device first).  NULL is a no-op. */
+void landau_destroy(landau_ctx* ctx);
+
+/* Sizes.  Arrays have one entry per grid (host, may be NULL to skip):
+ *   n_dof[g]  unknowns (equations) of one species on grid g,
+ *   nnz[g]    structural nonzeros of grid g's CSR pattern,
+ *   n_ip[g]   integration points of grid g,
+ *   n_cells[g] cells of grid g.
+ *   f_stride   doubles per batch entry of batch_f / out_rhs  = sum over species a of n_dof[grid(a)],
+ *   csr_stride doubles per batch entry of out_csr_vals       = sum over species a of nnz[grid(a)]. */
+int landau_sizes(const landau_ctx* ctx, int* n_dof, int* nnz, int* n_ip, int* n_cells, long long* f_stride,
+                 long long* csr_stride);
+
+/* (r,z) of every dof of grid g, in dof order: rz_host[2*i] = r, rz_host[2*i+1] = z   (host, n_dof[g] x 2). */
+int landau_dof_coords(const landau_ctx* ctx, int grid, double* rz_host);
+
+/* (r, z, w) of the integration points of grid g (host arrays of n_ip[g]; any may be NULL).
+ * w = Gauss weight x cell Jacobian x r (cylindrical measure, the common 2 pi dropped; reading A6). */
+int landau_ip_table(const landau_ctx* ctx, int grid, double* r_host, double* z_host, double* w_host);
+
+/* CSR pattern of grid g, shared by every species on the grid and every batch entry.  The pointers are DEVICE
+ * pointers owned by the context (valid until landau_destroy): rowptr[n_dof+1], colidx[nnz], columns ascending
+ * in each row, structural (every pair of dofs coupled by a cell, including parent-edge couplings of hanging
+ * nodes).  landau_csr_pattern_host copies the same arrays into caller-owned host memory. */
+int landau_csr_pattern(const landau_ctx* ctx, int grid, const int** rowptr_dev, const int** colidx_dev);
+int landau_csr_pattern_host(const landau_ctx* ctx, int grid, int* rowptr_host, int* colidx_host);
+
+/* The batched shifted Jacobian  M/dt - J[f]  (sparse, inner integrals frozen: PAPER.md:73).
+ *   batch_f_dev      : dev, [batch][species a][n_dof[grid(a)]]   nodal values (the paper's u = [f_1..f_S])
+ *   dt               : > 0; +infinity gives the unshifted -J
+ *   out_csr_vals_dev : dev, [batch][species a][nnz[grid(a)]]     every entry written exactly once
+ * J_ac = sum_q w_q [ -grad phi_a . D_a grad phi_c + (grad phi_a . K_a) phi_c ],  M_ac = sum_q w_q phi_a phi_c,
+ * D_a = sum_b nu_ab (m0/m_a)^2 INT U fb,  K_a = sum_b nu_ab (m0/m_a)(m0/m_b) INT U . grad fb   (eq. 2.1, 2.3).
+ * batch == 0 is a successful no-op. */
+int landau_jacobian(landau_ctx* ctx, const double* batch_f_dev, int batch, double dt, double* out_csr_vals_dev,
+                    void* cuda_stream);
+
+/* Operator application  rhs = J[f] f  (so that M df/dt = rhs; residual of the Newton iteration).
+ *   out_rhs_dev : dev, same layout as batch_f_dev. */
+int landau_apply(landau_ctx* ctx, const double* batch_f_dev, int batch, double* out_rhs_dev, void* cuda_stream);
+
+/* Host-buffer convenience: same as landau_jacobian / landau_apply with HOST pointers (pageable or pinned); the
+ * library stages H2D / D2H copies on `cuda_stream` in internal device buffers and synchronises the stream
+ * before returning. */
+int landau_jacobian_host(landau_ctx* ctx, const double* batch_f_host, int batch, double dt, double* out_csr_vals_host,
+                         void* cuda_stream);
+int landau_apply_host(landau_ctx* ctx, const double* batch_f_host, int batch, double* out_rhs_host, void* cuda_stream);
+
+/* Diagnostics -------------------------------------------------------------------------------------------- */
+
+/* Copy out the frozen coefficients of the LAST landau_jacobian / landau_apply call (synchronises the stream it
+ * ran on): dk_host[batch][species a][5][n_ip[grid(a)]] = (Drr, Drz, Dzz, Kr, Kz) at the integration points.
+ * Only the last pass is kept, so the call is meaningful when batch <= the batch chunk. */
+int landau_last_coefficients(landau_ctx* ctx, double* dk_host);
+
+/* Evaluate the 2V Landau tensor kernel on the device for n point pairs (dev arrays r,z,rb,zb of n doubles):
+ * out_dev[5*n] = (UD_rr, UD_rz, UD_zz, UK_rr, UK_zr) per pair, UK_rz = UD_rz, UK_zz = UD_zz; coincident
+ * pairs give zeros.  Same device function as the inner-integral kernel uses. */
+int landau_tensor_eval(const double* r_dev, const double* z_dev, const double* rb_dev, const double* zb_dev, int n,
+                       double* out_dev, void* cuda_stream);
+
+/* Elliptic pieces on the device: for n pairs (m[i], mp[i] = 1-m[i] given separately) out_dev[3*n] =
+ * (P0, Dc, Q) = INT_0^{pi/2} {1, cos^2, sin^2 cos^2} (1 - m sin^2)^{-3/2} dtheta. */
+int landau_ellip_eval(const double* m_dev, const double* mp_dev, int n, double* out_dev, void* cuda_stream);
+
+/* FP64 pipe probes used by bench.py for the roofline denominator: run `iters` rounds of register-resident
+ * DFMA (kind 0) or DMMA m8n8k4 (kind 1) on every SM; *tflops receives the achieved FP64 TFLOP/s
+ * (CUDA-event timed on `cuda_stream`, synchronises it). */
+int landau_fp64_probe(int kind, int iters, double* tflops, void* cuda_stream);
+
+/* Number of kernels the library launched on behalf of this context since creation (bench's gpu_launches). */
+long long landau_launch_count(const landau_ctx* ctx);
+
+/* Per-stage device time of the LAST jacobian/apply call in milliseconds (CUDA events recorded on the call's
+ * stream; synchronises it): ms[0] field evaluation, ms[1] inner integral, ms[2] coefficient combination,
+ * ms[3] element matrices + assembly (or apply).  Recording is enabled with landau_set_timing(ctx, 1). */
+int landau_set_timing(landau_ctx* ctx, int enabled);
+int landau_last_stage_ms(landau_ctx* ctx, float* ms4);
+
+/* Choose the inner-integral kernel: 0 auto, 1 plain DFMA kernel, 2 DMMA (tensor-pipe FP64) kernel. */
+int landau_set_inner_kernel(landau_ctx* ctx, int which);
+
+/* Batch entries pushed through the stages per pass (default 256); scratch is sized for one pass, so that the
+ * intermediates (source fields, partial sums, D/K) of a pass stay L2-resident.  chunk >= 1. */
+int landau_set_batch_chunk(landau_ctx* ctx, int chunk);
+
+const char* landau_last_error(const landau_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LANDAU_B200_H */

@@ -1,0 +1,342 @@
+// host_setup.cpp -- see host_setup.hpp.  Quadtree cells are addressed by (level, i, j); hanging faces are found
+// by neighbour look-up (a face whose neighbour region is covered by a coarser leaf), not by geometry sweeps.
+#include "host_setup.hpp"
+
+#include <algorithm>
+#include <cmath>
+#include <map>
+#include <tuple>
+#include <unordered_map>
+
+namespace landau {
+
+namespace {
+
+// Lagrange basis on k+1 equispaced nodes of [-1,1] (reading A9): values and derivatives at x.
+void equispaced_lagrange(int k, double x, double* v, double* d) {
+  // first-form barycentric-free evaluation with exact integer denominators: nodes t_c = (2c - k)/k
+  for (int c = 0; c <= k; ++c) {
+    double num = 1.0, den = 1.0;
+    for (int j = 0; j <= k; ++j) {
+      if (j == c) continue;
+      num *= (k * x - (2 * j - k));
+      den *= 2.0 * (c - j);
+    }
+    v[c] = num / den;
+    double acc = 0.0;
+    for (int skip = 0; skip <= k; ++skip) {
+      if (skip == c) continue;
+      double p = k;  // d/dx of (k x - (2 skip - k))
+      for (int j = 0; j <= k; ++j) {
+        if (j == c || j == skip) continue;
+        p *= (k * x - (2 * j - k));
+      }
+      acc += p;
+    }
+    d[c] = acc / den;
+  }
+}
+
+struct CellId {
+  int level, i, j;
+  bool operator<(const CellId& o) const { return std::tie(level, i, j) < std::tie(o.level, o.i, o.j); }
+};
+
+}  // namespace
+
+bool build_tables(int k, HostTables* t, std::string* msg) {
+  if (k != 2 && k != 3) {
+    *msg = "element degree must be 2 or 3";
+    return false;
+  }
+  t->k = k;
+  t->nq1 = k + 1;
+  t->nb = (k + 1) * (k + 1);
+  t->nq = t->nb;
+  // closed-form Gauss-Legendre rules
+  if (k == 2) {
+    const double a = std::sqrt(3.0 / 5.0);
+    t->gauss_x = {-a, 0.0, a};
+    t->gauss_w = {5.0 / 9.0, 8.0 / 9.0, 5.0 / 9.0};
+  } else {
+    const double s = std::sqrt(6.0 / 5.0);
+    const double a = std::sqrt(3.0 / 7.0 - 2.0 / 7.0 * s), b = std::sqrt(3.0 / 7.0 + 2.0 / 7.0 * s);
+    const double wa = (18.0 + std::sqrt(30.0)) / 36.0, wb = (18.0 - std::sqrt(30.0)) / 36.0;
+    t->gauss_x = {-b, -a, a, b};
+    t->gauss_w = {wb, wa, wa, wb};
+  }
+  const int n1 = k + 1;
+  std::vector<double> v(n1 * n1), d(n1 * n1);  // [q1][c]
+  for (int q = 0; q < n1; ++q) equispaced_lagrange(k, t->gauss_x[q], &v[q * n1], &d[q * n1]);
+  t->B.assign(t->nq * t->nb, 0.0);
+  t->dBxi.assign(t->nq * t->nb, 0.0);
+  t->dBeta.assign(t->nq * t->nb, 0.0);
+  for (int q2 = 0; q2 < n1; ++q2)
+    for (int q1 = 0; q1 < n1; ++q1)
+      for (int a2 = 0; a2 < n1; ++a2)
+        for (int a1 = 0; a1 < n1; ++a1) {
+          const int q = q1 + n1 * q2, a = a1 + n1 * a2;
+          t->B[q * t->nb + a] = v[q1 * n1 + a1] * v[q2 * n1 + a2];
+          t->dBxi[q * t->nb + a] = d[q1 * n1 + a1] * v[q2 * n1 + a2];
+          t->dBeta[q * t->nb + a] = v[q1 * n1 + a1] * d[q2 * n1 + a2];
+        }
+  return true;
+}
+
+int build_grid(const landau_grid_desc& d, const HostTables& t, HostGrid* g, std::string* msg) {
+  if (d.kind != 0 && d.kind != 1) {
+    *msg = "grid kind must be 0 (uniform) or 1 (quadtree)";
+    return LANDAU_UNSUPPORTED;
+  }
+  if (!(d.r_max > 0) || !(d.z_max > d.z_min) || d.nr < 1 || d.nz < 1 || (d.kind == 1 && (d.levels < 0 || d.levels > 12))) {
+    *msg = "bad grid extents or cell counts";
+    return LANDAU_INVALID_ARG;
+  }
+  const int k = t.k, n1 = k + 1, nb = t.nb, nq = t.nq;
+  const int L = d.kind == 1 ? d.levels : 0;
+  g->desc = d;
+  g->k = k;
+  g->nb = nb;
+  g->nq = nq;
+
+  // ---- leaves of the quadtree -------------------------------------------------------------------------
+  std::vector<CellId> leaves;
+  for (int j = 0; j < d.nz; ++j)
+    for (int i = 0; i < d.nr; ++i) leaves.push_back(CellId{0, i, j});
+  for (int l = 1; l <= L; ++l) {
+    std::vector<CellId> next;
+    const long long zspan = (long long)d.nz << l;  // 4 x (z centre in level-(l-1) cells) = 4 nz 2^(l-2)
+    for (const CellId& c : leaves) {
+      // cell (l-1, i, j) in units of level-(l-1) cells; box: r <= nr/2, z in [nz 2^(l-2) -+ nz/4]; times 4:
+      bool inside = c.level == l - 1 && 2LL * (c.i + 1) <= d.nr && 4LL * c.j >= zspan - d.nz &&
+                    4LL * (c.j + 1) <= zspan + d.nz;
+      if (!inside) {
+        next.push_back(c);
+        continue;
+      }
+      for (int cj = 0; cj < 2; ++cj)
+        for (int ci = 0; ci < 2; ++ci) next.push_back(CellId{l, 2 * c.i + ci, 2 * c.j + cj});
+    }
+    leaves.swap(next);
+  }
+  std::map<CellId, int> leaf_index;
+  for (size_t e = 0; e < leaves.size(); ++e) leaf_index[leaves[e]] = (int)e;
+  g->n_cells = (int)leaves.size();
+
+  // ---- lattice nodes: X = (i k + a1) 2^(L-level), Z likewise; key = Z * XW + X (sorted = z-major order) ----
+  const long long XW = ((long long)d.nr * k << L) + 1;
+  auto node_key = [&](const CellId& c, int a1, int a2) {
+    const long long X = ((long long)c.i * k + a1) << (L - c.level);
+    const long long Z = ((long long)c.j * k + a2) << (L - c.level);
+    return Z * XW + X;
+  };
+  // ---- hanging faces: constraint[key] = list of (master key, weight) ------------------------------------
+  std::unordered_map<long long, std::vector<std::pair<long long, double>>> constraint;
+  std::vector<double> lv(n1), ld(n1);
+  for (const CellId& c : leaves) {
+    for (int face = 0; face < 4; ++face) {  // 0: r-low, 1: r-high, 2: z-low, 3: z-high
+      int ni = c.i + (face == 0 ? -1 : face == 1 ? 1 : 0);
+      int nj = c.j + (face == 2 ? -1 : face == 3 ? 1 : 0);
+      if (ni < 0 || nj < 0 || ni >= (d.nr << c.level) || nj >= (d.nz << c.level)) continue;  // domain boundary
+      // the leaf covering the neighbour position is the neighbour itself (conforming), one of its ancestors
+      // (coarser: this face hangs), or neither (neighbour refined further: the finer side owns the constraint)
+      CellId nb_cell{c.level, ni, nj};
+      bool found = false;
+      for (int lev = c.level; lev >= 0; --lev) {
+        nb_cell = CellId{lev, ni >> (c.level - lev), nj >> (c.level - lev)};
+        if (leaf_index.count(nb_cell)) {
+          found = true;
+          break;
+        }
+      }
+      if (!found || nb_cell.level == c.level) continue;
+      // the face of c lies on an edge of the coarser leaf nb_cell: constrain c's face nodes that are not
+      // nodes of nb_cell to the k+1 nodes of that coarse edge
+      const int shift = c.level - nb_cell.level;
+      const bool along_z = face < 2;  // r-faces run along z
+      for (int a = 0; a <= k; ++a) {
+        const int a1 = along_z ? (face == 0 ? 0 : k) : a;
+        const int a2 = along_z ? a : (face == 2 ? 0 : k);
+        // position of the node along the coarse edge, in units of (coarse node spacing / 2^shift)
+        const long long fine_pos = along_z ? ((long long)c.j * k + a2) : ((long long)c.i * k + a1);
+        const long long coarse_org = (along_z ? (long long)nb_cell.j : (long long)nb_cell.i) * k << shift;
+        const long long rel = fine_pos - coarse_org;  // in [0, k 2^shift]
+        if (rel % (1LL << shift) == 0) continue;       // coincides with a coarse node
+        const double x = -1.0 + 2.0 * (double)rel / (double)((long long)k << shift);
+        equispaced_lagrange(k, x, lv.data(), ld.data());
+        std::vector<std::pair<long long, double>> row;
+        for (int cidx = 0; cidx <= k; ++cidx) {
+          // coarse edge node: on the coarse cell's face opposite to `face`
+          const int b1 = along_z ? (face == 0 ? k : 0) : cidx;
+          const int b2 = along_z ? cidx : (face == 2 ? k : 0);
+          row.push_back(std::make_pair(node_key(nb_cell, b1, b2), lv[cidx]));
+        }
+        constraint[node_key(c, a1, a2)] = row;
+      }
+    }
+  }
+  // ---- free nodes -> dofs in (z, r) order ---------------------------------------------------------------------
+  std::vector<long long> keys;
+  keys.reserve(leaves.size() * nb);
+  for (const CellId& c : leaves)
+    for (int a2 = 0; a2 <= k; ++a2)
+      for (int a1 = 0; a1 <= k; ++a1) {
+        long long key = node_key(c, a1, a2);
+        if (!constraint.count(key)) keys.push_back(key);
+      }
+  std::sort(keys.begin(), keys.end());
+  keys.erase(std::unique(keys.begin(), keys.end()), keys.end());
+  g->n_dof = (int)keys.size();
+  std::unordered_map<long long, int> dof_of;
+  dof_of.reserve(keys.size() * 2);
+  const double ur = d.r_max / (double)((long long)d.nr * k << L);
+  const double uz = (d.z_max - d.z_min) / (double)((long long)d.nz * k << L);
+  g->dof_r.resize(g->n_dof);
+  g->dof_z.resize(g->n_dof);
+  for (int n = 0; n < g->n_dof; ++n) {
+    dof_of[keys[n]] = n;
+    g->dof_r[n] = (double)(keys[n] % XW) * ur;
+    g->dof_z[n] = d.z_min + (double)(keys[n] / XW) * uz;
+  }
+  // ---- rows of P_e -------------------------------------------------------------------------------------------
+  g->en_ptr.assign(1, 0);
+  g->en_dof.clear();
+  g->en_w.clear();
+  bool chain_error = false;
+  std::vector<std::pair<long long, double>> work, nxt;
+  for (const CellId& c : leaves)
+    for (int a2 = 0; a2 <= k; ++a2)
+      for (int a1 = 0; a1 <= k; ++a1) {
+        work.assign(1, std::make_pair(node_key(c, a1, a2), 1.0));
+        for (int depth = 0; depth < 6; ++depth) {
+          bool again = false;
+          nxt.clear();
+          for (auto& kw : work) {
+            auto it = constraint.find(kw.first);
+            if (it == constraint.end()) {
+              nxt.push_back(kw);
+              continue;
+            }
+            again = true;
+            for (auto& mw : it->second) nxt.push_back(std::make_pair(mw.first, kw.second * mw.second));
+          }
+          work.swap(nxt);
+          if (!again) break;
+          if (depth == 5) chain_error = true;
+        }
+        std::map<int, double> merged;
+        for (auto& kw : work) {
+          auto it = dof_of.find(kw.first);
+          if (it == dof_of.end()) {
+            chain_error = true;
+            continue;
+          }
+          merged[it->second] += kw.second;
+        }
+        for (auto& dw : merged)
+          if (dw.second != 0.0) {
+            g->en_dof.push_back(dw.first);
+            g->en_w.push_back(dw.second);
+          }
+        g->en_ptr.push_back((int)g->en_dof.size());
+      }
+  if (chain_error) {
+    *msg = "unresolvable hanging-node constraints (mesh not 2:1 balanced)";
+    return LANDAU_UNSUPPORTED;
+  }
+  // ---- cell rectangles and integration points ----------------------------------------------------------------
+  g->cell_r0.resize(g->n_cells);
+  g->cell_z0.resize(g->n_cells);
+  g->cell_hr.resize(g->n_cells);
+  g->cell_hz.resize(g->n_cells);
+  g->n_ip = g->n_cells * nq;
+  g->ip_r.resize(g->n_ip);
+  g->ip_z.resize(g->n_ip);
+  g->ip_w.resize(g->n_ip);
+  for (int e = 0; e < g->n_cells; ++e) {
+    const CellId& c = leaves[e];
+    const double hr = d.r_max / (double)((long long)d.nr << c.level);
+    const double hz = (d.z_max - d.z_min) / (double)((long long)d.nz << c.level);
+    g->cell_hr[e] = hr;
+    g->cell_hz[e] = hz;
+    g->cell_r0[e] = c.i * hr;
+    g->cell_z0[e] = d.z_min + c.j * hz;
+    for (int q2 = 0; q2 < n1; ++q2)
+      for (int q1 = 0; q1 < n1; ++q1) {
+        const int ip = e * nq + q1 + n1 * q2;
+        const double r = g->cell_r0[e] + 0.5 * hr * (1.0 + t.gauss_x[q1]);
+        g->ip_r[ip] = r;
+        g->ip_z[ip] = g->cell_z0[e] + 0.5 * hz * (1.0 + t.gauss_x[q2]);
+        g->ip_w[ip] = t.gauss_w[q1] * t.gauss_w[q2] * 0.25 * hr * hz * r;
+      }
+  }
+  // ---- CSR pattern ----------------------------------------------------------------------------------------------
+  std::vector<std::vector<int>> rows(g->n_dof);
+  std::vector<int> touched;
+  for (int e = 0; e < g->n_cells; ++e) {
+    touched.assign(g->en_dof.begin() + g->en_ptr[e * nb], g->en_dof.begin() + g->en_ptr[(e + 1) * nb]);
+    std::sort(touched.begin(), touched.end());
+    touched.erase(std::unique(touched.begin(), touched.end()), touched.end());
+    for (int I : touched) rows[I].insert(rows[I].end(), touched.begin(), touched.end());
+  }
+  g->rowptr.assign(g->n_dof + 1, 0);
+  g->colidx.clear();
+  for (int I = 0; I < g->n_dof; ++I) {
+    std::sort(rows[I].begin(), rows[I].end());
+    rows[I].erase(std::unique(rows[I].begin(), rows[I].end()), rows[I].end());
+    g->colidx.insert(g->colidx.end(), rows[I].begin(), rows[I].end());
+    g->rowptr[I + 1] = (int)g->colidx.size();
+  }
+  g->nnz = (int)g->colidx.size();
+  // ---- gather tables -----------------------------------------------------------------------------------------------
+  {
+    std::vector<int> count(g->nnz, 0);
+    struct Entry {
+      int slot, code;
+      double w;
+    };
+    std::vector<Entry> entries;
+    for (int e = 0; e < g->n_cells; ++e)
+      for (int a = 0; a < nb; ++a)
+        for (int pa = g->en_ptr[e * nb + a]; pa < g->en_ptr[e * nb + a + 1]; ++pa) {
+          const int I = g->en_dof[pa];
+          const int* rb = &g->colidx[g->rowptr[I]];
+          const int* re = rb + (g->rowptr[I + 1] - g->rowptr[I]);
+          for (int c = 0; c < nb; ++c)
+            for (int pc = g->en_ptr[e * nb + c]; pc < g->en_ptr[e * nb + c + 1]; ++pc) {
+              const int slot = (int)(std::lower_bound(rb, re, g->en_dof[pc]) - &g->colidx[0]);
+              entries.push_back(Entry{slot, (e * nb + a) * nb + c, g->en_w[pa] * g->en_w[pc]});
+              ++count[slot];
+            }
+        }
+    g->as_ptr.assign(g->nnz + 1, 0);
+    for (int n = 0; n < g->nnz; ++n) g->as_ptr[n + 1] = g->as_ptr[n] + count[n];
+    g->as_code.resize(entries.size());
+    g->as_w.resize(entries.size());
+    std::vector<int> fill(g->as_ptr.begin(), g->as_ptr.end() - 1);
+    for (const Entry& en : entries) {  // entries are generated in (cell, a, c) order => deterministic lists
+      g->as_code[fill[en.slot]] = en.code;
+      g->as_w[fill[en.slot]] = en.w;
+      ++fill[en.slot];
+    }
+  }
+  {
+    std::vector<int> count(g->n_dof, 0);
+    for (size_t p = 0; p < g->en_dof.size(); ++p) ++count[g->en_dof[p]];
+    g->ap_ptr.assign(g->n_dof + 1, 0);
+    for (int n = 0; n < g->n_dof; ++n) g->ap_ptr[n + 1] = g->ap_ptr[n] + count[n];
+    g->ap_code.resize(g->en_dof.size());
+    g->ap_w.resize(g->en_dof.size());
+    std::vector<int> fill(g->ap_ptr.begin(), g->ap_ptr.end() - 1);
+    for (int ea = 0; ea < g->n_cells * nb; ++ea)
+      for (int p = g->en_ptr[ea]; p < g->en_ptr[ea + 1]; ++p) {
+        const int I = g->en_dof[p];
+        g->ap_code[fill[I]] = ea;
+        g->ap_w[fill[I]] = g->en_w[p];
+        ++fill[I];
+      }
+  }
+  return LANDAU_OK;
+}
+
+}  // namespace landau

@@ -1,0 +1,731 @@
+// landau_api.cu -- the C ABI of include/landau.h: context, scratch management and kernel launches.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/landau.h"
+#include "host_setup.hpp"
+#include "landau_kernels.cuh"
+
+using namespace landau;
+
+namespace {
+
+std::string g_create_error;
+
+struct Group {       // one launch of the inner-integral kernel
+  int j0;            // first source point (in the concatenated, padded IP arrays)
+  int nj_pad;        // number of source points (multiple of the tile)
+  int ncb;           // columns per batch entry
+  long long f_off;   // offset of the group's F block inside the F scratch (doubles), set per call
+};
+
+}  // namespace
+
+struct landau_ctx {
+  int device = 0;
+  int S = 0, G = 0, k = 0, nb = 0, nq = 0;
+  HostTables ht;
+  std::vector<HostGrid> hg;
+  std::vector<landau_species_desc> species;
+  std::vector<double> nu;
+  bool separable = false;
+  std::vector<long long> f_off, v_off, dk_off;  // per species offsets inside one batch entry
+  long long f_stride = 0, v_stride = 0, dk_stride = 0, fl_stride = 0;
+  std::vector<long long> fl_off;
+  // device tables
+  std::vector<void*> allocs;
+  DevTables* d_tab = nullptr;
+  std::vector<DevGrid> dg;
+  std::vector<const int*> d_rowptr, d_colidx;
+  double *d_ip_r = nullptr, *d_ip_z = nullptr;
+  int n_i_pad = 0;
+  std::vector<int> ip_off;
+  std::vector<Group> groups;
+  std::vector<MixTable> mix;          // per grid
+  std::vector<int> mix_group;         // group of each grid
+  std::vector<int> mix_col_in_group;  // first column (per batch entry) of the grid inside its group
+  std::vector<CombineTable> comb;     // per species
+  // scratch (grown on demand)
+  double *F = nullptr, *Gp = nullptr, *DK = nullptr, *FL = nullptr;
+  size_t F_cap = 0, Gp_cap = 0, DK_cap = 0, FL_cap = 0;
+  double *stage_in = nullptr, *stage_out = nullptr;
+  size_t stage_in_cap = 0, stage_out_cap = 0;
+  int chunk = 256;       // batch entries processed per pass through the stages
+  int inner_kernel = 0;  // 0 auto, 1 dfma, 2 dmma
+  int last_batch = 0;
+  cudaStream_t last_stream = nullptr;
+  bool timing = false;
+  cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  float stage_ms[4] = {0, 0, 0, 0};
+  long long launches = 0;
+  std::string err;
+};
+
+namespace {
+
+int fail(landau_ctx* ctx, int code, const std::string& msg) {
+  if (ctx)
+    ctx->err = msg;
+  else
+    g_create_error = msg;
+  return code;
+}
+
+#define CUDA_TRY(ctx, expr)                                                                       \
+  do {                                                                                            \
+    cudaError_t e_ = (expr);                                                                      \
+    if (e_ != cudaSuccess)                                                                        \
+      return fail(ctx, e_ == cudaErrorMemoryAllocation ? LANDAU_OUT_OF_MEMORY : LANDAU_CUDA_ERROR, \
+                  std::string(#expr) + ": " + cudaGetErrorString(e_));                            \
+  } while (0)
+
+template <class T>
+int upload(landau_ctx* ctx, const std::vector<T>& h, const T** out) {
+  T* d = nullptr;
+  size_t bytes = sizeof(T) * (h.empty() ? 1 : h.size());
+  CUDA_TRY(ctx, cudaMalloc(&d, bytes));
+  ctx->allocs.push_back(d);
+  if (!h.empty()) CUDA_TRY(ctx, cudaMemcpy(d, h.data(), sizeof(T) * h.size(), cudaMemcpyHostToDevice));
+  *out = d;
+  return LANDAU_OK;
+}
+
+int grow(landau_ctx* ctx, double** p, size_t* cap, size_t need, bool zero) {
+  if (need <= *cap) return LANDAU_OK;
+  if (*p) {
+    CUDA_TRY(ctx, cudaDeviceSynchronize());
+    CUDA_TRY(ctx, cudaFree(*p));
+    *p = nullptr;
+    *cap = 0;
+  }
+  CUDA_TRY(ctx, cudaMalloc(p, need * sizeof(double)));
+  if (zero) CUDA_TRY(ctx, cudaMemset(*p, 0, need * sizeof(double)));
+  *cap = need;
+  return LANDAU_OK;
+}
+
+int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+// is nu = a_a * b_b (rank one)?  fills a, b.
+bool rank_one(const std::vector<double>& nu, int S, std::vector<double>* a, std::vector<double>* b) {
+  int pr = -1, pc = -1;
+  for (int i = 0; i < S && pr < 0; ++i)
+    for (int j = 0; j < S; ++j)
+      if (nu[i * S + j] != 0.0) {
+        pr = i;
+        pc = j;
+        break;
+      }
+  a->assign(S, 0.0);
+  b->assign(S, 0.0);
+  if (pr < 0) return true;
+  for (int j = 0; j < S; ++j) (*b)[j] = nu[pr * S + j];
+  for (int i = 0; i < S; ++i) (*a)[i] = nu[i * S + pc] / nu[pr * S + pc];
+  for (int i = 0; i < S; ++i)
+    for (int j = 0; j < S; ++j) {
+      double ref = (*a)[i] * (*b)[j];
+      if (std::fabs(nu[i * S + j] - ref) > 1e-14 * std::fabs(ref) + 1e-300) return false;
+    }
+  return true;
+}
+
+int build_device_side(landau_ctx* ctx) {
+  const int G = ctx->G, S = ctx->S, nb = ctx->nb;
+  // basis tables
+  DevTables ht;
+  memset(&ht, 0, sizeof(ht));
+  for (int e = 0; e < ctx->nq * nb; ++e) {
+    ht.B[e] = ctx->ht.B[e];
+    ht.dBxi[e] = ctx->ht.dBxi[e];
+    ht.dBeta[e] = ctx->ht.dBeta[e];
+  }
+  CUDA_TRY(ctx, cudaMalloc(&ctx->d_tab, sizeof(DevTables)));
+  ctx->allocs.push_back(ctx->d_tab);
+  CUDA_TRY(ctx, cudaMemcpy(ctx->d_tab, &ht, sizeof(DevTables), cudaMemcpyHostToDevice));
+  // concatenated IP coordinates, every grid block padded to the tile; padding points sit at (1, 0) and carry F = 0
+  ctx->ip_off.assign(G + 1, 0);
+  for (int g = 0; g < G; ++g) ctx->ip_off[g + 1] = ctx->ip_off[g] + round_up(ctx->hg[g].n_ip, K2M_TJ);
+  ctx->n_i_pad = ctx->ip_off[G];
+  std::vector<double> r(ctx->n_i_pad, 1.0), z(ctx->n_i_pad, 0.0);
+  for (int g = 0; g < G; ++g)
+    for (int j = 0; j < ctx->hg[g].n_ip; ++j) {
+      r[ctx->ip_off[g] + j] = ctx->hg[g].ip_r[j];
+      z[ctx->ip_off[g] + j] = ctx->hg[g].ip_z[j];
+    }
+  const double* tmp;
+  if (int rc = upload(ctx, r, &tmp)) return rc;
+  ctx->d_ip_r = const_cast<double*>(tmp);
+  if (int rc = upload(ctx, z, &tmp)) return rc;
+  ctx->d_ip_z = const_cast<double*>(tmp);
+  ctx->dg.resize(G);
+  ctx->d_rowptr.resize(G);
+  ctx->d_colidx.resize(G);
+  for (int g = 0; g < G; ++g) {
+    const HostGrid& h = ctx->hg[g];
+    DevGrid& d = ctx->dg[g];
+    d.n_cells = h.n_cells;
+    d.n_dof = h.n_dof;
+    d.n_ip = h.n_ip;
+    d.nnz = h.nnz;
+    d.ip_off = ctx->ip_off[g];
+    std::vector<double> sr(h.n_cells), sz(h.n_cells);
+    for (int e = 0; e < h.n_cells; ++e) {
+      sr[e] = 2.0 / h.cell_hr[e];
+      sz[e] = 2.0 / h.cell_hz[e];
+    }
+    int rc = 0;
+    rc = rc ? rc : upload(ctx, sr, &d.cell_sr);
+    rc = rc ? rc : upload(ctx, sz, &d.cell_sz);
+    rc = rc ? rc : upload(ctx, h.ip_w, &d.ip_w);
+    rc = rc ? rc : upload(ctx, h.en_ptr, &d.en_ptr);
+    rc = rc ? rc : upload(ctx, h.en_dof, &d.en_dof);
+    rc = rc ? rc : upload(ctx, h.en_w, &d.en_w);
+    rc = rc ? rc : upload(ctx, h.as_ptr, &d.as_ptr);
+    rc = rc ? rc : upload(ctx, h.as_code, &d.as_code);
+    rc = rc ? rc : upload(ctx, h.as_w, &d.as_w);
+    rc = rc ? rc : upload(ctx, h.ap_ptr, &d.ap_ptr);
+    rc = rc ? rc : upload(ctx, h.ap_code, &d.ap_code);
+    rc = rc ? rc : upload(ctx, h.ap_w, &d.ap_w);
+    rc = rc ? rc : upload(ctx, h.rowptr, &ctx->d_rowptr[g]);
+    rc = rc ? rc : upload(ctx, h.colidx, &ctx->d_colidx[g]);
+    if (rc) return rc;
+  }
+  // source columns: separable nu => one group over all grids, one column per batch entry;
+  // general nu => one group per grid, one column per species of the grid.
+  std::vector<double> sa, sb;
+  ctx->separable = rank_one(ctx->nu, S, &sa, &sb);
+  ctx->mix.assign(G, MixTable());
+  ctx->mix_group.assign(G, 0);
+  ctx->mix_col_in_group.assign(G, 0);
+  ctx->groups.clear();
+  ctx->comb.assign(S, CombineTable());
+  if (ctx->separable) {
+    ctx->groups.push_back(Group{0, ctx->n_i_pad, 1, 0});
+    for (int g = 0; g < G; ++g) {
+      MixTable& m = ctx->mix[g];
+      memset(&m, 0, sizeof(m));
+      m.ncb = 1;
+      int n = 0;
+      for (int s = 0; s < S; ++s)
+        if (ctx->species[s].grid == g) {
+          if (n >= 16) return fail(ctx, LANDAU_UNSUPPORTED, "more than 16 species on one grid");
+          m.species_foff[n] = (int)ctx->f_off[s];
+          m.wD[n] = sb[s];
+          m.wK[n] = sb[s] / ctx->species[s].mass;
+          ++n;
+        }
+      m.n_entries = n;
+      m.ptr[0] = 0;
+      m.ptr[1] = n;
+    }
+    for (int s = 0; s < S; ++s) {
+      CombineTable& c = ctx->comb[s];
+      memset(&c, 0, sizeof(c));
+      const double ma = ctx->species[s].mass;
+      c.n_terms = 1;
+      c.col_base[0] = 0;
+      c.col_stride[0] = 1;
+      c.coefD[0] = sa[s] / (ma * ma);
+      c.coefK[0] = sa[s] / ma;
+    }
+  } else {
+    if (S > 16) return fail(ctx, LANDAU_UNSUPPORTED, "general (non rank-one) nu supports at most 16 species");
+    std::vector<int> local(S, 0);
+    for (int g = 0; g < G; ++g) {
+      MixTable& m = ctx->mix[g];
+      memset(&m, 0, sizeof(m));
+      int n = 0;
+      for (int s = 0; s < S; ++s)
+        if (ctx->species[s].grid == g) {
+          m.species_foff[n] = (int)ctx->f_off[s];
+          m.wD[n] = 1.0;
+          m.wK[n] = 1.0 / ctx->species[s].mass;
+          m.ptr[n] = n;
+          local[s] = n;
+          ++n;
+        }
+      m.ptr[n] = n;
+      m.ncb = n;
+      m.n_entries = n;
+      ctx->mix_group[g] = (int)ctx->groups.size();
+      ctx->groups.push_back(Group{ctx->ip_off[g], ctx->ip_off[g + 1] - ctx->ip_off[g], n, 0});
+    }
+    for (int s = 0; s < S; ++s) {
+      CombineTable& c = ctx->comb[s];
+      memset(&c, 0, sizeof(c));
+      const double ma = ctx->species[s].mass;
+      c.n_terms = S;
+      for (int t = 0; t < S; ++t) {
+        c.col_base[t] = -(ctx->species[t].grid + 1);  // resolved per call: group column base depends on the chunk size
+        c.col_stride[t] = local[t];                   // temporarily: local column
+        c.coefD[t] = ctx->nu[s * S + t] / (ma * ma);
+        c.coefK[t] = ctx->nu[s * S + t] / ma;
+      }
+    }
+  }
+  return LANDAU_OK;
+}
+
+template <int NC>
+void launch_dfma(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nsplit, long long split_stride,
+                 cudaStream_t st) {
+  dim3 grid((ctx->n_i_pad + 127) / 128, (ncols + NC - 1) / NC, nsplit);
+  k2_inner_dfma<NC><<<grid, 128, 0, st>>>(ctx->d_ip_r, ctx->d_ip_z, ctx->n_i_pad, gr.j0, gr.nj_pad, ctx->F + gr.f_off,
+                                          ncols, ctx->Gp, split_stride, gcol0);
+}
+
+template <int NT>
+int launch_dmma(landau_ctx* ctx, const Group& gr, int ncols, int ncols_pad, int gcol0, int nsplit,
+                long long split_stride, cudaStream_t st) {
+  constexpr int CT = 8 * NT;
+  const size_t smem = 2 * (CT * 3 * K2M_LD + 2 * K2M_TJ) * sizeof(double);
+  static bool configured = false;
+  if (!configured) {
+    CUDA_TRY(ctx, cudaFuncSetAttribute(k2_inner_dmma<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = true;
+  }
+  dim3 grid((ctx->n_i_pad + 63) / 64, (ncols + CT - 1) / CT, nsplit);
+  k2_inner_dmma<NT><<<grid, 256, smem, st>>>(ctx->d_ip_r, ctx->d_ip_z, ctx->n_i_pad, gr.j0, gr.nj_pad, ctx->F + gr.f_off,
+                                             ncols_pad, ncols, ctx->Gp, split_stride, gcol0);
+  return LANDAU_OK;
+}
+
+// stages a1..a2b for batch entries [b0, b0+nbc): leaves D,K in ctx->DK
+int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cudaStream_t st) {
+  const int G = ctx->G, S = ctx->S;
+  // column bookkeeping for this chunk
+  long long foff = 0;
+  int total_cols = 0;
+  std::vector<int> gcol0(ctx->groups.size()), ncols(ctx->groups.size()), ncols_pad(ctx->groups.size());
+  for (size_t q = 0; q < ctx->groups.size(); ++q) {
+    Group& gr = ctx->groups[q];
+    ncols[q] = nbc * gr.ncb;
+    ncols_pad[q] = round_up(ncols[q], 64);
+    gr.f_off = foff;
+    foff += (long long)ncols_pad[q] * 3 * gr.nj_pad;
+    gcol0[q] = total_cols;
+    total_cols += ncols[q];
+  }
+  // j-split so that small problems still fill the machine
+  int max_blocks = 1 << 30, nsplit = 1;
+  for (size_t q = 0; q < ctx->groups.size(); ++q) {
+    const bool dmma = ctx->inner_kernel == 2 || (ctx->inner_kernel == 0 && ncols[q] >= 8);
+    const int blocks = dmma ? ((ctx->n_i_pad + 63) / 64) * ((ncols[q] + 63) / 64) : ((ctx->n_i_pad + 127) / 128) * ((ncols[q] + 3) / 4);
+    if (blocks < max_blocks) max_blocks = blocks;
+  }
+  if (max_blocks < 296) {
+    nsplit = (296 + max_blocks - 1) / max_blocks;
+    int min_tiles = 1 << 30;
+    for (const Group& gr : ctx->groups) min_tiles = std::min(min_tiles, gr.nj_pad / K2M_TJ);
+    nsplit = std::max(1, std::min(std::min(nsplit, min_tiles), 64));
+  }
+  const long long split_stride = (long long)total_cols * 5 * ctx->n_i_pad;
+  if (int rc = grow(ctx, &ctx->F, &ctx->F_cap, (size_t)foff, true)) return rc;
+  if (int rc = grow(ctx, &ctx->Gp, &ctx->Gp_cap, (size_t)split_stride * nsplit, false)) return rc;
+  if (int rc = grow(ctx, &ctx->DK, &ctx->DK_cap, (size_t)ctx->dk_stride * nbc, false)) return rc;
+
+  if (ctx->timing) cudaEventRecord(ctx->ev[0], st);
+  // K1
+  for (int g = 0; g < G; ++g) {
+    const int q = ctx->mix_group[g];
+    const Group& gr = ctx->groups[q];
+    dim3 grid((ctx->hg[g].n_ip + 255) / 256, nbc);
+    const int joff = ctx->ip_off[g] - gr.j0;
+    if (ctx->nb == 9)
+      k1_fields<9><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->mix[g], batch_f, ctx->f_stride, b0, nbc,
+                                         ctx->F + gr.f_off, gr.nj_pad, joff, 0);
+    else
+      k1_fields<16><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->mix[g], batch_f, ctx->f_stride, b0, nbc,
+                                          ctx->F + gr.f_off, gr.nj_pad, joff, 0);
+    ++ctx->launches;
+  }
+  if (ctx->timing) cudaEventRecord(ctx->ev[1], st);
+  // K2
+  for (size_t q = 0; q < ctx->groups.size(); ++q) {
+    const Group& gr = ctx->groups[q];
+    const bool dmma = ctx->inner_kernel == 2 || (ctx->inner_kernel == 0 && ncols[q] >= 8);
+    if (dmma) {
+      int rc;
+      if (ncols[q] > 32)
+        rc = launch_dmma<8>(ctx, gr, ncols[q], ncols_pad[q], gcol0[q], nsplit, split_stride, st);
+      else if (ncols[q] > 16)
+        rc = launch_dmma<4>(ctx, gr, ncols[q], ncols_pad[q], gcol0[q], nsplit, split_stride, st);
+      else if (ncols[q] > 8)
+        rc = launch_dmma<2>(ctx, gr, ncols[q], ncols_pad[q], gcol0[q], nsplit, split_stride, st);
+      else
+        rc = launch_dmma<1>(ctx, gr, ncols[q], ncols_pad[q], gcol0[q], nsplit, split_stride, st);
+      if (rc) return rc;
+    } else {
+      if (ncols[q] >= 3)
+        launch_dfma<4>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st);
+      else if (ncols[q] == 2)
+        launch_dfma<2>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st);
+      else
+        launch_dfma<1>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st);
+    }
+    ++ctx->launches;
+  }
+  if (ctx->timing) cudaEventRecord(ctx->ev[2], st);
+  // K2b
+  for (int s = 0; s < S; ++s) {
+    CombineTable ct = ctx->comb[s];
+    if (!ctx->separable) {
+      for (int t = 0; t < ct.n_terms; ++t) {
+        const int g = -ct.col_base[t] - 1, q = ctx->mix_group[g];
+        ct.col_base[t] = gcol0[q] + ct.col_stride[t];
+        ct.col_stride[t] = ctx->groups[q].ncb;
+      }
+    }
+    const int g = ctx->species[s].grid;
+    dim3 grid((ctx->hg[g].n_ip + 255) / 256, nbc);
+    k2b_combine<<<grid, 256, 0, st>>>(ct, ctx->Gp, split_stride, nsplit, ctx->n_i_pad, ctx->ip_off[g], ctx->hg[g].n_ip, nbc,
+                                      ctx->DK, ctx->dk_stride, ctx->dk_off[s]);
+    ++ctx->launches;
+  }
+  if (ctx->timing) cudaEventRecord(ctx->ev[3], st);
+  CUDA_TRY(ctx, cudaGetLastError());
+  return LANDAU_OK;
+}
+
+void accumulate_timing(landau_ctx* ctx, cudaStream_t st) {
+  if (!ctx->timing) return;
+  cudaEventRecord(ctx->ev[4], st);
+  cudaEventSynchronize(ctx->ev[4]);
+  for (int k = 0; k < 4; ++k) {
+    float ms = 0;
+    cudaEventElapsedTime(&ms, ctx->ev[k], ctx->ev[k + 1]);
+    ctx->stage_ms[k] += ms;
+  }
+}
+
+int check_call(landau_ctx* ctx, const void* in, int batch, const void* out) {
+  if (!ctx) return LANDAU_INVALID_ARG;
+  if (batch < 0) return fail(ctx, LANDAU_INVALID_ARG, "negative batch");
+  if (batch > 0 && (!in || !out)) return fail(ctx, LANDAU_INVALID_ARG, "null buffer");
+  if (ctx->device < 0) return fail(ctx, LANDAU_CUDA_ERROR, "host-only context (cuda_device < 0): no compute, no CPU fallback");
+  CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+  return LANDAU_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int landau_create(const landau_grid_desc* grids, int n_grids, const landau_species_desc* species, int n_species,
+                  const landau_quadrature_desc* quadrature, const double* nu, int cuda_device, landau_ctx** out) {
+  if (!grids || !species || !quadrature || !out || n_grids < 1 || n_species < 1)
+    return fail(nullptr, LANDAU_INVALID_ARG, "null argument or empty grid/species list");
+  if (quadrature->n_gauss_1d != quadrature->degree + 1)
+    return fail(nullptr, LANDAU_UNSUPPORTED, "n_gauss_1d must be degree + 1");
+  landau_ctx* ctx = new (std::nothrow) landau_ctx();
+  if (!ctx) return fail(nullptr, LANDAU_OUT_OF_MEMORY, "host allocation failed");
+  std::string msg;
+  auto bail = [&](int code, const std::string& m) {
+    landau_destroy(ctx);
+    return fail(nullptr, code, m);
+  };
+  try {
+    if (!build_tables(quadrature->degree, &ctx->ht, &msg)) return bail(LANDAU_UNSUPPORTED, msg);
+    ctx->k = quadrature->degree;
+    ctx->nb = ctx->ht.nb;
+    ctx->nq = ctx->ht.nq;
+    ctx->G = n_grids;
+    ctx->S = n_species;
+    ctx->hg.resize(n_grids);
+    for (int g = 0; g < n_grids; ++g) {
+      int rc = build_grid(grids[g], ctx->ht, &ctx->hg[g], &msg);
+      if (rc) return bail(rc, msg);
+    }
+    ctx->species.assign(species, species + n_species);
+    ctx->nu.resize((size_t)n_species * n_species);
+    for (int a = 0; a < n_species; ++a) {
+      if (species[a].grid < 0 || species[a].grid >= n_grids || !(species[a].mass > 0))
+        return bail(LANDAU_INVALID_ARG, "species with bad grid index or mass");
+      for (int b = 0; b < n_species; ++b)
+        ctx->nu[a * n_species + b] = nu ? nu[a * n_species + b]
+                                        : species[a].charge * species[a].charge * species[b].charge * species[b].charge;
+    }
+    long long fo = 0, vo = 0, dko = 0, flo = 0;
+    for (int a = 0; a < n_species; ++a) {
+      const HostGrid& h = ctx->hg[species[a].grid];
+      ctx->f_off.push_back(fo);
+      ctx->v_off.push_back(vo);
+      ctx->dk_off.push_back(dko);
+      ctx->fl_off.push_back(flo);
+      fo += h.n_dof;
+      vo += h.nnz;
+      dko += 5LL * h.n_ip;
+      flo += 2LL * h.n_ip;
+    }
+    ctx->f_stride = fo;
+    ctx->v_stride = vo;
+    ctx->dk_stride = dko;
+    ctx->fl_stride = flo;
+  } catch (const std::bad_alloc&) {
+    return bail(LANDAU_OUT_OF_MEMORY, "host allocation failed");
+  }
+  ctx->device = cuda_device;
+  if (cuda_device < 0) {  // host-only context: geometry queries work, compute entry points refuse
+    *out = ctx;
+    return LANDAU_OK;
+  }
+  cudaError_t e = cudaSetDevice(cuda_device);
+  if (e != cudaSuccess) return bail(LANDAU_CUDA_ERROR, std::string("cudaSetDevice: ") + cudaGetErrorString(e));
+  int rc = build_device_side(ctx);
+  if (rc) {
+    std::string m = ctx->err;
+    return bail(rc, m);
+  }
+  for (int k = 0; k < 5; ++k) cudaEventCreate(&ctx->ev[k]);
+  *out = ctx;
+  return LANDAU_OK;
+}
+
+void landau_destroy(landau_ctx* ctx) {
+  if (!ctx) return;
+  if (ctx->device >= 0 && (!ctx->allocs.empty() || ctx->F || ctx->Gp || ctx->DK)) {
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+  }
+  for (void* p : ctx->allocs) cudaFree(p);
+  for (double* p : {ctx->F, ctx->Gp, ctx->DK, ctx->FL, ctx->stage_in, ctx->stage_out})
+    if (p) cudaFree(p);
+  for (int k = 0; k < 5; ++k)
+    if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
+  delete ctx;
+}
+
+int landau_sizes(const landau_ctx* ctx, int* n_dof, int* nnz, int* n_ip, int* n_cells, long long* f_stride,
+                 long long* csr_stride) {
+  if (!ctx) return LANDAU_INVALID_ARG;
+  for (int g = 0; g < ctx->G; ++g) {
+    if (n_dof) n_dof[g] = ctx->hg[g].n_dof;
+    if (nnz) nnz[g] = ctx->hg[g].nnz;
+    if (n_ip) n_ip[g] = ctx->hg[g].n_ip;
+    if (n_cells) n_cells[g] = ctx->hg[g].n_cells;
+  }
+  if (f_stride) *f_stride = ctx->f_stride;
+  if (csr_stride) *csr_stride = ctx->v_stride;
+  return LANDAU_OK;
+}
+
+int landau_dof_coords(const landau_ctx* ctx, int grid, double* rz_host) {
+  if (!ctx || !rz_host || grid < 0 || grid >= ctx->G) return LANDAU_INVALID_ARG;
+  const HostGrid& h = ctx->hg[grid];
+  for (int i = 0; i < h.n_dof; ++i) {
+    rz_host[2 * i] = h.dof_r[i];
+    rz_host[2 * i + 1] = h.dof_z[i];
+  }
+  return LANDAU_OK;
+}
+
+int landau_ip_table(const landau_ctx* ctx, int grid, double* r_host, double* z_host, double* w_host) {
+  if (!ctx || grid < 0 || grid >= ctx->G) return LANDAU_INVALID_ARG;
+  const HostGrid& h = ctx->hg[grid];
+  if (r_host) memcpy(r_host, h.ip_r.data(), sizeof(double) * h.n_ip);
+  if (z_host) memcpy(z_host, h.ip_z.data(), sizeof(double) * h.n_ip);
+  if (w_host) memcpy(w_host, h.ip_w.data(), sizeof(double) * h.n_ip);
+  return LANDAU_OK;
+}
+
+int landau_csr_pattern(const landau_ctx* ctx, int grid, const int** rowptr_dev, const int** colidx_dev) {
+  if (!ctx || grid < 0 || grid >= ctx->G || !rowptr_dev || !colidx_dev || ctx->device < 0) return LANDAU_INVALID_ARG;
+  *rowptr_dev = ctx->d_rowptr[grid];
+  *colidx_dev = ctx->d_colidx[grid];
+  return LANDAU_OK;
+}
+
+int landau_csr_pattern_host(const landau_ctx* ctx, int grid, int* rowptr_host, int* colidx_host) {
+  if (!ctx || grid < 0 || grid >= ctx->G || !rowptr_host || !colidx_host) return LANDAU_INVALID_ARG;
+  const HostGrid& h = ctx->hg[grid];
+  memcpy(rowptr_host, h.rowptr.data(), sizeof(int) * h.rowptr.size());
+  memcpy(colidx_host, h.colidx.data(), sizeof(int) * h.colidx.size());
+  return LANDAU_OK;
+}
+
+int landau_jacobian(landau_ctx* ctx, const double* batch_f_dev, int batch, double dt, double* out_csr_vals_dev,
+                    void* cuda_stream) {
+  if (int rc = check_call(ctx, batch_f_dev, batch, out_csr_vals_dev)) return rc;
+  if (!(dt > 0)) return fail(ctx, LANDAU_INVALID_ARG, "dt must be > 0 (use +inf for the unshifted -J)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const double inv_dt = std::isinf(dt) ? 0.0 : 1.0 / dt;
+  for (int k = 0; k < 4; ++k) ctx->stage_ms[k] = 0;
+  for (int b0 = 0; b0 < batch; b0 += ctx->chunk) {
+    const int nbc = std::min(ctx->chunk, batch - b0);
+    if (int rc = run_coefficients(ctx, batch_f_dev, b0, nbc, st)) return rc;
+    for (int s = 0; s < ctx->S; ++s) {
+      const int g = ctx->species[s].grid;
+      dim3 grid((ctx->hg[g].nnz + 255) / 256, nbc);
+      double* vals = out_csr_vals_dev + (long long)b0 * ctx->v_stride;
+      if (ctx->nb == 9)
+        k3_assemble<9><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, nbc,
+                                             vals, ctx->v_stride, ctx->v_off[s]);
+      else
+        k3_assemble<16><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, nbc,
+                                              vals, ctx->v_stride, ctx->v_off[s]);
+      ++ctx->launches;
+    }
+    CUDA_TRY(ctx, cudaGetLastError());
+    accumulate_timing(ctx, st);
+    ctx->last_batch = nbc;
+  }
+  ctx->last_stream = st;
+  return LANDAU_OK;
+}
+
+int landau_apply(landau_ctx* ctx, const double* batch_f_dev, int batch, double* out_rhs_dev, void* cuda_stream) {
+  if (int rc = check_call(ctx, batch_f_dev, batch, out_rhs_dev)) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  for (int k = 0; k < 4; ++k) ctx->stage_ms[k] = 0;
+  for (int b0 = 0; b0 < batch; b0 += ctx->chunk) {
+    const int nbc = std::min(ctx->chunk, batch - b0);
+    if (int rc = run_coefficients(ctx, batch_f_dev, b0, nbc, st)) return rc;
+    if (int rc = grow(ctx, &ctx->FL, &ctx->FL_cap, (size_t)ctx->fl_stride * nbc, false)) return rc;
+    for (int s = 0; s < ctx->S; ++s) {
+      const int g = ctx->species[s].grid;
+      dim3 g1((ctx->hg[g].n_ip + 255) / 256, nbc), g2((ctx->hg[g].n_dof + 255) / 256, nbc);
+      if (ctx->nb == 9) {
+        k3_flux<9><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,
+                                       ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);
+        k3_apply<9><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev,
+                                        ctx->f_stride, ctx->f_off[s], b0);
+      } else {
+        k3_flux<16><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,
+                                        ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);
+        k3_apply<16><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev,
+                                         ctx->f_stride, ctx->f_off[s], b0);
+      }
+      ctx->launches += 2;
+    }
+    CUDA_TRY(ctx, cudaGetLastError());
+    accumulate_timing(ctx, st);
+    ctx->last_batch = nbc;
+  }
+  ctx->last_stream = st;
+  return LANDAU_OK;
+}
+
+int landau_jacobian_host(landau_ctx* ctx, const double* batch_f_host, int batch, double dt, double* out_csr_vals_host,
+                         void* cuda_stream) {
+  if (int rc = check_call(ctx, batch_f_host, batch, out_csr_vals_host)) return rc;
+  if (batch == 0) return LANDAU_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t nin = (size_t)batch * ctx->f_stride, nout = (size_t)batch * ctx->v_stride;
+  if (int rc = grow(ctx, &ctx->stage_in, &ctx->stage_in_cap, nin, false)) return rc;
+  if (int rc = grow(ctx, &ctx->stage_out, &ctx->stage_out_cap, nout, false)) return rc;
+  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_in, batch_f_host, nin * sizeof(double), cudaMemcpyHostToDevice, st));
+  if (int rc = landau_jacobian(ctx, ctx->stage_in, batch, dt, ctx->stage_out, cuda_stream)) return rc;
+  CUDA_TRY(ctx, cudaMemcpyAsync(out_csr_vals_host, ctx->stage_out, nout * sizeof(double), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(ctx, cudaStreamSynchronize(st));
+  return LANDAU_OK;
+}
+
+int landau_apply_host(landau_ctx* ctx, const double* batch_f_host, int batch, double* out_rhs_host, void* cuda_stream) {
+  if (int rc = check_call(ctx, batch_f_host, batch, out_rhs_host)) return rc;
+  if (batch == 0) return LANDAU_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t n = (size_t)batch * ctx->f_stride;
+  if (int rc = grow(ctx, &ctx->stage_in, &ctx->stage_in_cap, n, false)) return rc;
+  if (int rc = grow(ctx, &ctx->stage_out, &ctx->stage_out_cap, n, false)) return rc;
+  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_in, batch_f_host, n * sizeof(double), cudaMemcpyHostToDevice, st));
+  if (int rc = landau_apply(ctx, ctx->stage_in, batch, ctx->stage_out, cuda_stream)) return rc;
+  CUDA_TRY(ctx, cudaMemcpyAsync(out_rhs_host, ctx->stage_out, n * sizeof(double), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(ctx, cudaStreamSynchronize(st));
+  return LANDAU_OK;
+}
+
+int landau_last_coefficients(landau_ctx* ctx, double* dk_host) {
+  if (!ctx || !dk_host) return LANDAU_INVALID_ARG;
+  if (ctx->device < 0 || ctx->last_batch == 0 || !ctx->DK) return fail(ctx, LANDAU_INVALID_ARG, "no previous jacobian/apply call");
+  CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+  CUDA_TRY(ctx, cudaStreamSynchronize(ctx->last_stream));
+  CUDA_TRY(ctx, cudaMemcpy(dk_host, ctx->DK, sizeof(double) * ctx->dk_stride * ctx->last_batch, cudaMemcpyDeviceToHost));
+  return LANDAU_OK;
+}
+
+int landau_tensor_eval(const double* r_dev, const double* z_dev, const double* rb_dev, const double* zb_dev, int n,
+                       double* out_dev, void* cuda_stream) {
+  if (n < 0 || (n > 0 && (!r_dev || !z_dev || !rb_dev || !zb_dev || !out_dev))) return LANDAU_INVALID_ARG;
+  if (n == 0) return LANDAU_OK;
+  k_tensor_eval<<<(n + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(r_dev, z_dev, rb_dev, zb_dev, n, out_dev);
+  return cudaGetLastError() == cudaSuccess ? LANDAU_OK : LANDAU_CUDA_ERROR;
+}
+
+int landau_ellip_eval(const double* m_dev, const double* mp_dev, int n, double* out_dev, void* cuda_stream) {
+  if (n < 0 || (n > 0 && (!m_dev || !mp_dev || !out_dev))) return LANDAU_INVALID_ARG;
+  if (n == 0) return LANDAU_OK;
+  k_ellip_eval<<<(n + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(m_dev, mp_dev, n, out_dev);
+  return cudaGetLastError() == cudaSuccess ? LANDAU_OK : LANDAU_CUDA_ERROR;
+}
+
+int landau_fp64_probe(int kind, int iters, double* tflops, void* cuda_stream) {
+  if (!tflops || iters < 1 || (kind != 0 && kind != 1)) return LANDAU_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0, nsm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return LANDAU_CUDA_ERROR;
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  const int nblk = nsm * 4;
+  double* out = nullptr;
+  if (cudaMalloc(&out, sizeof(double) * nblk * 256) != cudaSuccess) return LANDAU_OUT_OF_MEMORY;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  double best = 0;
+  for (int rep = 0; rep < 3; ++rep) {
+    cudaEventRecord(e0, st);
+    if (kind == 0)
+      k_probe_dfma<<<nblk, 256, 0, st>>>(out, iters, 1.0000001, 1e-9);
+    else
+      k_probe_dmma<<<nblk, 256, 0, st>>>(out, iters, 1.0000001, 1e-9);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) {
+      cudaFree(out);
+      return LANDAU_CUDA_ERROR;
+    }
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    // dfma: 64 FMA per thread per iteration; dmma: 32 mma per warp per iteration, 512 flop each = 16 flop/thread
+    const double flop = (kind == 0 ? 2.0 * 64 : 16.0 * 32) * (double)iters * nblk * 256;
+    best = std::max(best, flop / (ms * 1e-3) * 1e-12);
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(out);
+  *tflops = best;
+  return LANDAU_OK;
+}
+
+long long landau_launch_count(const landau_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int landau_set_timing(landau_ctx* ctx, int enabled) {
+  if (!ctx) return LANDAU_INVALID_ARG;
+  ctx->timing = enabled != 0;
+  return LANDAU_OK;
+}
+
+int landau_last_stage_ms(landau_ctx* ctx, float* ms4) {
+  if (!ctx || !ms4) return LANDAU_INVALID_ARG;
+  for (int k = 0; k < 4; ++k) ms4[k] = ctx->stage_ms[k];
+  return LANDAU_OK;
+}
+
+int landau_set_inner_kernel(landau_ctx* ctx, int which) {
+  if (!ctx || which < 0 || which > 2) return LANDAU_INVALID_ARG;
+  ctx->inner_kernel = which;
+  return LANDAU_OK;
+}
+
+int landau_set_batch_chunk(landau_ctx* ctx, int chunk) {
+  if (!ctx || chunk < 1) return LANDAU_INVALID_ARG;
+  ctx->chunk = chunk;
+  return LANDAU_OK;
+}
+
+const char* landau_last_error(const landau_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+}  // extern "C"

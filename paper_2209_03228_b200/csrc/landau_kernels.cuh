@@ -1,0 +1,552 @@
+// landau_kernels.cuh -- device code of the batched Landau Jacobian path (sm_100a).
+//
+//   K1  k1_fields        a1: source fields  F = w_j * (sum over species) {f, df/dr, df/dz} at the IPs
+//   K2  k2_inner_dfma    a2: inner integral, plain FP64 FMA version (few columns)
+//       k2_inner_dmma    a2: inner integral as a tensor-generating FP64 GEMM on the DMMA pipe (many columns)
+//   K2b k2b_combine      a2: D_a, K_a = species combination of the partial sums (also sums the j-splits)
+//   K3  k3_assemble      a3+a4: element-matrix entries formed on the fly, gathered into batched CSR
+//   K3' k3_flux, k3_apply a5: operator application
+//
+// Notation follows PAPER.md sec. 2 and DESIGN.md: i = field point, j = source point, U^D / U^K the gyro-averaged
+// Landau tensor contracted with the field / source unit vectors.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "ellip_coeffs.h"
+
+namespace landau {
+
+// ------------------------------------------------------------------------------------------------------------
+// Elliptic pieces.  Coefficients live in constant memory; after unrolling every coefficient is a constant-bank
+// operand of a DFMA (no loads).
+// ------------------------------------------------------------------------------------------------------------
+__constant__ double c_S_P0[] = LANDAU_ELLIP_S_P0_COEFFS;
+__constant__ double c_S_DC[] = LANDAU_ELLIP_S_DC_COEFFS;
+__constant__ double c_S_Q[] = LANDAU_ELLIP_S_Q_COEFFS;
+__constant__ double c_L_A_E[] = LANDAU_ELLIP_L_A_E_COEFFS;
+__constant__ double c_L_B_E[] = LANDAU_ELLIP_L_B_E_COEFFS;
+__constant__ double c_L_A_DC[] = LANDAU_ELLIP_L_A_DC_COEFFS;
+__constant__ double c_L_B_DC[] = LANDAU_ELLIP_L_B_DC_COEFFS;
+__constant__ double c_L_A_Q[] = LANDAU_ELLIP_L_A_Q_COEFFS;
+__constant__ double c_L_B_Q[] = LANDAU_ELLIP_L_B_Q_COEFFS;
+
+template <int DEG>
+__device__ __forceinline__ double horner(const double* __restrict__ c, double t) {
+  double acc = c[DEG];
+#pragma unroll
+  for (int n = DEG - 1; n >= 0; --n) acc = fma(acc, t, c[n]);
+  return acc;
+}
+
+// (m' P0, Dc, Q) at parameter m with complement mp = 1 - m given separately (never formed by subtraction).
+//   m' P0 = E,  Dc = (K-E)/m,  Q = ((2-m)K - 2E)/m^2   -- see gen_ellip_coeffs.py.
+// Returns P0 itself in the small-m branch (no pole there) and E in the log branch; `p0_is_E` tells which.
+__device__ __forceinline__ void ellip_pieces(double m, double mp, double& P0_or_E, double& Dc, double& Q, bool& p0_is_E) {
+  if (mp >= 1.0 - LANDAU_ELLIP_M_SPLIT) {
+    const double t = m - 0.5 * LANDAU_ELLIP_M_SPLIT;
+    P0_or_E = horner<LANDAU_ELLIP_S_P0_DEG>(c_S_P0, t);
+    Dc = horner<LANDAU_ELLIP_S_DC_DEG>(c_S_DC, t);
+    Q = horner<LANDAU_ELLIP_S_Q_DEG>(c_S_Q, t);
+    p0_is_E = false;
+  } else {
+    const double t = mp - 0.5 * (1.0 - LANDAU_ELLIP_M_SPLIT);
+    const double lg = -log(mp);
+    P0_or_E = fma(lg, horner<LANDAU_ELLIP_L_B_E_DEG>(c_L_B_E, t), horner<LANDAU_ELLIP_L_A_E_DEG>(c_L_A_E, t));
+    Dc = fma(lg, horner<LANDAU_ELLIP_L_B_DC_DEG>(c_L_B_DC, t), horner<LANDAU_ELLIP_L_A_DC_DEG>(c_L_A_DC, t));
+    Q = fma(lg, horner<LANDAU_ELLIP_L_B_Q_DEG>(c_L_B_Q, t), horner<LANDAU_ELLIP_L_A_Q_DEG>(c_L_A_Q, t));
+    p0_is_E = true;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// 2V Landau tensor for the pair (field point (r,z), source point (rb,zb)); DESIGN.md "tensor":
+//   s+- = (r +- rb)^2 + dz^2, m = 4 r rb / s+, m' = s-/s+, c = 4 / s+^{3/2}
+//   UD_rr = c (4 rb^2 Q + dz^2 P0)         UK_rr = c (4 r rb Q + dz^2 m P2),  m P2 = m (P0 - Dc - Q)
+//   UD_zz = c ((r-rb)^2 P0 + 4 r rb Dc)    UK_zz = UD_zz
+//   UD_rz = -dz c ((r-rb) P0 + 2 rb Dc)    UK_rz = UD_rz
+//                                          UK_zr =  dz c ((rb-r) P0 + 2 r Dc)
+// Coincident points (s- <= 1e-20 s+) give zero (reading A2).
+// ------------------------------------------------------------------------------------------------------------
+struct Tensor5 {
+  double UDrr, UDrz, UDzz, UKrr, UKzr;
+};
+
+__device__ __forceinline__ Tensor5 landau_tensor_2v(double r, double z, double rb, double zb) {
+  const double dr = r - rb, dz = z - zb;
+  const double dz2 = dz * dz;
+  double sm = fma(dr, dr, dz2);
+  const double rr4 = 4.0 * r * rb;
+  const double sp = sm + rr4;
+  const bool coincident = sm <= 1e-20 * sp;
+  sm = coincident ? sp : sm;
+  const double inv = 1.0 / (sp * sm);
+  const double isp = inv * sm;  // 1/s+
+  const double mp = sm * isp;
+  const double m = rr4 * isp;
+  double c = 4.0 * isp * rsqrt(sp);
+  c = coincident ? 0.0 : c;
+  double P0, Dc, Q;
+  bool p0_is_E;
+  ellip_pieces(m, mp, P0, Dc, Q, p0_is_E);
+  if (p0_is_E) P0 *= sp * sp * inv;  // E / m' = E s+ / s-
+  const double mP2 = m * (P0 - Dc - Q);
+  Tensor5 t;
+  t.UDrr = c * fma(4.0 * rb * rb, Q, dz2 * P0);
+  t.UDzz = c * fma(dr * dr, P0, rr4 * Dc);
+  t.UDrz = -dz * c * fma(dr, P0, 2.0 * rb * Dc);
+  t.UKrr = c * fma(rr4, Q, dz2 * mP2);
+  t.UKzr = dz * c * fma(-dr, P0, 2.0 * r * Dc);
+  return t;
+}
+
+__global__ void k_tensor_eval(const double* __restrict__ r, const double* __restrict__ z, const double* __restrict__ rb,
+                              const double* __restrict__ zb, int n, double* __restrict__ out) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  Tensor5 u = landau_tensor_2v(r[t], z[t], rb[t], zb[t]);
+  out[5 * t + 0] = u.UDrr;
+  out[5 * t + 1] = u.UDrz;
+  out[5 * t + 2] = u.UDzz;
+  out[5 * t + 3] = u.UKrr;
+  out[5 * t + 4] = u.UKzr;
+}
+
+__global__ void k_ellip_eval(const double* __restrict__ m, const double* __restrict__ mp, int n, double* __restrict__ out) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  double P0, Dc, Q;
+  bool isE;
+  ellip_pieces(m[t], mp[t], P0, Dc, Q, isE);
+  if (isE) P0 /= mp[t];
+  out[3 * t + 0] = P0;
+  out[3 * t + 1] = Dc;
+  out[3 * t + 2] = Q;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Device-side description of one grid (pointers into context-owned tables).
+// ------------------------------------------------------------------------------------------------------------
+struct DevGrid {
+  int n_cells, n_dof, n_ip, nnz;
+  int ip_off;  // offset of this grid's IPs in the concatenated IP arrays
+  const double* cell_sr;  // 2/hr per cell
+  const double* cell_sz;  // 2/hz per cell
+  const double* ip_w;     // [n_ip]
+  const int* en_ptr;      // [n_cells*nb + 1]
+  const int* en_dof;
+  const double* en_w;
+  const int* as_ptr;  // [nnz+1]
+  const int* as_code;
+  const double* as_w;
+  const int* ap_ptr;  // [n_dof+1]
+  const int* ap_code;
+  const double* ap_w;
+};
+
+// basis tabulation, [q][a]; nb = nq <= 16
+struct DevTables {
+  double B[256], dBxi[256], dBeta[256];
+};
+
+// ------------------------------------------------------------------------------------------------------------
+// K1: source fields.  One thread per (integration point j of grid g, batch entry b); q fastest so that the
+// threads of a cell share its dof loads and the stores along j are coalesced.
+//   F layout: [col][3][nj_pad], col = col0 + b*ncb + c;  comp 0: w f, 1: w df/dr, 2: w df/dz
+//   column c of the grid sums the species listed in (mix_ptr, mix_species, mix_wD, mix_wK).
+// ------------------------------------------------------------------------------------------------------------
+struct MixTable {  // per grid
+  int ncb;         // columns per batch entry
+  int n_entries;   // total entries
+  int ptr[17];     // per column c: entries ptr[c]..ptr[c+1]   (ncb <= 16)
+  int species_foff[16];  // offset of the species' dofs inside a batch entry
+  double wD[16], wK[16];
+};
+
+template <int NB>
+__global__ void __launch_bounds__(256)
+k1_fields(DevGrid g, const DevTables* __restrict__ tab, MixTable mix, const double* __restrict__ batch_f, long long f_stride,
+          int b0, int nbatch, double* __restrict__ F, long long nj_pad, int j_off_in_group, int col0) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const int b = blockIdx.y;
+  if (j >= g.n_ip || b >= nbatch) return;
+  const int cell = j / NB, q = j - cell * NB;
+  const double sr = g.cell_sr[cell], sz = g.cell_sz[cell], w = g.ip_w[j];
+  const double* fb = batch_f + (long long)(b0 + b) * f_stride;
+  for (int c = 0; c < mix.ncb; ++c) {
+    double aD = 0.0, aKr = 0.0, aKz = 0.0;
+    for (int e = mix.ptr[c]; e < mix.ptr[c + 1]; ++e) {
+      const double* fs = fb + mix.species_foff[e];
+      double v = 0.0, vx = 0.0, vy = 0.0;
+#pragma unroll 4
+      for (int a = 0; a < NB; ++a) {
+        const int p0 = g.en_ptr[cell * NB + a], p1 = g.en_ptr[cell * NB + a + 1];
+        double fa = 0.0;
+        for (int p = p0; p < p1; ++p) fa = fma(g.en_w[p], fs[g.en_dof[p]], fa);
+        v = fma(tab->B[q * NB + a], fa, v);
+        vx = fma(tab->dBxi[q * NB + a], fa, vx);
+        vy = fma(tab->dBeta[q * NB + a], fa, vy);
+      }
+      aD = fma(mix.wD[e], v, aD);
+      aKr = fma(mix.wK[e], vx * sr, aKr);
+      aKz = fma(mix.wK[e], vy * sz, aKz);
+    }
+    const long long col = col0 + (long long)b * mix.ncb + c;
+    double* dst = F + col * 3 * nj_pad + j_off_in_group + j;
+    dst[0] = w * aD;
+    dst[nj_pad] = w * aKr;
+    dst[2 * nj_pad] = w * aKz;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// K2 (plain FP64 FMA): thread = one field point i, NC columns; the block's 128 field points share source tiles
+// staged in shared memory (every lane reads the same address: broadcast).  blockIdx.z splits the j range.
+//   G layout: [split][col][5][n_i]   comp: 0 GD_rr, 1 GD_rz, 2 GD_zz, 3 GK_r, 4 GK_z
+// ------------------------------------------------------------------------------------------------------------
+constexpr int K2_TJ = 16;  // source points per shared-memory tile
+
+template <int NC>
+__global__ void __launch_bounds__(128)
+k2_inner_dfma(const double* __restrict__ ip_r, const double* __restrict__ ip_z, int n_i, int j0, int nj_pad,
+              const double* __restrict__ F, int ncols, double* __restrict__ G, long long g_split_stride, int gcol0) {
+  __shared__ double s_r[K2_TJ], s_z[K2_TJ];
+  __shared__ double s_F[NC][3][K2_TJ];
+  const int i = min((int)(blockIdx.x * blockDim.x + threadIdx.x), n_i - 1);
+  const double r = ip_r[i], z = ip_z[i];
+  const int colbase = blockIdx.y * NC;
+  const int ntiles = nj_pad / K2_TJ;
+  const int per = (ntiles + gridDim.z - 1) / gridDim.z;
+  const int t0 = blockIdx.z * per, t1 = min(t0 + per, ntiles);
+  double acc[NC][5];
+#pragma unroll
+  for (int c = 0; c < NC; ++c)
+#pragma unroll
+    for (int k = 0; k < 5; ++k) acc[c][k] = 0.0;
+  for (int t = t0; t < t1; ++t) {
+    __syncthreads();
+    if (threadIdx.x < K2_TJ) {
+      s_r[threadIdx.x] = ip_r[j0 + t * K2_TJ + threadIdx.x];
+      s_z[threadIdx.x] = ip_z[j0 + t * K2_TJ + threadIdx.x];
+    }
+    for (int e = threadIdx.x; e < NC * 3 * K2_TJ; e += blockDim.x) {
+      const int jj = e % K2_TJ, ck = e / K2_TJ;  // ck = c*3 + comp
+      const int col = colbase + ck / 3;
+      (&s_F[0][0][0])[e] = col < ncols ? F[((long long)col * 3 + ck % 3) * nj_pad + t * K2_TJ + jj] : 0.0;
+    }
+    __syncthreads();
+#pragma unroll 2
+    for (int jj = 0; jj < K2_TJ; ++jj) {
+      const Tensor5 u = landau_tensor_2v(r, z, s_r[jj], s_z[jj]);
+#pragma unroll
+      for (int c = 0; c < NC; ++c) {
+        const double wf = s_F[c][0][jj], wfr = s_F[c][1][jj], wfz = s_F[c][2][jj];
+        acc[c][0] = fma(u.UDrr, wf, acc[c][0]);
+        acc[c][1] = fma(u.UDrz, wf, acc[c][1]);
+        acc[c][2] = fma(u.UDzz, wf, acc[c][2]);
+        acc[c][3] = fma(u.UKrr, wfr, fma(u.UDrz, wfz, acc[c][3]));
+        acc[c][4] = fma(u.UKzr, wfr, fma(u.UDzz, wfz, acc[c][4]));
+      }
+    }
+  }
+  if (blockIdx.x * blockDim.x + threadIdx.x < n_i) {
+#pragma unroll
+    for (int c = 0; c < NC; ++c)
+      if (colbase + c < ncols) {
+        double* dst = G + blockIdx.z * g_split_stride + ((long long)(gcol0 + colbase + c) * 5) * n_i + i;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) dst[(long long)k * n_i] = acc[c][k];
+      }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// K2 (DMMA): the inner integral as a GEMM whose A operand is generated on the fly.
+//   G[i, comp, col] = sum_j U_comp(i,j) F[j, col]  -- per warp an 8(i) x 8NT(col) output tile, k = 4 source points per
+//   step.  Lane (g = lane/4, t = lane%4) evaluates the tensor of the pair (i0+g, j+t): exactly the A-fragment
+//   layout of mma.m8n8k4.f64, so the five tensor components go from registers straight into seven DMMAs per
+//   8-column tile (3 for G^D, 4 for G^K) with no shared-memory round trip.  B fragments (F[j+t][col0+g]) come
+//   from a shared-memory tile [col][3][TJ+4] (row stride 20 doubles: conflict-free), double-buffered with cp.async.
+//   Block = 8 warps = 64 field points; blockIdx.y = column tile; blockIdx.z = j split.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int K2M_TJ = 16;
+constexpr int K2M_LD = K2M_TJ + 4;
+
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(d0), "+d"(d1)
+               : "d"(a), "d"(b));
+}
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;" ::"n"(N));
+}
+
+template <int NT>
+__global__ void __launch_bounds__(256)
+k2_inner_dmma(const double* __restrict__ ip_r, const double* __restrict__ ip_z, int n_i, int j0, int nj_pad,
+              const double* __restrict__ F, int ncols_pad, int ncols, double* __restrict__ G, long long g_split_stride,
+              int gcol0) {
+  constexpr int CT = 8 * NT;
+  extern __shared__ __align__(16) double smem[];
+  // per stage: s_F[CT][3][K2M_LD], s_r[K2M_TJ], s_z[K2M_TJ]
+  constexpr int STAGE = CT * 3 * K2M_LD + 2 * K2M_TJ;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int gq = lane >> 2, tq = lane & 3;
+  const int i = min((int)(blockIdx.x * 64 + warp * 8 + gq), n_i - 1);
+  const double r = ip_r[i], z = ip_z[i];
+  const int colbase = blockIdx.y * CT;
+  const int ntiles = nj_pad / K2M_TJ;
+  const int per = (ntiles + gridDim.z - 1) / gridDim.z;
+  const int t0 = blockIdx.z * per, t1 = min(t0 + per, ntiles);
+
+  double acc[NT][5][2];
+#pragma unroll
+  for (int n = 0; n < NT; ++n)
+#pragma unroll
+    for (int k = 0; k < 5; ++k) acc[n][k][0] = acc[n][k][1] = 0.0;
+
+  auto issue_tile = [&](int t, int stage) {
+    double* sF = smem + stage * STAGE;
+    // CT*3 rows of K2M_TJ doubles = 8 x 16-byte chunks per row
+    for (int e = threadIdx.x; e < CT * 3 * (K2M_TJ / 2); e += 256) {
+      const int row = e / (K2M_TJ / 2), ch = e % (K2M_TJ / 2);
+      const double* src = F + ((long long)(colbase * 3 + row)) * nj_pad + (long long)t * K2M_TJ + ch * 2;
+      cp_async16(sF + row * K2M_LD + ch * 2, src);
+    }
+    if (threadIdx.x < K2M_TJ / 2) {
+      cp_async16(sF + CT * 3 * K2M_LD + threadIdx.x * 2, ip_r + j0 + t * K2M_TJ + threadIdx.x * 2);
+    } else if (threadIdx.x < K2M_TJ) {
+      const int c = threadIdx.x - K2M_TJ / 2;
+      cp_async16(sF + CT * 3 * K2M_LD + K2M_TJ + c * 2, ip_z + j0 + t * K2M_TJ + c * 2);
+    }
+    cp_async_commit();
+  };
+
+  if (t0 < t1) issue_tile(t0, 0);
+  for (int t = t0; t < t1; ++t) {
+    const int stage = (t - t0) & 1;
+    if (t + 1 < t1) {
+      issue_tile(t + 1, stage ^ 1);
+      cp_async_wait<1>();
+    } else {
+      cp_async_wait<0>();
+    }
+    __syncthreads();
+    const double* sF = smem + stage * STAGE;
+    const double* s_r = sF + CT * 3 * K2M_LD;
+    const double* s_z = s_r + K2M_TJ;
+#pragma unroll 1
+    for (int jj = 0; jj < K2M_TJ; jj += 4) {
+      const Tensor5 u = landau_tensor_2v(r, z, s_r[jj + tq], s_z[jj + tq]);
+#pragma unroll
+      for (int n = 0; n < NT; ++n) {
+        const double* col = sF + ((n * 8 + gq) * 3) * K2M_LD + jj + tq;
+        const double wf = col[0], wfr = col[K2M_LD], wfz = col[2 * K2M_LD];
+        dmma884(acc[n][0][0], acc[n][0][1], u.UDrr, wf);
+        dmma884(acc[n][1][0], acc[n][1][1], u.UDrz, wf);
+        dmma884(acc[n][2][0], acc[n][2][1], u.UDzz, wf);
+        dmma884(acc[n][3][0], acc[n][3][1], u.UKrr, wfr);
+        dmma884(acc[n][3][0], acc[n][3][1], u.UDrz, wfz);
+        dmma884(acc[n][4][0], acc[n][4][1], u.UKzr, wfr);
+        dmma884(acc[n][4][0], acc[n][4][1], u.UDzz, wfz);
+      }
+    }
+    __syncthreads();
+  }
+  // C fragment: row gq (field point), columns 2 tq, 2 tq + 1
+  if (blockIdx.x * 64 + warp * 8 + gq < n_i) {
+#pragma unroll
+    for (int n = 0; n < NT; ++n)
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int col = colbase + n * 8 + 2 * tq + h;
+        if (col < ncols) {
+          double* dst = G + blockIdx.z * g_split_stride + ((long long)(gcol0 + col) * 5) * n_i + i;
+#pragma unroll
+          for (int k = 0; k < 5; ++k) dst[(long long)k * n_i] = acc[n][k][h];
+        }
+      }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// K2b: species combination (eq. 2.1 prefactors) and sum over j splits.
+//   DK[b][species a][5][n_ip(g(a))] = sum_terms coef * sum_split G[split][col][comp][ip_off + i]
+// ------------------------------------------------------------------------------------------------------------
+struct CombineTable {   // per species alpha
+  int n_terms;
+  int col_base[16];     // column of batch entry 0
+  int col_stride[16];   // columns per batch entry of that group
+  double coefD[16], coefK[16];
+};
+
+__global__ void __launch_bounds__(256)
+k2b_combine(CombineTable ct, const double* __restrict__ G, long long g_split_stride, int n_split, int n_i_total,
+            int ip_off, int n_ip, int nbatch, double* __restrict__ DK, long long dk_stride, long long dk_off) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int b = blockIdx.y;
+  if (i >= n_ip || b >= nbatch) return;
+  double out[5] = {0, 0, 0, 0, 0};
+  for (int t = 0; t < ct.n_terms; ++t) {
+    const long long col = ct.col_base[t] + (long long)b * ct.col_stride[t];
+    double s[5] = {0, 0, 0, 0, 0};
+    for (int sp = 0; sp < n_split; ++sp) {
+      const double* src = G + sp * g_split_stride + col * 5 * n_i_total + ip_off + i;
+#pragma unroll
+      for (int k = 0; k < 5; ++k) s[k] += src[(long long)k * n_i_total];
+    }
+    out[0] = fma(ct.coefD[t], s[0], out[0]);
+    out[1] = fma(ct.coefD[t], s[1], out[1]);
+    out[2] = fma(ct.coefD[t], s[2], out[2]);
+    out[3] = fma(ct.coefK[t], s[3], out[3]);
+    out[4] = fma(ct.coefK[t], s[4], out[4]);
+  }
+  double* dst = DK + (long long)b * dk_stride + dk_off + i;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) dst[(long long)k * n_ip] = out[k];
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// K3: one thread per CSR slot of (batch entry, species): gathers its element-matrix contributions, each formed
+// on the fly  A_e[a][c] = sum_q w_q [ phi_a phi_c / dt + grad phi_a . D grad phi_c - (grad phi_a . K) phi_c ]
+// (eq. 2.4 with the sparse Jacobian of PAPER.md:73), weighted by the constraint products P[a][I] P[c][J].
+// Every CSR value is written exactly once, coalesced along the slot index; no atomics.
+// ------------------------------------------------------------------------------------------------------------
+template <int NB>
+__global__ void __launch_bounds__(256)
+k3_assemble(DevGrid g, const DevTables* __restrict__ tab, const double* __restrict__ DK, long long dk_stride,
+            long long dk_off, double inv_dt, int nbatch, double* __restrict__ vals, long long v_stride, long long v_off) {
+  __shared__ double sB[NB * NB], sX[NB * NB], sY[NB * NB];
+  for (int e = threadIdx.x; e < NB * NB; e += blockDim.x) {
+    sB[e] = tab->B[e];
+    sX[e] = tab->dBxi[e];
+    sY[e] = tab->dBeta[e];
+  }
+  __syncthreads();
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  const int b = blockIdx.y;
+  if (n >= g.nnz || b >= nbatch) return;
+  const double* dk = DK + (long long)b * dk_stride + dk_off;
+  double total = 0.0;
+  for (int p = g.as_ptr[n]; p < g.as_ptr[n + 1]; ++p) {
+    const int code = g.as_code[p];
+    const int c = code % NB, a = (code / NB) % NB, cell = code / (NB * NB);
+    const double sr = g.cell_sr[cell], sz = g.cell_sz[cell];
+    double s = 0.0;
+#pragma unroll 4
+    for (int q = 0; q < NB; ++q) {
+      const int ip = cell * NB + q;
+      const double w = g.ip_w[ip];
+      const double Drr = dk[ip], Drz = dk[g.n_ip + ip], Dzz = dk[2 * g.n_ip + ip], Kr = dk[3 * g.n_ip + ip],
+                   Kz = dk[4 * g.n_ip + ip];
+      const double pa = sB[q * NB + a], par = sX[q * NB + a] * sr, paz = sY[q * NB + a] * sz;
+      const double pc = sB[q * NB + c], pcr = sX[q * NB + c] * sr, pcz = sY[q * NB + c] * sz;
+      double v = inv_dt * pa * pc;
+      v = fma(par, fma(Drr, pcr, Drz * pcz), v);
+      v = fma(paz, fma(Drz, pcr, Dzz * pcz), v);
+      v = fma(-fma(par, Kr, paz * Kz), pc, v);
+      s = fma(w, v, s);
+    }
+    total = fma(g.as_w[p], s, total);
+  }
+  vals[(long long)b * v_stride + v_off + n] = total;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// K3' (apply): flux at the IPs, then gather into dofs:  rhs_a = - sum_q w_q grad phi_a . (D grad f - K f).
+// ------------------------------------------------------------------------------------------------------------
+template <int NB>
+__global__ void __launch_bounds__(256)
+k3_flux(DevGrid g, const DevTables* __restrict__ tab, const double* __restrict__ batch_f, long long f_stride,
+        long long f_off, int b0, const double* __restrict__ DK, long long dk_stride, long long dk_off, int nbatch,
+        double* __restrict__ FL, long long fl_stride, long long fl_off) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const int b = blockIdx.y;
+  if (j >= g.n_ip || b >= nbatch) return;
+  const int cell = j / NB, q = j - cell * NB;
+  const double* fs = batch_f + (long long)(b0 + b) * f_stride + f_off;
+  double v = 0.0, vx = 0.0, vy = 0.0;
+#pragma unroll 4
+  for (int a = 0; a < NB; ++a) {
+    double fa = 0.0;
+    for (int p = g.en_ptr[cell * NB + a]; p < g.en_ptr[cell * NB + a + 1]; ++p) fa = fma(g.en_w[p], fs[g.en_dof[p]], fa);
+    v = fma(tab->B[q * NB + a], fa, v);
+    vx = fma(tab->dBxi[q * NB + a], fa, vx);
+    vy = fma(tab->dBeta[q * NB + a], fa, vy);
+  }
+  const double fr = vx * g.cell_sr[cell], fz = vy * g.cell_sz[cell], w = g.ip_w[j];
+  const double* dk = DK + (long long)b * dk_stride + dk_off;
+  const double Drr = dk[j], Drz = dk[g.n_ip + j], Dzz = dk[2 * g.n_ip + j], Kr = dk[3 * g.n_ip + j], Kz = dk[4 * g.n_ip + j];
+  double* fl = FL + (long long)b * fl_stride + fl_off;
+  fl[j] = w * (fma(Drr, fr, Drz * fz) - Kr * v);
+  fl[g.n_ip + j] = w * (fma(Drz, fr, Dzz * fz) - Kz * v);
+}
+
+template <int NB>
+__global__ void __launch_bounds__(256)
+k3_apply(DevGrid g, const DevTables* __restrict__ tab, const double* __restrict__ FL, long long fl_stride, long long fl_off,
+         int nbatch, double* __restrict__ rhs, long long f_stride, long long f_off, int b0) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  const int b = blockIdx.y;
+  if (n >= g.n_dof || b >= nbatch) return;
+  const double* fl = FL + (long long)b * fl_stride + fl_off;
+  double total = 0.0;
+  for (int p = g.ap_ptr[n]; p < g.ap_ptr[n + 1]; ++p) {
+    const int code = g.ap_code[p];
+    const int a = code % NB, cell = code / NB;
+    const double sr = g.cell_sr[cell], sz = g.cell_sz[cell];
+    double s = 0.0;
+#pragma unroll 4
+    for (int q = 0; q < NB; ++q) {
+      const int ip = cell * NB + q;
+      s = fma(tab->dBxi[q * NB + a] * sr, fl[ip], s);
+      s = fma(tab->dBeta[q * NB + a] * sz, fl[g.n_ip + ip], s);
+    }
+    total = fma(g.ap_w[p], s, total);
+  }
+  rhs[(long long)(b0 + b) * f_stride + f_off + n] = -total;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// FP64 pipe probes (roofline denominators measured in-process by bench.py).
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_probe_dfma(double* out, int iters, double a, double b) {
+  double acc[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) acc[k] = threadIdx.x * 1e-3 + k;
+  for (int it = 0; it < iters; ++it)
+#pragma unroll
+    for (int u = 0; u < 8; ++u)
+#pragma unroll
+      for (int k = 0; k < 8; ++k) acc[k] = fma(acc[k], a, b);
+  double s = 0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) s += acc[k];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+__global__ void __launch_bounds__(256) k_probe_dmma(double* out, int iters, double a, double b) {
+  double c0[8], c1[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    c0[k] = threadIdx.x * 1e-3 + k;
+    c1[k] = k;
+  }
+  for (int it = 0; it < iters; ++it)
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+      for (int k = 0; k < 8; ++k) dmma884(c0[k], c1[k], a, b);
+  double s = 0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) s += c0[k] + c1[k];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+}  // namespace landau

@@ -1,0 +1,259 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on the same seeded
+inputs.  Bar (BASELINE.json north_star): relative Frobenius error <= 1e-10 per (batch entry, species) block for
+Jacobians and apply vectors; <= 1e-14 relative for the elliptic pieces; bit-exact for the integer CSR pattern.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2209_03228_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def Bn():
+    from paper_2209_03228_b200 import binding
+    binding.load()
+    return binding
+
+
+def _make(orc, Bn, cfg, nu=None):
+    o = orc.Oracle(cfg["grids"], cfg["species"], cfg["degree"], nu=nu)
+    L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"], nu=nu)
+    return o, L
+
+
+def _block_errors(L, got, ref, offs):
+    errs = []
+    for b in range(ref.shape[0]):
+        for s in range(L.S):
+            a, r = got[b, offs[s]:offs[s + 1]], ref[b, offs[s]:offs[s + 1]]
+            errs.append(np.linalg.norm(a - r) / np.linalg.norm(r))
+    return np.array(errs)
+
+
+# ------------------------------------------------------------------------------------------------ pieces
+def test_elliptic_pieces_device_accuracy(orc, Bn, torch_cuda):
+    torch = torch_cuda
+    ms, mps = [], []
+    for e in np.linspace(-7, math.log10(0.5), 400):       # m from 1e-7 up
+        ms.append(10 ** e); mps.append(1 - 10 ** e)
+    for e in np.linspace(-7, math.log10(0.5), 400):       # m' from 1e-7 up (m -> 1)
+        mps.append(10 ** e); ms.append(1 - 10 ** e)
+    for m in np.linspace(0.55, 0.65, 101):                # across the branch split
+        ms.append(m); mps.append(1 - m)
+    m = torch.tensor(ms, dtype=torch.float64, device="cuda")
+    mp = torch.tensor(mps, dtype=torch.float64, device="cuda")
+    out = torch.empty(3 * len(ms), dtype=torch.float64, device="cuda")
+    Bn.landau_ellip_eval(m, mp, out)
+    got = out.cpu().numpy().reshape(-1, 3)
+    worst = 0
+    for k in range(len(ms)):
+        e = orc.ellip(ms[k], mps[k])
+        for c, name in enumerate(["P0", "Dc", "Q"]):
+            worst = max(worst, abs(got[k, c] - e[name]) / e[name])
+    assert worst < 1e-14, worst
+
+
+def test_tensor_device_vs_oracle(orc, Bn, torch_cuda):
+    torch = torch_cuda
+    rng = np.random.default_rng(11)
+    n = 4000
+    r, rb = rng.uniform(1e-4, 5, n), rng.uniform(1e-4, 5, n)
+    z, zb = rng.uniform(-5, 5, n), rng.uniform(-5, 5, n)
+    near = rng.uniform(size=n) < 0.3
+    rb[near] = r[near] * (1 + 1e-3 * rng.normal(size=near.sum()))
+    zb[near] = z[near] + 1e-3 * rng.normal(size=near.sum())
+    far = rng.uniform(size=n) < 0.3
+    rb[far] *= 1e-3
+    zb[far] *= 1e-3
+    rb[:5], zb[:5] = r[:5], z[:5]                          # coincident pairs
+    dev = [torch.tensor(a, dtype=torch.float64, device="cuda") for a in (r, z, rb, zb)]
+    out = torch.empty(5 * n, dtype=torch.float64, device="cuda")
+    Bn.landau_tensor_eval(*dev, out)
+    got = out.cpu().numpy().reshape(n, 5)
+    assert np.all(got[:5] == 0)
+    worst = 0
+    for k in range(5, n):
+        ref, ok = orc.tensor(r[k], z[k], rb[k], zb[k])
+        worst = max(worst, np.abs(got[k] - ref).max() / np.abs(ref).max())
+    assert worst < 2e-14, worst
+
+
+# ------------------------------------------------------------------------------------------------ small, full batch
+@pytest.mark.parametrize("kind,degree", [("uniform", 2), ("uniform", 3), ("quadtree", 2), ("quadtree", 3)])
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_tiny_jacobian_apply_and_coefficients(orc, Bn, torch_cuda, kind, degree, kernel):
+    torch = torch_cuda
+    cfg = W.tiny_config(kind, degree, batch=3)
+    o, L = _make(orc, Bn, cfg)
+    Bn.landau_set_inner_kernel(L.ctx, kernel)
+    for g in range(o.G):   # bit-exact integer work + same dof convention
+        rp, ci = L.pattern(g)
+        rp2, ci2 = o.pattern(g)
+        assert np.array_equal(rp, rp2) and np.array_equal(ci, ci2)
+        assert np.abs(L.dof_coords(g) - o.dof_coords(g)).max() < 1e-14
+    f = W.make_batch_f(cfg, [o.dof_coords(g) for g in range(o.G)], batch=3)
+    fd = torch.tensor(f, device="cuda")
+    vals = L.jacobian(fd, cfg["dt"]).cpu().numpy()
+    ref = o.jacobian_batch(f, cfg["dt"])
+    assert _block_errors(L, vals, ref, L.v_off).max() < TOL
+    # frozen coefficients D, K at the IPs (IP order is implementation-private: match by coordinates)
+    dk = L.last_coefficients(3)
+    for b in range(3):
+        ref_dk = o.inner(f[b])
+        for s in range(L.S):
+            g = L.sgrid[s]
+            r1, z1, _ = L.ip_table(g)
+            r2, z2, _ = o.ip_table(g)
+            p1, p2 = np.lexsort((r1, z1)), np.lexsort((r2, z2))
+            a, r = dk[s][b].T[p1], ref_dk[s][p2]
+            assert np.linalg.norm(a - r) < 1e-12 * np.linalg.norm(r)
+    rhs = L.apply(fd).cpu().numpy()
+    ref_rhs = o.apply_batch(f)
+    assert _block_errors(L, rhs, ref_rhs, L.f_off).max() < TOL
+    # conservation on the GPU result too
+    for b in range(3):
+        mom, scale = np.zeros(3), np.zeros(3)
+        for s, sp in enumerate(cfg["species"]):
+            rz = o.dof_coords(sp["grid"])
+            blk = rhs[b, L.f_off[s]:L.f_off[s + 1]]
+            assert abs(blk.sum()) < 1e-12 * np.abs(blk).sum()
+            for k, psi in enumerate([rz[:, 1], rz[:, 0] ** 2 + rz[:, 1] ** 2]):
+                mom[k] += sp["mass"] * np.dot(psi, blk)
+                scale[k] += sp["mass"] * np.dot(np.abs(psi), np.abs(blk))
+        assert abs(mom[0]) < 1e-12 * scale[0] and abs(mom[1]) < 1e-12 * scale[1]
+    L.close()
+
+
+def test_general_nu_matrix_path(orc, Bn, torch_cuda):
+    """A nu matrix that is not rank one takes the per-species-column path."""
+    torch = torch_cuda
+    cfg = W.tiny_config("uniform", 2, batch=2)
+    cfg["species"] = cfg["species"] + [dict(mass=9.0, charge=1.0, grid=1)]
+    cfg["alpha"] = [1.0] * 3
+    nu = np.array([[1.0, 4.0, 1.5], [4.0, 16.0, 3.0], [1.5, 3.0, 1.0]])
+    o, L = _make(orc, Bn, cfg, nu=nu)
+    f = W.make_batch_f(cfg, [o.dof_coords(g) for g in range(o.G)], batch=2)
+    fd = torch.tensor(f, device="cuda")
+    for kernel in (1, 2):
+        Bn.landau_set_inner_kernel(L.ctx, kernel)
+        vals = L.jacobian(fd, 0.3).cpu().numpy()
+        assert _block_errors(L, vals, o.jacobian_batch(f, 0.3), L.v_off).max() < TOL
+        rhs = L.apply(fd).cpu().numpy()
+        assert _block_errors(L, rhs, o.apply_batch(f), L.f_off).max() < TOL
+    L.close()
+
+
+def test_edge_cases_and_errors(orc, Bn, torch_cuda):
+    torch = torch_cuda
+    cfg = W.tiny_config("quadtree", 2, two_species=False, batch=1)
+    o, L = _make(orc, Bn, cfg)
+    f = W.make_batch_f(cfg, [o.dof_coords(0)], batch=1)
+    fd = torch.tensor(f, device="cuda")
+    # batch == 0 is a no-op
+    out = torch.full((1, L.csr_stride), 7.0, dtype=torch.float64, device="cuda")
+    Bn.landau_jacobian(L.ctx, fd, 0, 1.0, out)
+    assert torch.all(out == 7.0)
+    # dt = +inf gives -J;  M/dt - J - (-J) = M/dt
+    a = L.jacobian(fd, 0.25).cpu().numpy()[0]
+    b = L.jacobian(fd, float("inf")).cpu().numpy()[0]
+    assert np.abs((a - b) - o.mass(0) / 0.25).max() < 1e-13 * np.abs(a).max()
+    assert np.linalg.norm(b - o.jacobian(f[0], float("inf"))) < TOL * np.linalg.norm(b)
+    # invalid arguments are reported, not executed
+    with pytest.raises(Bn.LandauError):
+        Bn.landau_jacobian(L.ctx, fd, 1, 0.0, out)
+    with pytest.raises(Bn.LandauError):
+        Bn.landau_jacobian(L.ctx, fd, -1, 1.0, out)
+    with pytest.raises(Bn.LandauError):
+        Bn.landau_create(cfg["grids"], cfg["species"], 5)
+    with pytest.raises(Bn.LandauError):
+        Bn.landau_create(cfg["grids"], [dict(mass=1.0, charge=-1.0, grid=3)], 2)
+    # host-buffer entry points agree with the device ones, bit for bit
+    hv = np.zeros((1, L.csr_stride))
+    Bn.landau_jacobian_host(L.ctx, f, 1, 0.25, hv)
+    assert np.array_equal(hv[0], a)
+    hr = np.zeros((1, L.f_stride))
+    Bn.landau_apply_host(L.ctx, f, 1, hr)
+    assert np.array_equal(hr, L.apply(fd).cpu().numpy())
+    # batch chunking does not change results
+    cfg3 = W.tiny_config("uniform", 2, batch=5)
+    o3, L3 = _make(orc, Bn, cfg3)
+    f3 = torch.tensor(W.make_batch_f(cfg3, [o3.dof_coords(g) for g in range(o3.G)], batch=5), device="cuda")
+    full = L3.jacobian(f3, 1.0).cpu().numpy()
+    Bn.landau_set_batch_chunk(L3.ctx, 2)
+    assert np.array_equal(L3.jacobian(f3, 1.0).cpu().numpy(), full)
+    L.close()
+    L3.close()
+
+
+# ------------------------------------------------------------------------------------------------ BASELINE configs
+def _sample_entries(B, seed):
+    """first, last and ceil(log2 B) seeded entries (BASELINE.md CPU-baseline plan)."""
+    rng = np.random.default_rng(seed)
+    extra = rng.choice(B, size=min(B, max(1, math.ceil(math.log2(max(B, 2))))), replace=False)
+    return sorted(set([0, B - 1] + [int(x) for x in extra]))
+
+
+def _config_parity(orc, Bn, torch, cfg, B, entries, kernel=0, check_apply=True):
+    o, L = _make(orc, Bn, cfg)
+    Bn.landau_set_inner_kernel(L.ctx, kernel)
+    coords = [L.dof_coords(g) for g in range(L.G)]
+    for g in range(L.G):
+        assert np.abs(coords[g] - o.dof_coords(g)).max() < 1e-14 * cfg["grids"][g]["r_max"]
+    f = W.make_batch_f(cfg, coords, batch=B)
+    fd = torch.tensor(f, device="cuda")
+    vals = L.jacobian(fd, cfg["dt"])
+    sub = vals[entries].cpu().numpy()
+    ref = np.stack([o.jacobian(f[b], cfg["dt"]) for b in entries])
+    errs = _block_errors(L, sub, ref, L.v_off)
+    assert errs.max() < TOL, errs.max()
+    # property that holds at any size: column sums of every J block vanish (1^T J = 0, conservation of density)
+    J = L.jacobian(fd, float("inf"))
+    for s in range(L.S):
+        g = L.sgrid[s]
+        _, ci = L.pattern(g)
+        cid = torch.tensor(ci.astype(np.int64), device="cuda")
+        blk = J[:, L.v_off[s]:L.v_off[s + 1]]
+        colsum = torch.zeros((B, int(L.n_dof[g])), dtype=torch.float64, device="cuda").index_add_(1, cid, blk)
+        colabs = torch.zeros((B, int(L.n_dof[g])), dtype=torch.float64, device="cuda").index_add_(1, cid, blk.abs())
+        assert float(colsum.abs().max() / colabs.max()) < 1e-12
+    if check_apply:
+        rhs = L.apply(fd)[entries].cpu().numpy()
+        ref_rhs = np.stack([o.apply(f[b]) for b in entries])
+        assert _block_errors(L, rhs, ref_rhs, L.f_off).max() < TOL
+    L.close()
+    return errs.max()
+
+
+def test_config1_full(orc, Bn, torch_cuda):
+    _config_parity(orc, Bn, torch_cuda, W.config(1), 1, [0])
+    _config_parity(orc, Bn, torch_cuda, W.config(1), 1, [0], kernel=2)
+
+
+def test_config2_batch64(orc, Bn, torch_cuda):
+    _config_parity(orc, Bn, torch_cuda, W.config(2), 64, _sample_entries(64, 2))
+
+
+@pytest.mark.parametrize("B", [1, 16, 64])
+def test_config3_ten_species(orc, Bn, torch_cuda, B):
+    _config_parity(orc, Bn, torch_cuda, W.config(3), B, _sample_entries(B, 3)[:4], check_apply=(B == 16))
+
+
+def test_config4_quadtree_bimaxwellian(orc, Bn, torch_cuda):
+    _config_parity(orc, Bn, torch_cuda, W.config(4), 256, _sample_entries(256, 4)[:5])
+
+
+def test_config5_bench_launch_configuration(orc, Bn, torch_cuda):
+    """Full size of the bench workload (B = 1024, default chunking), sampled entries against the oracle."""
+    _config_parity(orc, Bn, torch_cuda, W.config(5), 1024, [0, 517, 1023], check_apply=False)
