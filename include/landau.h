@@ -147,16 +147,21 @@ int landau_tensor_eval(const double* r_dev, const double* z_dev, const double* r
 int landau_ellip_eval(const double* m_dev, const double* mp_dev, int n, double* out_dev, void* cuda_stream);
 
 /* FP64 pipe probes used by bench.py for the roofline denominator: run `iters` rounds of register-resident
- * DFMA (kind 0) or DMMA m8n8k4 (kind 1) on every SM; *tflops receives the achieved FP64 TFLOP/s
+ * DFMA (kind 0), DMMA m8n8k4 (kind 1) or both interleaved (kind 2) on every SM; *tflops receives the achieved FP64 TFLOP/s
  * (CUDA-event timed on `cuda_stream`, synchronises it). */
 int landau_fp64_probe(int kind, int iters, double* tflops, void* cuda_stream);
+
+/* 1 if the collision-frequency matrix was detected as rank one (nu_ab = a_a b_b: one summed source column per
+ * batch entry), 0 if the general per-species-column path is used; negative on error. */
+int landau_is_separable(const landau_ctx* ctx);
 
 /* Number of kernels the library launched on behalf of this context since creation (bench's gpu_launches). */
 long long landau_launch_count(const landau_ctx* ctx);
 
-/* Per-stage device time of the LAST jacobian/apply call in milliseconds (CUDA events recorded on the call's
- * stream; synchronises it): ms[0] field evaluation, ms[1] inner integral, ms[2] coefficient combination,
- * ms[3] element matrices + assembly (or apply).  Recording is enabled with landau_set_timing(ctx, 1). */
+/* Per-stage device time of the LAST jacobian/apply call in milliseconds, summed over its passes: ms[0] field
+ * evaluation, ms[1] inner integral, ms[2] coefficient combination, ms[3] element matrices + assembly (or apply).
+ * Recording is enabled with landau_set_timing(ctx, 1): the compute calls then only RECORD CUDA events on their
+ * stream (no synchronisation is added to them); landau_last_stage_ms waits for the last event and reads them. */
 int landau_set_timing(landau_ctx* ctx, int enabled);
 int landau_last_stage_ms(landau_ctx* ctx, float* ms4);
 

@@ -20,7 +20,7 @@ STATUS = {0: "LANDAU_OK", -1: "LANDAU_INVALID_ARG", -2: "LANDAU_UNSUPPORTED", -3
 SYMBOLS = ["landau_create", "landau_destroy", "landau_sizes", "landau_dof_coords", "landau_ip_table",
            "landau_csr_pattern", "landau_csr_pattern_host", "landau_jacobian", "landau_apply", "landau_jacobian_host",
            "landau_apply_host", "landau_last_coefficients", "landau_tensor_eval", "landau_ellip_eval",
-           "landau_fp64_probe", "landau_launch_count", "landau_set_timing", "landau_last_stage_ms",
+           "landau_fp64_probe", "landau_launch_count", "landau_is_separable", "landau_set_timing", "landau_last_stage_ms",
            "landau_set_inner_kernel", "landau_set_batch_chunk", "landau_last_error"]
 
 
@@ -66,6 +66,11 @@ def _check(rc, ctx=None):
     if rc != LANDAU_OK:
         msg = load().landau_last_error(ctx)
         raise LandauError("%s: %s" % (STATUS.get(rc, rc), msg.decode() if msg else ""))
+
+
+def landau_last_error(ctx=None):
+    msg = load().landau_last_error(ctx)
+    return msg.decode() if msg else ""
 
 
 def _np(a):
@@ -193,6 +198,13 @@ def landau_fp64_probe(kind, iters=20000, stream=None):
 
 def landau_launch_count(ctx):
     return int(load().landau_launch_count(ctx))
+
+
+def landau_is_separable(ctx):
+    rc = load().landau_is_separable(ctx)
+    if rc < 0:
+        _check(rc, ctx)
+    return bool(rc)
 
 
 def landau_set_timing(ctx, enabled):

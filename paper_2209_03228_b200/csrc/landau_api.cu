@@ -34,6 +34,7 @@ struct landau_ctx {
   std::vector<landau_species_desc> species;
   std::vector<double> nu;
   bool separable = false;
+  bool separable_host = false;  // same decision, also known to host-only contexts
   std::vector<long long> f_off, v_off, dk_off;  // per species offsets inside one batch entry
   long long f_stride = 0, v_stride = 0, dk_stride = 0, fl_stride = 0;
   std::vector<long long> fl_off;
@@ -60,7 +61,8 @@ struct landau_ctx {
   int last_batch = 0;
   cudaStream_t last_stream = nullptr;
   bool timing = false;
-  cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  std::vector<cudaEvent_t> ev;  // 5 per pass of the last call (pool grows on demand, resolved lazily)
+  int ev_used = 0;
   float stage_ms[4] = {0, 0, 0, 0};
   long long launches = 0;
   std::string err;
@@ -110,6 +112,17 @@ int grow(landau_ctx* ctx, double** p, size_t* cap, size_t need, bool zero) {
 }
 
 int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+// stage timing: events are only recorded here (no synchronisation); landau_last_stage_ms resolves them
+void mark(landau_ctx* ctx, cudaStream_t st) {
+  if (!ctx->timing) return;
+  if (ctx->ev_used == (int)ctx->ev.size()) {
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    ctx->ev.push_back(e);
+  }
+  cudaEventRecord(ctx->ev[ctx->ev_used++], st);
+}
 
 // is nu = a_a * b_b (rank one)?  fills a, b.
 bool rank_one(const std::vector<double>& nu, int S, std::vector<double>* a, std::vector<double>* b) {
@@ -329,7 +342,7 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
   if (int rc = grow(ctx, &ctx->Gp, &ctx->Gp_cap, (size_t)split_stride * nsplit, false)) return rc;
   if (int rc = grow(ctx, &ctx->DK, &ctx->DK_cap, (size_t)ctx->dk_stride * nbc, false)) return rc;
 
-  if (ctx->timing) cudaEventRecord(ctx->ev[0], st);
+  mark(ctx, st);
   // K1
   for (int g = 0; g < G; ++g) {
     const int q = ctx->mix_group[g];
@@ -344,7 +357,7 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
                                           ctx->F + gr.f_off, gr.nj_pad, joff, 0);
     ++ctx->launches;
   }
-  if (ctx->timing) cudaEventRecord(ctx->ev[1], st);
+  mark(ctx, st);
   // K2
   for (size_t q = 0; q < ctx->groups.size(); ++q) {
     const Group& gr = ctx->groups[q];
@@ -370,7 +383,7 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
     }
     ++ctx->launches;
   }
-  if (ctx->timing) cudaEventRecord(ctx->ev[2], st);
+  mark(ctx, st);
   // K2b
   for (int s = 0; s < S; ++s) {
     CombineTable ct = ctx->comb[s];
@@ -387,21 +400,12 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
                                       ctx->DK, ctx->dk_stride, ctx->dk_off[s]);
     ++ctx->launches;
   }
-  if (ctx->timing) cudaEventRecord(ctx->ev[3], st);
+  mark(ctx, st);
   CUDA_TRY(ctx, cudaGetLastError());
   return LANDAU_OK;
 }
 
-void accumulate_timing(landau_ctx* ctx, cudaStream_t st) {
-  if (!ctx->timing) return;
-  cudaEventRecord(ctx->ev[4], st);
-  cudaEventSynchronize(ctx->ev[4]);
-  for (int k = 0; k < 4; ++k) {
-    float ms = 0;
-    cudaEventElapsedTime(&ms, ctx->ev[k], ctx->ev[k + 1]);
-    ctx->stage_ms[k] += ms;
-  }
-}
+void accumulate_timing(landau_ctx* ctx, cudaStream_t st) { mark(ctx, st); }
 
 int check_call(landau_ctx* ctx, const void* in, int batch, const void* out) {
   if (!ctx) return LANDAU_INVALID_ARG;
@@ -469,6 +473,10 @@ int landau_create(const landau_grid_desc* grids, int n_grids, const landau_speci
   } catch (const std::bad_alloc&) {
     return bail(LANDAU_OUT_OF_MEMORY, "host allocation failed");
   }
+  {
+    std::vector<double> sa, sb;
+    ctx->separable_host = rank_one(ctx->nu, ctx->S, &sa, &sb);
+  }
   ctx->device = cuda_device;
   if (cuda_device < 0) {  // host-only context: geometry queries work, compute entry points refuse
     *out = ctx;
@@ -481,7 +489,6 @@ int landau_create(const landau_grid_desc* grids, int n_grids, const landau_speci
     std::string m = ctx->err;
     return bail(rc, m);
   }
-  for (int k = 0; k < 5; ++k) cudaEventCreate(&ctx->ev[k]);
   *out = ctx;
   return LANDAU_OK;
 }
@@ -495,8 +502,7 @@ void landau_destroy(landau_ctx* ctx) {
   for (void* p : ctx->allocs) cudaFree(p);
   for (double* p : {ctx->F, ctx->Gp, ctx->DK, ctx->FL, ctx->stage_in, ctx->stage_out})
     if (p) cudaFree(p);
-  for (int k = 0; k < 5; ++k)
-    if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
+  for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
   delete ctx;
 }
 
@@ -554,7 +560,7 @@ int landau_jacobian(landau_ctx* ctx, const double* batch_f_dev, int batch, doubl
   if (!(dt > 0)) return fail(ctx, LANDAU_INVALID_ARG, "dt must be > 0 (use +inf for the unshifted -J)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const double inv_dt = std::isinf(dt) ? 0.0 : 1.0 / dt;
-  for (int k = 0; k < 4; ++k) ctx->stage_ms[k] = 0;
+  ctx->ev_used = 0;
   for (int b0 = 0; b0 < batch; b0 += ctx->chunk) {
     const int nbc = std::min(ctx->chunk, batch - b0);
     if (int rc = run_coefficients(ctx, batch_f_dev, b0, nbc, st)) return rc;
@@ -581,7 +587,7 @@ int landau_jacobian(landau_ctx* ctx, const double* batch_f_dev, int batch, doubl
 int landau_apply(landau_ctx* ctx, const double* batch_f_dev, int batch, double* out_rhs_dev, void* cuda_stream) {
   if (int rc = check_call(ctx, batch_f_dev, batch, out_rhs_dev)) return rc;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  for (int k = 0; k < 4; ++k) ctx->stage_ms[k] = 0;
+  ctx->ev_used = 0;
   for (int b0 = 0; b0 < batch; b0 += ctx->chunk) {
     const int nbc = std::min(ctx->chunk, batch - b0);
     if (int rc = run_coefficients(ctx, batch_f_dev, b0, nbc, st)) return rc;
@@ -664,7 +670,7 @@ int landau_ellip_eval(const double* m_dev, const double* mp_dev, int n, double* 
 }
 
 int landau_fp64_probe(int kind, int iters, double* tflops, void* cuda_stream) {
-  if (!tflops || iters < 1 || (kind != 0 && kind != 1)) return LANDAU_INVALID_ARG;
+  if (!tflops || iters < 1 || (kind < 0 || kind > 2)) return LANDAU_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int dev = 0, nsm = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return LANDAU_CUDA_ERROR;
@@ -680,8 +686,10 @@ int landau_fp64_probe(int kind, int iters, double* tflops, void* cuda_stream) {
     cudaEventRecord(e0, st);
     if (kind == 0)
       k_probe_dfma<<<nblk, 256, 0, st>>>(out, iters, 1.0000001, 1e-9);
-    else
+    else if (kind == 1)
       k_probe_dmma<<<nblk, 256, 0, st>>>(out, iters, 1.0000001, 1e-9);
+    else
+      k_probe_mixed<<<nblk, 256, 0, st>>>(out, iters, 1.0000001, 1e-9);
     cudaEventRecord(e1, st);
     if (cudaEventSynchronize(e1) != cudaSuccess) {
       cudaFree(out);
@@ -690,7 +698,8 @@ int landau_fp64_probe(int kind, int iters, double* tflops, void* cuda_stream) {
     float ms = 0;
     cudaEventElapsedTime(&ms, e0, e1);
     // dfma: 64 FMA per thread per iteration; dmma: 32 mma per warp per iteration, 512 flop each = 16 flop/thread
-    const double flop = (kind == 0 ? 2.0 * 64 : 16.0 * 32) * (double)iters * nblk * 256;
+    // mixed: per iteration 16 mma per warp (16 flop/thread each) + 32 FMA per thread
+    const double flop = (kind == 0 ? 2.0 * 64 : kind == 1 ? 16.0 * 32 : 16.0 * 16 + 2.0 * 32) * (double)iters * nblk * 256;
     best = std::max(best, flop / (ms * 1e-3) * 1e-12);
   }
   cudaEventDestroy(e0);
@@ -702,6 +711,11 @@ int landau_fp64_probe(int kind, int iters, double* tflops, void* cuda_stream) {
 
 long long landau_launch_count(const landau_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+int landau_is_separable(const landau_ctx* ctx) {
+  if (!ctx) return LANDAU_INVALID_ARG;
+  return ctx->separable_host ? 1 : 0;
+}
+
 int landau_set_timing(landau_ctx* ctx, int enabled) {
   if (!ctx) return LANDAU_INVALID_ARG;
   ctx->timing = enabled != 0;
@@ -710,6 +724,16 @@ int landau_set_timing(landau_ctx* ctx, int enabled) {
 
 int landau_last_stage_ms(landau_ctx* ctx, float* ms4) {
   if (!ctx || !ms4) return LANDAU_INVALID_ARG;
+  for (int k = 0; k < 4; ++k) ctx->stage_ms[k] = 0;
+  if (ctx->ev_used >= 5) {
+    CUDA_TRY(ctx, cudaEventSynchronize(ctx->ev[ctx->ev_used - 1]));
+    for (int p = 0; p + 5 <= ctx->ev_used; p += 5)
+      for (int k = 0; k < 4; ++k) {
+        float ms = 0;
+        cudaEventElapsedTime(&ms, ctx->ev[p + k], ctx->ev[p + k + 1]);
+        ctx->stage_ms[k] += ms;
+      }
+  }
   for (int k = 0; k < 4; ++k) ms4[k] = ctx->stage_ms[k];
   return LANDAU_OK;
 }

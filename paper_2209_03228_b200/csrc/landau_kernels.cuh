@@ -549,4 +549,32 @@ __global__ void __launch_bounds__(256) k_probe_dmma(double* out, int iters, doub
   out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+// mixed: 8 independent DFMA chains + 4 DMMA accumulator pairs per round -- are the two pipes concurrent?
+__global__ void __launch_bounds__(256) k_probe_mixed(double* out, int iters, double a, double b) {
+  double acc[8], c0[4], c1[4];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) acc[k] = threadIdx.x * 1e-3 + k;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    c0[k] = threadIdx.x * 1e-3 + k;
+    c1[k] = k;
+  }
+  for (int it = 0; it < iters; ++it)
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        dmma884(c0[k], c1[k], a, b);
+        acc[2 * k] = fma(acc[2 * k], a, b);
+        acc[2 * k + 1] = fma(acc[2 * k + 1], a, b);
+      }
+    }
+  double s = 0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) s += acc[k];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) s += c0[k] + c1[k];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 }  // namespace landau

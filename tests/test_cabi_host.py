@@ -1,0 +1,103 @@
+"""CPU-only checks of the product's boundary (no compute calls): the C-ABI library loads, exports every symbol
+include/landau.h declares, and its host set-up (meshes, dof numbering, constraints, CSR pattern, IP tables) -- written
+independently of the oracle -- agrees with the oracle's, bit for bit on the integer work."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2209_03228_b200 import binding as Bn
+from paper_2209_03228_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2209_03228_b200 import build
+    build.build()
+    return Bn.load()
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "landau.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(landau_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(lib):
+    names = _declared_symbols()
+    assert "landau_create" in names and "landau_jacobian" in names and "landau_apply" in names
+    for n in names:
+        assert hasattr(lib, n), "liblandau_b200.so does not export %s" % n
+    assert sorted(Bn.SYMBOLS) == names, "binding.SYMBOLS out of date with include/landau.h"
+    for n in names:  # the binding carries the same names
+        assert hasattr(Bn, n), "binding lacks %s" % n
+
+
+def test_no_cpu_fallback_compute_refuses_without_device(lib):
+    cfg = W.tiny_config("uniform", 2, batch=1)
+    ctx = Bn.landau_create(cfg["grids"], cfg["species"], cfg["degree"], cuda_device=-1)  # host-only context
+    f = np.zeros(8)
+    import ctypes as C
+    rc = lib.landau_jacobian_host(ctx, f.ctypes.data_as(C.c_void_p), C.c_int(1), C.c_double(1.0),
+                                  f.ctypes.data_as(C.c_void_p), None)
+    assert rc == -4  # LANDAU_CUDA_ERROR: there is no CPU path behind the ABI
+    assert b"no CPU fallback" in lib.landau_last_error(ctx)
+    rc = lib.landau_apply_host(ctx, f.ctypes.data_as(C.c_void_p), C.c_int(1), f.ctypes.data_as(C.c_void_p), None)
+    assert rc == -4
+    Bn.landau_destroy(ctx)
+
+
+def test_create_rejects_bad_arguments(lib):
+    cfg = W.tiny_config("uniform", 2, batch=1)
+    with pytest.raises(Bn.LandauError):
+        Bn.landau_create(cfg["grids"], cfg["species"], 5, cuda_device=-1)               # degree unsupported
+    with pytest.raises(Bn.LandauError):
+        Bn.landau_create(cfg["grids"], cfg["species"], dict(degree=2, n_gauss_1d=5), cuda_device=-1)
+    with pytest.raises(Bn.LandauError):
+        Bn.landau_create(cfg["grids"], [dict(mass=1.0, charge=-1.0, grid=7)], 2, cuda_device=-1)
+    with pytest.raises(Bn.LandauError):
+        Bn.landau_create(cfg["grids"], [dict(mass=-1.0, charge=-1.0, grid=0)], 2, cuda_device=-1)
+
+
+@pytest.mark.parametrize("cfg", [W.tiny_config("uniform", 2), W.tiny_config("quadtree", 3), W.config(1), W.config(4),
+                                 W.config(3)], ids=lambda c: c["name"])
+def test_host_setup_matches_oracle(orc, lib, cfg):
+    """dof numbering, CSR pattern (bit-exact), IP tables (as sets) of the product's own host set-up vs the oracle's."""
+    o = orc.Oracle(cfg["grids"], cfg["species"], cfg["degree"])
+    L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"], device=-1)
+    assert list(L.n_dof) == list(o.n_dof) and list(L.nnz) == list(o.nnz)
+    assert list(L.n_ip) == list(o.n_ip) and list(L.n_cells) == list(o.n_cells)
+    assert L.f_stride == o.f_stride and L.csr_stride == o.v_stride
+    for g in range(L.G):
+        rp, ci = L.pattern(g)
+        rp2, ci2 = o.pattern(g)
+        assert np.array_equal(rp, rp2) and np.array_equal(ci, ci2)
+        scale = cfg["grids"][g]["r_max"]
+        assert np.abs(L.dof_coords(g) - o.dof_coords(g)).max() <= 1e-14 * scale
+        r1, z1, w1 = L.ip_table(g)
+        r2, z2, w2 = o.ip_table(g)
+        p1, p2 = np.lexsort((r1, z1)), np.lexsort((r2, z2))
+        assert np.abs(r1[p1] - r2[p2]).max() <= 1e-14 * scale and np.abs(z1[p1] - z2[p2]).max() <= 1e-14 * scale
+        assert np.abs(w1[p1] - w2[p2]).max() <= 1e-13 * np.abs(w2).max()
+    L.close()
+
+
+def test_paper_mesh_statistics_from_the_product_side(lib):
+    """4x2 base + one level at the origin: 14 Q3 cells, 142 equations, 22.2 nnz/row."""
+    grids = [dict(kind=1, r_max=5.0, z_min=-5.0, z_max=5.0, nr=2, nz=4, levels=1)]
+    L = Bn.Landau(grids, [dict(mass=1.0, charge=-1.0, grid=0)], 3, device=-1)
+    assert int(L.n_cells[0]) == 14 and int(L.n_dof[0]) == 142 and int(L.nnz[0]) == 3154
+    L.close()
+
+
+def test_separable_detection(lib):
+    cfg = W.tiny_config("uniform", 2)
+    ctx = Bn.landau_create(cfg["grids"], cfg["species"], 2, cuda_device=-1)
+    assert Bn.landau_is_separable(ctx)
+    Bn.landau_destroy(ctx)
+    ctx = Bn.landau_create(cfg["grids"], cfg["species"], 2, nu=np.array([[1.0, 2.0], [2.0, 1.0]]), cuda_device=-1)
+    assert not Bn.landau_is_separable(ctx)
+    Bn.landau_destroy(ctx)
