@@ -165,7 +165,8 @@ long long landau_launch_count(const landau_ctx* ctx);
 int landau_set_timing(landau_ctx* ctx, int enabled);
 int landau_last_stage_ms(landau_ctx* ctx, float* ms4);
 
-/* Choose the inner-integral kernel: 0 auto, 1 plain DFMA kernel, 2 DMMA (tensor-pipe FP64) kernel. */
+/* Choose the inner-integral kernel: 0 auto (by column count), 1 plain DFMA kernel, 2 DMMA kernel with per-warp
+ * tensor generation, 3 DMMA GEMM kernel with the tensor tile shared by the CTA (TMA-staged source tiles). */
 int landau_set_inner_kernel(landau_ctx* ctx, int which);
 
 /* Batch entries pushed through the stages per pass (default 256); scratch is sized for one pass, so that the

@@ -1,0 +1,187 @@
+// k2_gemm.cuh -- K2 for many source columns: the inner integral as an FP64
+// contraction whose A operand (the Landau tensor) is generated ONCE per CTA per (i,j) tile and shared by all warps.
+//
+//   G_k[i, col] = sum_j U_k(i,j) * F_l[j, col]      seven (k,l) products, DMMA m8n8k4 (SASS: DMMA)
+//
+// CTA tile: TI field points x TC columns, K loop over source tiles of 16 points.
+//   * B operand (source fields F): global layout is already the shared-memory image of a stage
+//     ([col tile][j tile][comp 3][col in tile][16 j, 4-blocks XOR-swizzled by col&3]), so one elected thread moves a
+//     stage with ONE bulk async copy (TMA, cp.async.bulk -> SASS UBLKCP) that signals an mbarrier; NST stages.
+//   * A operand (tensor): all threads evaluate the TI x 16 tensor tile of the NEXT step while the DMMAs of the
+//     current step are in flight (other warps), and store it in DMMA A-fragment order ([comp][i block][k4][lane]),
+//     double buffered; every warp then reads its fragments with conflict-free contiguous 256-byte loads.
+//   * one __syncthreads per 16 source points.
+// Warp tile: (8 WI_T) field points x (8 WC_T) columns; WGI x WGC warps.
+#pragma once
+#include <cstdint>
+
+namespace landau {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+
+template <int WI_T, int WC_T, int WGI, int WGC, int NST>
+struct K2G {
+  static constexpr int NTHREADS = 32 * WGI * WGC;
+  static constexpr int TI = 8 * WI_T * WGI;
+  static constexpr int TC = 8 * WC_T * WGC;
+  static constexpr int STAGE_DOUBLES = 3 * TC * K2G_TJ;
+  static constexpr int A_DOUBLES = 5 * (TI / 8) * 4 * 32;  // one buffer
+  static constexpr int PAIRS_PER_THREAD = TI * K2G_TJ / NTHREADS;
+  static constexpr size_t SMEM_BYTES = (size_t)(NST * STAGE_DOUBLES + 2 * A_DOUBLES) * 8 + NST * 8;
+  static_assert(TI * K2G_TJ % NTHREADS == 0, "tensor tile must divide over the threads");
+};
+
+template <int WI_T, int WC_T, int WGI, int WGC, int NST>
+__global__ void __launch_bounds__(32 * WGI * WGC, 1)
+k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, int n_i, int j0, int njt,
+              const double* __restrict__ F, int ncols, double* __restrict__ G, long long g_split_stride, int gcol0) {
+  using C = K2G<WI_T, WC_T, WGI, WGC, NST>;
+  extern __shared__ __align__(128) double smem_g[];
+  double* smem = smem_g;
+  double* sB = smem;                                  // [NST][3][TC][16]
+  double* sA = smem + NST * C::STAGE_DOUBLES;         // [2][5][TI/8][4][32]
+  uint64_t* full = reinterpret_cast<uint64_t*>(sA + 2 * C::A_DOUBLES);
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wi = warp / WGC, wc = warp - wi * WGC;
+  const int gq = lane >> 2, tq = lane & 3;
+  const int i0 = blockIdx.x * C::TI;
+  const int per = (njt + gridDim.z - 1) / gridDim.z;
+  const int t0 = blockIdx.z * per, t1 = min(t0 + per, njt);
+  const int nt = t1 - t0;
+  const double* Fct = F + (long long)blockIdx.y * njt * C::STAGE_DOUBLES;
+
+  if (tid == 0) {
+    for (int s = 0; s < NST; ++s) mbar_init(&full[s], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid == 0) {
+    for (int s = 0; s < NST && s < nt; ++s) {
+      mbar_expect_tx(&full[s], C::STAGE_DOUBLES * 8);
+      bulk_g2s(sB + s * C::STAGE_DOUBLES, Fct + (long long)(t0 + s) * C::STAGE_DOUBLES, C::STAGE_DOUBLES * 8, &full[s]);
+    }
+  }
+
+  // field points of this thread's tensor evaluations (pair p = tid + NTHREADS*u: i = p/16, j = p%16)
+  double ri[C::PAIRS_PER_THREAD], zi[C::PAIRS_PER_THREAD];
+  int a_slot[C::PAIRS_PER_THREAD];
+  const int jl = tid & 15;
+#pragma unroll
+  for (int u = 0; u < C::PAIRS_PER_THREAD; ++u) {
+    const int il = (tid + C::NTHREADS * u) >> 4;
+    const int ig = min(i0 + il, n_i - 1);
+    ri[u] = ip_r[ig];
+    zi[u] = ip_z[ig];
+    a_slot[u] = (((il >> 3) * 4 + (jl >> 2)) << 5) + ((il & 7) << 2) + (jl & 3);
+  }
+  auto eval_tile = [&](int t, int buf) {
+    const double rj = ip_r[j0 + t * K2G_TJ + jl], zj = ip_z[j0 + t * K2G_TJ + jl];
+    double* dst = sA + buf * C::A_DOUBLES;
+#pragma unroll
+    for (int u = 0; u < C::PAIRS_PER_THREAD; ++u) {
+      const Tensor5 U = landau_tensor_2v(ri[u], zi[u], rj, zj);
+      constexpr int CS = (C::TI / 8) * 4 * 32;
+      dst[a_slot[u]] = U.UDrr;
+      dst[CS + a_slot[u]] = U.UDrz;
+      dst[2 * CS + a_slot[u]] = U.UDzz;
+      dst[3 * CS + a_slot[u]] = U.UKrr;
+      dst[4 * CS + a_slot[u]] = U.UKzr;
+    }
+  };
+
+  double acc[WI_T][WC_T][5][2];
+#pragma unroll
+  for (int x = 0; x < WI_T; ++x)
+#pragma unroll
+    for (int n = 0; n < WC_T; ++n)
+#pragma unroll
+      for (int k = 0; k < 5; ++k) acc[x][n][k][0] = acc[x][n][k][1] = 0.0;
+
+  if (nt > 0) eval_tile(t0, 0);
+  __syncthreads();
+
+  for (int tt = 0; tt < nt; ++tt) {
+    const int stage = tt % NST;
+    if (tt + 1 < nt) eval_tile(t0 + tt + 1, (tt + 1) & 1);
+    mbar_wait(&full[stage], (tt / NST) & 1);
+    const double* A = sA + (tt & 1) * C::A_DOUBLES;
+    const double* Bst = sB + stage * C::STAGE_DOUBLES;
+    constexpr int CS = (C::TI / 8) * 4 * 32;
+#pragma unroll
+    for (int ks = 0; ks < 4; ++ks) {
+      double a[WI_T][5];
+#pragma unroll
+      for (int x = 0; x < WI_T; ++x)
+#pragma unroll
+        for (int k = 0; k < 5; ++k) a[x][k] = A[k * CS + (((wi * WI_T + x) * 4 + ks) << 5) + lane];
+#pragma unroll
+      for (int n = 0; n < WC_T; ++n) {
+        const int cl = (wc * WC_T + n) * 8 + gq;
+        const double* bp = Bst + cl * 16 + (((ks ^ (gq & 3)) << 2) | tq);
+        const double wf = bp[0], wfr = bp[C::TC * 16], wfz = bp[2 * C::TC * 16];
+#pragma unroll
+        for (int x = 0; x < WI_T; ++x) {
+          dmma884(acc[x][n][0][0], acc[x][n][0][1], a[x][0], wf);
+          dmma884(acc[x][n][1][0], acc[x][n][1][1], a[x][1], wf);
+          dmma884(acc[x][n][2][0], acc[x][n][2][1], a[x][2], wf);
+          dmma884(acc[x][n][3][0], acc[x][n][3][1], a[x][3], wfr);
+          dmma884(acc[x][n][4][0], acc[x][n][4][1], a[x][4], wfr);
+          dmma884(acc[x][n][3][0], acc[x][n][3][1], a[x][1], wfz);
+          dmma884(acc[x][n][4][0], acc[x][n][4][1], a[x][2], wfz);
+        }
+      }
+    }
+    __syncthreads();
+    if (tid == 0 && tt + NST < nt) {
+      mbar_expect_tx(&full[stage], C::STAGE_DOUBLES * 8);
+      bulk_g2s(sB + stage * C::STAGE_DOUBLES, Fct + (long long)(t0 + tt + NST) * C::STAGE_DOUBLES, C::STAGE_DOUBLES * 8,
+               &full[stage]);
+    }
+  }
+
+  // C fragment: row gq (field point), columns 2 tq, 2 tq + 1
+#pragma unroll
+  for (int x = 0; x < WI_T; ++x) {
+    const int i = i0 + (wi * WI_T + x) * 8 + gq;
+    if (i < n_i) {
+#pragma unroll
+      for (int n = 0; n < WC_T; ++n)
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int col = blockIdx.y * C::TC + (wc * WC_T + n) * 8 + 2 * tq + h;
+          if (col < ncols) {
+            double* dst = G + blockIdx.z * g_split_stride + ((long long)(gcol0 + col) * 5) * n_i + i;
+#pragma unroll
+            for (int k = 0; k < 5; ++k) dst[(long long)k * n_i] = acc[x][n][k][h];
+          }
+        }
+    }
+  }
+}
+
+}  // namespace landau

@@ -56,6 +56,7 @@ struct landau_ctx {
   size_t F_cap = 0, Gp_cap = 0, DK_cap = 0, FL_cap = 0;
   double *stage_in = nullptr, *stage_out = nullptr;
   size_t stage_in_cap = 0, stage_out_cap = 0;
+  long long f_layout_key = -1;
   int chunk = 256;       // batch entries processed per pass through the stages
   int inner_kernel = 0;  // 0 auto, 1 dfma, 2 dmma
   int last_batch = 0;
@@ -308,17 +309,46 @@ int launch_dmma(landau_ctx* ctx, const Group& gr, int ncols, int ncols_pad, int 
   return LANDAU_OK;
 }
 
+// many-column kernel (k2_gemm.cuh): TI=32 x TC=128 CTA tile, 8 warps of 16 x 32
+using K2Big = K2G<2, 4, 2, 4, 3>;
+constexpr int K2BIG_TC = K2Big::TC;
+
+int launch_gemm(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nsplit, long long split_stride,
+                cudaStream_t st) {
+  static bool configured = false;
+  if (!configured) {
+    CUDA_TRY(ctx, cudaFuncSetAttribute(k2_inner_gemm<2, 4, 2, 4, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)K2Big::SMEM_BYTES));
+    configured = true;
+  }
+  dim3 grid((ctx->n_i_pad + K2Big::TI - 1) / K2Big::TI, (ncols + K2Big::TC - 1) / K2Big::TC, nsplit);
+  k2_inner_gemm<2, 4, 2, 4, 3><<<grid, K2Big::NTHREADS, K2Big::SMEM_BYTES, st>>>(
+      ctx->d_ip_r, ctx->d_ip_z, ctx->n_i_pad, gr.j0, gr.nj_pad / K2G_TJ, ctx->F + gr.f_off, ncols, ctx->Gp, split_stride,
+      gcol0);
+  return LANDAU_OK;
+}
+
+// which inner-integral kernel a group of `ncols` columns takes: 1 DFMA, 2 DMMA (per-warp tensor), 3 GEMM (shared tensor)
+int pick_kernel(const landau_ctx* ctx, int ncols) {
+  if (ctx->inner_kernel) return ctx->inner_kernel;
+  return ncols > 64 ? 3 : (ncols >= 8 ? 2 : 1);
+}
+
 // stages a1..a2b for batch entries [b0, b0+nbc): leaves D,K in ctx->DK
 int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cudaStream_t st) {
   const int G = ctx->G, S = ctx->S;
   // column bookkeeping for this chunk
   long long foff = 0;
   int total_cols = 0;
-  std::vector<int> gcol0(ctx->groups.size()), ncols(ctx->groups.size()), ncols_pad(ctx->groups.size());
+  std::vector<int> gcol0(ctx->groups.size()), ncols(ctx->groups.size()), ncols_pad(ctx->groups.size()),
+      kern(ctx->groups.size());
+  long long layout_key = 0;
   for (size_t q = 0; q < ctx->groups.size(); ++q) {
     Group& gr = ctx->groups[q];
     ncols[q] = nbc * gr.ncb;
-    ncols_pad[q] = round_up(ncols[q], 64);
+    kern[q] = pick_kernel(ctx, ncols[q]);
+    ncols_pad[q] = round_up(ncols[q], kern[q] == 3 ? K2BIG_TC : 64);
+    layout_key = layout_key * 1000003 + ncols_pad[q] * 4 + kern[q];
     gr.f_off = foff;
     foff += (long long)ncols_pad[q] * 3 * gr.nj_pad;
     gcol0[q] = total_cols;
@@ -327,8 +357,9 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
   // j-split so that small problems still fill the machine
   int max_blocks = 1 << 30, nsplit = 1;
   for (size_t q = 0; q < ctx->groups.size(); ++q) {
-    const bool dmma = ctx->inner_kernel == 2 || (ctx->inner_kernel == 0 && ncols[q] >= 8);
-    const int blocks = dmma ? ((ctx->n_i_pad + 63) / 64) * ((ncols[q] + 63) / 64) : ((ctx->n_i_pad + 127) / 128) * ((ncols[q] + 3) / 4);
+    const int blocks = kern[q] == 3   ? ((ctx->n_i_pad + K2Big::TI - 1) / K2Big::TI) * (ncols_pad[q] / K2BIG_TC)
+                       : kern[q] == 2 ? ((ctx->n_i_pad + 63) / 64) * ((ncols[q] + 63) / 64)
+                                      : ((ctx->n_i_pad + 127) / 128) * ((ncols[q] + 3) / 4);
     if (blocks < max_blocks) max_blocks = blocks;
   }
   if (max_blocks < 296) {
@@ -338,7 +369,14 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
     nsplit = std::max(1, std::min(std::min(nsplit, min_tiles), 64));
   }
   const long long split_stride = (long long)total_cols * 5 * ctx->n_i_pad;
-  if (int rc = grow(ctx, &ctx->F, &ctx->F_cap, (size_t)foff, true)) return rc;
+  {
+    const size_t cap0 = ctx->F_cap;
+    if (int rc = grow(ctx, &ctx->F, &ctx->F_cap, (size_t)foff, true)) return rc;
+    // padding columns / padding source points must read as zero: re-zero when the layout changes
+    if (layout_key != ctx->f_layout_key && cap0 == ctx->F_cap)
+      CUDA_TRY(ctx, cudaMemsetAsync(ctx->F, 0, (size_t)foff * sizeof(double), st));
+    ctx->f_layout_key = layout_key;
+  }
   if (int rc = grow(ctx, &ctx->Gp, &ctx->Gp_cap, (size_t)split_stride * nsplit, false)) return rc;
   if (int rc = grow(ctx, &ctx->DK, &ctx->DK_cap, (size_t)ctx->dk_stride * nbc, false)) return rc;
 
@@ -351,18 +389,19 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
     const int joff = ctx->ip_off[g] - gr.j0;
     if (ctx->nb == 9)
       k1_fields<9><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->mix[g], batch_f, ctx->f_stride, b0, nbc,
-                                         ctx->F + gr.f_off, gr.nj_pad, joff, 0);
+                                         ctx->F + gr.f_off, gr.nj_pad, joff, 0, kern[q] == 3 ? K2BIG_TC : 0);
     else
       k1_fields<16><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->mix[g], batch_f, ctx->f_stride, b0, nbc,
-                                          ctx->F + gr.f_off, gr.nj_pad, joff, 0);
+                                          ctx->F + gr.f_off, gr.nj_pad, joff, 0, kern[q] == 3 ? K2BIG_TC : 0);
     ++ctx->launches;
   }
   mark(ctx, st);
   // K2
   for (size_t q = 0; q < ctx->groups.size(); ++q) {
     const Group& gr = ctx->groups[q];
-    const bool dmma = ctx->inner_kernel == 2 || (ctx->inner_kernel == 0 && ncols[q] >= 8);
-    if (dmma) {
+    if (kern[q] == 3) {
+      if (int rc = launch_gemm(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
+    } else if (kern[q] == 2) {
       int rc;
       if (ncols[q] > 32)
         rc = launch_dmma<8>(ctx, gr, ncols[q], ncols_pad[q], gcol0[q], nsplit, split_stride, st);
@@ -739,7 +778,7 @@ int landau_last_stage_ms(landau_ctx* ctx, float* ms4) {
 }
 
 int landau_set_inner_kernel(landau_ctx* ctx, int which) {
-  if (!ctx || which < 0 || which > 2) return LANDAU_INVALID_ARG;
+  if (!ctx || which < 0 || which > 3) return LANDAU_INVALID_ARG;
   ctx->inner_kernel = which;
   return LANDAU_OK;
 }

@@ -162,10 +162,20 @@ struct MixTable {  // per grid
   double wD[16], wK[16];
 };
 
+constexpr int K2G_TJ = 16;
+
+// offset (in doubles) of source value (col, comp, j) in the tiled F layout of a group with njt source tiles
+__host__ __device__ __forceinline__ long long k2g_f_offset(int TC, int njt, int col, int comp, int j) {
+  const int ct = col / TC, cl = col - ct * TC;
+  const int jt = j >> 4, jj = j & 15;
+  const int pos = (((jj >> 2) ^ (cl & 3)) << 2) | (jj & 3);
+  return ((((long long)ct * njt + jt) * 3 + comp) * TC + cl) * 16 + pos;
+}
+
 template <int NB>
 __global__ void __launch_bounds__(256)
 k1_fields(DevGrid g, const DevTables* __restrict__ tab, MixTable mix, const double* __restrict__ batch_f, long long f_stride,
-          int b0, int nbatch, double* __restrict__ F, long long nj_pad, int j_off_in_group, int col0) {
+          int b0, int nbatch, double* __restrict__ F, long long nj_pad, int j_off_in_group, int col0, int tiled_tc) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   const int b = blockIdx.y;
   if (j >= g.n_ip || b >= nbatch) return;
@@ -191,10 +201,17 @@ k1_fields(DevGrid g, const DevTables* __restrict__ tab, MixTable mix, const doub
       aKz = fma(mix.wK[e], vy * sz, aKz);
     }
     const long long col = col0 + (long long)b * mix.ncb + c;
-    double* dst = F + col * 3 * nj_pad + j_off_in_group + j;
-    dst[0] = w * aD;
-    dst[nj_pad] = w * aKr;
-    dst[2 * nj_pad] = w * aKz;
+    if (tiled_tc) {  // stage-image layout of k2_inner_gemm
+      const int njt = (int)(nj_pad >> 4), jg = j_off_in_group + j;
+      F[k2g_f_offset(tiled_tc, njt, (int)col, 0, jg)] = w * aD;
+      F[k2g_f_offset(tiled_tc, njt, (int)col, 1, jg)] = w * aKr;
+      F[k2g_f_offset(tiled_tc, njt, (int)col, 2, jg)] = w * aKz;
+    } else {
+      double* dst = F + col * 3 * nj_pad + j_off_in_group + j;
+      dst[0] = w * aD;
+      dst[nj_pad] = w * aKr;
+      dst[2 * nj_pad] = w * aKz;
+    }
   }
 }
 
@@ -374,6 +391,10 @@ k2_inner_dmma(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
       }
   }
 }
+
+}  // namespace landau
+#include "k2_gemm.cuh"
+namespace landau {
 
 // ------------------------------------------------------------------------------------------------------------
 // K2b: species combination (eq. 2.1 prefactors) and sum over j splits.
