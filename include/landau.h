@@ -169,6 +169,16 @@ int landau_last_stage_ms(landau_ctx* ctx, float* ms4);
  * tensor generation, 3 DMMA GEMM kernel with the tensor tile shared by the CTA (TMA-staged source tiles). */
 int landau_set_inner_kernel(landau_ctx* ctx, int which);
 
+/* Choose the element-matrix + assembly kernel: 0 auto (k3_ring: DMMA sum-factorised element matrices kept in a
+ * shared-memory ring, CSR slots gathered from it; used for every grid whose ring fits in shared memory),
+ * 1 force the general slot-gather kernel (k3_assemble: one thread per CSR slot, scalar FP64). */
+int landau_set_assembly_kernel(landau_ctx* ctx, int which);
+
+/* Schedule of the ring assembly kernel for grid g (host query, works on host-only contexts): ring_cells = element
+ * matrices kept in shared memory (0: the ring does not fit, the slot-gather kernel is used for this grid),
+ * n_steps = panels of 16 cells, n_simple_slots = CSR slots fed by exactly one element-matrix entry with weight 1. */
+int landau_assembly_info(const landau_ctx* ctx, int grid, int* ring_cells, int* n_steps, int* n_simple_slots);
+
 /* Batch entries pushed through the stages per pass (default 256); scratch is sized for one pass, so that the
  * intermediates (source fields, partial sums, D/K) of a pass stay L2-resident.  chunk >= 1. */
 int landau_set_batch_chunk(landau_ctx* ctx, int chunk);

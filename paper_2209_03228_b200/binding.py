@@ -21,7 +21,7 @@ SYMBOLS = ["landau_create", "landau_destroy", "landau_sizes", "landau_dof_coords
            "landau_csr_pattern", "landau_csr_pattern_host", "landau_jacobian", "landau_apply", "landau_jacobian_host",
            "landau_apply_host", "landau_last_coefficients", "landau_tensor_eval", "landau_ellip_eval",
            "landau_fp64_probe", "landau_launch_count", "landau_is_separable", "landau_set_timing", "landau_last_stage_ms",
-           "landau_set_inner_kernel", "landau_set_batch_chunk", "landau_last_error"]
+           "landau_set_inner_kernel", "landau_set_assembly_kernel", "landau_assembly_info", "landau_set_batch_chunk", "landau_last_error"]
 
 
 class LandauError(RuntimeError):
@@ -219,6 +219,16 @@ def landau_last_stage_ms(ctx):
 
 def landau_set_inner_kernel(ctx, which):
     _check(load().landau_set_inner_kernel(ctx, C.c_int(which)), ctx)
+
+
+def landau_set_assembly_kernel(ctx, which):
+    _check(load().landau_set_assembly_kernel(ctx, C.c_int(which)), ctx)
+
+
+def landau_assembly_info(ctx, grid):
+    rc, ns, nsimple = C.c_int(), C.c_int(), C.c_int()
+    _check(load().landau_assembly_info(ctx, C.c_int(grid), C.byref(rc), C.byref(ns), C.byref(nsimple)), ctx)
+    return dict(ring_cells=rc.value, n_steps=ns.value, n_simple_slots=nsimple.value)
 
 
 def landau_set_batch_chunk(ctx, chunk):

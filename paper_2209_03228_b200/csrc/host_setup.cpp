@@ -68,6 +68,31 @@ bool build_tables(int k, HostTables* t, std::string* msg) {
   const int n1 = k + 1;
   std::vector<double> v(n1 * n1), d(n1 * n1);  // [q1][c]
   for (int q = 0; q < n1; ++q) equispaced_lagrange(k, t->gauss_x[q], &v[q * n1], &d[q * n1]);
+  t->lag_v = v;
+  t->lag_d = d;
+  {
+    // 1-D product tables P[x][y][ac][q] = l^(x)_a(q) l^(y)_c(q), ac = a n1 + c  (zero outside the valid range)
+    auto P = [&](int x, int y, int ac, int q) -> double {
+      if (ac >= n1 * n1 || q >= n1) return 0.0;
+      const int a = ac / n1, c = ac % n1;
+      return (x ? d[q * n1 + a] : v[q * n1 + a]) * (y ? d[q * n1 + c] : v[q * n1 + c]);
+    };
+    // table order used by both directions: 0: P00, 1: P11, 2: P10 (derivative on the test function a), 3: P01
+    const int tx[4] = {0, 1, 1, 0}, ty[4] = {0, 1, 0, 1};
+    t->k3_frag.assign(16 * 32, 0.0);
+    for (int lane = 0; lane < 32; ++lane) {
+      const int g = lane >> 2, tq = lane & 3;
+      for (int zt = 0; zt < 4; ++zt)
+        for (int mt = 0; mt < 2; ++mt)  // stage 1: A[m = a2c2][k = q2]
+          t->k3_frag[(zt * 2 + mt) * 32 + lane] = P(tx[zt], ty[zt], g + 8 * mt, tq);
+      for (int nt = 0; nt < 2; ++nt)
+        for (int h = 0; h < 2; ++h)
+          for (int mt = 0; mt < 2; ++mt) {  // stage 2: A[m = a1c1][k -> (rtab = 2 nt + tq/2, q1 = 2 (tq%2) + h)]
+            const int rt = 2 * nt + (tq >> 1), q1 = 2 * (tq & 1) + h;
+            t->k3_frag[(8 + (nt * 2 + h) * 2 + mt) * 32 + lane] = P(tx[rt], ty[rt], g + 8 * mt, q1);
+          }
+    }
+  }
   t->B.assign(t->nq * t->nb, 0.0);
   t->dBxi.assign(t->nq * t->nb, 0.0);
   t->dBeta.assign(t->nq * t->nb, 0.0);
@@ -318,6 +343,48 @@ int build_grid(const landau_grid_desc& d, const HostTables& t, HostGrid* g, std:
       g->as_code[fill[en.slot]] = en.code;
       g->as_w[fill[en.slot]] = en.w;
       ++fill[en.slot];
+    }
+  }
+  // ---- K3 ring schedule --------------------------------------------------------------------------------------------
+  {
+    const int nb2 = nb * nb;
+    int span = 0;
+    std::vector<int> last(g->nnz, 0);
+    for (int n = 0; n < g->nnz; ++n) {
+      int lo = g->n_cells, hi = -1;
+      for (int p = g->as_ptr[n]; p < g->as_ptr[n + 1]; ++p) {
+        const int cell = g->as_code[p] / nb2;
+        lo = std::min(lo, cell);
+        hi = std::max(hi, cell);
+      }
+      last[n] = hi;
+      span = std::max(span, hi - lo);
+    }
+    int rc = (span + K3_PC + K3_PC - 1) / K3_PC * K3_PC;
+    g->k3_nsteps = (g->n_cells + K3_PC - 1) / K3_PC;
+    if ((long long)rc * K3_RS * 8 > K3_RING_MAX_BYTES || (long long)rc * K3_RS > 0xFFFF) rc = 0;
+    g->k3_rc = rc;
+    if (rc) {
+      g->as_roff.resize(g->as_code.size());
+      for (size_t p = 0; p < g->as_code.size(); ++p) {
+        const int code = g->as_code[p], cell = code / nb2, a = (code / nb) % nb, c = code % nb;
+        const int a1 = a % n1, a2 = a / n1, c1 = c % n1, c2 = c / n1;
+        g->as_roff[p] = (cell % rc) * K3_RS + (a2 * n1 + c2) * K3_LD + (a1 * n1 + c1);
+      }
+      std::vector<int> count(g->k3_nsteps + 1, 0);
+      for (int n = 0; n < g->nnz; ++n) ++count[last[n] / K3_PC + 1];
+      g->em_ptr.assign(g->k3_nsteps + 1, 0);
+      for (int s = 0; s < g->k3_nsteps; ++s) g->em_ptr[s + 1] = g->em_ptr[s] + count[s + 1];
+      g->em_n.resize(g->nnz);
+      g->em_off.resize(g->nnz);
+      std::vector<int> fill(g->em_ptr.begin(), g->em_ptr.end() - 1);
+      for (int n = 0; n < g->nnz; ++n) {  // ascending n inside every step
+        const int e = fill[last[n] / K3_PC]++;
+        const int p0 = g->as_ptr[n];
+        const bool simple = g->as_ptr[n + 1] - p0 == 1 && g->as_w[p0] == 1.0;
+        g->em_n[e] = n;
+        g->em_off[e] = simple ? (unsigned short)g->as_roff[p0] : (unsigned short)0xFFFF;
+      }
     }
   }
   {

@@ -10,6 +10,14 @@
 
 namespace landau {
 
+// K3 (element matrices + assembly) schedule constants, shared by host set-up and the kernel:
+// cells are processed in panels of K3_PC cells (cell order); each element matrix occupies K3_RS doubles of a
+// shared-memory ring, entry (a, c) at  (a2 n1 + c2) * K3_LD + (a1 n1 + c1)  (a = a1 + n1 a2, c = c1 + n1 c2).
+constexpr int K3_PC = 16;
+constexpr int K3_LD = 18;
+constexpr int K3_RS = 16 * K3_LD;
+constexpr int K3_RING_MAX_BYTES = 220 * 1024;
+
 struct HostGrid {
   landau_grid_desc desc;
   int k = 0, nb = 0, nq = 0;
@@ -28,6 +36,13 @@ struct HostGrid {
   // as_code = cell*nb*nb + a*nb + c
   std::vector<int> as_ptr, as_code;
   std::vector<double> as_w;
+  // K3 ring schedule: step s computes cells [s K3_PC, (s+1) K3_PC) into ring positions (cell % k3_rc) and then
+  // emits the CSR slots em_n[em_ptr[s] .. em_ptr[s+1]) whose last contributing cell lies in that panel.
+  // em_off: ring offset of the single contribution (weight 1) or 0xFFFF = walk as_ptr/as_roff/as_w.
+  // k3_rc == 0: the ring would not fit in shared memory, the slot-gather kernel is used for this grid.
+  int k3_rc = 0, k3_nsteps = 0;
+  std::vector<int> em_ptr, em_n, as_roff;
+  std::vector<unsigned short> em_off;
   // apply gather: dof i receives sum of ap_w * r_cell[a], ap_code = cell*nb + a
   std::vector<int> ap_ptr, ap_code;
   std::vector<double> ap_w;
@@ -37,6 +52,10 @@ struct HostTables {
   int k = 0, nq1 = 0, nb = 0, nq = 0;
   std::vector<double> gauss_x, gauss_w;  // on [-1,1]
   std::vector<double> B, dBxi, dBeta;    // [q][a]
+  std::vector<double> lag_v, lag_d;      // 1-D Lagrange values / derivatives at the Gauss points, [q1][c]
+  // constant DMMA A-fragments of K3 (see k3_ring.cuh): [16][32 lanes]; 0..7 = z-direction tables (ztab*2 + mt),
+  // 8..15 = r-direction tables ((nt*2 + h)*2 + mt2)
+  std::vector<double> k3_frag;
 };
 
 // Fills tables for degree k (2 or 3).  Returns false with msg on unsupported degree.

@@ -10,6 +10,7 @@
 #include "../../include/landau.h"
 #include "host_setup.hpp"
 #include "landau_kernels.cuh"
+#include "k3_ring.cuh"
 
 using namespace landau;
 
@@ -51,6 +52,13 @@ struct landau_ctx {
   std::vector<int> mix_group;         // group of each grid
   std::vector<int> mix_col_in_group;  // first column (per batch entry) of the grid inside its group
   std::vector<CombineTable> comb;     // per species
+  // K3 ring kernel: device schedule per grid, species list (only species whose grid has a ring schedule)
+  K3Grid* d_k3grid = nullptr;
+  K3Species* d_k3spec = nullptr;
+  const double* d_k3frag = nullptr;
+  int k3_nspec = 0, k3_min_steps = 0;
+  size_t k3_smem = 0;
+  std::vector<char> k3_ring_ok;  // per species
   // scratch (grown on demand)
   double *F = nullptr, *Gp = nullptr, *DK = nullptr, *FL = nullptr;
   size_t F_cap = 0, Gp_cap = 0, DK_cap = 0, FL_cap = 0;
@@ -59,6 +67,7 @@ struct landau_ctx {
   long long f_layout_key = -1;
   int chunk = 256;       // batch entries processed per pass through the stages
   int inner_kernel = 0;  // 0 auto, 1 dfma, 2 dmma
+  int assembly_kernel = 0;  // 0 auto (ring kernel where the grid has a schedule), 1 slot-gather kernel
   int last_batch = 0;
   cudaStream_t last_stream = nullptr;
   bool timing = false;
@@ -208,6 +217,55 @@ int build_device_side(landau_ctx* ctx) {
     rc = rc ? rc : upload(ctx, h.rowptr, &ctx->d_rowptr[g]);
     rc = rc ? rc : upload(ctx, h.colidx, &ctx->d_colidx[g]);
     if (rc) return rc;
+  }
+  // K3 ring schedules
+  {
+    std::vector<K3Grid> kg(G);
+    for (int g = 0; g < G; ++g) {
+      const HostGrid& h = ctx->hg[g];
+      K3Grid& d = kg[g];
+      memset(&d, 0, sizeof(d));
+      d.n_cells = h.n_cells;
+      d.nq = h.nq;
+      d.n1 = h.k + 1;
+      d.rc = h.k3_rc;
+      d.nsteps = h.k3_nsteps;
+      d.cell_sr = ctx->dg[g].cell_sr;
+      d.cell_sz = ctx->dg[g].cell_sz;
+      d.ip_w = ctx->dg[g].ip_w;
+      d.as_ptr = ctx->dg[g].as_ptr;
+      d.as_w = ctx->dg[g].as_w;
+      if (h.k3_rc) {
+        int rc = 0;
+        rc = rc ? rc : upload(ctx, h.em_ptr, &d.em_ptr);
+        rc = rc ? rc : upload(ctx, h.em_n, &d.em_n);
+        rc = rc ? rc : upload(ctx, h.em_off, &d.em_off);
+        rc = rc ? rc : upload(ctx, h.as_roff, &d.as_roff);
+        if (rc) return rc;
+      }
+    }
+    std::vector<K3Species> ks;
+    ctx->k3_ring_ok.assign(S, 0);
+    ctx->k3_smem = 0;
+    ctx->k3_min_steps = 1 << 30;
+    for (int s = 0; s < S; ++s) {
+      const HostGrid& h = ctx->hg[ctx->species[s].grid];
+      if (!h.k3_rc) continue;
+      ctx->k3_ring_ok[s] = 1;
+      ks.push_back(K3Species{ctx->species[s].grid, ctx->dk_off[s], ctx->v_off[s], (long long)h.n_ip});
+      ctx->k3_smem = std::max(ctx->k3_smem, (size_t)h.k3_rc * K3_RS * sizeof(double));
+      ctx->k3_min_steps = std::min(ctx->k3_min_steps, h.k3_nsteps);
+    }
+    ctx->k3_nspec = (int)ks.size();
+    const K3Grid* tg;
+    const K3Species* tsp;
+    if (int rc = upload(ctx, kg, &tg)) return rc;
+    if (int rc = upload(ctx, ks, &tsp)) return rc;
+    if (int rc = upload(ctx, ctx->ht.k3_frag, &ctx->d_k3frag)) return rc;
+    ctx->d_k3grid = const_cast<K3Grid*>(tg);
+    ctx->d_k3spec = const_cast<K3Species*>(tsp);
+    if (ctx->k3_nspec)
+      CUDA_TRY(ctx, cudaFuncSetAttribute(k3_ring, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->k3_smem));
   }
   // source columns: separable nu => one group over all grids, one column per batch entry;
   // general nu => one group per grid, one column per species of the grid.
@@ -603,10 +661,21 @@ int landau_jacobian(landau_ctx* ctx, const double* batch_f_dev, int batch, doubl
   for (int b0 = 0; b0 < batch; b0 += ctx->chunk) {
     const int nbc = std::min(ctx->chunk, batch - b0);
     if (int rc = run_coefficients(ctx, batch_f_dev, b0, nbc, st)) return rc;
+    double* vals = out_csr_vals_dev + (long long)b0 * ctx->v_stride;
+    if (ctx->k3_nspec && ctx->assembly_kernel != 1) {
+      // enough CTAs for ~2 waves of 3 CTAs/SM; cell segments (with a recomputed halo) when the batch is small
+      const int ctas = nbc * ctx->k3_nspec;
+      int nseg = 1;
+      if (ctas < 888) nseg = std::max(1, std::min(ctx->k3_min_steps, (888 + ctas - 1) / ctas));
+      k3_ring<<<ctas * nseg, K3_THREADS, ctx->k3_smem, st>>>(ctx->d_k3grid, ctx->d_k3spec, ctx->k3_nspec, nseg,
+                                                             ctx->d_k3frag, ctx->DK, ctx->dk_stride, inv_dt, vals,
+                                                             ctx->v_stride);
+      ++ctx->launches;
+    }
     for (int s = 0; s < ctx->S; ++s) {
+      if (ctx->k3_ring_ok[s] && ctx->assembly_kernel != 1) continue;
       const int g = ctx->species[s].grid;
       dim3 grid((ctx->hg[g].nnz + 255) / 256, nbc);
-      double* vals = out_csr_vals_dev + (long long)b0 * ctx->v_stride;
       if (ctx->nb == 9)
         k3_assemble<9><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, nbc,
                                              vals, ctx->v_stride, ctx->v_off[s]);
@@ -780,6 +849,25 @@ int landau_last_stage_ms(landau_ctx* ctx, float* ms4) {
 int landau_set_inner_kernel(landau_ctx* ctx, int which) {
   if (!ctx || which < 0 || which > 3) return LANDAU_INVALID_ARG;
   ctx->inner_kernel = which;
+  return LANDAU_OK;
+}
+
+int landau_set_assembly_kernel(landau_ctx* ctx, int which) {
+  if (!ctx || which < 0 || which > 1) return LANDAU_INVALID_ARG;
+  ctx->assembly_kernel = which;
+  return LANDAU_OK;
+}
+
+int landau_assembly_info(const landau_ctx* ctx, int grid, int* ring_cells, int* n_steps, int* n_simple_slots) {
+  if (!ctx || grid < 0 || grid >= ctx->G) return LANDAU_INVALID_ARG;
+  const HostGrid& h = ctx->hg[grid];
+  if (ring_cells) *ring_cells = h.k3_rc;
+  if (n_steps) *n_steps = h.k3_nsteps;
+  if (n_simple_slots) {
+    int n = 0;
+    for (unsigned short o : h.em_off) n += o != 0xFFFF;
+    *n_simple_slots = n;
+  }
   return LANDAU_OK;
 }
 

@@ -101,3 +101,19 @@ def test_separable_detection(lib):
     ctx = Bn.landau_create(cfg["grids"], cfg["species"], 2, nu=np.array([[1.0, 2.0], [2.0, 1.0]]), cuda_device=-1)
     assert not Bn.landau_is_separable(ctx)
     Bn.landau_destroy(ctx)
+
+
+@pytest.mark.parametrize("c", [1, 2, 3, 4, 5])
+def test_ring_assembly_schedule_exists_for_every_baseline_config(lib, c):
+    """Every BASELINE.json grid gets a shared-memory ring schedule for the assembly kernel (no gather fallback), the
+    ring fits one CTA, and most CSR slots are single-contribution slots (K3)."""
+    cfg = W.config(c)
+    ctx = Bn.landau_create(cfg["grids"], cfg["species"], cfg["degree"], cuda_device=-1)
+    sz = Bn.landau_sizes(ctx, len(cfg["grids"]))
+    for g in range(len(cfg["grids"])):
+        info = Bn.landau_assembly_info(ctx, g)
+        assert info["ring_cells"] >= 32 and info["ring_cells"] % 16 == 0
+        assert info["ring_cells"] * 288 * 8 <= 220 * 1024
+        assert info["n_steps"] == (int(sz["n_cells"][g]) + 15) // 16
+        assert 0.7 * sz["nnz"][g] < info["n_simple_slots"] <= sz["nnz"][g]
+    Bn.landau_destroy(ctx)

@@ -108,6 +108,12 @@ def test_tiny_jacobian_apply_and_coefficients(orc, Bn, torch_cuda, kind, degree,
     vals = L.jacobian(fd, cfg["dt"]).cpu().numpy()
     ref = o.jacobian_batch(f, cfg["dt"])
     assert _block_errors(L, vals, ref, L.v_off).max() < TOL
+    # the general slot-gather assembly kernel agrees with the default ring kernel (summation order differs only)
+    Bn.landau_set_assembly_kernel(L.ctx, 1)
+    vals1 = L.jacobian(fd, cfg["dt"]).cpu().numpy()
+    Bn.landau_set_assembly_kernel(L.ctx, 0)
+    assert _block_errors(L, vals1, ref, L.v_off).max() < TOL
+    assert _block_errors(L, vals1, vals, L.v_off).max() < 1e-13
     # frozen coefficients D, K at the IPs (IP order is implementation-private: match by coordinates)
     dk = L.last_coefficients(3)
     for b in range(3):
