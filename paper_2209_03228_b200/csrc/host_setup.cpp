@@ -362,29 +362,56 @@ int build_grid(const landau_grid_desc& d, const HostTables& t, HostGrid* g, std:
     }
     int rc = (span + K3_PC + K3_PC - 1) / K3_PC * K3_PC;
     g->k3_nsteps = (g->n_cells + K3_PC - 1) / K3_PC;
-    if ((long long)rc * K3_RS * 8 > K3_RING_MAX_BYTES || (long long)rc * K3_RS > 0xFFFF) rc = 0;
+    if ((long long)rc * K3_RS * 8 + 64 > K3_RING_MAX_BYTES || (long long)rc * K3_RS + 8 >= (1 << (32 - K3_NBITS))) rc = 0;
     g->k3_rc = rc;
     if (rc) {
+      const int S1 = g->k3_nsteps + 1;
       g->as_roff.resize(g->as_code.size());
       for (size_t p = 0; p < g->as_code.size(); ++p) {
         const int code = g->as_code[p], cell = code / nb2, a = (code / nb) % nb, c = code % nb;
         const int a1 = a % n1, a2 = a / n1, c1 = c % n1, c2 = c / n1;
         g->as_roff[p] = (cell % rc) * K3_RS + (a2 * n1 + c2) * K3_LD + (a1 * n1 + c1);
       }
-      std::vector<int> count(g->k3_nsteps + 1, 0);
-      for (int n = 0; n < g->nnz; ++n) ++count[last[n] / K3_PC + 1];
-      g->em_ptr.assign(g->k3_nsteps + 1, 0);
-      for (int s = 0; s < g->k3_nsteps; ++s) g->em_ptr[s + 1] = g->em_ptr[s] + count[s + 1];
-      g->em_n.resize(g->nnz);
-      g->em_off.resize(g->nnz);
-      std::vector<int> fill(g->em_ptr.begin(), g->em_ptr.end() - 1);
-      for (int n = 0; n < g->nnz; ++n) {  // ascending n inside every step
-        const int e = fill[last[n] / K3_PC]++;
-        const int p0 = g->as_ptr[n];
-        const bool simple = g->as_ptr[n + 1] - p0 == 1 && g->as_w[p0] == 1.0;
-        g->em_n[e] = n;
-        g->em_off[e] = simple ? (unsigned short)g->as_roff[p0] : (unsigned short)0xFFFF;
+      // classify, bucket by step (slots visited in ascending n, so every list is ascending)
+      std::vector<std::vector<int>> l1(g->k3_nsteps), l4(g->k3_nsteps), lg(g->k3_nsteps);
+      for (int n = 0; n < g->nnz; ++n) {
+        const int p0 = g->as_ptr[n], cnt = g->as_ptr[n + 1] - p0;
+        bool unit = cnt <= 4;
+        for (int p = p0; p < p0 + cnt && unit; ++p) unit = g->as_w[p] == 1.0;
+        (unit ? (cnt == 1 ? l1 : l4) : lg)[last[n] / K3_PC].push_back(n);
       }
+      g->em_ptr.assign(3 * S1, 0);
+      g->em_base.assign(g->k3_nsteps, 0);
+      g->em1.clear();
+      g->em4.clear();
+      g->emg.clear();
+      const unsigned zero_off = (unsigned)(rc * K3_RS);
+      for (int st = 0; st < g->k3_nsteps && rc; ++st) {
+        int base = g->nnz;
+        for (const auto* l : {&l1[st], &l4[st], &lg[st]})
+          if (!l->empty()) base = std::min(base, l->front());
+        g->em_base[st] = base;
+        g->em_ptr[st] = (int)g->em1.size();
+        g->em_ptr[S1 + st] = (int)g->em4.size() / 4;
+        g->em_ptr[2 * S1 + st] = (int)g->emg.size();
+        for (int n : l1[st]) {
+          if (n - base >= (1 << K3_NBITS)) rc = 0;
+          g->em1.push_back((unsigned)g->as_roff[g->as_ptr[n]] << K3_NBITS | (unsigned)(n - base));
+        }
+        for (int n : l4[st]) {
+          unsigned off[4] = {zero_off, zero_off, zero_off, zero_off};
+          for (int p = g->as_ptr[n]; p < g->as_ptr[n + 1]; ++p) off[p - g->as_ptr[n]] = (unsigned)g->as_roff[p];
+          g->em4.push_back((unsigned)(n - base));
+          g->em4.push_back(off[0] | off[1] << 16);
+          g->em4.push_back(off[2] | off[3] << 16);
+          g->em4.push_back(0u);
+        }
+        for (int n : lg[st]) g->emg.push_back(n);
+      }
+      g->em_ptr[g->k3_nsteps] = (int)g->em1.size();
+      g->em_ptr[S1 + g->k3_nsteps] = (int)g->em4.size() / 4;
+      g->em_ptr[2 * S1 + g->k3_nsteps] = (int)g->emg.size();
+      g->k3_rc = rc;  // 0 if a packed word overflowed
     }
   }
   {

@@ -17,6 +17,7 @@ constexpr int K3_PC = 16;
 constexpr int K3_LD = 18;
 constexpr int K3_RS = 16 * K3_LD;
 constexpr int K3_RING_MAX_BYTES = 220 * 1024;
+constexpr int K3_NBITS = 17;  // bits of (slot - step base) in a packed single-contribution word
 
 struct HostGrid {
   landau_grid_desc desc;
@@ -37,12 +38,16 @@ struct HostGrid {
   std::vector<int> as_ptr, as_code;
   std::vector<double> as_w;
   // K3 ring schedule: step s computes cells [s K3_PC, (s+1) K3_PC) into ring positions (cell % k3_rc) and then
-  // emits the CSR slots em_n[em_ptr[s] .. em_ptr[s+1]) whose last contributing cell lies in that panel.
-  // em_off: ring offset of the single contribution (weight 1) or 0xFFFF = walk as_ptr/as_roff/as_w.
-  // k3_rc == 0: the ring would not fit in shared memory, the slot-gather kernel is used for this grid.
+  // emits the CSR slots whose last contributing cell lies in that panel, from three lists (each ascending in n):
+  //   em1[em_ptr[s] ..)            one contribution, weight 1:   word = ring offset << K3_NBITS | (n - em_base[s])
+  //   em4[em_ptr[S1 + s] ..)       2..4 contributions, all weight 1: {n - base, off0 | off1 << 16, off2 | off3 << 16, 0}
+  //                                (unused offsets point at the zero pad behind the ring, offset k3_rc * K3_RS)
+  //   emg[em_ptr[2 S1 + s] ..)     anything else (hanging-node weights): n, walks as_ptr / as_roff / as_w
+  // with S1 = k3_nsteps + 1.  k3_rc == 0: no ring schedule (ring too large for shared memory or offsets too wide
+  // for the packed words), the slot-gather kernel is used for this grid.
   int k3_rc = 0, k3_nsteps = 0;
-  std::vector<int> em_ptr, em_n, as_roff;
-  std::vector<unsigned short> em_off;
+  std::vector<int> em_ptr, em_base, emg, as_roff;
+  std::vector<unsigned> em1, em4;
   // apply gather: dof i receives sum of ap_w * r_cell[a], ap_code = cell*nb + a
   std::vector<int> ap_ptr, ap_code;
   std::vector<double> ap_w;

@@ -7,7 +7,10 @@
 // K3_PC; the element matrices of the last `rc` cells live in a shared-memory ring, and after every panel the CSR
 // slots whose last contributing cell lies in that panel are gathered from the ring and written ONCE, in ascending
 // slot order (coalesced streaming stores, no atomics, deterministic).  The schedule (em_*, as_*) is built on the
-// host (host_setup.cpp, "K3 ring schedule").
+// host (host_setup.cpp, "K3 ring schedule"): packed 4-byte words for the ~88 % of slots fed by one element-matrix
+// entry, 16-byte records for shared-node slots (<= 4 unit-weight entries), index lists for hanging-node slots, each
+// list homogeneous so that warps do not diverge.  The quadrature-point data (w, D, K) of the next panel is fetched
+// while the current panel is being emitted.
 //
 // Element matrix = sum-factorised FP64 contraction on the DMMA pipe, one warp per cell.  With the tensor-product
 // basis phi_a = l_a1(xi) l_a2(eta) and the 1-D product tables Pxy[ac][q] = l^(x)_a(q) l^(y)_c(q):
@@ -21,7 +24,7 @@
 //   P10r        | -Wkr        .        .       Wrz
 //   P01r        |   .         .       Wrz       .
 //
-// Both stages are m8n8k4 DMMAs whose A operands are CONSTANT fragments (16 registers per lane, loaded once); the
+// Both stages are m8n8k4 DMMAs whose A operands are CONSTANT fragments (16 doubles per lane, kept in shared memory); the
 // stage-1 C fragments are exactly the stage-2 B fragments (the contraction index is only permuted, and the constant
 // stage-2 A fragments are built with the same permutation), so the chain never leaves registers: 12 + 16 DMMAs per
 // cell instead of ~14k scalar FMAs.  Works for Q2 and Q3 (tables zero-padded to 16 x 4).
@@ -30,11 +33,12 @@
 
 namespace landau {
 
-struct K3Grid {  // device copy of one grid's K3 schedule
+struct K3Grid {  // device copy of one grid's K3 schedule (host_setup.hpp, "K3 ring schedule")
   int n_cells, nq, n1, rc, nsteps;
   const double *cell_sr, *cell_sz, *ip_w;
-  const int *em_ptr, *em_n;
-  const unsigned short* em_off;
+  const int *em_ptr, *em_base, *emg;
+  const unsigned* em1;
+  const uint4* em4;
   const int *as_ptr, *as_roff;
   const double* as_w;
 };
@@ -45,6 +49,10 @@ struct K3Species {
 };
 
 constexpr int K3_THREADS = 256;
+constexpr int K3_CPW = K3_PC / (K3_THREADS / 32);  // cells per warp per step
+
+// dynamic shared memory: ring [rc][K3_RS] | zero pad [8] | constant fragments [16][32]
+__host__ __device__ constexpr size_t k3_smem_bytes(int rc) { return ((size_t)rc * K3_RS + 8 + 16 * 32) * sizeof(double); }
 
 __global__ void __launch_bounds__(K3_THREADS, 3)
 k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, int n_spec, int nseg,
@@ -58,92 +66,129 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
   bid /= nseg;
   const int sidx = bid % n_spec, b = bid / n_spec;
   const K3Species sp = spec[sidx];
-  const K3Grid g = grids[sp.grid];
-  const int s_lo = (int)((long long)seg * g.nsteps / nseg), s_hi = (int)((long long)(seg + 1) * g.nsteps / nseg);
+  const K3Grid* __restrict__ g = grids + sp.grid;
+  const int nsteps = g->nsteps, rc = g->rc, n_cells = g->n_cells, n1 = g->n1, nq = g->nq;
+  const int s_lo = (int)((long long)seg * nsteps / nseg), s_hi = (int)((long long)(seg + 1) * nsteps / nseg);
   if (s_lo >= s_hi) return;
-  const int s_begin = max(0, s_lo - (g.rc / K3_PC - 1));
+  const int s_begin = max(0, s_lo - (rc / K3_PC - 1));
 
-  double az[8], ar[8];
-#pragma unroll
-  for (int x = 0; x < 8; ++x) {
-    az[x] = frag[x * 32 + lane];
-    ar[x] = frag[(8 + x) * 32 + lane];
-  }
+  double* zero_pad = ring + rc * K3_RS;
+  double* sfrag = zero_pad + 8;
+  if (tid < 8) zero_pad[tid] = 0.0;
+  for (int e = tid; e < 16 * 32; e += K3_THREADS) sfrag[e] = frag[e];
+  const double* fr = sfrag + lane;
+
   const int q1 = gq & 3, q2 = tq;
   const bool hi = gq >= 4;
-  const bool valid = q1 < g.n1 && q2 < g.n1;
-  const int qidx = q1 + g.n1 * q2;
-  const double* dk = DK + (long long)b * dk_stride + sp.dk_off;
-  double* out = vals + (long long)b * v_stride + sp.v_off;
+  const bool valid = q1 < n1 && q2 < n1;
+  const int qidx = q1 + n1 * q2;
+  const double* __restrict__ dk = DK + (long long)b * dk_stride + sp.dk_off;
+  const double* __restrict__ ip_w = g->ip_w;
+  const double* __restrict__ cell_sr = g->cell_sr;
+  const double* __restrict__ cell_sz = g->cell_sz;
+  double* __restrict__ out = vals + (long long)b * v_stride + sp.v_off;
+  const int S1 = nsteps + 1;
+
+  // this lane's quadrature-point data of the warp's cells, fetched one step ahead of its use
+  double wv[K3_CPW][6], sc[K3_CPW][2];
+  auto fetch = [&](int s) {
+#pragma unroll
+    for (int u = 0; u < K3_CPW; ++u) {
+      const int cell = s * K3_PC + warp + u * (K3_THREADS / 32);
+      const bool ok = cell < n_cells;
+      const long long ip = (long long)(ok ? cell : 0) * nq + (valid ? qidx : 0);
+      const double m = (ok && valid) ? 1.0 : 0.0;
+      wv[u][0] = m * ip_w[ip];
+#pragma unroll
+      for (int k = 0; k < 5; ++k) wv[u][1 + k] = dk[k * sp.n_ip + ip];
+      sc[u][0] = cell_sr[ok ? cell : 0];
+      sc[u][1] = cell_sz[ok ? cell : 0];
+    }
+  };
+  fetch(s_begin);
+  __syncthreads();
 
   for (int s = s_begin; s < s_hi; ++s) {
-#pragma unroll 1
-    for (int cc = warp; cc < K3_PC; cc += K3_THREADS / 32) {
-      const int cell = s * K3_PC + cc;
-      if (cell >= g.n_cells) break;
-      double w = 0.0, Drr = 0.0, Drz = 0.0, Dzz = 0.0, Kr = 0.0, Kz = 0.0;
-      if (valid) {
-        const long long ip = (long long)cell * g.nq + qidx;
-        w = g.ip_w[ip];
-        Drr = dk[ip];
-        Drz = dk[sp.n_ip + ip];
-        Dzz = dk[2 * sp.n_ip + ip];
-        Kr = dk[3 * sp.n_ip + ip];
-        Kz = dk[4 * sp.n_ip + ip];
-      }
-      const double sr = g.cell_sr[cell], sz = g.cell_sz[cell];
-      const double wr = w * sr, wz = w * sz;
-      const double Wm = w * inv_dt, Wrr = wr * sr * Drr, Wzz = wz * sz * Dzz, Wrz = wr * sz * Drz, Wkr = wr * Kr,
-                   Wkz = wz * Kz;
-      // stage-1 B fragments: B[k = q2][n = (rtab, q1)], rtab = 2 nt + (gq >= 4)
-      const double b00 = hi ? Wrr : Wm, b01 = hi ? 0.0 : Wzz, b02 = hi ? 0.0 : -Wkz;
-      const double b10 = hi ? 0.0 : -Wkr, b12 = hi ? Wrz : 0.0, b13 = hi ? 0.0 : Wrz;
-      double y[2][2][2];
 #pragma unroll
-      for (int mt = 0; mt < 2; ++mt) {
-        y[mt][0][0] = y[mt][0][1] = y[mt][1][0] = y[mt][1][1] = 0.0;
-        dmma884(y[mt][0][0], y[mt][0][1], az[0 * 2 + mt], b00);
-        dmma884(y[mt][1][0], y[mt][1][1], az[0 * 2 + mt], b10);
-        dmma884(y[mt][0][0], y[mt][0][1], az[1 * 2 + mt], b01);
-        dmma884(y[mt][1][0], y[mt][1][1], az[2 * 2 + mt], b12);
-        dmma884(y[mt][0][0], y[mt][0][1], az[2 * 2 + mt], b02);
-        dmma884(y[mt][1][0], y[mt][1][1], az[3 * 2 + mt], b13);
-      }
-      // stage 2: A[m = a1c1][n = a2c2]; k-step (nt, h) takes y[.][nt][h] as its B fragment
-      double o[2][2][2];
+    for (int u = 0; u < K3_CPW; ++u) {
+      const int cell = s * K3_PC + warp + u * (K3_THREADS / 32);
+      if (cell < n_cells) {
+        const double w = wv[u][0], sr = sc[u][0], sz = sc[u][1];
+        const double wr = w * sr, wz = w * sz;
+        const double Wm = w * inv_dt, Wrr = wr * sr * wv[u][1], Wrz = wr * sz * wv[u][2], Wzz = wz * sz * wv[u][3],
+                     Wkr = wr * wv[u][4], Wkz = wz * wv[u][5];
+        // stage-1 B fragments: B[k = q2][n = (rtab, q1)], rtab = 2 nt + (gq >= 4)
+        const double b00 = hi ? Wrr : Wm, b01 = hi ? 0.0 : Wzz, b02 = hi ? 0.0 : -Wkz;
+        const double b10 = hi ? 0.0 : -Wkr, b12 = hi ? Wrz : 0.0, b13 = hi ? 0.0 : Wrz;
+        double y[2][2][2];
 #pragma unroll
-      for (int mt2 = 0; mt2 < 2; ++mt2)
+        for (int mt = 0; mt < 2; ++mt) {
+          y[mt][0][0] = y[mt][0][1] = y[mt][1][0] = y[mt][1][1] = 0.0;
+          dmma884(y[mt][0][0], y[mt][0][1], fr[(0 * 2 + mt) * 32], b00);
+          dmma884(y[mt][1][0], y[mt][1][1], fr[(0 * 2 + mt) * 32], b10);
+          dmma884(y[mt][0][0], y[mt][0][1], fr[(1 * 2 + mt) * 32], b01);
+          dmma884(y[mt][1][0], y[mt][1][1], fr[(2 * 2 + mt) * 32], b12);
+          dmma884(y[mt][0][0], y[mt][0][1], fr[(2 * 2 + mt) * 32], b02);
+          dmma884(y[mt][1][0], y[mt][1][1], fr[(3 * 2 + mt) * 32], b13);
+        }
+        // stage 2: A[m = a1c1][n = a2c2]; k-step ks = (nt, h) takes y[.][nt][h] as its B fragment
+        double o[2][2][2];
 #pragma unroll
-        for (int nt2 = 0; nt2 < 2; ++nt2) o[mt2][nt2][0] = o[mt2][nt2][1] = 0.0;
+        for (int mt2 = 0; mt2 < 2; ++mt2)
 #pragma unroll
-      for (int ks = 0; ks < 4; ++ks)
+          for (int nt2 = 0; nt2 < 2; ++nt2) o[mt2][nt2][0] = o[mt2][nt2][1] = 0.0;
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks)
+#pragma unroll
+          for (int mt2 = 0; mt2 < 2; ++mt2) {
+            const double a = fr[(8 + ks * 2 + mt2) * 32];
+#pragma unroll
+            for (int nt2 = 0; nt2 < 2; ++nt2) dmma884(o[mt2][nt2][0], o[mt2][nt2][1], a, y[nt2][ks >> 1][ks & 1]);
+          }
+        double* dst = ring + (cell % rc) * K3_RS;
 #pragma unroll
         for (int mt2 = 0; mt2 < 2; ++mt2)
 #pragma unroll
           for (int nt2 = 0; nt2 < 2; ++nt2)
-            dmma884(o[mt2][nt2][0], o[mt2][nt2][1], ar[ks * 2 + mt2], y[nt2][ks >> 1][ks & 1]);
-      double* dst = ring + (cell % g.rc) * K3_RS;
 #pragma unroll
-      for (int mt2 = 0; mt2 < 2; ++mt2)
-#pragma unroll
-        for (int nt2 = 0; nt2 < 2; ++nt2)
-#pragma unroll
-          for (int h = 0; h < 2; ++h) dst[(2 * tq + h + 8 * nt2) * K3_LD + gq + 8 * mt2] = o[mt2][nt2][h];
+            for (int h = 0; h < 2; ++h) dst[(2 * tq + h + 8 * nt2) * K3_LD + gq + 8 * mt2] = o[mt2][nt2][h];
+      }
     }
+    if (s + 1 < s_hi) fetch(s + 1);
     __syncthreads();
     if (s >= s_lo) {
-      const int e1 = g.em_ptr[s + 1];
-      for (int e = g.em_ptr[s] + tid; e < e1; e += K3_THREADS) {
-        const int n = g.em_n[e];
-        const unsigned off = g.em_off[e];
-        double v;
-        if (off != 0xFFFFu) {
-          v = ring[off];
-        } else {
-          v = 0.0;
-          for (int p = g.as_ptr[n]; p < g.as_ptr[n + 1]; ++p) v = fma(g.as_w[p], ring[g.as_roff[p]], v);
+      const int base = g->em_base[s];
+      {  // one contribution, weight 1
+        const unsigned* __restrict__ em1 = g->em1;
+        const int e1 = g->em_ptr[s + 1];
+#pragma unroll 4
+        for (int e = g->em_ptr[s] + tid; e < e1; e += K3_THREADS) {
+          const unsigned wd = em1[e];
+          __stcs(out + base + (int)(wd & ((1u << K3_NBITS) - 1)), ring[wd >> K3_NBITS]);
         }
-        __stcs(out + n, v);
+      }
+      {  // 2..4 contributions, weight 1
+        const uint4* __restrict__ em4 = g->em4;
+        const int e1 = g->em_ptr[S1 + s + 1];
+#pragma unroll 2
+        for (int e = g->em_ptr[S1 + s] + tid; e < e1; e += K3_THREADS) {
+          const uint4 d = em4[e];
+          const double v = ((ring[d.y & 0xFFFFu] + ring[d.y >> 16]) + ring[d.z & 0xFFFFu]) + ring[d.z >> 16];
+          __stcs(out + base + (int)d.x, v);
+        }
+      }
+      {  // general: hanging-node weights
+        const int* __restrict__ emg = g->emg;
+        const int* __restrict__ as_ptr = g->as_ptr;
+        const int* __restrict__ as_roff = g->as_roff;
+        const double* __restrict__ as_w = g->as_w;
+        const int e1 = g->em_ptr[2 * S1 + s + 1];
+        for (int e = g->em_ptr[2 * S1 + s] + tid; e < e1; e += K3_THREADS) {
+          const int n = emg[e];
+          double v = 0.0;
+          for (int p = as_ptr[n]; p < as_ptr[n + 1]; ++p) v = fma(as_w[p], ring[as_roff[p]], v);
+          __stcs(out + n, v);
+        }
       }
     }
     __syncthreads();

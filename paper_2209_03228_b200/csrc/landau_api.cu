@@ -237,10 +237,14 @@ int build_device_side(landau_ctx* ctx) {
       d.as_w = ctx->dg[g].as_w;
       if (h.k3_rc) {
         int rc = 0;
+        const unsigned* em4 = nullptr;
         rc = rc ? rc : upload(ctx, h.em_ptr, &d.em_ptr);
-        rc = rc ? rc : upload(ctx, h.em_n, &d.em_n);
-        rc = rc ? rc : upload(ctx, h.em_off, &d.em_off);
+        rc = rc ? rc : upload(ctx, h.em_base, &d.em_base);
+        rc = rc ? rc : upload(ctx, h.emg, &d.emg);
+        rc = rc ? rc : upload(ctx, h.em1, &d.em1);
+        rc = rc ? rc : upload(ctx, h.em4, &em4);
         rc = rc ? rc : upload(ctx, h.as_roff, &d.as_roff);
+        d.em4 = reinterpret_cast<const uint4*>(em4);
         if (rc) return rc;
       }
     }
@@ -253,7 +257,7 @@ int build_device_side(landau_ctx* ctx) {
       if (!h.k3_rc) continue;
       ctx->k3_ring_ok[s] = 1;
       ks.push_back(K3Species{ctx->species[s].grid, ctx->dk_off[s], ctx->v_off[s], (long long)h.n_ip});
-      ctx->k3_smem = std::max(ctx->k3_smem, (size_t)h.k3_rc * K3_RS * sizeof(double));
+      ctx->k3_smem = std::max(ctx->k3_smem, k3_smem_bytes(h.k3_rc));
       ctx->k3_min_steps = std::min(ctx->k3_min_steps, h.k3_nsteps);
     }
     ctx->k3_nspec = (int)ks.size();
@@ -863,11 +867,7 @@ int landau_assembly_info(const landau_ctx* ctx, int grid, int* ring_cells, int* 
   const HostGrid& h = ctx->hg[grid];
   if (ring_cells) *ring_cells = h.k3_rc;
   if (n_steps) *n_steps = h.k3_nsteps;
-  if (n_simple_slots) {
-    int n = 0;
-    for (unsigned short o : h.em_off) n += o != 0xFFFF;
-    *n_simple_slots = n;
-  }
+  if (n_simple_slots) *n_simple_slots = (int)h.em1.size();
   return LANDAU_OK;
 }
 
