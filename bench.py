@@ -49,6 +49,7 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel", type=int, default=0, help="inner-integral kernel: 0 auto, 1 DFMA, 2 DMMA")
+    ap.add_argument("--chunk", type=int, default=0, help="batch entries per pass through the stages (0: library default)")
     return ap.parse_args()
 
 
@@ -188,6 +189,8 @@ def run_ours(args):
     B = args.batch or cfg["batch"]
     L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"], device=local)
     Bn.landau_set_inner_kernel(L.ctx, args.kernel)
+    if args.chunk:
+        Bn.landau_set_batch_chunk(L.ctx, args.chunk)
     coords = [L.dof_coords(g) for g in range(L.G)]
     # weak scaling: rank r owns the global batch entries [r*B, (r+1)*B) -- independent problems, no collective
     entries = sharding.shard_entries(rank, world, B * world, mode="weak")

@@ -179,7 +179,7 @@ int landau_set_assembly_kernel(landau_ctx* ctx, int which);
  * n_steps = panels of 16 cells, n_simple_slots = CSR slots fed by exactly one element-matrix entry with weight 1. */
 int landau_assembly_info(const landau_ctx* ctx, int grid, int* ring_cells, int* n_steps, int* n_simple_slots);
 
-/* Batch entries pushed through the stages per pass (default 256); scratch is sized for one pass, so that the
+/* Batch entries pushed through the stages per pass (default 1024); scratch is sized for one pass, so that the
  * intermediates (source fields, partial sums, D/K) of a pass stay L2-resident.  chunk >= 1. */
 int landau_set_batch_chunk(landau_ctx* ctx, int chunk);
 

@@ -50,6 +50,7 @@ struct K3Species {
 
 constexpr int K3_THREADS = 256;
 constexpr int K3_CPW = K3_PC / (K3_THREADS / 32);  // cells per warp per step
+constexpr int K3_EB = 8;                            // emission: descriptor words per thread per batch
 
 // dynamic shared memory: ring [rc][K3_RS] | zero pad [8] | constant fragments [16][32]
 __host__ __device__ constexpr size_t k3_smem_bytes(int rc) { return ((size_t)rc * K3_RS + 8 + 16 * 32) * sizeof(double); }
@@ -158,23 +159,37 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
     __syncthreads();
     if (s >= s_lo) {
       const int base = g->em_base[s];
-      {  // one contribution, weight 1
+      {  // one contribution, weight 1: K3_EB descriptor words per thread in flight before the first store
         const unsigned* __restrict__ em1 = g->em1;
         const int e1 = g->em_ptr[s + 1];
-#pragma unroll 4
-        for (int e = g->em_ptr[s] + tid; e < e1; e += K3_THREADS) {
-          const unsigned wd = em1[e];
-          __stcs(out + base + (int)(wd & ((1u << K3_NBITS) - 1)), ring[wd >> K3_NBITS]);
+        for (int e0 = g->em_ptr[s] + tid; e0 < e1; e0 += K3_THREADS * K3_EB) {
+          unsigned wd[K3_EB];
+#pragma unroll
+          for (int k = 0; k < K3_EB; ++k) {
+            const int e = e0 + k * K3_THREADS;
+            wd[k] = e < e1 ? __ldg(em1 + e) : 0xFFFFFFFFu;
+          }
+#pragma unroll
+          for (int k = 0; k < K3_EB; ++k)
+            if (wd[k] != 0xFFFFFFFFu) __stcs(out + base + (int)(wd[k] & ((1u << K3_NBITS) - 1)), ring[wd[k] >> K3_NBITS]);
         }
       }
       {  // 2..4 contributions, weight 1
         const uint4* __restrict__ em4 = g->em4;
         const int e1 = g->em_ptr[S1 + s + 1];
-#pragma unroll 2
-        for (int e = g->em_ptr[S1 + s] + tid; e < e1; e += K3_THREADS) {
-          const uint4 d = em4[e];
-          const double v = ((ring[d.y & 0xFFFFu] + ring[d.y >> 16]) + ring[d.z & 0xFFFFu]) + ring[d.z >> 16];
-          __stcs(out + base + (int)d.x, v);
+        for (int e0 = g->em_ptr[S1 + s] + tid; e0 < e1; e0 += K3_THREADS * 2) {
+          uint4 d[2];
+#pragma unroll
+          for (int k = 0; k < 2; ++k) {
+            const int e = e0 + k * K3_THREADS;
+            d[k] = e < e1 ? __ldg(em4 + e) : make_uint4(0xFFFFFFFFu, 0, 0, 0);
+          }
+#pragma unroll
+          for (int k = 0; k < 2; ++k)
+            if (d[k].x != 0xFFFFFFFFu) {
+              const double v = ((ring[d[k].y & 0xFFFFu] + ring[d[k].y >> 16]) + ring[d[k].z & 0xFFFFu]) + ring[d[k].z >> 16];
+              __stcs(out + base + (int)d[k].x, v);
+            }
         }
       }
       {  // general: hanging-node weights

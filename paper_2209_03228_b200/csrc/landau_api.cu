@@ -65,7 +65,7 @@ struct landau_ctx {
   double *stage_in = nullptr, *stage_out = nullptr;
   size_t stage_in_cap = 0, stage_out_cap = 0;
   long long f_layout_key = -1;
-  int chunk = 256;       // batch entries processed per pass through the stages
+  int chunk = 1024;      // batch entries processed per pass through the stages
   int inner_kernel = 0;  // 0 auto, 1 dfma, 2 dmma
   int assembly_kernel = 0;  // 0 auto (ring kernel where the grid has a schedule), 1 slot-gather kernel
   int last_batch = 0;
