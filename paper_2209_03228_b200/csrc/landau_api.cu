@@ -10,6 +10,7 @@
 #include "../../include/landau.h"
 #include "host_setup.hpp"
 #include "landau_kernels.cuh"
+#include "k2_ws.cuh"
 #include "k3_ring.cuh"
 
 using namespace landau;
@@ -390,6 +391,31 @@ int launch_gemm(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nspl
   return LANDAU_OK;
 }
 
+// warp-specialised many-column kernels (k2_ws.cuh): kern 4 = 32 x 128 CTA tile, kern 5 = 16 x 256 CTA tile
+using K2Ws4 = K2W<2, 4, 2, 4, 3, 2>;
+using K2Ws5 = K2W<2, 4, 1, 8, 2, 2>;
+
+template <int WI_T, int WC_T, int WGI, int WGC, int NST, int NA>
+int launch_ws(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nsplit, long long split_stride,
+              cudaStream_t st) {
+  using C = K2W<WI_T, WC_T, WGI, WGC, NST, NA>;
+  static bool configured = false;
+  if (!configured) {
+    CUDA_TRY(ctx, cudaFuncSetAttribute(k2_inner_ws<WI_T, WC_T, WGI, WGC, NST, NA>,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
+    configured = true;
+  }
+  dim3 grid((ctx->n_i_pad + C::TI - 1) / C::TI, (ncols + C::TC - 1) / C::TC, nsplit);
+  k2_inner_ws<WI_T, WC_T, WGI, WGC, NST, NA><<<grid, C::NTHREADS, C::SMEM_BYTES, st>>>(
+      ctx->d_ip_r, ctx->d_ip_z, ctx->n_i_pad, gr.j0, gr.nj_pad / K2G_TJ, ctx->F + gr.f_off, ncols, ctx->Gp, split_stride,
+      gcol0);
+  return LANDAU_OK;
+}
+
+// column-tile width of the tiled F layout a kernel reads (0: plain layout), field points per CTA
+int kern_tc(int kern) { return kern == 3 ? K2BIG_TC : kern == 4 ? K2Ws4::TC : kern == 5 ? K2Ws5::TC : 0; }
+int kern_ti(int kern) { return kern == 3 ? K2Big::TI : kern == 4 ? K2Ws4::TI : kern == 5 ? K2Ws5::TI : 0; }
+
 // which inner-integral kernel a group of `ncols` columns takes: 1 DFMA, 2 DMMA (per-warp tensor), 3 GEMM (shared tensor)
 int pick_kernel(const landau_ctx* ctx, int ncols) {
   if (ctx->inner_kernel) return ctx->inner_kernel;
@@ -409,7 +435,7 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
     Group& gr = ctx->groups[q];
     ncols[q] = nbc * gr.ncb;
     kern[q] = pick_kernel(ctx, ncols[q]);
-    ncols_pad[q] = round_up(ncols[q], kern[q] == 3 ? K2BIG_TC : 64);
+    ncols_pad[q] = round_up(ncols[q], kern[q] >= 3 ? kern_tc(kern[q]) : 64);
     layout_key = layout_key * 1000003 + ncols_pad[q] * 4 + kern[q];
     gr.f_off = foff;
     foff += (long long)ncols_pad[q] * 3 * gr.nj_pad;
@@ -419,7 +445,7 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
   // j-split so that small problems still fill the machine
   int max_blocks = 1 << 30, nsplit = 1;
   for (size_t q = 0; q < ctx->groups.size(); ++q) {
-    const int blocks = kern[q] == 3   ? ((ctx->n_i_pad + K2Big::TI - 1) / K2Big::TI) * (ncols_pad[q] / K2BIG_TC)
+    const int blocks = kern[q] >= 3   ? ((ctx->n_i_pad + kern_ti(kern[q]) - 1) / kern_ti(kern[q])) * (ncols_pad[q] / kern_tc(kern[q]))
                        : kern[q] == 2 ? ((ctx->n_i_pad + 63) / 64) * ((ncols[q] + 63) / 64)
                                       : ((ctx->n_i_pad + 127) / 128) * ((ncols[q] + 3) / 4);
     if (blocks < max_blocks) max_blocks = blocks;
@@ -451,17 +477,21 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
     const int joff = ctx->ip_off[g] - gr.j0;
     if (ctx->nb == 9)
       k1_fields<9><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->mix[g], batch_f, ctx->f_stride, b0, nbc,
-                                         ctx->F + gr.f_off, gr.nj_pad, joff, 0, kern[q] == 3 ? K2BIG_TC : 0);
+                                         ctx->F + gr.f_off, gr.nj_pad, joff, 0, kern_tc(kern[q]));
     else
       k1_fields<16><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->mix[g], batch_f, ctx->f_stride, b0, nbc,
-                                          ctx->F + gr.f_off, gr.nj_pad, joff, 0, kern[q] == 3 ? K2BIG_TC : 0);
+                                          ctx->F + gr.f_off, gr.nj_pad, joff, 0, kern_tc(kern[q]));
     ++ctx->launches;
   }
   mark(ctx, st);
   // K2
   for (size_t q = 0; q < ctx->groups.size(); ++q) {
     const Group& gr = ctx->groups[q];
-    if (kern[q] == 3) {
+    if (kern[q] == 5) {
+      if (int rc = launch_ws<2, 4, 1, 8, 2, 2>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
+    } else if (kern[q] == 4) {
+      if (int rc = launch_ws<2, 4, 2, 4, 3, 2>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
+    } else if (kern[q] == 3) {
       if (int rc = launch_gemm(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
     } else if (kern[q] == 2) {
       int rc;
@@ -851,7 +881,7 @@ int landau_last_stage_ms(landau_ctx* ctx, float* ms4) {
 }
 
 int landau_set_inner_kernel(landau_ctx* ctx, int which) {
-  if (!ctx || which < 0 || which > 3) return LANDAU_INVALID_ARG;
+  if (!ctx || which < 0 || which > 5) return LANDAU_INVALID_ARG;
   ctx->inner_kernel = which;
   return LANDAU_OK;
 }

@@ -17,25 +17,35 @@
 namespace landau {
 
 // ------------------------------------------------------------------------------------------------------------
-// Elliptic pieces.  Coefficients live in constant memory; after unrolling every coefficient is a constant-bank
-// operand of a DFMA (no loads).
+// Elliptic pieces.  Coefficients are compile-time constants: every Horner step is a DFMA with an immediate / uniform-
+// register operand that the assembler rematerialises where needed (no loads, nothing to hoist out of the tile loops
+// and spill -- __constant__ tables were hoisted by the compiler into registers and from there into local memory).
 // ------------------------------------------------------------------------------------------------------------
-__constant__ double c_S_P0[] = LANDAU_ELLIP_S_P0_COEFFS;
-__constant__ double c_S_DC[] = LANDAU_ELLIP_S_DC_COEFFS;
-__constant__ double c_S_Q[] = LANDAU_ELLIP_S_Q_COEFFS;
-__constant__ double c_L_A_E[] = LANDAU_ELLIP_L_A_E_COEFFS;
-__constant__ double c_L_B_E[] = LANDAU_ELLIP_L_B_E_COEFFS;
-__constant__ double c_L_A_DC[] = LANDAU_ELLIP_L_A_DC_COEFFS;
-__constant__ double c_L_B_DC[] = LANDAU_ELLIP_L_B_DC_COEFFS;
-__constant__ double c_L_A_Q[] = LANDAU_ELLIP_L_A_Q_COEFFS;
-__constant__ double c_L_B_Q[] = LANDAU_ELLIP_L_B_Q_COEFFS;
+static constexpr double c_S_P0[] = LANDAU_ELLIP_S_P0_COEFFS;
+static constexpr double c_S_DC[] = LANDAU_ELLIP_S_DC_COEFFS;
+static constexpr double c_S_Q[] = LANDAU_ELLIP_S_Q_COEFFS;
+static constexpr double c_L_A_E[] = LANDAU_ELLIP_L_A_E_COEFFS;
+static constexpr double c_L_B_E[] = LANDAU_ELLIP_L_B_E_COEFFS;
+static constexpr double c_L_A_DC[] = LANDAU_ELLIP_L_A_DC_COEFFS;
+static constexpr double c_L_B_DC[] = LANDAU_ELLIP_L_B_DC_COEFFS;
+static constexpr double c_L_A_Q[] = LANDAU_ELLIP_L_A_Q_COEFFS;
+static constexpr double c_L_B_Q[] = LANDAU_ELLIP_L_B_Q_COEFFS;
 
-template <int DEG>
-__device__ __forceinline__ double horner(const double* __restrict__ c, double t) {
-  double acc = c[DEG];
-#pragma unroll
-  for (int n = DEG - 1; n >= 0; --n) acc = fma(acc, t, c[n]);
-  return acc;
+template <const double* C, int N>
+struct HornerStep {
+  static __device__ __forceinline__ double run(double acc, double t) {
+    constexpr double c = C[N];
+    return HornerStep<C, N - 1>::run(fma(acc, t, c), t);
+  }
+};
+template <const double* C>
+struct HornerStep<C, -1> {
+  static __device__ __forceinline__ double run(double acc, double) { return acc; }
+};
+template <const double* C, int DEG>
+__device__ __forceinline__ double horner(double t) {
+  constexpr double top = C[DEG];
+  return HornerStep<C, DEG - 1>::run(top, t);
 }
 
 // (m' P0, Dc, Q) at parameter m with complement mp = 1 - m given separately (never formed by subtraction).
@@ -44,16 +54,16 @@ __device__ __forceinline__ double horner(const double* __restrict__ c, double t)
 __device__ __forceinline__ void ellip_pieces(double m, double mp, double& P0_or_E, double& Dc, double& Q, bool& p0_is_E) {
   if (mp >= 1.0 - LANDAU_ELLIP_M_SPLIT) {
     const double t = m - 0.5 * LANDAU_ELLIP_M_SPLIT;
-    P0_or_E = horner<LANDAU_ELLIP_S_P0_DEG>(c_S_P0, t);
-    Dc = horner<LANDAU_ELLIP_S_DC_DEG>(c_S_DC, t);
-    Q = horner<LANDAU_ELLIP_S_Q_DEG>(c_S_Q, t);
+    P0_or_E = horner<c_S_P0, LANDAU_ELLIP_S_P0_DEG>(t);
+    Dc = horner<c_S_DC, LANDAU_ELLIP_S_DC_DEG>(t);
+    Q = horner<c_S_Q, LANDAU_ELLIP_S_Q_DEG>(t);
     p0_is_E = false;
   } else {
     const double t = mp - 0.5 * (1.0 - LANDAU_ELLIP_M_SPLIT);
     const double lg = -log(mp);
-    P0_or_E = fma(lg, horner<LANDAU_ELLIP_L_B_E_DEG>(c_L_B_E, t), horner<LANDAU_ELLIP_L_A_E_DEG>(c_L_A_E, t));
-    Dc = fma(lg, horner<LANDAU_ELLIP_L_B_DC_DEG>(c_L_B_DC, t), horner<LANDAU_ELLIP_L_A_DC_DEG>(c_L_A_DC, t));
-    Q = fma(lg, horner<LANDAU_ELLIP_L_B_Q_DEG>(c_L_B_Q, t), horner<LANDAU_ELLIP_L_A_Q_DEG>(c_L_A_Q, t));
+    P0_or_E = fma(lg, horner<c_L_B_E, LANDAU_ELLIP_L_B_E_DEG>(t), horner<c_L_A_E, LANDAU_ELLIP_L_A_E_DEG>(t));
+    Dc = fma(lg, horner<c_L_B_DC, LANDAU_ELLIP_L_B_DC_DEG>(t), horner<c_L_A_DC, LANDAU_ELLIP_L_A_DC_DEG>(t));
+    Q = fma(lg, horner<c_L_B_Q, LANDAU_ELLIP_L_B_Q_DEG>(t), horner<c_L_A_Q, LANDAU_ELLIP_L_A_Q_DEG>(t));
     p0_is_E = true;
   }
 }
