@@ -50,8 +50,12 @@ struct K2G {
   static constexpr int STAGE_DOUBLES = 3 * TC * K2G_TJ;
   static constexpr int A_DOUBLES = 5 * (TI / 8) * 4 * 32;  // one buffer
   static constexpr int PAIRS_PER_THREAD = TI * K2G_TJ / NTHREADS;
-  static constexpr size_t SMEM_BYTES = (size_t)(NST * STAGE_DOUBLES + 2 * A_DOUBLES) * 8 + NST * 8;
+  static constexpr int TAB_DOUBLES = 4 * LANDAU_ELLIP_TAB_BINADES * (LANDAU_ELLIP_TAB_DEG + 1) * 4;
+  static constexpr int XY_DOUBLES = 4 * 2 * K2G_TJ;  // ring of four source-tile coordinate blocks (r[16], z[16])
+  static constexpr size_t SMEM_BYTES =
+      (size_t)(NST * STAGE_DOUBLES + 2 * A_DOUBLES + TAB_DOUBLES + XY_DOUBLES) * 8 + NST * 8;
   static_assert(TI * K2G_TJ % NTHREADS == 0, "tensor tile must divide over the threads");
+  static_assert((NTHREADS / 32) % 4 == 0, "warps must cover whole groups of the four k4 blocks");
 };
 
 template <int WI_T, int WC_T, int WGI, int WGC, int NST>
@@ -63,7 +67,9 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
   double* smem = smem_g;
   double* sB = smem;                                  // [NST][3][TC][16]
   double* sA = smem + NST * C::STAGE_DOUBLES;         // [2][5][TI/8][4][32]
-  uint64_t* full = reinterpret_cast<uint64_t*>(sA + 2 * C::A_DOUBLES);
+  double* sTab = sA + 2 * C::A_DOUBLES;               // elliptic table T (13 KB), copied once
+  double* sXY = sTab + C::TAB_DOUBLES;                // [4][2][16] source-point coordinates, filled by cp.async
+  uint64_t* full = reinterpret_cast<uint64_t*>(sXY + C::XY_DOUBLES);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wi = warp / WGC, wc = warp - wi * WGC;
@@ -74,6 +80,13 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
   const int nt = t1 - t0;
   const double* Fct = F + (long long)blockIdx.y * njt * C::STAGE_DOUBLES;
 
+  for (int e = tid; e < C::TAB_DOUBLES; e += C::NTHREADS) sTab[e] = g_ellip_tab[e];
+  // coordinates of the first two source tiles (later tiles arrive by cp.async two steps ahead of their use)
+  if (tid < 4 * K2G_TJ && (tid >> 5) < nt) {
+    const int tl = tid >> 5, e = tid & 31;
+    const double* src = (e < K2G_TJ ? ip_r : ip_z) + j0 + (t0 + tl) * K2G_TJ + (e & (K2G_TJ - 1));
+    sXY[tl * 2 * K2G_TJ + e] = *src;
+  }
   if (tid == 0) {
     for (int s = 0; s < NST; ++s) mbar_init(&full[s], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -87,30 +100,31 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
     }
   }
 
-  // field points of this thread's tensor evaluations (pair p = tid + NTHREADS*u: i = p/16, j = p%16)
-  double ri[C::PAIRS_PER_THREAD], zi[C::PAIRS_PER_THREAD];
-  int a_slot[C::PAIRS_PER_THREAD];
-  const int jl = tid & 15;
+  // Tensor pairs of this thread: lane (gq, tq) of warp w evaluates (i = 8 iblk + gq, j = 4 k4 + tq) for the fragment
+  // blocks blk = w + NWARPS u = iblk * 4 + k4 -- one warp store per component = 32 consecutive doubles (no conflicts).
+  constexpr int NW = C::NTHREADS / 32, NU = C::PAIRS_PER_THREAD;
+  double ri[NU], zi[NU];
 #pragma unroll
-  for (int u = 0; u < C::PAIRS_PER_THREAD; ++u) {
-    const int il = (tid + C::NTHREADS * u) >> 4;
-    const int ig = min(i0 + il, n_i - 1);
+  for (int u = 0; u < NU; ++u) {
+    const int ig = min(i0 + ((warp + NW * u) >> 2) * 8 + gq, n_i - 1);
     ri[u] = ip_r[ig];
     zi[u] = ip_z[ig];
-    a_slot[u] = (((il >> 3) * 4 + (jl >> 2)) << 5) + ((il & 7) << 2) + (jl & 3);
   }
-  auto eval_tile = [&](int t, int buf) {
-    const double rj = ip_r[j0 + t * K2G_TJ + jl], zj = ip_z[j0 + t * K2G_TJ + jl];
-    double* dst = sA + buf * C::A_DOUBLES;
+  // NW is a multiple of 4, so every block of this thread has the same k4 = warp & 3: one source point per tile
+  const int jl = (warp & 3) * 4 + tq;
+  constexpr int CS = (C::TI / 8) * 4 * 32;
+  PairEval pe[NU];
+  auto store_tile = [&](int buf) {
+    double* dst = sA + buf * C::A_DOUBLES + (warp << 5) + lane;
 #pragma unroll
-    for (int u = 0; u < C::PAIRS_PER_THREAD; ++u) {
-      const Tensor5 U = landau_tensor_2v(ri[u], zi[u], rj, zj);
-      constexpr int CS = (C::TI / 8) * 4 * 32;
-      dst[a_slot[u]] = U.UDrr;
-      dst[CS + a_slot[u]] = U.UDrz;
-      dst[2 * CS + a_slot[u]] = U.UDzz;
-      dst[3 * CS + a_slot[u]] = U.UKrr;
-      dst[4 * CS + a_slot[u]] = U.UKzr;
+    for (int u = 0; u < NU; ++u) {
+      const Tensor5 U = pe[u].finish();
+      double* d = dst + ((NW * u) << 5);
+      d[0] = U.UDrr;
+      d[CS] = U.UDrz;
+      d[2 * CS] = U.UDzz;
+      d[3 * CS] = U.UKrr;
+      d[4 * CS] = U.UKzr;
     }
   };
 
@@ -122,16 +136,36 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
 #pragma unroll
       for (int k = 0; k < 5; ++k) acc[x][n][k][0] = acc[x][n][k][1] = 0.0;
 
-  if (nt > 0) eval_tile(t0, 0);
+  if (nt > 0) {
+#pragma unroll
+    for (int u = 0; u < NU; ++u) {
+      pe[u].geometry(ri[u], zi[u], sXY[jl], sXY[K2G_TJ + jl], sTab);
+      pe[u].template steps<LANDAU_ELLIP_TAB_DEG - 1, 0>();
+    }
+    store_tile(0);
+  }
   __syncthreads();
 
+  // Horner steps of the NEXT tile's tensor, cut in four and placed between the four k-blocks of DMMAs
+  constexpr int D = LANDAU_ELLIP_TAB_DEG, H1 = D - 1 - D / 3, H2 = H1 - D / 3;
   for (int tt = 0; tt < nt; ++tt) {
     const int stage = tt % NST;
-    if (tt + 1 < nt) eval_tile(t0 + tt + 1, (tt + 1) & 1);
+    const bool more = tt + 1 < nt;
     mbar_wait(&full[stage], (tt / NST) & 1);
     const double* A = sA + (tt & 1) * C::A_DOUBLES;
     const double* Bst = sB + stage * C::STAGE_DOUBLES;
-    constexpr int CS = (C::TI / 8) * 4 * 32;
+    if (tt + 2 < nt && tid < K2G_TJ) {  // coordinates of the tile after next: 16 x 16 bytes, landed by the end of the step
+      const int e = tid * 2;        // doubles 0..15 = r, 16..31 = z
+      const double* src = (e < K2G_TJ ? ip_r : ip_z) + j0 + (t0 + tt + 2) * K2G_TJ + (e & (K2G_TJ - 1));
+      cp_async16(sXY + ((tt + 2) & 3) * 2 * K2G_TJ + e, src);
+    }
+    cp_async_commit();
+    if (more) {
+      const double* xy = sXY + ((tt + 1) & 3) * 2 * K2G_TJ;
+      const double rj = xy[jl], zj = xy[K2G_TJ + jl];
+#pragma unroll
+      for (int u = 0; u < NU; ++u) pe[u].geometry(ri[u], zi[u], rj, zj, sTab);
+    }
 #pragma unroll
     for (int ks = 0; ks < 4; ++ks) {
       double a[WI_T][5];
@@ -155,7 +189,17 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
           dmma884(acc[x][n][4][0], acc[x][n][4][1], a[x][2], wfz);
         }
       }
+      if (more) {
+#pragma unroll
+        for (int u = 0; u < NU; ++u) {
+          if (ks == 0) pe[u].template steps<D - 1, H1 + 1>();
+          if (ks == 1) pe[u].template steps<H1, H2 + 1>();
+          if (ks == 2) pe[u].template steps<H2, 0>();
+        }
+        if (ks == 3) store_tile((tt + 1) & 1);
+      }
     }
+    cp_async_wait<0>();
     __syncthreads();
     if (tid == 0 && tt + NST < nt) {
       mbar_expect_tx(&full[stage], C::STAGE_DOUBLES * 8);

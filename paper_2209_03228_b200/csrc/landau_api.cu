@@ -376,19 +376,29 @@ int launch_dmma(landau_ctx* ctx, const Group& gr, int ncols, int ncols_pad, int 
 using K2Big = K2G<2, 4, 2, 4, 3>;
 constexpr int K2BIG_TC = K2Big::TC;
 
-int launch_gemm(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nsplit, long long split_stride,
-                cudaStream_t st) {
+// wide variant: 16 x 256 CTA tile (one tensor pair per thread per source tile), 2 B stages
+using K2Wide = K2G<2, 4, 1, 8, 2>;
+
+template <int WI_T, int WC_T, int WGI, int WGC, int NST>
+int launch_gemm_t(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nsplit, long long split_stride,
+                  cudaStream_t st) {
+  using C = K2G<WI_T, WC_T, WGI, WGC, NST>;
   static bool configured = false;
   if (!configured) {
-    CUDA_TRY(ctx, cudaFuncSetAttribute(k2_inner_gemm<2, 4, 2, 4, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)K2Big::SMEM_BYTES));
+    CUDA_TRY(ctx, cudaFuncSetAttribute(k2_inner_gemm<WI_T, WC_T, WGI, WGC, NST>,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
     configured = true;
   }
-  dim3 grid((ctx->n_i_pad + K2Big::TI - 1) / K2Big::TI, (ncols + K2Big::TC - 1) / K2Big::TC, nsplit);
-  k2_inner_gemm<2, 4, 2, 4, 3><<<grid, K2Big::NTHREADS, K2Big::SMEM_BYTES, st>>>(
+  dim3 grid((ctx->n_i_pad + C::TI - 1) / C::TI, (ncols + C::TC - 1) / C::TC, nsplit);
+  k2_inner_gemm<WI_T, WC_T, WGI, WGC, NST><<<grid, C::NTHREADS, C::SMEM_BYTES, st>>>(
       ctx->d_ip_r, ctx->d_ip_z, ctx->n_i_pad, gr.j0, gr.nj_pad / K2G_TJ, ctx->F + gr.f_off, ncols, ctx->Gp, split_stride,
       gcol0);
   return LANDAU_OK;
+}
+
+int launch_gemm(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nsplit, long long split_stride,
+                cudaStream_t st) {
+  return launch_gemm_t<2, 4, 2, 4, 3>(ctx, gr, ncols, gcol0, nsplit, split_stride, st);
 }
 
 // warp-specialised many-column kernels (k2_ws.cuh): kern 4 = 32 x 128 CTA tile, kern 5 = 16 x 256 CTA tile
@@ -413,13 +423,17 @@ int launch_ws(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nsplit
 }
 
 // column-tile width of the tiled F layout a kernel reads (0: plain layout), field points per CTA
-int kern_tc(int kern) { return kern == 3 ? K2BIG_TC : kern == 4 ? K2Ws4::TC : kern == 5 ? K2Ws5::TC : 0; }
-int kern_ti(int kern) { return kern == 3 ? K2Big::TI : kern == 4 ? K2Ws4::TI : kern == 5 ? K2Ws5::TI : 0; }
+int kern_tc(int kern) {
+  return kern == 3 ? K2BIG_TC : kern == 4 ? K2Ws4::TC : kern == 5 ? K2Ws5::TC : kern == 6 ? K2Wide::TC : 0;
+}
+int kern_ti(int kern) {
+  return kern == 3 ? K2Big::TI : kern == 4 ? K2Ws4::TI : kern == 5 ? K2Ws5::TI : kern == 6 ? K2Wide::TI : 0;
+}
 
 // which inner-integral kernel a group of `ncols` columns takes: 1 DFMA, 2 DMMA (per-warp tensor), 3 GEMM (shared tensor)
 int pick_kernel(const landau_ctx* ctx, int ncols) {
   if (ctx->inner_kernel) return ctx->inner_kernel;
-  return ncols > 64 ? 3 : (ncols >= 8 ? 2 : 1);
+  return ncols > 128 ? 6 : ncols > 64 ? 3 : (ncols >= 8 ? 2 : 1);
 }
 
 // stages a1..a2b for batch entries [b0, b0+nbc): leaves D,K in ctx->DK
@@ -487,7 +501,9 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
   // K2
   for (size_t q = 0; q < ctx->groups.size(); ++q) {
     const Group& gr = ctx->groups[q];
-    if (kern[q] == 5) {
+    if (kern[q] == 6) {
+      if (int rc = launch_gemm_t<2, 4, 1, 8, 2>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
+    } else if (kern[q] == 5) {
       if (int rc = launch_ws<2, 4, 1, 8, 2, 2>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
     } else if (kern[q] == 4) {
       if (int rc = launch_ws<2, 4, 2, 4, 3, 2>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
@@ -881,7 +897,7 @@ int landau_last_stage_ms(landau_ctx* ctx, float* ms4) {
 }
 
 int landau_set_inner_kernel(landau_ctx* ctx, int which) {
-  if (!ctx || which < 0 || which > 5) return LANDAU_INVALID_ARG;
+  if (!ctx || which < 0 || which > 6) return LANDAU_INVALID_ARG;
   ctx->inner_kernel = which;
   return LANDAU_OK;
 }

@@ -21,9 +21,6 @@ namespace landau {
 // register operand that the assembler rematerialises where needed (no loads, nothing to hoist out of the tile loops
 // and spill -- __constant__ tables were hoisted by the compiler into registers and from there into local memory).
 // ------------------------------------------------------------------------------------------------------------
-static constexpr double c_S_P0[] = LANDAU_ELLIP_S_P0_COEFFS;
-static constexpr double c_S_DC[] = LANDAU_ELLIP_S_DC_COEFFS;
-static constexpr double c_S_Q[] = LANDAU_ELLIP_S_Q_COEFFS;
 static constexpr double c_L_A_E[] = LANDAU_ELLIP_L_A_E_COEFFS;
 static constexpr double c_L_B_E[] = LANDAU_ELLIP_L_B_E_COEFFS;
 static constexpr double c_L_A_DC[] = LANDAU_ELLIP_L_A_DC_COEFFS;
@@ -48,23 +45,64 @@ __device__ __forceinline__ double horner(double t) {
   return HornerStep<C, DEG - 1>::run(top, t);
 }
 
-// (m' P0, Dc, Q) at parameter m with complement mp = 1 - m given separately (never formed by subtraction).
-//   m' P0 = E,  Dc = (K-E)/m,  Q = ((2-m)K - 2E)/m^2   -- see gen_ellip_coeffs.py.
-// Returns P0 itself in the small-m branch (no pole there) and E in the log branch; `p0_is_E` tells which.
-__device__ __forceinline__ void ellip_pieces(double m, double mp, double& P0_or_E, double& Dc, double& Q, bool& p0_is_E) {
-  if (mp >= 1.0 - LANDAU_ELLIP_M_SPLIT) {
-    const double t = m - 0.5 * LANDAU_ELLIP_M_SPLIT;
-    P0_or_E = horner<c_S_P0, LANDAU_ELLIP_S_P0_DEG>(t);
-    Dc = horner<c_S_DC, LANDAU_ELLIP_S_DC_DEG>(t);
-    Q = horner<c_S_Q, LANDAU_ELLIP_S_Q_DEG>(t);
-    p0_is_E = false;
+// (E, Dc, Q) at complement x = m' = 1 - m (given directly, never formed by subtraction), E = m' P0:
+//   Dc = (K-E)/m,  Q = ((2-m)K - 2E)/m^2   -- see gen_ellip_coeffs.py.
+// x >= 2^-TAB_BINADES (all but near-coincident pairs): table T.  The interval index is the exponent and the top two
+// mantissa bits of x, the interval centre is x with the lower mantissa bits replaced by 100..0, so t = x - centre is
+// exact; three degree-TAB_DEG Horner chains share the loads of one table row (L1-resident, 13 KB).  No branch on m,
+// no logarithm: 3 (TAB_DEG) DFMA instead of 73 (old small-m fit) or ~140 (logarithmic form).
+// x < 2^-TAB_BINADES: f = A_f(x) + ln(1/x) B_f(x) (fits valid for x < 1 - M_SPLIT).
+__device__ __align__(16) const double g_ellip_tab[] = LANDAU_ELLIP_TAB_COEFFS;
+constexpr double ELLIP_TAB_XMIN = 1.0 / (1 << LANDAU_ELLIP_TAB_BINADES);
+
+// logarithmic form, x < 1 - M_SPLIT
+__device__ __forceinline__ void ellip_pieces_log(double x, double& E, double& Dc, double& Q) {
+  const double t = x - 0.5 * (1.0 - LANDAU_ELLIP_M_SPLIT);
+  const double lg = -log(x);
+  E = fma(lg, horner<c_L_B_E, LANDAU_ELLIP_L_B_E_DEG>(t), horner<c_L_A_E, LANDAU_ELLIP_L_A_E_DEG>(t));
+  Dc = fma(lg, horner<c_L_B_DC, LANDAU_ELLIP_L_B_DC_DEG>(t), horner<c_L_A_DC, LANDAU_ELLIP_L_A_DC_DEG>(t));
+  Q = fma(lg, horner<c_L_B_Q, LANDAU_ELLIP_L_B_Q_DEG>(t), horner<c_L_A_Q, LANDAU_ELLIP_L_A_Q_DEG>(t));
+}
+
+// Table evaluation in stages, so that a kernel can interleave the Horner steps with other work:
+//   start(x) -> steps<HI, LO>() ... -> E, Dc, Q valid after steps down to 0 (x >= ELLIP_TAB_XMIN; smaller x index the
+//   first interval and must be redone with ellip_pieces_log).
+struct EllipTable {
+  double t, E, Dc, Q;
+  const double* row;
+  __device__ __forceinline__ void start(double x, const double* __restrict__ tab) {
+    constexpr int BIAS = (1023 - LANDAU_ELLIP_TAB_BINADES) << 2, D = LANDAU_ELLIP_TAB_DEG;
+    const int idx = max(min((__double2hiint(x) >> 18) - BIAS, 4 * LANDAU_ELLIP_TAB_BINADES - 1), 0);  // x == 1: last
+    t = x - __hiloint2double(((idx + BIAS) << 18) | 0x20000, 0);
+    row = tab + idx * (D + 1) * 4;
+    const double2 ed = *reinterpret_cast<const double2*>(row + 4 * D);
+    E = ed.x;
+    Dc = ed.y;
+    Q = row[4 * D + 2];
+  }
+  template <int HI, int LO>
+  __device__ __forceinline__ void steps() {
+#pragma unroll
+    for (int n = HI; n >= LO; --n) {
+      const double2 ed = *reinterpret_cast<const double2*>(row + 4 * n);
+      const double q = row[4 * n + 2];
+      E = fma(E, t, ed.x);
+      Dc = fma(Dc, t, ed.y);
+      Q = fma(Q, t, q);
+    }
+  }
+};
+
+__device__ __forceinline__ void ellip_pieces(double x, double& E, double& Dc, double& Q) {
+  if (x >= ELLIP_TAB_XMIN) {
+    EllipTable e;
+    e.start(x, g_ellip_tab);
+    e.template steps<LANDAU_ELLIP_TAB_DEG - 1, 0>();
+    E = e.E;
+    Dc = e.Dc;
+    Q = e.Q;
   } else {
-    const double t = mp - 0.5 * (1.0 - LANDAU_ELLIP_M_SPLIT);
-    const double lg = -log(mp);
-    P0_or_E = fma(lg, horner<c_L_B_E, LANDAU_ELLIP_L_B_E_DEG>(t), horner<c_L_A_E, LANDAU_ELLIP_L_A_E_DEG>(t));
-    Dc = fma(lg, horner<c_L_B_DC, LANDAU_ELLIP_L_B_DC_DEG>(t), horner<c_L_A_DC, LANDAU_ELLIP_L_A_DC_DEG>(t));
-    Q = fma(lg, horner<c_L_B_Q, LANDAU_ELLIP_L_B_Q_DEG>(t), horner<c_L_A_Q, LANDAU_ELLIP_L_A_Q_DEG>(t));
-    p0_is_E = true;
+    ellip_pieces_log(x, E, Dc, Q);
   }
 }
 
@@ -76,37 +114,60 @@ __device__ __forceinline__ void ellip_pieces(double m, double mp, double& P0_or_
 //   UD_rz = -dz c ((r-rb) P0 + 2 rb Dc)    UK_rz = UD_rz
 //                                          UK_zr =  dz c ((rb-r) P0 + 2 r Dc)
 // Coincident points (s- <= 1e-20 s+) give zero (reading A2).
+// PairEval is the same computation cut into stages (geometry -> Horner steps of the table -> finish) for kernels that
+// interleave it with their DMMA stream; landau_tensor_2v runs the stages back to back.
 // ------------------------------------------------------------------------------------------------------------
 struct Tensor5 {
   double UDrr, UDrz, UDzz, UKrr, UKzr;
 };
 
-__device__ __forceinline__ Tensor5 landau_tensor_2v(double r, double z, double rb, double zb) {
-  const double dr = r - rb, dz = z - zb;
-  const double dz2 = dz * dz;
-  double sm = fma(dr, dr, dz2);
-  const double rr4 = 4.0 * r * rb;
-  const double sp = sm + rr4;
-  const bool coincident = sm <= 1e-20 * sp;
-  sm = coincident ? sp : sm;
-  const double inv = 1.0 / (sp * sm);
-  const double isp = inv * sm;  // 1/s+
-  const double mp = sm * isp;
-  const double m = rr4 * isp;
-  double c = 4.0 * isp * rsqrt(sp);
-  c = coincident ? 0.0 : c;
-  double P0, Dc, Q;
-  bool p0_is_E;
-  ellip_pieces(m, mp, P0, Dc, Q, p0_is_E);
-  if (p0_is_E) P0 *= sp * sp * inv;  // E / m' = E s+ / s-
-  const double mP2 = m * (P0 - Dc - Q);
-  Tensor5 t;
-  t.UDrr = c * fma(4.0 * rb * rb, Q, dz2 * P0);
-  t.UDzz = c * fma(dr * dr, P0, rr4 * Dc);
-  t.UDrz = -dz * c * fma(dr, P0, 2.0 * rb * Dc);
-  t.UKrr = c * fma(rr4, Q, dz2 * mP2);
-  t.UKzr = dz * c * fma(-dr, P0, 2.0 * r * Dc);
-  return t;
+struct PairEval {
+  double r, rb, dr, dz, rr4, ratio, c, m, x;
+  EllipTable el;
+  __device__ __forceinline__ void geometry(double r_, double z, double rb_, double zb, const double* __restrict__ tab) {
+    r = r_;
+    rb = rb_;
+    dr = r - rb;
+    dz = z - zb;
+    double sm = fma(dr, dr, dz * dz);
+    rr4 = 4.0 * r * rb;
+    const double sp = sm + rr4;
+    const bool coincident = sm <= 1e-20 * sp;
+    sm = coincident ? sp : sm;
+    const double inv = 1.0 / (sp * sm);
+    const double isp = inv * sm;  // 1/s+
+    x = sm * isp;                 // m' = s-/s+
+    m = rr4 * isp;
+    ratio = sp * sp * inv;        // s+/s-
+    c = coincident ? 0.0 : 4.0 * isp * rsqrt(sp);
+    el.start(x, tab);
+  }
+  template <int HI, int LO>
+  __device__ __forceinline__ void steps() {
+    el.template steps<HI, LO>();
+  }
+  __device__ __forceinline__ Tensor5 finish() {
+    double E = el.E, Dc = el.Dc, Q = el.Q;
+    if (x < ELLIP_TAB_XMIN) ellip_pieces_log(x, E, Dc, Q);  // near-coincident pairs only
+    const double P0 = E * ratio;  // P0 = E / m'
+    const double mP2 = m * (P0 - Dc - Q);
+    const double dz2 = dz * dz;
+    Tensor5 u;
+    u.UDrr = c * fma(4.0 * rb * rb, Q, dz2 * P0);
+    u.UDzz = c * fma(dr * dr, P0, rr4 * Dc);
+    u.UDrz = -dz * c * fma(dr, P0, 2.0 * rb * Dc);
+    u.UKrr = c * fma(rr4, Q, dz2 * mP2);
+    u.UKzr = dz * c * fma(-dr, P0, 2.0 * r * Dc);
+    return u;
+  }
+};
+
+__device__ __forceinline__ Tensor5 landau_tensor_2v(double r, double z, double rb, double zb,
+                                                    const double* __restrict__ tab = g_ellip_tab) {
+  PairEval p;
+  p.geometry(r, z, rb, zb, tab);
+  p.template steps<LANDAU_ELLIP_TAB_DEG - 1, 0>();
+  return p.finish();
 }
 
 __global__ void k_tensor_eval(const double* __restrict__ r, const double* __restrict__ z, const double* __restrict__ rb,
@@ -125,9 +186,8 @@ __global__ void k_ellip_eval(const double* __restrict__ m, const double* __restr
   int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n) return;
   double P0, Dc, Q;
-  bool isE;
-  ellip_pieces(m[t], mp[t], P0, Dc, Q, isE);
-  if (isE) P0 /= mp[t];
+  ellip_pieces(mp[t], P0, Dc, Q);
+  P0 /= mp[t];
   out[3 * t + 0] = P0;
   out[3 * t + 1] = Dc;
   out[3 * t + 2] = Q;
@@ -299,7 +359,7 @@ constexpr int K2M_TJ = 16;
 constexpr int K2M_LD = K2M_TJ + 4;
 
 __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                : "+d"(d0), "+d"(d1)
                : "d"(a), "d"(b));
 }
