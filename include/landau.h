@@ -166,9 +166,8 @@ int landau_set_timing(landau_ctx* ctx, int enabled);
 int landau_last_stage_ms(landau_ctx* ctx, float* ms4);
 
 /* Choose the inner-integral kernel: 0 auto (by column count), 1 plain DFMA kernel, 2 DMMA kernel with per-warp
- * tensor generation, 3 DMMA GEMM kernel with the tensor tile shared by the CTA (TMA-staged source tiles),
- * 4 / 5 warp-specialised DMMA GEMM kernel (producer warps evaluate the tensor, consumer warps issue the DMMAs;
- * 32 x 128 / 16 x 256 CTA tile). */
+ * tensor generation, 3 / 4 DMMA GEMM kernel with the tensor tile evaluated once per CTA and shared by its warps
+ * (TMA-staged source tiles; 32 x 128 / 16 x 256 CTA tile: 4 is the default for more than 128 source columns). */
 int landau_set_inner_kernel(landau_ctx* ctx, int which);
 
 /* Choose the element-matrix + assembly kernel: 0 auto (k3_ring: DMMA sum-factorised element matrices kept in a

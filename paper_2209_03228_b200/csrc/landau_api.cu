@@ -10,7 +10,6 @@
 #include "../../include/landau.h"
 #include "host_setup.hpp"
 #include "landau_kernels.cuh"
-#include "k2_ws.cuh"
 #include "k3_ring.cuh"
 
 using namespace landau;
@@ -401,39 +400,15 @@ int launch_gemm(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nspl
   return launch_gemm_t<2, 4, 2, 4, 3>(ctx, gr, ncols, gcol0, nsplit, split_stride, st);
 }
 
-// warp-specialised many-column kernels (k2_ws.cuh): kern 4 = 32 x 128 CTA tile, kern 5 = 16 x 256 CTA tile
-using K2Ws4 = K2W<2, 4, 2, 4, 3, 2>;
-using K2Ws5 = K2W<2, 4, 1, 8, 2, 2>;
-
-template <int WI_T, int WC_T, int WGI, int WGC, int NST, int NA>
-int launch_ws(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nsplit, long long split_stride,
-              cudaStream_t st) {
-  using C = K2W<WI_T, WC_T, WGI, WGC, NST, NA>;
-  static bool configured = false;
-  if (!configured) {
-    CUDA_TRY(ctx, cudaFuncSetAttribute(k2_inner_ws<WI_T, WC_T, WGI, WGC, NST, NA>,
-                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
-    configured = true;
-  }
-  dim3 grid((ctx->n_i_pad + C::TI - 1) / C::TI, (ncols + C::TC - 1) / C::TC, nsplit);
-  k2_inner_ws<WI_T, WC_T, WGI, WGC, NST, NA><<<grid, C::NTHREADS, C::SMEM_BYTES, st>>>(
-      ctx->d_ip_r, ctx->d_ip_z, ctx->n_i_pad, gr.j0, gr.nj_pad / K2G_TJ, ctx->F + gr.f_off, ncols, ctx->Gp, split_stride,
-      gcol0);
-  return LANDAU_OK;
-}
-
 // column-tile width of the tiled F layout a kernel reads (0: plain layout), field points per CTA
-int kern_tc(int kern) {
-  return kern == 3 ? K2BIG_TC : kern == 4 ? K2Ws4::TC : kern == 5 ? K2Ws5::TC : kern == 6 ? K2Wide::TC : 0;
-}
-int kern_ti(int kern) {
-  return kern == 3 ? K2Big::TI : kern == 4 ? K2Ws4::TI : kern == 5 ? K2Ws5::TI : kern == 6 ? K2Wide::TI : 0;
-}
+int kern_tc(int kern) { return kern == 3 ? K2BIG_TC : kern == 4 ? K2Wide::TC : 0; }
+int kern_ti(int kern) { return kern == 3 ? K2Big::TI : kern == 4 ? K2Wide::TI : 0; }
 
-// which inner-integral kernel a group of `ncols` columns takes: 1 DFMA, 2 DMMA (per-warp tensor), 3 GEMM (shared tensor)
+// which inner-integral kernel a group of `ncols` columns takes: 1 DFMA, 2 DMMA (per-warp tensor), 3 / 4 GEMM with the
+// tensor tile shared by the CTA (32 x 128 / 16 x 256 CTA tile)
 int pick_kernel(const landau_ctx* ctx, int ncols) {
   if (ctx->inner_kernel) return ctx->inner_kernel;
-  return ncols > 128 ? 6 : ncols > 64 ? 3 : (ncols >= 8 ? 2 : 1);
+  return ncols > 128 ? 4 : ncols > 64 ? 3 : (ncols >= 8 ? 2 : 1);
 }
 
 // stages a1..a2b for batch entries [b0, b0+nbc): leaves D,K in ctx->DK
@@ -501,12 +476,8 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
   // K2
   for (size_t q = 0; q < ctx->groups.size(); ++q) {
     const Group& gr = ctx->groups[q];
-    if (kern[q] == 6) {
+    if (kern[q] == 4) {
       if (int rc = launch_gemm_t<2, 4, 1, 8, 2>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
-    } else if (kern[q] == 5) {
-      if (int rc = launch_ws<2, 4, 1, 8, 2, 2>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
-    } else if (kern[q] == 4) {
-      if (int rc = launch_ws<2, 4, 2, 4, 3, 2>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
     } else if (kern[q] == 3) {
       if (int rc = launch_gemm(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
     } else if (kern[q] == 2) {
@@ -897,7 +868,7 @@ int landau_last_stage_ms(landau_ctx* ctx, float* ms4) {
 }
 
 int landau_set_inner_kernel(landau_ctx* ctx, int which) {
-  if (!ctx || which < 0 || which > 6) return LANDAU_INVALID_ARG;
+  if (!ctx || which < 0 || which > 4) return LANDAU_INVALID_ARG;
   ctx->inner_kernel = which;
   return LANDAU_OK;
 }
