@@ -123,8 +123,9 @@ int landau_jacobian(landau_ctx* ctx, const double* batch_f_dev, int batch, doubl
 int landau_apply(landau_ctx* ctx, const double* batch_f_dev, int batch, double* out_rhs_dev, void* cuda_stream);
 
 /* Host-buffer convenience: same as landau_jacobian / landau_apply with HOST pointers (pageable or pinned); the
- * library stages H2D / D2H copies on `cuda_stream` in internal device buffers and synchronises the stream
- * before returning. */
+ * library stages the copies in internal device buffers and synchronises before returning.  landau_jacobian_host
+ * cuts the batch into pieces and copies the CSR values of a finished piece to the host on a second (internal)
+ * stream while the kernels of the next piece run on `cuda_stream`; results are identical to the one-piece path. */
 int landau_jacobian_host(landau_ctx* ctx, const double* batch_f_host, int batch, double dt, double* out_csr_vals_host,
                          void* cuda_stream);
 int landau_apply_host(landau_ctx* ctx, const double* batch_f_host, int batch, double* out_rhs_host, void* cuda_stream);

@@ -63,6 +63,8 @@ struct landau_ctx {
   double *F = nullptr, *Gp = nullptr, *DK = nullptr, *FL = nullptr;
   size_t F_cap = 0, Gp_cap = 0, DK_cap = 0, FL_cap = 0;
   double *stage_in = nullptr, *stage_out = nullptr;
+  cudaStream_t copy_stream = nullptr;  // D2H copies of landau_jacobian_host, overlapped with the next piece's kernels
+  std::vector<cudaEvent_t> copy_ev;
   size_t stage_in_cap = 0, stage_out_cap = 0;
   long long f_layout_key = -1;
   int chunk = 1024;      // batch entries processed per pass through the stages
@@ -462,14 +464,14 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
   for (int g = 0; g < G; ++g) {
     const int q = ctx->mix_group[g];
     const Group& gr = ctx->groups[q];
-    dim3 grid((ctx->hg[g].n_ip + 255) / 256, nbc);
+    dim3 grid(ctx->hg[g].n_cells, (nbc + K1T_BT - 1) / K1T_BT);
     const int joff = ctx->ip_off[g] - gr.j0;
     if (ctx->nb == 9)
       k1_fields<9><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->mix[g], batch_f, ctx->f_stride, b0, nbc,
-                                         ctx->F + gr.f_off, gr.nj_pad, joff, 0, kern_tc(kern[q]));
+                                              ctx->F + gr.f_off, gr.nj_pad, joff, 0, kern_tc(kern[q]));
     else
       k1_fields<16><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->mix[g], batch_f, ctx->f_stride, b0, nbc,
-                                          ctx->F + gr.f_off, gr.nj_pad, joff, 0, kern_tc(kern[q]));
+                                               ctx->F + gr.f_off, gr.nj_pad, joff, 0, kern_tc(kern[q]));
     ++ctx->launches;
   }
   mark(ctx, st);
@@ -621,6 +623,8 @@ void landau_destroy(landau_ctx* ctx) {
   for (double* p : {ctx->F, ctx->Gp, ctx->DK, ctx->FL, ctx->stage_in, ctx->stage_out})
     if (p) cudaFree(p);
   for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+  for (cudaEvent_t e : ctx->copy_ev) cudaEventDestroy(e);
+  if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
   delete ctx;
 }
 
@@ -753,11 +757,47 @@ int landau_jacobian_host(landau_ctx* ctx, const double* batch_f_host, int batch,
   const size_t nin = (size_t)batch * ctx->f_stride, nout = (size_t)batch * ctx->v_stride;
   if (int rc = grow(ctx, &ctx->stage_in, &ctx->stage_in_cap, nin, false)) return rc;
   if (int rc = grow(ctx, &ctx->stage_out, &ctx->stage_out_cap, nout, false)) return rc;
-  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_in, batch_f_host, nin * sizeof(double), cudaMemcpyHostToDevice, st));
-  if (int rc = landau_jacobian(ctx, ctx->stage_in, batch, dt, ctx->stage_out, cuda_stream)) return rc;
-  CUDA_TRY(ctx, cudaMemcpyAsync(out_csr_vals_host, ctx->stage_out, nout * sizeof(double), cudaMemcpyDeviceToHost, st));
+  if (!ctx->copy_stream) CUDA_TRY(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+  // Pieces of the batch go through H2D -> kernels on `cuda_stream`; the D2H copy of a finished piece runs on a
+  // second stream under the kernels of the next piece.  Pieces: whole chunks, then the rest with its last 256
+  // entries split off, so that only a small copy is left exposed at the end.
+  std::vector<int> pieces;
+  int left = batch;
+  while (left > ctx->chunk) {
+    pieces.push_back(ctx->chunk);
+    left -= ctx->chunk;
+  }
+  if (left >= 512) {
+    pieces.push_back(left - 256);
+    left = 256;
+  }
+  pieces.push_back(left);
+  while (ctx->copy_ev.size() < pieces.size()) {
+    cudaEvent_t e = nullptr;
+    CUDA_TRY(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    ctx->copy_ev.push_back(e);
+  }
+  const bool timing = ctx->timing;
+  ctx->timing = false;  // stage events of a piece would be overwritten by the next one
+  int b0 = 0, status = LANDAU_OK;
+  for (size_t k = 0; k < pieces.size() && status == LANDAU_OK; ++k) {
+    const int nb = pieces[k];
+    const double* fin = ctx->stage_in + (size_t)b0 * ctx->f_stride;
+    double* vout = ctx->stage_out + (size_t)b0 * ctx->v_stride;
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_in + (size_t)b0 * ctx->f_stride, batch_f_host + (size_t)b0 * ctx->f_stride,
+                                  (size_t)nb * ctx->f_stride * sizeof(double), cudaMemcpyHostToDevice, st));
+    status = landau_jacobian(ctx, fin, nb, dt, vout, cuda_stream);
+    if (status != LANDAU_OK) break;
+    CUDA_TRY(ctx, cudaEventRecord(ctx->copy_ev[k], st));
+    CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->copy_ev[k], 0));
+    CUDA_TRY(ctx, cudaMemcpyAsync(out_csr_vals_host + (size_t)b0 * ctx->v_stride, vout,
+                                  (size_t)nb * ctx->v_stride * sizeof(double), cudaMemcpyDeviceToHost, ctx->copy_stream));
+    b0 += nb;
+  }
+  ctx->timing = timing;
+  CUDA_TRY(ctx, cudaStreamSynchronize(ctx->copy_stream));
   CUDA_TRY(ctx, cudaStreamSynchronize(st));
-  return LANDAU_OK;
+  return status;
 }
 
 int landau_apply_host(landau_ctx* ctx, const double* batch_f_host, int batch, double* out_rhs_host, void* cuda_stream) {

@@ -219,8 +219,7 @@ struct DevTables {
 };
 
 // ------------------------------------------------------------------------------------------------------------
-// K1: source fields.  One thread per (integration point j of grid g, batch entry b); q fastest so that the
-// threads of a cell share its dof loads and the stores along j are coalesced.
+// K1: source fields (kernel k1_fields below).
 //   F layout: [col][3][nj_pad], col = col0 + b*ncb + c;  comp 0: w f, 1: w df/dr, 2: w df/dz
 //   column c of the grid sums the species listed in (mix_ptr, mix_species, mix_wD, mix_wK).
 // ------------------------------------------------------------------------------------------------------------
@@ -242,45 +241,73 @@ __host__ __device__ __forceinline__ long long k2g_f_offset(int TC, int njt, int 
   return ((((long long)ct * njt + jt) * 3 + comp) * TC + cl) * 16 + pos;
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// K1: one CTA = one cell x 16 batch entries.  The cell's nodal values (constraints and species mix applied:
+// fD = sum_e wD_e f_e for the value, fK = sum_e wK_e f_e for the gradient) are staged in shared memory once, then
+// thread (q, entry) contracts them with the basis tabulation (stored [a][q]: conflict-free) and writes its three
+// source values; the 16 points of a cell are contiguous in either F layout, so every warp store covers whole
+// 128-byte lines.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int K1T_BT = 16;
+
 template <int NB>
 __global__ void __launch_bounds__(256)
-k1_fields(DevGrid g, const DevTables* __restrict__ tab, MixTable mix, const double* __restrict__ batch_f, long long f_stride,
-          int b0, int nbatch, double* __restrict__ F, long long nj_pad, int j_off_in_group, int col0, int tiled_tc) {
-  const int j = blockIdx.x * blockDim.x + threadIdx.x;
-  const int b = blockIdx.y;
-  if (j >= g.n_ip || b >= nbatch) return;
-  const int cell = j / NB, q = j - cell * NB;
-  const double sr = g.cell_sr[cell], sz = g.cell_sz[cell], w = g.ip_w[j];
-  const double* fb = batch_f + (long long)(b0 + b) * f_stride;
+k1_fields(DevGrid g, const DevTables* __restrict__ tab, MixTable mix, const double* __restrict__ batch_f,
+               long long f_stride, int b0, int nbatch, double* __restrict__ F, long long nj_pad, int j_off_in_group,
+               int col0, int tiled_tc) {
+  __shared__ double sT[3][NB][16];       // B, dBxi, dBeta as [a][q]
+  __shared__ double sD[NB][K1T_BT], sK[NB][K1T_BT];
+  const int tid = threadIdx.x, lo = tid & 15, bl = tid >> 4;
+  const int cell = blockIdx.x, b = blockIdx.y * K1T_BT + bl;
+  for (int e = tid; e < NB * NB; e += 256) {
+    const int q = e / NB, a = e - q * NB;
+    sT[0][a][q] = tab->B[e];
+    sT[1][a][q] = tab->dBxi[e];
+    sT[2][a][q] = tab->dBeta[e];
+  }
+  const double sr = g.cell_sr[cell], sz = g.cell_sz[cell];
+  const int j = cell * NB + lo;
+  const double w = lo < NB ? g.ip_w[j] : 0.0;
+  const bool live = b < nbatch;
+  const double* fb = batch_f + (long long)(b0 + (live ? b : 0)) * f_stride;
   for (int c = 0; c < mix.ncb; ++c) {
-    double aD = 0.0, aKr = 0.0, aKz = 0.0;
-    for (int e = mix.ptr[c]; e < mix.ptr[c + 1]; ++e) {
-      const double* fs = fb + mix.species_foff[e];
-      double v = 0.0, vx = 0.0, vy = 0.0;
-#pragma unroll 4
-      for (int a = 0; a < NB; ++a) {
-        const int p0 = g.en_ptr[cell * NB + a], p1 = g.en_ptr[cell * NB + a + 1];
+    __syncthreads();
+    if (lo < NB) {  // lo = basis function a
+      double fD = 0.0, fK = 0.0;
+      const int p0 = g.en_ptr[cell * NB + lo], p1 = g.en_ptr[cell * NB + lo + 1];
+      for (int e = mix.ptr[c]; e < mix.ptr[c + 1]; ++e) {
+        const double* fs = fb + mix.species_foff[e];
         double fa = 0.0;
         for (int p = p0; p < p1; ++p) fa = fma(g.en_w[p], fs[g.en_dof[p]], fa);
-        v = fma(tab->B[q * NB + a], fa, v);
-        vx = fma(tab->dBxi[q * NB + a], fa, vx);
-        vy = fma(tab->dBeta[q * NB + a], fa, vy);
+        fD = fma(mix.wD[e], fa, fD);
+        fK = fma(mix.wK[e], fa, fK);
       }
-      aD = fma(mix.wD[e], v, aD);
-      aKr = fma(mix.wK[e], vx * sr, aKr);
-      aKz = fma(mix.wK[e], vy * sz, aKz);
+      sD[lo][bl] = fD;
+      sK[lo][bl] = fK;
     }
-    const long long col = col0 + (long long)b * mix.ncb + c;
-    if (tiled_tc) {  // stage-image layout of k2_inner_gemm
-      const int njt = (int)(nj_pad >> 4), jg = j_off_in_group + j;
-      F[k2g_f_offset(tiled_tc, njt, (int)col, 0, jg)] = w * aD;
-      F[k2g_f_offset(tiled_tc, njt, (int)col, 1, jg)] = w * aKr;
-      F[k2g_f_offset(tiled_tc, njt, (int)col, 2, jg)] = w * aKz;
-    } else {
-      double* dst = F + col * 3 * nj_pad + j_off_in_group + j;
-      dst[0] = w * aD;
-      dst[nj_pad] = w * aKr;
-      dst[2 * nj_pad] = w * aKz;
+    __syncthreads();
+    if (lo < NB && live) {  // lo = quadrature point q
+      double v = 0.0, vx = 0.0, vy = 0.0;
+#pragma unroll
+      for (int a = 0; a < NB; ++a) {
+        const double fd = sD[a][bl], fk = sK[a][bl];
+        v = fma(sT[0][a][lo], fd, v);
+        vx = fma(sT[1][a][lo], fk, vx);
+        vy = fma(sT[2][a][lo], fk, vy);
+      }
+      const long long col = col0 + (long long)b * mix.ncb + c;
+      const double o0 = w * v, o1 = w * (vx * sr), o2 = w * (vy * sz);
+      if (tiled_tc) {
+        const int njt = (int)(nj_pad >> 4), jg = j_off_in_group + j;
+        F[k2g_f_offset(tiled_tc, njt, (int)col, 0, jg)] = o0;
+        F[k2g_f_offset(tiled_tc, njt, (int)col, 1, jg)] = o1;
+        F[k2g_f_offset(tiled_tc, njt, (int)col, 2, jg)] = o2;
+      } else {
+        double* dst = F + col * 3 * nj_pad + j_off_in_group + j;
+        dst[0] = o0;
+        dst[nj_pad] = o1;
+        dst[2 * nj_pad] = o2;
+      }
     }
   }
 }
