@@ -50,7 +50,7 @@ struct K3Species {
 
 constexpr int K3_THREADS = 256;
 constexpr int K3_CPW = K3_PC / (K3_THREADS / 32);  // cells per warp per step
-constexpr int K3_EB = 8;                            // emission: descriptor words per thread per batch
+constexpr int K3_EB = 16;                           // emission: descriptor words per thread per batch
 
 // dynamic shared memory: ring [rc][K3_RS] | zero pad [8] | constant fragments [16][32]
 __host__ __device__ constexpr size_t k3_smem_bytes(int rc) { return ((size_t)rc * K3_RS + 8 + 16 * 32) * sizeof(double); }
@@ -156,40 +156,55 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
       }
     }
     if (s + 1 < s_hi) fetch(s + 1);
+    // first batch of this panel's emission descriptors: issued before the barrier, consumed after it
+    const bool emit = s >= s_lo;
+    const int base = g->em_base[s];
+    const unsigned* __restrict__ em1 = g->em1;
+    const uint4* __restrict__ em4 = g->em4;
+    const int e1_lo = g->em_ptr[s] + tid, e1_hi = emit ? g->em_ptr[s + 1] : 0;
+    const int e4_lo = g->em_ptr[S1 + s] + tid, e4_hi = emit ? g->em_ptr[S1 + s + 1] : 0;
+    unsigned wd[K3_EB];
+    uint4 d4[2];
+#pragma unroll
+    for (int k = 0; k < K3_EB; ++k) {
+      const int e = e1_lo + k * K3_THREADS;
+      wd[k] = e < e1_hi ? __ldg(em1 + e) : 0xFFFFFFFFu;
+    }
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const int e = e4_lo + k * K3_THREADS;
+      d4[k] = e < e4_hi ? __ldg(em4 + e) : make_uint4(0xFFFFFFFFu, 0, 0, 0);
+    }
     __syncthreads();
-    if (s >= s_lo) {
-      const int base = g->em_base[s];
-      {  // one contribution, weight 1: K3_EB descriptor words per thread in flight before the first store
-        const unsigned* __restrict__ em1 = g->em1;
-        const int e1 = g->em_ptr[s + 1];
-        for (int e0 = g->em_ptr[s] + tid; e0 < e1; e0 += K3_THREADS * K3_EB) {
-          unsigned wd[K3_EB];
+    if (emit) {
+      // one contribution, weight 1
+      for (int e0 = e1_lo;;) {
 #pragma unroll
-          for (int k = 0; k < K3_EB; ++k) {
-            const int e = e0 + k * K3_THREADS;
-            wd[k] = e < e1 ? __ldg(em1 + e) : 0xFFFFFFFFu;
-          }
+        for (int k = 0; k < K3_EB; ++k)
+          if (wd[k] != 0xFFFFFFFFu) __stcs(out + base + (int)(wd[k] & ((1u << K3_NBITS) - 1)), ring[wd[k] >> K3_NBITS]);
+        e0 += K3_THREADS * K3_EB;
+        if (e0 >= e1_hi) break;
 #pragma unroll
-          for (int k = 0; k < K3_EB; ++k)
-            if (wd[k] != 0xFFFFFFFFu) __stcs(out + base + (int)(wd[k] & ((1u << K3_NBITS) - 1)), ring[wd[k] >> K3_NBITS]);
+        for (int k = 0; k < K3_EB; ++k) {
+          const int e = e0 + k * K3_THREADS;
+          wd[k] = e < e1_hi ? __ldg(em1 + e) : 0xFFFFFFFFu;
         }
       }
-      {  // 2..4 contributions, weight 1
-        const uint4* __restrict__ em4 = g->em4;
-        const int e1 = g->em_ptr[S1 + s + 1];
-        for (int e0 = g->em_ptr[S1 + s] + tid; e0 < e1; e0 += K3_THREADS * 2) {
-          uint4 d[2];
+      // 2..4 contributions, weight 1
+      for (int e0 = e4_lo;;) {
 #pragma unroll
-          for (int k = 0; k < 2; ++k) {
-            const int e = e0 + k * K3_THREADS;
-            d[k] = e < e1 ? __ldg(em4 + e) : make_uint4(0xFFFFFFFFu, 0, 0, 0);
+        for (int k = 0; k < 2; ++k)
+          if (d4[k].x != 0xFFFFFFFFu) {
+            const double v =
+                ((ring[d4[k].y & 0xFFFFu] + ring[d4[k].y >> 16]) + ring[d4[k].z & 0xFFFFu]) + ring[d4[k].z >> 16];
+            __stcs(out + base + (int)d4[k].x, v);
           }
+        e0 += K3_THREADS * 2;
+        if (e0 >= e4_hi) break;
 #pragma unroll
-          for (int k = 0; k < 2; ++k)
-            if (d[k].x != 0xFFFFFFFFu) {
-              const double v = ((ring[d[k].y & 0xFFFFu] + ring[d[k].y >> 16]) + ring[d[k].z & 0xFFFFu]) + ring[d[k].z >> 16];
-              __stcs(out + base + (int)d[k].x, v);
-            }
+        for (int k = 0; k < 2; ++k) {
+          const int e = e0 + k * K3_THREADS;
+          d4[k] = e < e4_hi ? __ldg(em4 + e) : make_uint4(0xFFFFFFFFu, 0, 0, 0);
         }
       }
       {  // general: hanging-node weights
