@@ -107,6 +107,16 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
     }
   };
   fetch(s_begin);
+  // list bounds of the panel to emit, loaded one step ahead: em1 [pa[0], pa[1]), em4 [pa[2], pa[3]), slot base pa[4]
+  int pa[5];
+  auto fetch_bounds = [&](int s) {
+    pa[0] = g->em_ptr[s];
+    pa[1] = g->em_ptr[s + 1];
+    pa[2] = g->em_ptr[S1 + s];
+    pa[3] = g->em_ptr[S1 + s + 1];
+    pa[4] = g->em_base[s];
+  };
+  fetch_bounds(s_begin);
   __syncthreads();
 
   for (int s = s_begin; s < s_hi; ++s) {
@@ -158,11 +168,11 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
     if (s + 1 < s_hi) fetch(s + 1);
     // first batch of this panel's emission descriptors: issued before the barrier, consumed after it
     const bool emit = s >= s_lo;
-    const int base = g->em_base[s];
+    const int base = pa[4];
     const unsigned* __restrict__ em1 = g->em1;
     const uint4* __restrict__ em4 = g->em4;
-    const int e1_lo = g->em_ptr[s] + tid, e1_hi = emit ? g->em_ptr[s + 1] : 0;
-    const int e4_lo = g->em_ptr[S1 + s] + tid, e4_hi = emit ? g->em_ptr[S1 + s + 1] : 0;
+    const int e1_lo = pa[0] + tid, e1_hi = emit ? pa[1] : 0;
+    const int e4_lo = pa[2] + tid, e4_hi = emit ? pa[3] : 0;
     unsigned wd[K3_EB];
     uint4 d4[2];
 #pragma unroll
@@ -175,6 +185,7 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
       const int e = e4_lo + k * K3_THREADS;
       d4[k] = e < e4_hi ? __ldg(em4 + e) : make_uint4(0xFFFFFFFFu, 0, 0, 0);
     }
+    if (s + 1 < s_hi) fetch_bounds(s + 1);
     __syncthreads();
     if (emit) {
       // one contribution, weight 1
