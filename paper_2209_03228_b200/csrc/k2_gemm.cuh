@@ -61,7 +61,8 @@ struct K2G {
 template <int WI_T, int WC_T, int WGI, int WGC, int NST>
 __global__ void __launch_bounds__(32 * WGI * WGC, 1)
 k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, int n_i, int j0, int njt,
-              const double* __restrict__ F, int ncols, double* __restrict__ G, long long g_split_stride, int gcol0) {
+              const double* __restrict__ F, int ncols, double* __restrict__ G, long long g_split_stride, int gcol0,
+              int stream_itiles, int stream_tiles) {
   using C = K2G<WI_T, WC_T, WGI, WGC, NST>;
   extern __shared__ __align__(128) double smem_g[];
   double* smem = smem_g;
@@ -74,42 +75,35 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wi = warp / WGC, wc = warp - wi * WGC;
   const int gq = lane >> 2, tq = lane & 3;
-  const int i0 = blockIdx.x * C::TI;
-  const int per = (njt + gridDim.z - 1) / gridDim.z;
-  const int t0 = blockIdx.z * per, t1 = min(t0 + per, njt);
-  const int nt = t1 - t0;
-  const double* Fct = F + (long long)blockIdx.y * njt * C::STAGE_DOUBLES;
-
-  for (int e = tid; e < C::TAB_DOUBLES; e += C::NTHREADS) sTab[e] = g_ellip_tab[e];
-  // coordinates of the first two source tiles (later tiles arrive by cp.async two steps ahead of their use)
-  if (tid < 4 * K2G_TJ && (tid >> 5) < nt) {
-    const int tl = tid >> 5, e = tid & 31;
-    const double* src = (e < K2G_TJ ? ip_r : ip_z) + j0 + (t0 + tl) * K2G_TJ + (e & (K2G_TJ - 1));
-    sXY[tl * 2 * K2G_TJ + e] = *src;
+  // Work of this CTA.  Grid mode (stream_tiles == 0): one segment = tile (blockIdx.x, blockIdx.y), source tiles of
+  // j-split blockIdx.z, plain stores into split plane blockIdx.z.  Stream mode: gridDim.x persistent CTAs share
+  // stream_tiles x njt (tile, source tile) steps evenly (tiles ordered column tile slowest); a CTA's range is cut at
+  // tile boundaries into segments; a segment that covers its whole tile is stored, a partial one is ADDED into the
+  // zeroed G (at most two partial segments per tile when a CTA's share is at least one tile, so the sum is
+  // order-independent).
+  long long w0, w1;
+  if (stream_tiles) {
+    const long long W = (long long)stream_tiles * njt;
+    w0 = W * blockIdx.x / gridDim.x;
+    w1 = W * (blockIdx.x + 1) / gridDim.x;
+  } else {
+    const int per = (njt + gridDim.z - 1) / gridDim.z;
+    const int ta = blockIdx.z * per, tb = min(ta + per, njt);
+    w0 = ta;
+    w1 = max(tb, ta);
   }
+  for (int e = tid; e < C::TAB_DOUBLES; e += C::NTHREADS) sTab[e] = g_ellip_tab[e];
   if (tid == 0) {
     for (int s = 0; s < NST; ++s) mbar_init(&full[s], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncthreads();
-  if (tid == 0) {
-    for (int s = 0; s < NST && s < nt; ++s) {
-      mbar_expect_tx(&full[s], C::STAGE_DOUBLES * 8);
-      bulk_g2s(sB + s * C::STAGE_DOUBLES, Fct + (long long)(t0 + s) * C::STAGE_DOUBLES, C::STAGE_DOUBLES * 8, &full[s]);
-    }
-  }
 
   // Tensor pairs of this thread: lane (gq, tq) of warp w evaluates (i = 8 iblk + gq, j = 4 k4 + tq) for the fragment
   // blocks blk = w + NWARPS u = iblk * 4 + k4 -- one warp store per component = 32 consecutive doubles (no conflicts).
   constexpr int NW = C::NTHREADS / 32, NU = C::PAIRS_PER_THREAD;
   double ri[NU], zi[NU];
-#pragma unroll
-  for (int u = 0; u < NU; ++u) {
-    const int ig = min(i0 + ((warp + NW * u) >> 2) * 8 + gq, n_i - 1);
-    ri[u] = ip_r[ig];
-    zi[u] = ip_z[ig];
-  }
   // NW is a multiple of 4, so every block of this thread has the same k4 = warp & 3: one source point per tile
   const int jl = (warp & 3) * 4 + tq;
   constexpr int CS = (C::TI / 8) * 4 * 32;
@@ -136,7 +130,51 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
 #pragma unroll
       for (int k = 0; k < 5; ++k) acc[x][n][k][0] = acc[x][n][k][1] = 0.0;
 
-  if (nt > 0) {
+  unsigned cnt = 0;  // source-tile steps done by this CTA: stage = cnt % NST, mbarrier parity = (cnt / NST) & 1
+  do {
+  int it, ct, t0, nt, plane;
+  bool whole;
+  if (stream_tiles) {
+    const int tile = (int)(w0 / njt);
+    t0 = (int)(w0 - (long long)tile * njt);
+    nt = (int)min((long long)(njt - t0), w1 - w0);
+    ct = tile / stream_itiles;
+    it = tile - ct * stream_itiles;
+    plane = 0;
+    whole = nt == njt;
+  } else {
+    it = blockIdx.x;
+    ct = blockIdx.y;
+    t0 = (int)w0;
+    nt = (int)(w1 - w0);
+    plane = blockIdx.z;
+    whole = true;
+  }
+  w0 += nt;
+  const int i0 = it * C::TI;
+  const double* Fct = F + (long long)ct * njt * C::STAGE_DOUBLES;
+  if (tid == 0) {
+    for (int s = 0; s < NST && s < nt; ++s) {
+      uint64_t* bar = &full[(cnt + s) % NST];
+      mbar_expect_tx(bar, C::STAGE_DOUBLES * 8);
+      bulk_g2s(sB + ((cnt + s) % NST) * C::STAGE_DOUBLES, Fct + (long long)(t0 + s) * C::STAGE_DOUBLES,
+               C::STAGE_DOUBLES * 8, bar);
+    }
+  }
+  // coordinates of the first two source tiles (later tiles arrive by cp.async two steps ahead of their use)
+  if (tid < 4 * K2G_TJ && (tid >> 5) < nt) {
+    const int tl = tid >> 5, e = tid & 31;
+    const double* src = (e < K2G_TJ ? ip_r : ip_z) + j0 + (t0 + tl) * K2G_TJ + (e & (K2G_TJ - 1));
+    sXY[tl * 2 * K2G_TJ + e] = *src;
+  }
+#pragma unroll
+  for (int u = 0; u < NU; ++u) {
+    const int ig = min(i0 + ((warp + NW * u) >> 2) * 8 + gq, n_i - 1);
+    ri[u] = ip_r[ig];
+    zi[u] = ip_z[ig];
+  }
+  __syncthreads();
+  {
 #pragma unroll
     for (int u = 0; u < NU; ++u) {
       pe[u].geometry(ri[u], zi[u], sXY[jl], sXY[K2G_TJ + jl], sTab);
@@ -148,10 +186,10 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
 
   // Horner steps of the NEXT tile's tensor, cut in four and placed between the four k-blocks of DMMAs
   constexpr int D = LANDAU_ELLIP_TAB_DEG, H1 = D - 1 - D / 3, H2 = H1 - D / 3;
-  for (int tt = 0; tt < nt; ++tt) {
-    const int stage = tt % NST;
+  for (int tt = 0; tt < nt; ++tt, ++cnt) {
+    const int stage = cnt % NST;
     const bool more = tt + 1 < nt;
-    mbar_wait(&full[stage], (tt / NST) & 1);
+    mbar_wait(&full[stage], (cnt / NST) & 1);
     const double* A = sA + (tt & 1) * C::A_DOUBLES;
     const double* Bst = sB + stage * C::STAGE_DOUBLES;
     if (tt + 2 < nt && tid < K2G_TJ) {  // coordinates of the tile after next: 16 x 16 bytes, landed by the end of the step
@@ -212,20 +250,26 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
 #pragma unroll
   for (int x = 0; x < WI_T; ++x) {
     const int i = i0 + (wi * WI_T + x) * 8 + gq;
-    if (i < n_i) {
 #pragma unroll
-      for (int n = 0; n < WC_T; ++n)
+    for (int n = 0; n < WC_T; ++n)
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          const int col = blockIdx.y * C::TC + (wc * WC_T + n) * 8 + 2 * tq + h;
-          if (col < ncols) {
-            double* dst = G + blockIdx.z * g_split_stride + ((long long)(gcol0 + col) * 5) * n_i + i;
+      for (int h = 0; h < 2; ++h) {
+        const int col = ct * C::TC + (wc * WC_T + n) * 8 + 2 * tq + h;
+        if (i < n_i && col < ncols) {
+          double* dst = G + plane * g_split_stride + ((long long)(gcol0 + col) * 5) * n_i + i;
 #pragma unroll
-            for (int k = 0; k < 5; ++k) dst[(long long)k * n_i] = acc[x][n][k][h];
+          for (int k = 0; k < 5; ++k) {
+            if (whole)
+              dst[(long long)k * n_i] = acc[x][n][k][h];
+            else
+              atomicAdd(dst + (long long)k * n_i, acc[x][n][k][h]);
           }
         }
-    }
+#pragma unroll
+        for (int k = 0; k < 5; ++k) acc[x][n][k][h] = 0.0;
+      }
   }
+  } while (w0 < w1);  // segments (an empty j-split still stores its zeros)
 }
 
 }  // namespace landau

@@ -69,6 +69,8 @@ struct landau_ctx {
   long long f_layout_key = -1;
   int chunk = 1024;      // batch entries processed per pass through the stages
   int inner_kernel = 0;  // 0 auto, 1 dfma, 2 dmma
+  int n_sm = 148;
+  bool stream_k = true;  // many-column K2: persistent CTAs sharing the steps evenly when the tiles do not fill whole waves
   int assembly_kernel = 0;  // 0 auto (ring kernel where the grid has a schedule), 1 slot-gather kernel
   int last_batch = 0;
   cudaStream_t last_stream = nullptr;
@@ -390,10 +392,22 @@ int launch_gemm_t(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int ns
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
     configured = true;
   }
-  dim3 grid((ctx->n_i_pad + C::TI - 1) / C::TI, (ncols + C::TC - 1) / C::TC, nsplit);
+  const int n_it = (ctx->n_i_pad + C::TI - 1) / C::TI, n_ct = (ncols + C::TC - 1) / C::TC;
+  const bool stream = ctx->stream_k && nsplit == 1 && n_it * n_ct >= ctx->n_sm && (n_it * n_ct) % ctx->n_sm != 0;
+  if (stream) {
+    // persistent CTAs, one per SM, share the (tile, source tile) steps evenly: no partial last wave.  Partial tiles are
+    // added into G, which is zeroed first.
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->Gp + (long long)gcol0 * 5 * ctx->n_i_pad, 0,
+                                  sizeof(double) * (size_t)ncols * 5 * ctx->n_i_pad, st));
+    k2_inner_gemm<WI_T, WC_T, WGI, WGC, NST><<<dim3(ctx->n_sm, 1, 1), C::NTHREADS, C::SMEM_BYTES, st>>>(
+        ctx->d_ip_r, ctx->d_ip_z, ctx->n_i_pad, gr.j0, gr.nj_pad / K2G_TJ, ctx->F + gr.f_off, ncols, ctx->Gp,
+        split_stride, gcol0, n_it, n_it * n_ct);
+    return LANDAU_OK;
+  }
+  dim3 grid(n_it, n_ct, nsplit);
   k2_inner_gemm<WI_T, WC_T, WGI, WGC, NST><<<grid, C::NTHREADS, C::SMEM_BYTES, st>>>(
       ctx->d_ip_r, ctx->d_ip_z, ctx->n_i_pad, gr.j0, gr.nj_pad / K2G_TJ, ctx->F + gr.f_off, ncols, ctx->Gp, split_stride,
-      gcol0);
+      gcol0, 0, 0);
   return LANDAU_OK;
 }
 
@@ -604,6 +618,7 @@ int landau_create(const landau_grid_desc* grids, int n_grids, const landau_speci
   }
   cudaError_t e = cudaSetDevice(cuda_device);
   if (e != cudaSuccess) return bail(LANDAU_CUDA_ERROR, std::string("cudaSetDevice: ") + cudaGetErrorString(e));
+  cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, cuda_device);
   int rc = build_device_side(ctx);
   if (rc) {
     std::string m = ctx->err;
