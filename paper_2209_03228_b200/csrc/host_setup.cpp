@@ -348,20 +348,47 @@ int build_grid(const landau_grid_desc& d, const HostTables& t, HostGrid* g, std:
   // ---- K3 ring schedule --------------------------------------------------------------------------------------------
   {
     const int nb2 = nb * nb;
-    int span = 0;
-    std::vector<int> last(g->nnz, 0);
-    for (int n = 0; n < g->nnz; ++n) {
-      int lo = g->n_cells, hi = -1;
-      for (int p = g->as_ptr[n]; p < g->as_ptr[n + 1]; ++p) {
-        const int cell = g->as_code[p] / nb2;
-        lo = std::min(lo, cell);
-        hi = std::max(hi, cell);
-      }
-      last[n] = hi;
-      span = std::max(span, hi - lo);
-    }
-    int rc = (span + K3_PC + K3_PC - 1) / K3_PC * K3_PC;
     g->k3_nsteps = (g->n_cells + K3_PC - 1) / K3_PC;
+    // emission step of every CSR slot = step of its last contributing cell; an element matrix stays in the ring from
+    // the step that computes it to the last step that emits one of its slots
+    std::vector<int> last(g->nnz, 0), dies(g->n_cells, 0);
+    for (int c = 0; c < g->n_cells; ++c) dies[c] = c / K3_PC;
+    for (int n = 0; n < g->nnz; ++n) {
+      int hi = -1;
+      for (int p = g->as_ptr[n]; p < g->as_ptr[n + 1]; ++p) hi = std::max(hi, g->as_code[p] / nb2);
+      last[n] = hi;
+      for (int p = g->as_ptr[n]; p < g->as_ptr[n + 1]; ++p) {
+        int& d = dies[g->as_code[p] / nb2];
+        d = std::max(d, hi / K3_PC);
+      }
+    }
+    // ring positions: a cell takes the lowest free position when its step starts; positions of matrices whose last
+    // emission was an earlier step are free again (the kernel's second barrier of a step orders reuse after emission)
+    g->cell_pos.assign(g->n_cells, 0);
+    g->halo_begin.assign(g->k3_nsteps, 0);
+    int rc = 0;
+    {
+      std::vector<int> free_pos, owner;  // owner[pos] = cell or -1
+      for (int st = 0; st < g->k3_nsteps; ++st) {
+        int hb = st;
+        for (size_t pos = 0; pos < owner.size(); ++pos)
+          if (owner[pos] >= 0) {
+            if (dies[owner[pos]] < st)
+              owner[pos] = -1;
+            else
+              hb = std::min(hb, owner[pos] / K3_PC);
+          }
+        g->halo_begin[st] = hb;
+        for (int c = st * K3_PC; c < std::min(g->n_cells, (st + 1) * K3_PC); ++c) {
+          size_t pos = 0;
+          while (pos < owner.size() && owner[pos] >= 0) ++pos;
+          if (pos == owner.size()) owner.push_back(-1);
+          owner[pos] = c;
+          g->cell_pos[c] = (int)pos;
+        }
+        rc = std::max(rc, (int)owner.size());
+      }
+    }
     if ((long long)rc * K3_RS * 8 + 64 > K3_RING_MAX_BYTES || (long long)rc * K3_RS + 8 >= (1 << (32 - K3_NBITS))) rc = 0;
     g->k3_rc = rc;
     if (rc) {
@@ -370,7 +397,7 @@ int build_grid(const landau_grid_desc& d, const HostTables& t, HostGrid* g, std:
       for (size_t p = 0; p < g->as_code.size(); ++p) {
         const int code = g->as_code[p], cell = code / nb2, a = (code / nb) % nb, c = code % nb;
         const int a1 = a % n1, a2 = a / n1, c1 = c % n1, c2 = c / n1;
-        g->as_roff[p] = (cell % rc) * K3_RS + (a2 * n1 + c2) * K3_LD + (a1 * n1 + c1);
+        g->as_roff[p] = g->cell_pos[cell] * K3_RS + (a2 * n1 + c2) * K3_LD + (a1 * n1 + c1);
       }
       // classify, bucket by step (slots visited in ascending n, so every list is ascending)
       std::vector<std::vector<int>> l1(g->k3_nsteps), l4(g->k3_nsteps), lg(g->k3_nsteps);

@@ -12,7 +12,7 @@ namespace landau {
 
 // K3 (element matrices + assembly) schedule constants, shared by host set-up and the kernel:
 // cells are processed in panels of K3_PC cells (cell order); each element matrix occupies K3_RS doubles of a
-// shared-memory ring, entry (a, c) at  (a2 n1 + c2) * K3_LD + (a1 n1 + c1)  (a = a1 + n1 a2, c = c1 + n1 c2).
+// shared-memory ring (a pool of k3_rc matrix positions), entry (a, c) at  (a2 n1 + c2) * K3_LD + (a1 n1 + c1)  (a = a1 + n1 a2, c = c1 + n1 c2).
 constexpr int K3_PC = 16;
 constexpr int K3_LD = 18;
 constexpr int K3_RS = 16 * K3_LD;
@@ -37,7 +37,9 @@ struct HostGrid {
   // as_code = cell*nb*nb + a*nb + c
   std::vector<int> as_ptr, as_code;
   std::vector<double> as_w;
-  // K3 ring schedule: step s computes cells [s K3_PC, (s+1) K3_PC) into ring positions (cell % k3_rc) and then
+  // K3 ring schedule: step s computes cells [s K3_PC, (s+1) K3_PC) into ring positions cell_pos[cell] (< k3_rc; a
+  // position is reused once the last slot fed by its matrix has been emitted; halo_begin[s] = first step a CTA that
+  // starts emitting at step s must recompute to have every live matrix in its ring) and then
   // emits the CSR slots whose last contributing cell lies in that panel, from three lists (each ascending in n):
   //   em1[em_ptr[s] ..)            one contribution, weight 1:   word = ring offset << K3_NBITS | (n - em_base[s])
   //   em4[em_ptr[S1 + s] ..)       2..4 contributions, all weight 1: {n - base, off0 | off1 << 16, off2 | off3 << 16, 0}
@@ -46,7 +48,7 @@ struct HostGrid {
   // with S1 = k3_nsteps + 1.  k3_rc == 0: no ring schedule (ring too large for shared memory or offsets too wide
   // for the packed words), the slot-gather kernel is used for this grid.
   int k3_rc = 0, k3_nsteps = 0;
-  std::vector<int> em_ptr, em_base, emg, as_roff;
+  std::vector<int> em_ptr, em_base, emg, as_roff, cell_pos, halo_begin;
   std::vector<unsigned> em1, em4;
   // apply gather: dof i receives sum of ap_w * r_cell[a], ap_code = cell*nb + a
   std::vector<int> ap_ptr, ap_code;

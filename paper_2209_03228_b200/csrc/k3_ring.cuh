@@ -41,6 +41,7 @@ struct K3Grid {  // device copy of one grid's K3 schedule (host_setup.hpp, "K3 r
   const uint4* em4;
   const int *as_ptr, *as_roff;
   const double* as_w;
+  const int *cell_pos, *halo_begin;
 };
 
 struct K3Species {
@@ -71,7 +72,7 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
   const int nsteps = g->nsteps, rc = g->rc, n_cells = g->n_cells, n1 = g->n1, nq = g->nq;
   const int s_lo = (int)((long long)seg * nsteps / nseg), s_hi = (int)((long long)(seg + 1) * nsteps / nseg);
   if (s_lo >= s_hi) return;
-  const int s_begin = max(0, s_lo - (rc / K3_PC - 1));
+  const int s_begin = g->halo_begin[s_lo];
 
   double* zero_pad = ring + rc * K3_RS;
   double* sfrag = zero_pad + 8;
@@ -92,6 +93,8 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
 
   // this lane's quadrature-point data of the warp's cells, fetched one step ahead of its use
   double wv[K3_CPW][6], sc[K3_CPW][2];
+  int pos[K3_CPW];
+  const int* __restrict__ cell_pos = g->cell_pos;
   auto fetch = [&](int s) {
 #pragma unroll
     for (int u = 0; u < K3_CPW; ++u) {
@@ -104,6 +107,7 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
       for (int k = 0; k < 5; ++k) wv[u][1 + k] = dk[k * sp.n_ip + ip];
       sc[u][0] = cell_sr[ok ? cell : 0];
       sc[u][1] = cell_sz[ok ? cell : 0];
+      pos[u] = cell_pos[ok ? cell : 0];
     }
   };
   fetch(s_begin);
@@ -156,7 +160,7 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
 #pragma unroll
             for (int nt2 = 0; nt2 < 2; ++nt2) dmma884(o[mt2][nt2][0], o[mt2][nt2][1], a, y[nt2][ks >> 1][ks & 1]);
           }
-        double* dst = ring + (cell % rc) * K3_RS;
+        double* dst = ring + pos[u] * K3_RS;
 #pragma unroll
         for (int mt2 = 0; mt2 < 2; ++mt2)
 #pragma unroll

@@ -248,6 +248,8 @@ int build_device_side(landau_ctx* ctx) {
         rc = rc ? rc : upload(ctx, h.em1, &d.em1);
         rc = rc ? rc : upload(ctx, h.em4, &em4);
         rc = rc ? rc : upload(ctx, h.as_roff, &d.as_roff);
+        rc = rc ? rc : upload(ctx, h.cell_pos, &d.cell_pos);
+        rc = rc ? rc : upload(ctx, h.halo_begin, &d.halo_begin);
         d.em4 = reinterpret_cast<const uint4*>(em4);
         if (rc) return rc;
       }
@@ -703,10 +705,11 @@ int landau_jacobian(landau_ctx* ctx, const double* batch_f_dev, int batch, doubl
     if (int rc = run_coefficients(ctx, batch_f_dev, b0, nbc, st)) return rc;
     double* vals = out_csr_vals_dev + (long long)b0 * ctx->v_stride;
     if (ctx->k3_nspec && ctx->assembly_kernel != 1) {
-      // enough CTAs for ~2 waves of 3 CTAs/SM; cell segments (with a recomputed halo) when the batch is small
-      const int ctas = nbc * ctx->k3_nspec;
+      // at least one wave of 3 CTAs per SM; the cell range is cut into segments (each with a recomputed halo) only
+      // when the batch alone gives fewer blocks than that
+      const int ctas = nbc * ctx->k3_nspec, want = 3 * ctx->n_sm;
       int nseg = 1;
-      if (ctas < 888) nseg = std::max(1, std::min(ctx->k3_min_steps, (888 + ctas - 1) / ctas));
+      if (ctas < want) nseg = std::max(1, std::min(ctx->k3_min_steps, (want + ctas - 1) / ctas));
       k3_ring<<<ctas * nseg, K3_THREADS, ctx->k3_smem, st>>>(ctx->d_k3grid, ctx->d_k3spec, ctx->k3_nspec, nseg,
                                                              ctx->d_k3frag, ctx->DK, ctx->dk_stride, inv_dt, vals,
                                                              ctx->v_stride);
