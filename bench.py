@@ -261,8 +261,12 @@ def run_ours(args):
             Bn.landau_jacobian_host(L.ctx, f_host, B, cfg["dt"], out_host)  # synchronous
         torch.cuda.synchronize()
         t_e2e = sharding.max_over_ranks((time.perf_counter() - t0) * 1e3, world, dev) / n_e2e
-        if not np.array_equal(out_host[0].numpy(), out_dev[0].cpu().numpy()) and (args.steps - 1) & 1 == 0:
-            raise SystemExit("bench sanity failed: host-buffer path differs from device path")
+        # same values up to summation order: the host path runs the batch in pieces, and the persistent K2 cuts the
+        # source range of a few tiles at piece-dependent places (K2 stream mode)
+        if (args.steps - 1) & 1 == 0:
+            a, b = out_host[0].numpy(), out_dev[0].cpu().numpy()
+            if not np.linalg.norm(a - b) <= 1e-13 * np.linalg.norm(b):
+                raise SystemExit("bench sanity failed: host-buffer path differs from device path")
         e2e = {"value": world * B / (t_e2e * 1e-3), "unit": UNIT, "ms_per_step": t_e2e,
                "h2d_bytes_per_step": int(f_host.numel() * 8), "d2h_bytes_per_step": int(out_host.numel() * 8),
                "steps": n_e2e, "api": "landau_jacobian_host (pinned host buffers)"}

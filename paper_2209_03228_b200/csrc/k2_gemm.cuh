@@ -50,6 +50,7 @@ struct K2G {
   static constexpr int STAGE_DOUBLES = 3 * TC * K2G_TJ;
   static constexpr int A_DOUBLES = 5 * (TI / 8) * 4 * 32;  // one buffer
   static constexpr int PAIRS_PER_THREAD = TI * K2G_TJ / NTHREADS;
+  static constexpr int ACC_PER_THREAD = WI_T * WC_T * 10;
   static constexpr int TAB_DOUBLES = 4 * LANDAU_ELLIP_TAB_BINADES * (LANDAU_ELLIP_TAB_DEG + 1) * 4;
   static constexpr int XY_DOUBLES = 4 * 2 * K2G_TJ;  // ring of four source-tile coordinate blocks (r[16], z[16])
   static constexpr size_t SMEM_BYTES =
@@ -62,7 +63,8 @@ template <int WI_T, int WC_T, int WGI, int WGC, int NST>
 __global__ void __launch_bounds__(32 * WGI * WGC, 1)
 k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, int n_i, int j0, int njt,
               const double* __restrict__ F, int ncols, double* __restrict__ G, long long g_split_stride, int gcol0,
-              int stream_itiles, int stream_tiles) {
+              int stream_itiles, int stream_tiles, double* __restrict__ part_buf, int part_stride,
+              int* __restrict__ part_count) {
   using C = K2G<WI_T, WC_T, WGI, WGC, NST>;
   extern __shared__ __align__(128) double smem_g[];
   double* smem = smem_g;
@@ -76,16 +78,19 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
   const int wi = warp / WGC, wc = warp - wi * WGC;
   const int gq = lane >> 2, tq = lane & 3;
   // Work of this CTA.  Grid mode (stream_tiles == 0): one segment = tile (blockIdx.x, blockIdx.y), source tiles of
-  // j-split blockIdx.z, plain stores into split plane blockIdx.z.  Stream mode: gridDim.x persistent CTAs share
-  // stream_tiles x njt (tile, source tile) steps evenly (tiles ordered column tile slowest); a CTA's range is cut at
-  // tile boundaries into segments; a segment that covers its whole tile is stored, a partial one is ADDED into the
-  // zeroed G (at most two partial segments per tile when a CTA's share is at least one tile, so the sum is
-  // order-independent).
+  // j-split blockIdx.z, plain stores into split plane blockIdx.z.
+  // Stream mode: P = gridDim.x persistent CTAs, tiles ordered column tile slowest.  CTA p first takes the whole tiles
+  // p, p + P, .. of the q = T / P full waves (resident CTAs walk the same F column tile in step: L2 reuse as in grid
+  // mode); the r = T mod P tiles of the last, partial wave are cut evenly: their r * njt source-tile steps are shared
+  // by all P CTAs.  A CTA that holds only part of a tile dumps its accumulators to `part_buf`; the CTA that arrives
+  // last at the tile's counter adds the parts IN PART ORDER and stores the tile (deterministic, no atomics on G).
   long long w0, w1;
+  int seg_k = 0, seg_q = 0;
   if (stream_tiles) {
-    const long long W = (long long)stream_tiles * njt;
-    w0 = W * blockIdx.x / gridDim.x;
-    w1 = W * (blockIdx.x + 1) / gridDim.x;
+    seg_q = stream_tiles / (int)gridDim.x;
+    const long long R = (long long)(stream_tiles - seg_q * (int)gridDim.x) * njt;
+    w0 = R * blockIdx.x / gridDim.x;
+    w1 = R * (blockIdx.x + 1) / gridDim.x;
   } else {
     const int per = (njt + gridDim.z - 1) / gridDim.z;
     const int ta = blockIdx.z * per, tb = min(ta + per, njt);
@@ -134,10 +139,22 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
   do {
   int it, ct, t0, nt, plane;
   bool whole;
+  int rem_tile = -1;  // index of a partial-wave tile held in part
   if (stream_tiles) {
-    const int tile = (int)(w0 / njt);
-    t0 = (int)(w0 - (long long)tile * njt);
-    nt = (int)min((long long)(njt - t0), w1 - w0);
+    int tile;
+    if (seg_k < seg_q) {
+      tile = seg_k * (int)gridDim.x + (int)blockIdx.x;
+      ++seg_k;
+      t0 = 0;
+      nt = njt;
+    } else {
+      const int tr = (int)(w0 / njt);
+      tile = seg_q * (int)gridDim.x + tr;
+      t0 = (int)(w0 - (long long)tr * njt);
+      nt = (int)min((long long)(njt - t0), w1 - w0);
+      w0 += nt;
+      if (nt < njt) rem_tile = tr;
+    }
     ct = tile / stream_itiles;
     it = tile - ct * stream_itiles;
     plane = 0;
@@ -149,8 +166,8 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
     nt = (int)(w1 - w0);
     plane = blockIdx.z;
     whole = true;
+    w0 += nt;
   }
-  w0 += nt;
   const int i0 = it * C::TI;
   const double* Fct = F + (long long)ct * njt * C::STAGE_DOUBLES;
   if (tid == 0) {
@@ -246,6 +263,54 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
     }
   }
 
+  if (!whole) {
+    // Partial tile: parts are numbered by CTA.  first = lowest CTA whose share [lo(p), lo(p+1)) of the partial wave
+    // meets this tile, lo(p) = floor(R p / P).
+    const long long R = (long long)(stream_tiles - seg_q * (int)gridDim.x) * njt, P = gridDim.x;
+    const long long tb = (long long)rem_tile * njt, te = tb + njt;
+    int first = (int)(tb * P / R);
+    while (first > 0 && R * first / P > tb) --first;
+    while (R * (first + 1) / P <= tb) ++first;
+    int lastp = (int)((te - 1) * P / R);
+    while (lastp + 1 < (int)P && R * (lastp + 1) / P < te) ++lastp;
+    while (R * lastp / P >= te) --lastp;
+    const int nparts = lastp - first + 1, mypart = (int)blockIdx.x - first;
+    double* mine = part_buf + ((long long)rem_tile * part_stride + mypart) * (C::ACC_PER_THREAD * C::NTHREADS) + tid;
+    {
+      int e = 0;
+#pragma unroll
+      for (int x = 0; x < WI_T; ++x)
+#pragma unroll
+        for (int n = 0; n < WC_T; ++n)
+#pragma unroll
+          for (int k = 0; k < 5; ++k)
+#pragma unroll
+            for (int h = 0; h < 2; ++h, ++e) mine[e * C::NTHREADS] = acc[x][n][k][h];
+    }
+    __threadfence();
+    __syncthreads();
+    __shared__ int s_last;
+    if (tid == 0) s_last = atomicAdd(part_count + rem_tile, 1) == nparts - 1;
+    __syncthreads();
+    whole = s_last;
+    if (whole) {  // every part is visible: add them in part order
+      __threadfence();
+      const double* src = part_buf + (long long)rem_tile * part_stride * (C::ACC_PER_THREAD * C::NTHREADS) + tid;
+      int e = 0;
+#pragma unroll
+      for (int x = 0; x < WI_T; ++x)
+#pragma unroll
+        for (int n = 0; n < WC_T; ++n)
+#pragma unroll
+          for (int k = 0; k < 5; ++k)
+#pragma unroll
+            for (int h = 0; h < 2; ++h, ++e) {
+              double sum = 0.0;
+              for (int q = 0; q < nparts; ++q) sum += __ldcg(src + ((long long)q * C::ACC_PER_THREAD + e) * C::NTHREADS);
+              acc[x][n][k][h] = sum;
+            }
+    }
+  }
   // C fragment: row gq (field point), columns 2 tq, 2 tq + 1
 #pragma unroll
   for (int x = 0; x < WI_T; ++x) {
@@ -255,21 +320,16 @@ k2_inner_gemm(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         const int col = ct * C::TC + (wc * WC_T + n) * 8 + 2 * tq + h;
-        if (i < n_i && col < ncols) {
+        if (whole && i < n_i && col < ncols) {
           double* dst = G + plane * g_split_stride + ((long long)(gcol0 + col) * 5) * n_i + i;
 #pragma unroll
-          for (int k = 0; k < 5; ++k) {
-            if (whole)
-              dst[(long long)k * n_i] = acc[x][n][k][h];
-            else
-              atomicAdd(dst + (long long)k * n_i, acc[x][n][k][h]);
-          }
+          for (int k = 0; k < 5; ++k) dst[(long long)k * n_i] = acc[x][n][k][h];
         }
 #pragma unroll
         for (int k = 0; k < 5; ++k) acc[x][n][k][h] = 0.0;
       }
   }
-  } while (w0 < w1);  // segments (an empty j-split still stores its zeros)
+  } while (seg_k < seg_q || w0 < w1);  // segments (an empty j-split still stores its zeros)
 }
 
 }  // namespace landau

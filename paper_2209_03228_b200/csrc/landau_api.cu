@@ -60,8 +60,8 @@ struct landau_ctx {
   size_t k3_smem = 0;
   std::vector<char> k3_ring_ok;  // per species
   // scratch (grown on demand)
-  double *F = nullptr, *Gp = nullptr, *DK = nullptr, *FL = nullptr;
-  size_t F_cap = 0, Gp_cap = 0, DK_cap = 0, FL_cap = 0;
+  double *F = nullptr, *Gp = nullptr, *DK = nullptr, *FL = nullptr, *part_buf = nullptr;
+  size_t F_cap = 0, Gp_cap = 0, DK_cap = 0, FL_cap = 0, part_cap = 0;
   double *stage_in = nullptr, *stage_out = nullptr;
   cudaStream_t copy_stream = nullptr;  // D2H copies of landau_jacobian_host, overlapped with the next piece's kernels
   std::vector<cudaEvent_t> copy_ev;
@@ -397,19 +397,24 @@ int launch_gemm_t(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int ns
   const int n_it = (ctx->n_i_pad + C::TI - 1) / C::TI, n_ct = (ncols + C::TC - 1) / C::TC;
   const bool stream = ctx->stream_k && nsplit == 1 && n_it * n_ct >= ctx->n_sm && (n_it * n_ct) % ctx->n_sm != 0;
   if (stream) {
-    // persistent CTAs, one per SM, share the (tile, source tile) steps evenly: no partial last wave.  Partial tiles are
-    // added into G, which is zeroed first.
-    CUDA_TRY(ctx, cudaMemsetAsync(ctx->Gp + (long long)gcol0 * 5 * ctx->n_i_pad, 0,
-                                  sizeof(double) * (size_t)ncols * 5 * ctx->n_i_pad, st));
-    k2_inner_gemm<WI_T, WC_T, WGI, WGC, NST><<<dim3(ctx->n_sm, 1, 1), C::NTHREADS, C::SMEM_BYTES, st>>>(
+    // persistent CTAs, one per SM: whole tiles for the full waves, the tiles of the last partial wave cut evenly over all
+    // CTAs; parts of a cut tile meet in part_buf and are added in part order by the last CTA to arrive (k2_gemm.cuh)
+    const int T = n_it * n_ct, P = ctx->n_sm, r = T % P;
+    const int part_stride = (P + r - 1) / r + 2;  // parts per cut tile, upper bound
+    const size_t per_part = (size_t)C::ACC_PER_THREAD * C::NTHREADS;
+    if (int rc = grow(ctx, &ctx->part_buf, &ctx->part_cap, (size_t)r * part_stride * per_part + (size_t)(P + 1) / 2 + 1, false))
+      return rc;
+    int* part_count = reinterpret_cast<int*>(ctx->part_buf + (size_t)r * part_stride * per_part);
+    CUDA_TRY(ctx, cudaMemsetAsync(part_count, 0, sizeof(int) * P, st));
+    k2_inner_gemm<WI_T, WC_T, WGI, WGC, NST><<<dim3(P, 1, 1), C::NTHREADS, C::SMEM_BYTES, st>>>(
         ctx->d_ip_r, ctx->d_ip_z, ctx->n_i_pad, gr.j0, gr.nj_pad / K2G_TJ, ctx->F + gr.f_off, ncols, ctx->Gp,
-        split_stride, gcol0, n_it, n_it * n_ct);
+        split_stride, gcol0, n_it, T, ctx->part_buf, part_stride, part_count);
     return LANDAU_OK;
   }
   dim3 grid(n_it, n_ct, nsplit);
   k2_inner_gemm<WI_T, WC_T, WGI, WGC, NST><<<grid, C::NTHREADS, C::SMEM_BYTES, st>>>(
       ctx->d_ip_r, ctx->d_ip_z, ctx->n_i_pad, gr.j0, gr.nj_pad / K2G_TJ, ctx->F + gr.f_off, ncols, ctx->Gp, split_stride,
-      gcol0, 0, 0);
+      gcol0, 0, 0, nullptr, 0, nullptr);
   return LANDAU_OK;
 }
 
@@ -426,7 +431,7 @@ int kern_ti(int kern) { return kern == 3 ? K2Big::TI : kern == 4 ? K2Wide::TI : 
 // tensor tile shared by the CTA (32 x 128 / 16 x 256 CTA tile)
 int pick_kernel(const landau_ctx* ctx, int ncols) {
   if (ctx->inner_kernel) return ctx->inner_kernel;
-  return ncols > 128 ? 4 : ncols > 64 ? 3 : (ncols >= 8 ? 2 : 1);
+  return ncols > 128 ? 4 : ncols > 96 ? 3 : (ncols >= 8 ? 2 : 1);  // crossovers measured on config 2 (N = 4096)
 }
 
 // stages a1..a2b for batch entries [b0, b0+nbc): leaves D,K in ctx->DK
@@ -637,7 +642,7 @@ void landau_destroy(landau_ctx* ctx) {
     cudaDeviceSynchronize();
   }
   for (void* p : ctx->allocs) cudaFree(p);
-  for (double* p : {ctx->F, ctx->Gp, ctx->DK, ctx->FL, ctx->stage_in, ctx->stage_out})
+  for (double* p : {ctx->F, ctx->Gp, ctx->DK, ctx->FL, ctx->part_buf, ctx->stage_in, ctx->stage_out})
     if (p) cudaFree(p);
   for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
   for (cudaEvent_t e : ctx->copy_ev) cudaEventDestroy(e);
