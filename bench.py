@@ -290,8 +290,10 @@ def run_ours(args):
         k3_ms = stage[3] / args.steps
         csr_bytes = float(B) * L.csr_stride * 8
         dk_bytes = float(B) * L.dk_stride * 8
+        traffic = ncu_traffic(workload_name(cfg, B))
         roofline = {"kernel": "K2 inner integral (k2_inner_*)", "bound": "alu", "achieved": achieved, "peak": peak,
-                    "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                    "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic.get("k2_dram_bytes_per_launch"),
+                    "traffic_source": traffic.get("source"),
                     "peak_source": "in-process FP64 probe (DFMA %.2f, DMMA m8n8k4 %.2f TFLOP/s), max taken"
                                    % (peak_dfma, peak_dmma),
                     "k2_ms_per_step": k2_ms, "share_of_step": k2_ms / (sum(stage) / args.steps),
@@ -299,7 +301,8 @@ def run_ours(args):
                     "assembly": {"kernel": "K3 element matrices + assembly (k3_*)", "bound": "hbm",
                                  "achieved": (csr_bytes + dk_bytes) / (k3_ms * 1e-3) / 1e9, "peak": hbm_peak(),
                                  "unit": "GB/s", "frac": (csr_bytes + dk_bytes) / (k3_ms * 1e-3) / 1e9 / hbm_peak(),
-                                 "k3_ms_per_step": k3_ms, "algorithmic_bytes_per_step": csr_bytes + dk_bytes}}
+                                 "k3_ms_per_step": k3_ms, "algorithmic_bytes_per_step": csr_bytes + dk_bytes,
+                                 "traffic": traffic.get("k3_dram_bytes_per_launch")}}
         cpu = None
         if not args.no_cpu_baseline and world == 1:
             v, n_done, threads, times = oracle_sample(cfg, args.cpu_seconds)
@@ -324,6 +327,17 @@ def run_ours(args):
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
+
+
+def ncu_traffic(workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of this
+    workload (profiles/r1_traffic_v4.json.txt); empty when the workload is another one (traffic = null)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r1_traffic_v4.json.txt")) as fh:
+            t = json.load(fh)
+        return t if workload.startswith(t["workload"]) else {}
+    except (OSError, KeyError, ValueError):
+        return {}
 
 
 def hbm_peak():
