@@ -122,6 +122,30 @@ int landau_jacobian(landau_ctx* ctx, const double* batch_f_dev, int batch, doubl
  *   out_rhs_dev : dev, same layout as batch_f_dev. */
 int landau_apply(landau_ctx* ctx, const double* batch_f_dev, int batch, double* out_rhs_dev, void* cuda_stream);
 
+/* Batched CSR product  y = A x  for every (entry, species) block of a value array in the layout of out_csr_vals_dev
+ * (pattern of the block's grid); x_dev, y_dev in the layout of batch_f_dev.  With the values of M/dt - J and of -J
+ * (dt = +inf) it gives the right-hand side (M/dt) f of the implicit step. */
+int landau_spmv(landau_ctx* ctx, const double* csr_vals_dev, const double* x_dev, int batch, double* y_dev,
+                void* cuda_stream);
+
+/* Batched linear solve  A x = b  of every (entry, species) block, the step that follows the Jacobian construction in
+ * the implicit advance (sec. 3.2, 127): TFQMR with Jacobi preconditioning, one system per thread
+ * block, the whole batch in one launch (reading A18 for the iteration the paper only cites).
+ *   csr_vals_dev : dev, [batch][species a][nnz[grid(a)]]      e.g. the output of landau_jacobian
+ *   rhs_dev      : dev, [batch][species a][n_dof[grid(a)]]
+ *   x_dev        : dev, same layout; ON INPUT the initial guess (zeros are fine), on output the solution
+ *   rtol         : a run stops when the TFQMR residual bound  tau sqrt(m)  <=  rtol * || D^-1 (b - A x0) ||; the true
+ *                  Jacobi-scaled residual is then computed and, if it misses the tolerance (the recursive bound drifts
+ *                  on ill-conditioned blocks), the iteration restarts from the current x (at most 4 restarts)
+ *   max_it       : at most 2 max_it half-steps (max_it products with A beyond the first)
+ *   iters_dev    : dev, [batch][species] or NULL: half-steps taken; negative (-m-1) when the tolerance was not reached
+ *                  in 2 max_it half-steps or the iteration broke down (x then holds the last iterate)
+ *   relres_dev   : dev, [batch][species] or NULL: last residual norm (true if converged, else the bound) relative to
+ *                  the initial Jacobi-scaled residual
+ * Asynchronous on cuda_stream.  Zero diagonal entries are not supported (Jacobi). */
+int landau_solve(landau_ctx* ctx, const double* csr_vals_dev, const double* rhs_dev, int batch, double rtol, int max_it,
+                 double* x_dev, int* iters_dev, double* relres_dev, void* cuda_stream);
+
 /* Host-buffer convenience: same as landau_jacobian / landau_apply with HOST pointers (pageable or pinned); the
  * library stages the copies in internal device buffers and synchronises before returning.  landau_jacobian_host
  * cuts the batch into pieces and copies the CSR values of a finished piece to the host on a second (internal)

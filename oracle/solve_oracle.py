@@ -42,8 +42,10 @@ def residual(rowptr, colidx, vals, x, rhs):
     return np.linalg.norm(rhs - csr_matvec(rowptr, colidx, vals, x)) / np.linalg.norm(rhs)
 
 
-def tfqmr_reference(rowptr, colidx, vals, rhs, rtol, max_it):
-    """TFQMR on diag(A)^{-1} A x = diag(A)^{-1} b from x0 = 0.  Returns (x, half-steps m done, converged)."""
+def tfqmr_reference(rowptr, colidx, vals, rhs, rtol, max_it, max_restarts=4):
+    """TFQMR on diag(A)^{-1} A x = diag(A)^{-1} b from x0 = 0.  A run that meets the bound  tau sqrt(k) <= rtol ||r0||
+    is checked against the true scaled residual and restarted from the current x if that misses the tolerance (the
+    tolerance stays relative to the first residual).  Returns (x, half-steps done, converged)."""
     n = len(rhs)
     diag = np.array([vals[rowptr[i]:rowptr[i + 1]][list(colidx[rowptr[i]:rowptr[i + 1]]).index(i)] for i in range(n)])
 
@@ -51,46 +53,56 @@ def tfqmr_reference(rowptr, colidx, vals, rhs, rtol, max_it):
         return csr_matvec(rowptr, colidx, vals, u) / diag
 
     x = np.zeros(n)
-    r0 = rhs / diag
-    w = r0.copy()
-    u = r0.copy()
-    rs = r0.copy()
-    au = op(u)
-    v = au.copy()
-    d = np.zeros(n)
-    tau = np.linalg.norm(r0)
-    r0norm = tau
-    theta = eta = 0.0
-    rho = float(rs @ r0)
-    alpha = 0.0
-    if r0norm == 0.0:
-        return x, 0, True
-    for m in range(2 * max_it):
-        if m % 2 == 0:
-            sigma = float(rs @ v)
-            if sigma == 0.0:
-                return x, m, False
-            alpha = rho / sigma
-        w = w - alpha * au
-        d = u + (theta * theta * eta / alpha) * d
-        theta = np.linalg.norm(w) / tau
-        c = 1.0 / np.sqrt(1.0 + theta * theta)
-        tau = tau * theta * c
-        eta = c * c * alpha
-        x = x + eta * d
-        if tau * np.sqrt(m + 1.0) <= rtol * r0norm:
-            return x, m + 1, True
-        if m % 2 == 0:
-            u = u - alpha * v
-            au = op(u)
-        else:
-            rho_new = float(rs @ w)
-            if rho == 0.0:
-                return x, m + 1, False
-            beta = rho_new / rho
-            rho = rho_new
-            u_new = w + beta * u
-            au_new = op(u_new)
-            v = au_new + beta * (au + beta * v)
-            u, au = u_new, au_new
-    return x, 2 * max_it, False
+    m = 0
+    r0norm = None
+    for restart in range(max_restarts + 1):
+        r = (rhs - csr_matvec(rowptr, colidx, vals, x)) / diag
+        tau = np.linalg.norm(r)
+        if r0norm is None:
+            r0norm = tau
+        if tau <= rtol * r0norm:
+            return x, m, True
+        if m >= 2 * max_it:
+            return x, m, False
+        w, u, rs = r.copy(), r.copy(), r.copy()
+        au = op(u)
+        v = au.copy()
+        d = np.zeros(n)
+        theta = eta = alpha = 0.0
+        rho = float(rs @ r)
+        bound_met = False
+        k = 0
+        while not bound_met and m < 2 * max_it:
+            even = k % 2 == 0
+            if even:
+                sigma = float(rs @ v)
+                if sigma == 0.0:
+                    return x, m, False
+                alpha = rho / sigma
+            w = w - alpha * au
+            d = u + (theta * theta * eta / alpha) * d
+            theta = np.linalg.norm(w) / tau
+            c = 1.0 / np.sqrt(1.0 + theta * theta)
+            tau = tau * theta * c
+            eta = c * c * alpha
+            x = x + eta * d
+            m += 1
+            if tau * np.sqrt(k + 1.0) <= rtol * r0norm:
+                bound_met = True
+            elif even:
+                u = u - alpha * v
+                au = op(u)
+            else:
+                rho_new = float(rs @ w)
+                if rho == 0.0:
+                    return x, m, False
+                beta = rho_new / rho
+                rho = rho_new
+                u_new = w + beta * u
+                au_new = op(u_new)
+                v = au_new + beta * (au + beta * v)
+                u, au = u_new, au_new
+            k += 1
+        if not bound_met:
+            return x, m, False
+    return x, m, False

@@ -18,7 +18,7 @@ STATUS = {0: "LANDAU_OK", -1: "LANDAU_INVALID_ARG", -2: "LANDAU_UNSUPPORTED", -3
 
 # every symbol include/landau.h declares (tests check that the library exports all of them)
 SYMBOLS = ["landau_create", "landau_destroy", "landau_sizes", "landau_dof_coords", "landau_ip_table",
-           "landau_csr_pattern", "landau_csr_pattern_host", "landau_jacobian", "landau_apply", "landau_jacobian_host",
+           "landau_csr_pattern", "landau_csr_pattern_host", "landau_jacobian", "landau_apply", "landau_spmv", "landau_solve", "landau_jacobian_host",
            "landau_apply_host", "landau_last_coefficients", "landau_tensor_eval", "landau_ellip_eval",
            "landau_fp64_probe", "landau_launch_count", "landau_is_separable", "landau_set_timing", "landau_last_stage_ms",
            "landau_set_inner_kernel", "landau_set_assembly_kernel", "landau_assembly_info", "landau_set_batch_chunk", "landau_last_error"]
@@ -155,6 +155,18 @@ def landau_apply(ctx, batch_f, batch, out_rhs, stream=None):
     _check(load().landau_apply(ctx, _dev_ptr(batch_f), C.c_int(batch), _dev_ptr(out_rhs), _stream(stream)), ctx)
 
 
+def landau_spmv(ctx, csr_vals, x, batch, y, stream=None):
+    _check(load().landau_spmv(ctx, _dev_ptr(csr_vals), _dev_ptr(x), C.c_int(batch), _dev_ptr(y), _stream(stream)), ctx)
+
+
+def landau_solve(ctx, csr_vals, rhs, batch, rtol, max_it, x, iters=None, relres=None, stream=None):
+    """x: initial guess in, solution out.  iters (int32 CUDA tensor [batch, S]) / relres (float64) optional."""
+    ip = C.c_void_p(iters.data_ptr()) if iters is not None else None
+    rp = C.c_void_p(relres.data_ptr()) if relres is not None else None
+    _check(load().landau_solve(ctx, _dev_ptr(csr_vals), _dev_ptr(rhs), C.c_int(batch), C.c_double(rtol), C.c_int(max_it),
+                               _dev_ptr(x), ip, rp, _stream(stream)), ctx)
+
+
 def _host_ptr(a):
     """numpy array or CPU (pinned) torch tensor -> pointer."""
     if isinstance(a, np.ndarray):
@@ -285,6 +297,22 @@ class Landau:
             out = torch.empty((B, self.f_stride), dtype=torch.float64, device=batch_f.device)
         landau_apply(self.ctx, batch_f, B, out, stream)
         return out
+
+    def spmv(self, csr_vals, x, stream=None):
+        import torch
+        y = torch.empty_like(x)
+        landau_spmv(self.ctx, csr_vals, x, x.shape[0], y, stream)
+        return y
+
+    def solve(self, csr_vals, rhs, rtol=1e-10, max_it=200, x0=None, stream=None):
+        """Returns (x, half-steps [B, S] int32, residual bounds [B, S])."""
+        import torch
+        B = rhs.shape[0]
+        x = torch.zeros_like(rhs) if x0 is None else x0.clone()
+        iters = torch.zeros((B, self.S), dtype=torch.int32, device=rhs.device)
+        relres = torch.zeros((B, self.S), dtype=torch.float64, device=rhs.device)
+        landau_solve(self.ctx, csr_vals, rhs, B, rtol, max_it, x, iters, relres, stream)
+        return x, iters, relres
 
     def last_coefficients(self, batch):
         """list over species of arrays [batch, 5, n_ip]."""

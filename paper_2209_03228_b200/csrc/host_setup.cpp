@@ -313,6 +313,10 @@ int build_grid(const landau_grid_desc& d, const HostTables& t, HostGrid* g, std:
     g->rowptr[I + 1] = (int)g->colidx.size();
   }
   g->nnz = (int)g->colidx.size();
+  g->diag.resize(g->n_dof);
+  for (int I = 0; I < g->n_dof; ++I)
+    g->diag[I] = (int)(std::lower_bound(g->colidx.begin() + g->rowptr[I], g->colidx.begin() + g->rowptr[I + 1], I) -
+                       g->colidx.begin());
   // ---- gather tables -----------------------------------------------------------------------------------------------
   {
     std::vector<int> count(g->nnz, 0);

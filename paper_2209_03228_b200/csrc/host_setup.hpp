@@ -31,8 +31,8 @@ struct HostGrid {
   // element-node -> dof expansion (rows of P_e): entries en_ptr[cell*nb+a] .. en_ptr[cell*nb+a+1]
   std::vector<int> en_ptr, en_dof;
   std::vector<double> en_w;
-  // CSR pattern
-  std::vector<int> rowptr, colidx;
+  // CSR pattern; diag[i] = position of the diagonal entry of row i in colidx / the value array
+  std::vector<int> rowptr, colidx, diag;
   // assembly gather: CSR slot n receives sum over entries as_ptr[n]..as_ptr[n+1] of as_w * A_cell[a][c],
   // as_code = cell*nb*nb + a*nb + c
   std::vector<int> as_ptr, as_code;

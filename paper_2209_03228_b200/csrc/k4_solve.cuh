@@ -1,0 +1,198 @@
+// k4_solve.cuh -- batched linear solve of the shifted systems the Jacobian construction produces:
+//
+//     (M/dt - J[f]) x = b      one system per (batch entry, species)
+//
+// TFQMR (Freund; Saad Alg. 7.8) with left Jacobi preconditioning, the whole iteration of one system in ONE CTA, one
+// launch for the batch (the paper's batched solver: "the entire solve requires a single kernel launch,
+// each solve can run asynchronously, exiting the kernel as soon as it converges").  The seven Krylov vectors of a
+// system live in shared memory (7 n doubles: 205 KB for the 3655 unknowns of the 14 x 28 Q3 grid, one CTA per SM), x
+// in global memory; the CSR values of the systems in flight (148 x 0.7 MB) stay L2-resident over the iterations, the
+// pattern (rowptr / colidx / diagonal positions) is shared by all systems of a grid.  SpMV: 8 lanes per row (24 nonzeros
+// per row on Q3 grids), rows contiguous in the value array.  Systems whose vectors do not fit in shared memory take
+// the same code with the vectors in a global workspace.
+#pragma once
+
+namespace landau {
+
+struct K4Grid {
+  int n, nnz;
+  const int *rowptr, *colidx, *diag;  // diag[i] = position of a_ii in the row-major value array
+};
+
+struct K4Species {
+  int grid;
+  long long f_off, v_off;
+};
+
+constexpr int K4_THREADS = 512;
+constexpr int K4_NVEC = 7;
+constexpr int K4_MAX_RESTARTS = 4;
+
+// sums of two values over the CTA (deterministic order), result in every thread
+__device__ __forceinline__ void k4_block_sum2(double& a, double& b, double* red) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    a += __shfl_xor_sync(0xffffffffu, a, o);
+    b += __shfl_xor_sync(0xffffffffu, b, o);
+  }
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  __syncthreads();  // red may still be read from the previous reduction
+  if (lane == 0) {
+    red[2 * warp] = a;
+    red[2 * warp + 1] = b;
+  }
+  __syncthreads();
+  a = 0.0;
+  b = 0.0;
+#pragma unroll
+  for (int wv = 0; wv < K4_THREADS / 32; ++wv) {
+    a += red[2 * wv];
+    b += red[2 * wv + 1];
+  }
+}
+
+// y_i = s_i * sum_k a_ik in_k  (s = 1 / a_ii: left Jacobi), 8 lanes per row
+template <class Out>
+__device__ __forceinline__ void k4_spmv(const K4Grid& g, const double* __restrict__ vals, const double* in, Out out) {
+  const int l8 = threadIdx.x & 7, sub = (threadIdx.x & 31) >> 3;
+  // warp-uniform trip count: the shuffles below need all 32 lanes, rows past the end contribute nothing
+  for (int row0 = (threadIdx.x >> 5) * 4; row0 < g.n; row0 += K4_THREADS / 8) {
+    const int row = row0 + sub;
+    const bool live = row < g.n;
+    const int k0 = live ? g.rowptr[row] : 0, k1 = live ? g.rowptr[row + 1] : 0;
+    double s = 0.0;
+    for (int k = k0 + l8; k < k1; k += 8) s = fma(__ldg(vals + k), in[g.colidx[k]], s);
+    s += __shfl_xor_sync(0xffffffffu, s, 4);
+    s += __shfl_xor_sync(0xffffffffu, s, 2);
+    s += __shfl_xor_sync(0xffffffffu, s, 1);
+    if (live && l8 == 0) out(row, s);
+  }
+}
+
+__global__ void __launch_bounds__(K4_THREADS, 1)
+k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, int n_spec, const double* __restrict__ vals,
+         long long v_stride, const double* __restrict__ rhs, long long f_stride, double* __restrict__ x, double rtol,
+         int max_it, int* __restrict__ iters, double* __restrict__ relres, double* __restrict__ ws, long long ws_stride,
+         int smem_n) {
+  extern __shared__ __align__(16) double k4_smem[];
+  double* red = k4_smem;  // [2 * warps]
+  const int sidx = blockIdx.x % n_spec, b = blockIdx.x / n_spec;
+  const K4Species sp = spec[sidx];
+  const K4Grid g = grids[sp.grid];
+  const int n = g.n, tid = threadIdx.x;
+  double* vec = n <= smem_n ? k4_smem + 2 * (K4_THREADS / 32) : ws + (long long)blockIdx.x * ws_stride;
+  double *rs = vec, *w = vec + n, *u = vec + 2 * n, *v = vec + 3 * n, *d = vec + 4 * n, *au = vec + 5 * n, *idg = vec + 6 * n;
+  const double* a = vals + (long long)b * v_stride + sp.v_off;
+  const double* bb = rhs + (long long)b * f_stride + sp.f_off;
+  double* xx = x + (long long)b * f_stride + sp.f_off;
+
+  for (int i = tid; i < n; i += K4_THREADS) idg[i] = 1.0 / a[g.diag[i]];
+  __syncthreads();
+  // TFQMR's residual bound is updated recursively and drifts away from the true residual on ill-conditioned blocks,
+  // so a converged run is CHECKED against the true (Jacobi-scaled) residual and restarted from the current x if it
+  // misses the tolerance, which stays relative to the first residual.
+  double r0norm = 0.0, tau = 0.0;
+  int m = 0, status = 0;  // 1 converged, 2 breakdown, 0 running / not converged
+  for (int restart = 0; restart <= K4_MAX_RESTARTS && !status; ++restart) {
+    // r = D^-1 (b - A x);  w = u = rs = r, d = 0
+    k4_spmv(g, a, xx, [&](int row, double s) {
+      const double r = idg[row] * (bb[row] - s);
+      rs[row] = r;
+      w[row] = r;
+      u[row] = r;
+      d[row] = 0.0;
+    });
+    __syncthreads();
+    double p0 = 0.0, p1 = 0.0;
+    for (int i = tid; i < n; i += K4_THREADS) p0 = fma(rs[i], rs[i], p0);
+    k4_block_sum2(p0, p1, red);
+    double rho = p0, theta = 0.0, eta = 0.0, alpha = 0.0;
+    tau = sqrt(p0);
+    if (restart == 0) r0norm = tau;
+    if (tau <= rtol * r0norm) {  // true residual within tolerance (also: zero right-hand side)
+      status = 1;
+      break;
+    }
+    if (m >= 2 * max_it) break;
+    k4_spmv(g, a, u, [&](int row, double s) {
+      const double t = idg[row] * s;
+      au[row] = t;
+      v[row] = t;
+    });
+    __syncthreads();
+    bool bound_met = false;
+    for (int k = 0; !bound_met && !status && m < 2 * max_it; ++k) {  // k: half-step of this run
+      const bool even = (k & 1) == 0;
+      if (even) {
+        double sg = 0.0, z = 0.0;
+        for (int i = tid; i < n; i += K4_THREADS) sg = fma(rs[i], v[i], sg);
+        k4_block_sum2(sg, z, red);
+        if (sg == 0.0) {
+          status = 2;
+          break;
+        }
+        alpha = rho / sg;
+      }
+      // w -= alpha A u;  d = u + (theta^2 eta / alpha) d;  ||w||^2 and (rs, w)
+      const double cd = theta * theta * eta / alpha;
+      double ww = 0.0, rw = 0.0;
+      for (int i = tid; i < n; i += K4_THREADS) {
+        const double wi = fma(-alpha, au[i], w[i]);
+        w[i] = wi;
+        d[i] = fma(cd, d[i], u[i]);
+        ww = fma(wi, wi, ww);
+        rw = fma(rs[i], wi, rw);
+      }
+      k4_block_sum2(ww, rw, red);
+      theta = sqrt(ww) / tau;
+      const double c = 1.0 / sqrt(1.0 + theta * theta);
+      tau = tau * theta * c;
+      eta = c * c * alpha;
+      for (int i = tid; i < n; i += K4_THREADS) xx[i] = fma(eta, d[i], xx[i]);
+      ++m;
+      if (tau * sqrt((double)(k + 1)) <= rtol * r0norm) {
+        bound_met = true;
+      } else if (even) {
+        for (int i = tid; i < n; i += K4_THREADS) u[i] = fma(-alpha, v[i], u[i]);
+        __syncthreads();
+        k4_spmv(g, a, u, [&](int row, double s) { au[row] = idg[row] * s; });
+      } else {
+        if (rho == 0.0) {
+          status = 2;
+          break;
+        }
+        const double beta = rw / rho;
+        rho = rw;
+        for (int i = tid; i < n; i += K4_THREADS) u[i] = fma(beta, u[i], w[i]);
+        __syncthreads();
+        // v = A u_new + beta (A u_old + beta v);  au = A u_new
+        k4_spmv(g, a, u, [&](int row, double s) {
+          const double t = idg[row] * s;
+          v[row] = fma(beta, fma(beta, v[row], au[row]), t);
+          au[row] = t;
+        });
+      }
+      __syncthreads();
+    }
+    if (!bound_met) break;  // out of iterations or breakdown
+  }
+  if (tid == 0) {
+    if (iters) iters[blockIdx.x] = status == 1 ? m : -m - 1;  // half-steps; negative: not converged / breakdown
+    if (relres) relres[blockIdx.x] = r0norm > 0.0 ? tau / r0norm : 0.0;  // last true residual seen (or bound)
+  }
+}
+
+// y = A x for every (entry, species) block (residual checks, right-hand sides M f / dt)
+__global__ void __launch_bounds__(K4_THREADS)
+k4_spmv_batch(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, int n_spec,
+              const double* __restrict__ vals, long long v_stride, const double* __restrict__ x, long long f_stride,
+              double* __restrict__ y) {
+  const int sidx = blockIdx.x % n_spec, b = blockIdx.x / n_spec;
+  const K4Species sp = spec[sidx];
+  const K4Grid g = grids[sp.grid];
+  double* yy = y + (long long)b * f_stride + sp.f_off;
+  k4_spmv(g, vals + (long long)b * v_stride + sp.v_off, x + (long long)b * f_stride + sp.f_off,
+          [&](int row, double s) { yy[row] = s; });
+}
+
+}  // namespace landau

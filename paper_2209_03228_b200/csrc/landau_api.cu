@@ -11,6 +11,7 @@
 #include "host_setup.hpp"
 #include "landau_kernels.cuh"
 #include "k3_ring.cuh"
+#include "k4_solve.cuh"
 
 using namespace landau;
 
@@ -59,6 +60,13 @@ struct landau_ctx {
   int k3_nspec = 0, k3_min_steps = 0;
   size_t k3_smem = 0;
   std::vector<char> k3_ring_ok;  // per species
+  // batched solve (k4_solve.cuh)
+  K4Grid* d_k4grid = nullptr;
+  K4Species* d_k4spec = nullptr;
+  int k4_max_n = 0, k4_smem_n = 0;
+  size_t k4_smem = 0;
+  double* solve_ws = nullptr;
+  size_t solve_ws_cap = 0;
   // scratch (grown on demand)
   double *F = nullptr, *Gp = nullptr, *DK = nullptr, *FL = nullptr, *part_buf = nullptr;
   size_t F_cap = 0, Gp_cap = 0, DK_cap = 0, FL_cap = 0, part_cap = 0;
@@ -276,6 +284,30 @@ int build_device_side(landau_ctx* ctx) {
     ctx->d_k3spec = const_cast<K3Species*>(tsp);
     if (ctx->k3_nspec)
       CUDA_TRY(ctx, cudaFuncSetAttribute(k3_ring, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->k3_smem));
+  }
+  // batched solve: pattern views per grid, block offsets per species
+  {
+    std::vector<K4Grid> kg(G);
+    std::vector<const int*> d_diag(G);
+    for (int g = 0; g < G; ++g) {
+      if (int rc = upload(ctx, ctx->hg[g].diag, &d_diag[g])) return rc;
+      kg[g] = K4Grid{ctx->hg[g].n_dof, ctx->hg[g].nnz, ctx->d_rowptr[g], ctx->d_colidx[g], d_diag[g]};
+      ctx->k4_max_n = std::max(ctx->k4_max_n, ctx->hg[g].n_dof);
+    }
+    std::vector<K4Species> ks(S);
+    for (int s = 0; s < S; ++s) ks[s] = K4Species{ctx->species[s].grid, ctx->f_off[s], ctx->v_off[s]};
+    const K4Grid* tg;
+    const K4Species* tsp;
+    if (int rc = upload(ctx, kg, &tg)) return rc;
+    if (int rc = upload(ctx, ks, &tsp)) return rc;
+    ctx->d_k4grid = const_cast<K4Grid*>(tg);
+    ctx->d_k4spec = const_cast<K4Species*>(tsp);
+    // Krylov vectors in shared memory when 7 n doubles fit beside the reduction scratch (227 KB per CTA on sm_100)
+    const size_t limit = 227 * 1024, fixed = 2 * (K4_THREADS / 32) * sizeof(double);
+    ctx->k4_smem_n = (int)((limit - fixed) / (K4_NVEC * sizeof(double)));
+    const int n_in_smem = std::min(ctx->k4_max_n, ctx->k4_smem_n);
+    ctx->k4_smem = fixed + (size_t)K4_NVEC * n_in_smem * sizeof(double);
+    CUDA_TRY(ctx, cudaFuncSetAttribute(k4_tfqmr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->k4_smem));
   }
   // source columns: separable nu => one group over all grids, one column per batch entry;
   // general nu => one group per grid, one column per species of the grid.
@@ -642,7 +674,7 @@ void landau_destroy(landau_ctx* ctx) {
     cudaDeviceSynchronize();
   }
   for (void* p : ctx->allocs) cudaFree(p);
-  for (double* p : {ctx->F, ctx->Gp, ctx->DK, ctx->FL, ctx->part_buf, ctx->stage_in, ctx->stage_out})
+  for (double* p : {ctx->F, ctx->Gp, ctx->DK, ctx->FL, ctx->part_buf, ctx->solve_ws, ctx->stage_in, ctx->stage_out})
     if (p) cudaFree(p);
   for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
   for (cudaEvent_t e : ctx->copy_ev) cudaEventDestroy(e);
@@ -834,6 +866,37 @@ int landau_apply_host(landau_ctx* ctx, const double* batch_f_host, int batch, do
   if (int rc = landau_apply(ctx, ctx->stage_in, batch, ctx->stage_out, cuda_stream)) return rc;
   CUDA_TRY(ctx, cudaMemcpyAsync(out_rhs_host, ctx->stage_out, n * sizeof(double), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(ctx, cudaStreamSynchronize(st));
+  return LANDAU_OK;
+}
+
+int landau_spmv(landau_ctx* ctx, const double* csr_vals_dev, const double* x_dev, int batch, double* y_dev,
+                void* cuda_stream) {
+  if (int rc = check_call(ctx, csr_vals_dev, batch, y_dev)) return rc;
+  if (batch > 0 && !x_dev) return fail(ctx, LANDAU_INVALID_ARG, "null buffer");
+  if (batch == 0) return LANDAU_OK;
+  k4_spmv_batch<<<batch * ctx->S, K4_THREADS, 0, (cudaStream_t)cuda_stream>>>(
+      ctx->d_k4grid, ctx->d_k4spec, ctx->S, csr_vals_dev, ctx->v_stride, x_dev, ctx->f_stride, y_dev);
+  ++ctx->launches;
+  CUDA_TRY(ctx, cudaGetLastError());
+  return LANDAU_OK;
+}
+
+int landau_solve(landau_ctx* ctx, const double* csr_vals_dev, const double* rhs_dev, int batch, double rtol, int max_it,
+                 double* x_dev, int* iters_dev, double* relres_dev, void* cuda_stream) {
+  if (int rc = check_call(ctx, csr_vals_dev, batch, x_dev)) return rc;
+  if (batch > 0 && !rhs_dev) return fail(ctx, LANDAU_INVALID_ARG, "null buffer");
+  if (!(rtol > 0) || max_it < 1) return fail(ctx, LANDAU_INVALID_ARG, "rtol must be > 0 and max_it >= 1");
+  if (batch == 0) return LANDAU_OK;
+  long long ws_stride = 0;
+  if (ctx->k4_max_n > ctx->k4_smem_n) {  // some grid's vectors do not fit in shared memory: global workspace
+    ws_stride = (long long)K4_NVEC * ctx->k4_max_n;
+    if (int rc = grow(ctx, &ctx->solve_ws, &ctx->solve_ws_cap, (size_t)ws_stride * batch * ctx->S, false)) return rc;
+  }
+  k4_tfqmr<<<batch * ctx->S, K4_THREADS, ctx->k4_smem, (cudaStream_t)cuda_stream>>>(
+      ctx->d_k4grid, ctx->d_k4spec, ctx->S, csr_vals_dev, ctx->v_stride, rhs_dev, ctx->f_stride, x_dev, rtol, max_it,
+      iters_dev, relres_dev, ctx->solve_ws, ws_stride, ctx->k4_smem_n);
+  ++ctx->launches;
+  CUDA_TRY(ctx, cudaGetLastError());
   return LANDAU_OK;
 }
 
