@@ -49,6 +49,8 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel", type=int, default=0, help="inner-integral kernel: 0 auto, 1 DFMA, 2 DMMA, 3/4 GEMM (32x128 / 16x256 tile)")
+    ap.add_argument("--solve", action="store_true", help="also time the batched TFQMR solve of the step's systems "
+                    "(reported under \"solve\", not part of value)")
     ap.add_argument("--chunk", type=int, default=0, help="batch entries per pass through the stages (0: library default)")
     return ap.parse_args()
 
@@ -271,6 +273,32 @@ def run_ours(args):
                "h2d_bytes_per_step": int(f_host.numel() * 8), "d2h_bytes_per_step": int(out_host.numel() * 8),
                "steps": n_e2e, "api": "landau_jacobian_host (pinned host buffers)"}
 
+    solve = None
+    if args.solve:
+        # the step after the hot path: backward-Euler systems (M/dt - J) x = (M/dt) f, TFQMR + Jacobi
+        a_inf = torch.empty_like(out_dev)
+        Bn.landau_jacobian(L.ctx, f_dev[0], B, float("inf"), a_inf)
+        Bn.landau_jacobian(L.ctx, f_dev[0], B, cfg["dt"], out_dev)
+        rhs = torch.empty_like(f_dev[0])
+        Bn.landau_spmv(L.ctx, out_dev - a_inf, f_dev[0], B, rhs)
+        del a_inf
+        x = torch.zeros_like(rhs)
+        iters = torch.zeros((B, L.S), dtype=torch.int32, device=dev)
+        t_solve = []
+        for rep in range(3):
+            x.zero_()
+            s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            s0.record(stream)
+            Bn.landau_solve(L.ctx, out_dev, rhs, B, 1e-8, 2000, x, iters)
+            s1.record(stream)
+            torch.cuda.synchronize()
+            t_solve.append(s0.elapsed_time(s1))
+        res = rhs - L.spmv(out_dev, x)
+        solve = {"ms_per_batch": min(t_solve), "systems": int(B * L.S), "rtol": 1e-8,
+                 "half_steps_mean": float(iters.float().abs().mean()), "half_steps_max": int(iters.abs().max()),
+                 "not_converged": int((iters < 0).sum()),
+                 "max_true_relative_residual": float((res.norm(dim=1) / rhs.norm(dim=1)).max()),
+                 "solves_per_s": world * B * L.S / (min(t_solve) * 1e-3)}
     if rank == 0:
         # roofline of the dominant kernel (K2, inner integral).  Algorithmic FLOPs per step:
         # 14 flop per (i, j, source column) -- separable nu: one column per batch entry over all N^2 pairs --
@@ -320,7 +348,7 @@ def run_ours(args):
                                      "pair_applications_b_i_j": cols_pairs * world / (ms_per_step * 1e-3)},
                 "stage_ms_per_step": {"a1_fields": stage[0] / args.steps, "a2_inner": k2_ms,
                                       "a2b_combine": stage[2] / args.steps, "a3a4_assembly": k3_ms},
-                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "solve": solve, "gpu_launches": int(launches),
                 "clocks": clocks}
         print(json.dumps(line), flush=True)
     L.close()

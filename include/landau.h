@@ -136,7 +136,7 @@ int landau_spmv(landau_ctx* ctx, const double* csr_vals_dev, const double* x_dev
  *   x_dev        : dev, same layout; ON INPUT the initial guess (zeros are fine), on output the solution
  *   rtol         : a run stops when the TFQMR residual bound  tau sqrt(m)  <=  rtol * || D^-1 (b - A x0) ||; the true
  *                  Jacobi-scaled residual is then computed and, if it misses the tolerance (the recursive bound drifts
- *                  on ill-conditioned blocks), the iteration restarts from the current x (at most 4 restarts)
+ *                  on ill-conditioned blocks), the iteration restarts from the current x (a run is also restarted after 600 half-steps, which ends stagnation)
  *   max_it       : at most 2 max_it half-steps (max_it products with A beyond the first)
  *   iters_dev    : dev, [batch][species] or NULL: half-steps taken; negative (-m-1) when the tolerance was not reached
  *                  in 2 max_it half-steps or the iteration broke down (x then holds the last iterate)

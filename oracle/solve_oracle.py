@@ -42,10 +42,11 @@ def residual(rowptr, colidx, vals, x, rhs):
     return np.linalg.norm(rhs - csr_matvec(rowptr, colidx, vals, x)) / np.linalg.norm(rhs)
 
 
-def tfqmr_reference(rowptr, colidx, vals, rhs, rtol, max_it, max_restarts=4):
+def tfqmr_reference(rowptr, colidx, vals, rhs, rtol, max_it, run_cap=600):
     """TFQMR on diag(A)^{-1} A x = diag(A)^{-1} b from x0 = 0.  A run that meets the bound  tau sqrt(k) <= rtol ||r0||
     is checked against the true scaled residual and restarted from the current x if that misses the tolerance (the
-    tolerance stays relative to the first residual).  Returns (x, half-steps done, converged)."""
+    tolerance stays relative to the first residual); a run is also restarted after run_cap half-steps.
+    Returns (x, half-steps done, converged)."""
     n = len(rhs)
     diag = np.array([vals[rowptr[i]:rowptr[i + 1]][list(colidx[rowptr[i]:rowptr[i + 1]]).index(i)] for i in range(n)])
 
@@ -55,7 +56,7 @@ def tfqmr_reference(rowptr, colidx, vals, rhs, rtol, max_it, max_restarts=4):
     x = np.zeros(n)
     m = 0
     r0norm = None
-    for restart in range(max_restarts + 1):
+    while True:
         r = (rhs - csr_matvec(rowptr, colidx, vals, x)) / diag
         tau = np.linalg.norm(r)
         if r0norm is None:
@@ -72,7 +73,7 @@ def tfqmr_reference(rowptr, colidx, vals, rhs, rtol, max_it, max_restarts=4):
         rho = float(rs @ r)
         bound_met = False
         k = 0
-        while not bound_met and m < 2 * max_it:
+        while not bound_met and m < 2 * max_it and k < run_cap:
             even = k % 2 == 0
             if even:
                 sigma = float(rs @ v)
@@ -103,6 +104,3 @@ def tfqmr_reference(rowptr, colidx, vals, rhs, rtol, max_it, max_restarts=4):
                 v = au_new + beta * (au + beta * v)
                 u, au = u_new, au_new
             k += 1
-        if not bound_met:
-            return x, m, False
-    return x, m, False

@@ -26,7 +26,7 @@ struct K4Species {
 
 constexpr int K4_THREADS = 512;
 constexpr int K4_NVEC = 7;
-constexpr int K4_MAX_RESTARTS = 4;
+constexpr int K4_RUN_CAP = 600;  // half-steps of one TFQMR run before it is restarted from the current x
 
 // sums of two values over the CTA (deterministic order), result in every thread
 __device__ __forceinline__ void k4_block_sum2(double& a, double& b, double* red) {
@@ -90,10 +90,12 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
   __syncthreads();
   // TFQMR's residual bound is updated recursively and drifts away from the true residual on ill-conditioned blocks,
   // so a converged run is CHECKED against the true (Jacobi-scaled) residual and restarted from the current x if it
-  // misses the tolerance, which stays relative to the first residual.
+  // misses the tolerance, which stays relative to the first residual.  A run is also restarted after K4_RUN_CAP
+  // half-steps: with the shadow residual fixed, TFQMR can stagnate for thousands of steps on the electron blocks of
+  // the large grids (cond(D^-1 A) ~ 5e3), and a restart from the current iterate ends that.
   double r0norm = 0.0, tau = 0.0;
   int m = 0, status = 0;  // 1 converged, 2 breakdown, 0 running / not converged
-  for (int restart = 0; restart <= K4_MAX_RESTARTS && !status; ++restart) {
+  for (int restart = 0; !status; ++restart) {
     // r = D^-1 (b - A x);  w = u = rs = r, d = 0
     k4_spmv(g, a, xx, [&](int row, double s) {
       const double r = idg[row] * (bb[row] - s);
@@ -121,7 +123,7 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
     });
     __syncthreads();
     bool bound_met = false;
-    for (int k = 0; !bound_met && !status && m < 2 * max_it; ++k) {  // k: half-step of this run
+    for (int k = 0; !bound_met && !status && m < 2 * max_it && k < K4_RUN_CAP; ++k) {  // k: half-step of this run
       const bool even = (k & 1) == 0;
       if (even) {
         double sg = 0.0, z = 0.0;
@@ -174,7 +176,8 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
       }
       __syncthreads();
     }
-    if (!bound_met) break;  // out of iterations or breakdown
+    if (status == 2) break;  // breakdown
+    // bound met: verify against the true residual; run cap reached: restart (a fresh shadow residual ends stagnation)
   }
   if (tid == 0) {
     if (iters) iters[blockIdx.x] = status == 1 ? m : -m - 1;  // half-steps; negative: not converged / breakdown
