@@ -51,21 +51,62 @@ __device__ __forceinline__ void k4_block_sum2(double& a, double& b, double* red)
   }
 }
 
-// y_i = s_i * sum_k a_ik in_k  (s = 1 / a_ii: left Jacobi), 8 lanes per row
+// out(row, sum_k a_ik in_k) for every row: 8 lanes per row, two rows per lane group in flight, the first 56 entries of
+// a row as unrolled predicated loads (all independent: the product is bound by the latency of the value loads from
+// L2, so memory-level parallelism is what counts), longer rows (hanging-node rows) finish in a tail loop.
+__device__ __forceinline__ double k4_row(const double* __restrict__ vals, const int* __restrict__ colidx, const double* in,
+                                         int k0, int k1, int l8) {
+  double s = 0.0;
+#pragma unroll
+  for (int t = 0; t < 7; ++t) {
+    const int k = k0 + l8 + 8 * t;
+    if (k < k1) s = fma(__ldg(vals + k), in[__ldg(colidx + k)], s);
+  }
+  for (int k = k0 + l8 + 56; k < k1; k += 8) s = fma(__ldg(vals + k), in[__ldg(colidx + k)], s);
+  return s;
+}
+
 template <class Out>
 __device__ __forceinline__ void k4_spmv(const K4Grid& g, const double* __restrict__ vals, const double* in, Out out) {
   const int l8 = threadIdx.x & 7, sub = (threadIdx.x & 31) >> 3;
-  // warp-uniform trip count: the shuffles below need all 32 lanes, rows past the end contribute nothing
-  for (int row0 = (threadIdx.x >> 5) * 4; row0 < g.n; row0 += K4_THREADS / 8) {
-    const int row = row0 + sub;
-    const bool live = row < g.n;
-    const int k0 = live ? g.rowptr[row] : 0, k1 = live ? g.rowptr[row + 1] : 0;
-    double s = 0.0;
-    for (int k = k0 + l8; k < k1; k += 8) s = fma(__ldg(vals + k), in[g.colidx[k]], s);
-    s += __shfl_xor_sync(0xffffffffu, s, 4);
-    s += __shfl_xor_sync(0xffffffffu, s, 2);
-    s += __shfl_xor_sync(0xffffffffu, s, 1);
-    if (live && l8 == 0) out(row, s);
+  constexpr int RS = K4_THREADS / 8;  // rows per sweep of the CTA
+  constexpr int U = 4;                // rows per lane group in flight
+  // warp-uniform trip count (the shuffles need all 32 lanes; rows past the end contribute nothing); the row bounds of
+  // the next iteration are fetched while the current rows are summed
+  int k0[U], k1[U];
+  const int first = (threadIdx.x >> 5) * 4;
+  auto bounds = [&](int row0) {
+#pragma unroll
+    for (int j = 0; j < U; ++j) {
+      const int r = row0 + j * RS + sub;
+      const bool live = r < g.n;
+      k0[j] = live ? __ldg(g.rowptr + r) : 0;
+      k1[j] = live ? __ldg(g.rowptr + r + 1) : 0;
+    }
+  };
+  bounds(first);
+  for (int row0 = first; row0 < g.n; row0 += U * RS) {
+    double sum[U];
+    int c0[U], c1[U];
+#pragma unroll
+    for (int j = 0; j < U; ++j) {
+      c0[j] = k0[j];
+      c1[j] = k1[j];
+    }
+    if (row0 + U * RS < g.n) bounds(row0 + U * RS);
+#pragma unroll
+    for (int j = 0; j < U; ++j) sum[j] = k4_row(vals, g.colidx, in, c0[j], c1[j], l8);
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1)
+#pragma unroll
+      for (int j = 0; j < U; ++j) sum[j] += __shfl_xor_sync(0xffffffffu, sum[j], o);
+    if (l8 == 0) {
+#pragma unroll
+      for (int j = 0; j < U; ++j) {
+        const int r = row0 + j * RS + sub;
+        if (r < g.n) out(r, sum[j]);
+      }
+    }
   }
 }
 
