@@ -51,28 +51,19 @@ __device__ __forceinline__ void k4_block_sum2(double& a, double& b, double* red)
   }
 }
 
-// out(row, sum_k a_ik in_k) for every row: 8 lanes per row, two rows per lane group in flight, the first 56 entries of
-// a row as unrolled predicated loads (all independent: the product is bound by the latency of the value loads from
-// L2, so memory-level parallelism is what counts), longer rows (hanging-node rows) finish in a tail loop.
-__device__ __forceinline__ double k4_row(const double* __restrict__ vals, const int* __restrict__ colidx, const double* in,
-                                         int k0, int k1, int l8) {
-  double s = 0.0;
-#pragma unroll
-  for (int t = 0; t < 7; ++t) {
-    const int k = k0 + l8 + 8 * t;
-    if (k < k1) s = fma(__ldg(vals + k), in[__ldg(colidx + k)], s);
-  }
-  for (int k = k0 + l8 + 56; k < k1; k += 8) s = fma(__ldg(vals + k), in[__ldg(colidx + k)], s);
-  return s;
-}
+// out(row, sum_k a_ik in_k) for every row: 8 lanes per row, two rows per lane group in flight, the first 48 entries of
+// a row loaded into registers before the first use (values and indices come from L2: memory-level parallelism is what
+// counts), longer rows (hanging-node rows) finish in a tail loop.
+constexpr int K4_T = 6;  // entries per lane held in registers per row (8 lanes: rows up to 48 entries without a tail)
 
 template <class Out>
 __device__ __forceinline__ void k4_spmv(const K4Grid& g, const double* __restrict__ vals, const double* in, Out out) {
   const int l8 = threadIdx.x & 7, sub = (threadIdx.x & 31) >> 3;
   constexpr int RS = K4_THREADS / 8;  // rows per sweep of the CTA
-  constexpr int U = 4;                // rows per lane group in flight
+  constexpr int U = 2;                // rows per lane group in flight
   // warp-uniform trip count (the shuffles need all 32 lanes; rows past the end contribute nothing); the row bounds of
-  // the next iteration are fetched while the current rows are summed
+  // the next iteration are fetched while the current rows are summed.  All value / index loads of an iteration are
+  // issued before the first use: the product is bound by the latency of those loads (L2), not by their volume.
   int k0[U], k1[U];
   const int first = (threadIdx.x >> 5) * 4;
   auto bounds = [&](int row0) {
@@ -86,16 +77,30 @@ __device__ __forceinline__ void k4_spmv(const K4Grid& g, const double* __restric
   };
   bounds(first);
   for (int row0 = first; row0 < g.n; row0 += U * RS) {
-    double sum[U];
-    int c0[U], c1[U];
+    double av[U][K4_T];
+    int ci[U][K4_T], c0[U], c1[U];
 #pragma unroll
     for (int j = 0; j < U; ++j) {
       c0[j] = k0[j];
       c1[j] = k1[j];
+#pragma unroll
+      for (int t = 0; t < K4_T; ++t) {
+        const int k = c0[j] + l8 + 8 * t;
+        const bool p = k < c1[j];
+        av[j][t] = p ? __ldg(vals + k) : 0.0;
+        ci[j][t] = p ? __ldg(g.colidx + k) : 0;
+      }
     }
     if (row0 + U * RS < g.n) bounds(row0 + U * RS);
+    double sum[U];
 #pragma unroll
-    for (int j = 0; j < U; ++j) sum[j] = k4_row(vals, g.colidx, in, c0[j], c1[j], l8);
+    for (int j = 0; j < U; ++j) {
+      double sj = 0.0;
+#pragma unroll
+      for (int t = 0; t < K4_T; ++t) sj = fma(av[j][t], in[ci[j][t]], sj);
+      for (int k = c0[j] + l8 + 8 * K4_T; k < c1[j]; k += 8) sj = fma(__ldg(vals + k), in[__ldg(g.colidx + k)], sj);
+      sum[j] = sj;
+    }
 #pragma unroll
     for (int o = 4; o > 0; o >>= 1)
 #pragma unroll
