@@ -78,6 +78,7 @@ struct landau_ctx {
   int chunk = 1024;      // batch entries processed per pass through the stages
   int inner_kernel = 0;  // 0 auto, 1 dfma, 2 dmma
   int n_sm = 148;
+  unsigned func_configured = 0;  // kernels whose dynamic shared-memory limit has been raised on this device
   bool stream_k = true;  // many-column K2: persistent CTAs sharing the steps evenly when the tiles do not fill whole waves
   int assembly_kernel = 0;  // 0 auto (ring kernel where the grid has a schedule), 1 slot-gather kernel
   int last_batch = 0;
@@ -398,10 +399,10 @@ int launch_dmma(landau_ctx* ctx, const Group& gr, int ncols, int ncols_pad, int 
                 long long split_stride, cudaStream_t st) {
   constexpr int CT = 8 * NT;
   const size_t smem = 2 * (CT * 3 * K2M_LD + 2 * K2M_TJ) * sizeof(double);
-  static bool configured = false;
-  if (!configured) {
+  // per context (= per device), not per process: the attribute belongs to the device's copy of the function
+  if (!(ctx->func_configured & (1u << NT))) {
     CUDA_TRY(ctx, cudaFuncSetAttribute(k2_inner_dmma<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = true;
+    ctx->func_configured |= 1u << NT;
   }
   dim3 grid((ctx->n_i_pad + 63) / 64, (ncols + CT - 1) / CT, nsplit);
   k2_inner_dmma<NT><<<grid, 256, smem, st>>>(ctx->d_ip_r, ctx->d_ip_z, ctx->n_i_pad, gr.j0, gr.nj_pad, ctx->F + gr.f_off,
@@ -420,11 +421,11 @@ template <int WI_T, int WC_T, int WGI, int WGC, int NST>
 int launch_gemm_t(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nsplit, long long split_stride,
                   cudaStream_t st) {
   using C = K2G<WI_T, WC_T, WGI, WGC, NST>;
-  static bool configured = false;
-  if (!configured) {
+  constexpr unsigned bit = 1u << (16 + WGC);
+  if (!(ctx->func_configured & bit)) {
     CUDA_TRY(ctx, cudaFuncSetAttribute(k2_inner_gemm<WI_T, WC_T, WGI, WGC, NST>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
-    configured = true;
+    ctx->func_configured |= bit;
   }
   const int n_it = (ctx->n_i_pad + C::TI - 1) / C::TI, n_ct = (ncols + C::TC - 1) / C::TC;
   const bool stream = ctx->stream_k && nsplit == 1 && n_it * n_ct >= ctx->n_sm && (n_it * n_ct) % ctx->n_sm != 0;

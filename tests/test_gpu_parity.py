@@ -280,3 +280,36 @@ def test_stream_mode_reproducible_and_batch_independent(Bn, torch_cuda):
     num = (c - a[:300]).norm(dim=1)
     assert float((num / a[:300].norm(dim=1)).max()) < 1e-13
     L.close()
+
+
+def test_config5_maximum_batch(orc, Bn, torch_cuda):
+    """BASELINE.json's largest size (config 5, B = 4096: 5.8 GB of CSR values, four passes of the default chunk): the
+    first and the last entry against the oracle, every block's column sums, and the first pass bit-identical to a
+    stand-alone run of the same 1024 entries."""
+    torch = torch_cuda
+    cfg = W.config(5)
+    B = 4096
+    o, L = _make(orc, Bn, cfg)
+    coords = [L.dof_coords(g) for g in range(L.G)]
+    f = W.make_batch_f(cfg, coords, batch=B)
+    fd = torch.tensor(f, device="cuda")
+    vals = L.jacobian(fd, cfg["dt"])
+    entries = [0, B - 1]
+    ref = np.stack([o.jacobian(f[b], cfg["dt"]) for b in entries])
+    assert _block_errors(L, vals[entries].cpu().numpy(), ref, L.v_off).max() < TOL
+    first = L.jacobian(fd[:1024].contiguous(), cfg["dt"])
+    assert torch.equal(first, vals[:1024])
+    del first
+    vals.copy_(L.jacobian(fd, float("inf")))
+    for s in range(L.S):
+        g = L.sgrid[s]
+        _, ci = L.pattern(g)
+        cid = torch.tensor(ci.astype(np.int64), device="cuda")
+        worst = 0.0
+        for b0 in range(0, B, 512):
+            blk = vals[b0:b0 + 512, L.v_off[s]:L.v_off[s + 1]]
+            colsum = torch.zeros((blk.shape[0], int(L.n_dof[g])), dtype=torch.float64, device="cuda").index_add_(1, cid, blk)
+            colabs = torch.zeros((blk.shape[0], int(L.n_dof[g])), dtype=torch.float64, device="cuda").index_add_(1, cid, blk.abs())
+            worst = max(worst, float(colsum.abs().max() / colabs.max()))
+        assert worst < 1e-12
+    L.close()
