@@ -53,6 +53,12 @@ constexpr int K3_THREADS = 256;
 constexpr int K3_CPW = K3_PC / (K3_THREADS / 32);  // cells per warp per step
 constexpr int K3_EB = 16;                           // emission: descriptor words per thread per batch
 
+__device__ __forceinline__ double k3_lds(unsigned addr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+  return v;
+}
+
 // dynamic shared memory: ring [rc][K3_RS] | zero pad [8] | constant fragments [16][32]
 __host__ __device__ constexpr size_t k3_smem_bytes(int rc) { return ((size_t)rc * K3_RS + 8 + 16 * 32) * sizeof(double); }
 
@@ -74,6 +80,7 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
   if (s_lo >= s_hi) return;
   const int s_begin = g->halo_begin[s_lo];
 
+  const unsigned ring_s = smem_u32(ring);
   double* zero_pad = ring + rc * K3_RS;
   double* sfrag = zero_pad + 8;
   if (tid < 8) zero_pad[tid] = 0.0;
@@ -192,11 +199,13 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
     if (s + 1 < s_hi) fetch_bounds(s + 1);
     __syncthreads();
     if (emit) {
+      double* __restrict__ outb = out + base;
       // one contribution, weight 1
       for (int e0 = e1_lo;;) {
 #pragma unroll
         for (int k = 0; k < K3_EB; ++k)
-          if (wd[k] != 0xFFFFFFFFu) __stcs(out + base + (int)(wd[k] & ((1u << K3_NBITS) - 1)), ring[wd[k] >> K3_NBITS]);
+          if (wd[k] != 0xFFFFFFFFu)  // 32-bit shared address, one widening multiply-add for the global one
+            __stcs(outb + (wd[k] & ((1u << K3_NBITS) - 1)), k3_lds(ring_s + ((wd[k] >> (K3_NBITS - 3)) & ~7u)));
         e0 += K3_THREADS * K3_EB;
         if (e0 >= e1_hi) break;
 #pragma unroll
@@ -210,9 +219,10 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
 #pragma unroll
         for (int k = 0; k < 2; ++k)
           if (d4[k].x != 0xFFFFFFFFu) {
-            const double v =
-                ((ring[d4[k].y & 0xFFFFu] + ring[d4[k].y >> 16]) + ring[d4[k].z & 0xFFFFu]) + ring[d4[k].z >> 16];
-            __stcs(out + base + (int)d4[k].x, v);
+            const double v = ((k3_lds(ring_s + (d4[k].y & 0xFFFFu) * 8) + k3_lds(ring_s + (d4[k].y >> 16) * 8)) +
+                              k3_lds(ring_s + (d4[k].z & 0xFFFFu) * 8)) +
+                             k3_lds(ring_s + (d4[k].z >> 16) * 8);
+            __stcs(outb + d4[k].x, v);
           }
         e0 += K3_THREADS * 2;
         if (e0 >= e4_hi) break;
