@@ -783,17 +783,17 @@ int landau_apply(landau_ctx* ctx, const double* batch_f_dev, int batch, double* 
     if (int rc = grow(ctx, &ctx->FL, &ctx->FL_cap, (size_t)ctx->fl_stride * nbc, false)) return rc;
     for (int s = 0; s < ctx->S; ++s) {
       const int g = ctx->species[s].grid;
-      dim3 g1((ctx->hg[g].n_ip + 255) / 256, nbc), g2((ctx->hg[g].n_dof + 255) / 256, nbc);
+      dim3 g1(ctx->hg[g].n_cells, (nbc + K1T_BT - 1) / K1T_BT), g2((ctx->hg[g].n_dof + 255) / 256, nbc);
       if (ctx->nb == 9) {
-        k3_flux<9><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,
-                                       ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);
-        k3_apply<9><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev,
-                                        ctx->f_stride, ctx->f_off[s], b0);
+        k3_elem_apply<9><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,
+                                             ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);
+        k3_apply_gather<9><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev,
+                                               ctx->f_stride, ctx->f_off[s], b0);
       } else {
-        k3_flux<16><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,
-                                        ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);
-        k3_apply<16><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev,
-                                         ctx->f_stride, ctx->f_off[s], b0);
+        k3_elem_apply<16><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,
+                                              ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);
+        k3_apply_gather<16><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev,
+                                                ctx->f_stride, ctx->f_off[s], b0);
       }
       ctx->launches += 2;
     }

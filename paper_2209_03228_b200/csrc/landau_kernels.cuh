@@ -577,57 +577,75 @@ k3_assemble(DevGrid g, const DevTables* __restrict__ tab, const double* __restri
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// K3' (apply): flux at the IPs, then gather into dofs:  rhs_a = - sum_q w_q grad phi_a . (D grad f - K f).
+// K3' (apply):  rhs_a = - sum_q w_q grad phi_a . (D grad f - K f).
+//   k3_elem_apply: one CTA = one cell x 16 batch entries (as K1): nodal values staged in shared memory, thread
+//     (q, entry) forms f, grad f and the weighted flux at its point, thread (a, entry) contracts the fluxes with the
+//     basis gradients -> element vector RE[entry][cell * NB + a] (contiguous 128-byte lines per entry).
+//   k3_apply_gather: one thread per (dof, entry) sums its element-vector entries (constraint weights), coalesced along
+//     the dof index.
 // ------------------------------------------------------------------------------------------------------------
 template <int NB>
 __global__ void __launch_bounds__(256)
-k3_flux(DevGrid g, const DevTables* __restrict__ tab, const double* __restrict__ batch_f, long long f_stride,
-        long long f_off, int b0, const double* __restrict__ DK, long long dk_stride, long long dk_off, int nbatch,
-        double* __restrict__ FL, long long fl_stride, long long fl_off) {
-  const int j = blockIdx.x * blockDim.x + threadIdx.x;
-  const int b = blockIdx.y;
-  if (j >= g.n_ip || b >= nbatch) return;
-  const int cell = j / NB, q = j - cell * NB;
-  const double* fs = batch_f + (long long)(b0 + b) * f_stride + f_off;
-  double v = 0.0, vx = 0.0, vy = 0.0;
-#pragma unroll 4
-  for (int a = 0; a < NB; ++a) {
-    double fa = 0.0;
-    for (int p = g.en_ptr[cell * NB + a]; p < g.en_ptr[cell * NB + a + 1]; ++p) fa = fma(g.en_w[p], fs[g.en_dof[p]], fa);
-    v = fma(tab->B[q * NB + a], fa, v);
-    vx = fma(tab->dBxi[q * NB + a], fa, vx);
-    vy = fma(tab->dBeta[q * NB + a], fa, vy);
+k3_elem_apply(DevGrid g, const DevTables* __restrict__ tab, const double* __restrict__ batch_f, long long f_stride,
+              long long f_off, int b0, const double* __restrict__ DK, long long dk_stride, long long dk_off, int nbatch,
+              double* __restrict__ RE, long long re_stride, long long re_off) {
+  __shared__ double sT[3][NB][16];  // B, dBxi, dBeta as [a][q]
+  __shared__ double sF[NB][K1T_BT], sFl[2][NB][K1T_BT];
+  const int tid = threadIdx.x, lo = tid & 15, bl = tid >> 4;
+  const int cell = blockIdx.x, b = blockIdx.y * K1T_BT + bl;
+  const bool live = b < nbatch;
+  for (int e = tid; e < NB * NB; e += 256) {
+    const int q = e / NB, a = e - q * NB;
+    sT[0][a][q] = tab->B[e];
+    sT[1][a][q] = tab->dBxi[e];
+    sT[2][a][q] = tab->dBeta[e];
   }
-  const double fr = vx * g.cell_sr[cell], fz = vy * g.cell_sz[cell], w = g.ip_w[j];
-  const double* dk = DK + (long long)b * dk_stride + dk_off;
-  const double Drr = dk[j], Drz = dk[g.n_ip + j], Dzz = dk[2 * g.n_ip + j], Kr = dk[3 * g.n_ip + j], Kz = dk[4 * g.n_ip + j];
-  double* fl = FL + (long long)b * fl_stride + fl_off;
-  fl[j] = w * (fma(Drr, fr, Drz * fz) - Kr * v);
-  fl[g.n_ip + j] = w * (fma(Drz, fr, Dzz * fz) - Kz * v);
+  const double sr = g.cell_sr[cell], sz = g.cell_sz[cell];
+  if (lo < NB) {  // lo = basis function a: constrained nodal value
+    const double* fs = batch_f + (long long)(b0 + (live ? b : 0)) * f_stride + f_off;
+    double fa = 0.0;
+    for (int p = g.en_ptr[cell * NB + lo]; p < g.en_ptr[cell * NB + lo + 1]; ++p) fa = fma(g.en_w[p], fs[g.en_dof[p]], fa);
+    sF[lo][bl] = fa;
+  }
+  __syncthreads();
+  if (lo < NB) {  // lo = quadrature point q
+    double v = 0.0, vx = 0.0, vy = 0.0;
+#pragma unroll
+    for (int a = 0; a < NB; ++a) {
+      const double fa = sF[a][bl];
+      v = fma(sT[0][a][lo], fa, v);
+      vx = fma(sT[1][a][lo], fa, vx);
+      vy = fma(sT[2][a][lo], fa, vy);
+    }
+    const int j = cell * NB + lo;
+    const double fr = vx * sr, fz = vy * sz, w = g.ip_w[j];
+    const double* dk = DK + (long long)(live ? b : 0) * dk_stride + dk_off;
+    const double Drr = dk[j], Drz = dk[g.n_ip + j], Dzz = dk[2 * g.n_ip + j], Kr = dk[3 * g.n_ip + j], Kz = dk[4 * g.n_ip + j];
+    sFl[0][lo][bl] = w * (fma(Drr, fr, Drz * fz) - Kr * v);
+    sFl[1][lo][bl] = w * (fma(Drz, fr, Dzz * fz) - Kz * v);
+  }
+  __syncthreads();
+  if (lo < NB && live) {  // lo = basis function a again
+    double r = 0.0;
+#pragma unroll
+    for (int q = 0; q < NB; ++q) {
+      r = fma(sT[1][lo][q] * sr, sFl[0][q][bl], r);
+      r = fma(sT[2][lo][q] * sz, sFl[1][q][bl], r);
+    }
+    RE[(long long)b * re_stride + re_off + cell * NB + lo] = r;
+  }
 }
 
 template <int NB>
 __global__ void __launch_bounds__(256)
-k3_apply(DevGrid g, const DevTables* __restrict__ tab, const double* __restrict__ FL, long long fl_stride, long long fl_off,
-         int nbatch, double* __restrict__ rhs, long long f_stride, long long f_off, int b0) {
+k3_apply_gather(DevGrid g, const double* __restrict__ RE, long long re_stride, long long re_off, int nbatch,
+                double* __restrict__ rhs, long long f_stride, long long f_off, int b0) {
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
   const int b = blockIdx.y;
   if (n >= g.n_dof || b >= nbatch) return;
-  const double* fl = FL + (long long)b * fl_stride + fl_off;
+  const double* re = RE + (long long)b * re_stride + re_off;
   double total = 0.0;
-  for (int p = g.ap_ptr[n]; p < g.ap_ptr[n + 1]; ++p) {
-    const int code = g.ap_code[p];
-    const int a = code % NB, cell = code / NB;
-    const double sr = g.cell_sr[cell], sz = g.cell_sz[cell];
-    double s = 0.0;
-#pragma unroll 4
-    for (int q = 0; q < NB; ++q) {
-      const int ip = cell * NB + q;
-      s = fma(tab->dBxi[q * NB + a] * sr, fl[ip], s);
-      s = fma(tab->dBeta[q * NB + a] * sz, fl[g.n_ip + ip], s);
-    }
-    total = fma(g.ap_w[p], s, total);
-  }
+  for (int p = g.ap_ptr[n]; p < g.ap_ptr[n + 1]; ++p) total = fma(g.ap_w[p], re[g.ap_code[p]], total);
   rhs[(long long)(b0 + b) * f_stride + f_off + n] = -total;
 }
 
