@@ -2,10 +2,13 @@
 //
 //   K1  k1_fields        a1: source fields  F = w_j * (sum over species) {f, df/dr, df/dz} at the IPs
 //   K2  k2_inner_dfma    a2: inner integral, plain FP64 FMA version (few columns)
-//       k2_inner_dmma    a2: inner integral as a tensor-generating FP64 GEMM on the DMMA pipe (many columns)
+//       k2_inner_dmma    a2: inner integral on the DMMA pipe, tensor generated per warp (8 .. 96 columns)
+//       k2_inner_gemm    a2: (k2_gemm.cuh) tensor tile shared by the CTA, TMA-staged source tiles (many columns)
 //   K2b k2b_combine      a2: D_a, K_a = species combination of the partial sums (also sums the j-splits)
-//   K3  k3_assemble      a3+a4: element-matrix entries formed on the fly, gathered into batched CSR
-//   K3' k3_flux, k3_apply a5: operator application
+//   K3  k3_ring          a3+a4: (k3_ring.cuh) DMMA element matrices in a shared-memory ring, gathered into batched CSR
+//       k3_assemble      a3+a4: general fallback, one thread per CSR slot
+//   K3' k3_elem_apply, k3_apply_gather   a5: operator application
+//   K4  k4_tfqmr         (k4_solve.cuh) batched TFQMR + Jacobi solve, the step after the path
 //
 // Notation follows PAPER.md sec. 2 and DESIGN.md: i = field point, j = source point, U^D / U^K the gyro-averaged
 // Landau tensor contracted with the field / source unit vectors.
