@@ -401,7 +401,7 @@ int build_grid(const landau_grid_desc& d, const HostTables& t, HostGrid* g, std:
       for (size_t p = 0; p < g->as_code.size(); ++p) {
         const int code = g->as_code[p], cell = code / nb2, a = (code / nb) % nb, c = code % nb;
         const int a1 = a % n1, a2 = a / n1, c1 = c % n1, c2 = c / n1;
-        g->as_roff[p] = g->cell_pos[cell] * K3_RS + (a2 * n1 + c2) * K3_LD + (a1 * n1 + c1);
+        g->as_roff[p] = g->cell_pos[cell] * K3_RS + k3_entry_offset(a2 * n1 + c2, a1 * n1 + c1);
       }
       // classify, bucket by step (slots visited in ascending n, so every list is ascending)
       std::vector<std::vector<int>> l1(g->k3_nsteps), l4(g->k3_nsteps), lg(g->k3_nsteps);

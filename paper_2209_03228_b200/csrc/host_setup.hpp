@@ -12,10 +12,15 @@ namespace landau {
 
 // K3 (element matrices + assembly) schedule constants, shared by host set-up and the kernel:
 // cells are processed in panels of K3_PC cells (cell order); each element matrix occupies K3_RS doubles of a
-// shared-memory ring (a pool of k3_rc matrix positions), entry (a, c) at  (a2 n1 + c2) * K3_LD + (a1 n1 + c1)  (a = a1 + n1 a2, c = c1 + n1 c2).
-constexpr int K3_PC = 16;
-constexpr int K3_LD = 18;
-constexpr int K3_RS = 16 * K3_LD;
+// shared-memory ring (a pool of k3_rc matrix positions), entry (a, c) at  k3_entry_offset(a2 n1 + c2, a1 n1 + c1)  (a = a1 + n1 a2, c = c1 + n1 c2).
+constexpr int K3_PC = 8;
+constexpr int K3_RS = 256;
+// offset of entry (n = a2 n1 + c2, m = a1 n1 + c1) inside one element matrix: row n, column m XOR-swizzled by n so that
+// the DMMA C-fragment stores of a warp (lanes differ in n / 2 and in m) fall on 32 distinct doubles
+#ifdef __CUDACC__
+__host__ __device__
+#endif
+constexpr int k3_entry_offset(int n, int m) { return n * 16 + (m ^ (((n >> 1) & 3) << 2)); }
 constexpr int K3_RING_MAX_BYTES = 220 * 1024;
 constexpr int K3_NBITS = 17;  // bits of (slot - step base) in a packed single-contribution word
 

@@ -51,7 +51,7 @@ struct K3Species {
 
 constexpr int K3_THREADS = 256;
 constexpr int K3_CPW = K3_PC / (K3_THREADS / 32);  // cells per warp per step
-constexpr int K3_EB = 16;                           // emission: descriptor words per thread per batch
+constexpr int K3_EB = 8;                            // emission: descriptor words per thread per batch
 
 __device__ __forceinline__ double k3_lds(unsigned addr) {
   double v;
@@ -62,7 +62,7 @@ __device__ __forceinline__ double k3_lds(unsigned addr) {
 // dynamic shared memory: ring [rc][K3_RS] | zero pad [8] | constant fragments [16][32]
 __host__ __device__ constexpr size_t k3_smem_bytes(int rc) { return ((size_t)rc * K3_RS + 8 + 16 * 32) * sizeof(double); }
 
-__global__ void __launch_bounds__(K3_THREADS, 3)
+__global__ void __launch_bounds__(K3_THREADS, 4)
 k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, int n_spec, int nseg,
         const double* __restrict__ frag, const double* __restrict__ DK, long long dk_stride, double inv_dt,
         double* __restrict__ vals, long long v_stride) {
@@ -118,14 +118,17 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
     }
   };
   fetch(s_begin);
-  // list bounds of the panel to emit, loaded one step ahead: em1 [pa[0], pa[1]), em4 [pa[2], pa[3]), slot base pa[4]
-  int pa[5];
+  // list bounds of the panel to emit, loaded one step ahead: em1 [pa[0], pa[1]), em4 [pa[2], pa[3]), slot base pa[4],
+  // general list [pa[5], pa[6])
+  int pa[7];
   auto fetch_bounds = [&](int s) {
     pa[0] = g->em_ptr[s];
     pa[1] = g->em_ptr[s + 1];
     pa[2] = g->em_ptr[S1 + s];
     pa[3] = g->em_ptr[S1 + s + 1];
     pa[4] = g->em_base[s];
+    pa[5] = g->em_ptr[2 * S1 + s];
+    pa[6] = g->em_ptr[2 * S1 + s + 1];
   };
   fetch_bounds(s_begin);
   __syncthreads();
@@ -173,7 +176,7 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
 #pragma unroll
           for (int nt2 = 0; nt2 < 2; ++nt2)
 #pragma unroll
-            for (int h = 0; h < 2; ++h) dst[(2 * tq + h + 8 * nt2) * K3_LD + gq + 8 * mt2] = o[mt2][nt2][h];
+            for (int h = 0; h < 2; ++h) dst[k3_entry_offset(2 * tq + h + 8 * nt2, gq + 8 * mt2)] = o[mt2][nt2][h];
       }
     }
     if (s + 1 < s_hi) fetch(s + 1);
@@ -184,6 +187,7 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
     const uint4* __restrict__ em4 = g->em4;
     const int e1_lo = pa[0] + tid, e1_hi = emit ? pa[1] : 0;
     const int e4_lo = pa[2] + tid, e4_hi = emit ? pa[3] : 0;
+    const int eg_lo = pa[5] + tid, eg_hi = pa[6];
     unsigned wd[K3_EB];
     uint4 d4[2];
 #pragma unroll
@@ -237,8 +241,7 @@ k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, in
         const int* __restrict__ as_ptr = g->as_ptr;
         const int* __restrict__ as_roff = g->as_roff;
         const double* __restrict__ as_w = g->as_w;
-        const int e1 = g->em_ptr[2 * S1 + s + 1];
-        for (int e = g->em_ptr[2 * S1 + s] + tid; e < e1; e += K3_THREADS) {
+        for (int e = eg_lo; e < eg_hi; e += K3_THREADS) {
           const int n = emg[e];
           double v = 0.0;
           for (int p = as_ptr[n]; p < as_ptr[n + 1]; ++p) v = fma(as_w[p], ring[as_roff[p]], v);

@@ -743,9 +743,9 @@ int landau_jacobian(landau_ctx* ctx, const double* batch_f_dev, int batch, doubl
     if (int rc = run_coefficients(ctx, batch_f_dev, b0, nbc, st)) return rc;
     double* vals = out_csr_vals_dev + (long long)b0 * ctx->v_stride;
     if (ctx->k3_nspec && ctx->assembly_kernel != 1) {
-      // at least one wave of 3 CTAs per SM; the cell range is cut into segments (each with a recomputed halo) only
+      // at least one wave of 4 CTAs per SM; the cell range is cut into segments (each with a recomputed halo) only
       // when the batch alone gives fewer blocks than that
-      const int ctas = nbc * ctx->k3_nspec, want = 3 * ctx->n_sm;
+      const int ctas = nbc * ctx->k3_nspec, want = 4 * ctx->n_sm;
       int nseg = 1;
       if (ctas < want) nseg = std::max(1, std::min(ctx->k3_min_steps, (want + ctas - 1) / ctas));
       k3_ring<<<ctas * nseg, K3_THREADS, ctx->k3_smem, st>>>(ctx->d_k3grid, ctx->d_k3spec, ctx->k3_nspec, nseg,

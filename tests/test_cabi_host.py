@@ -112,8 +112,8 @@ def test_ring_assembly_schedule_exists_for_every_baseline_config(lib, c):
     sz = Bn.landau_sizes(ctx, len(cfg["grids"]))
     for g in range(len(cfg["grids"])):
         info = Bn.landau_assembly_info(ctx, g)
-        assert 16 <= info["ring_cells"] <= 48          # pool of element-matrix positions, reused as matrices die
-        assert info["ring_cells"] * 288 * 8 <= 220 * 1024
-        assert info["n_steps"] == (int(sz["n_cells"][g]) + 15) // 16
+        assert 8 <= info["ring_cells"] <= 48           # pool of element-matrix positions, reused as matrices die
+        assert info["ring_cells"] * 256 * 8 <= 220 * 1024
+        assert info["n_steps"] == (int(sz["n_cells"][g]) + 7) // 8
         assert 0.7 * sz["nnz"][g] < info["n_simple_slots"] <= sz["nnz"][g]
     Bn.landau_destroy(ctx)
