@@ -313,3 +313,32 @@ def test_config5_maximum_batch(orc, Bn, torch_cuda):
             worst = max(worst, float(colsum.abs().max() / colabs.max()))
         assert worst < 1e-12
     L.close()
+
+
+def test_degenerate_cases(orc, Bn, torch_cuda):
+    """Degenerate inputs of the method: (a) two species on two IDENTICAL grids -- every integration point of one grid
+    coincides with one of the other, so the coincident-pair rule (reading A2) is exercised across grids; (b) a grid of
+    a single cell; (c) a species that is absent (f = 0): its block must reduce to M/dt plus the field of the others."""
+    torch = torch_cuda
+    same = dict(kind=0, r_max=4.0, z_min=-4.0, z_max=4.0, nr=3, nz=5, levels=0)
+    one = dict(kind=0, r_max=2.0, z_min=-2.0, z_max=2.0, nr=1, nz=1, levels=0)
+    cfg = dict(name="degenerate", index=97, grids=[same, dict(same), one],
+               species=[dict(mass=1.0, charge=-1.0, grid=0), dict(mass=2.0, charge=1.0, grid=1),
+                        dict(mass=4.0, charge=2.0, grid=2)],
+               degree=2, dt=0.3, batch=2, state="shifted", alpha=[1.0, 1.0, 1.0])
+    o, L = _make(orc, Bn, cfg)
+    f = W.make_batch_f(cfg, [o.dof_coords(g) for g in range(o.G)], batch=2)
+    f[1, L.f_off[1]:L.f_off[2]] = 0.0                      # (c): species 1 absent in entry 1
+    fd = torch.tensor(f, device="cuda")
+    for kernel in (1, 2):
+        Bn.landau_set_inner_kernel(L.ctx, kernel)
+        vals = L.jacobian(fd, cfg["dt"]).cpu().numpy()
+        assert _block_errors(L, vals, o.jacobian_batch(f, cfg["dt"]), L.v_off).max() < TOL
+        rhs = L.apply(fd).cpu().numpy()
+        ref = o.apply_batch(f)
+        for b in range(2):
+            for s in range(L.S):
+                a, r = rhs[b, L.f_off[s]:L.f_off[s + 1]], ref[b, L.f_off[s]:L.f_off[s + 1]]
+                assert np.linalg.norm(a - r) <= TOL * max(np.linalg.norm(r), 1e-300) or np.abs(r).max() == 0.0
+    assert np.all(rhs[1, L.f_off[1]:L.f_off[2]] == 0.0)     # J[f] applied to f = 0 is exactly zero
+    L.close()
