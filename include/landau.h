@@ -146,6 +146,24 @@ int landau_spmv(landau_ctx* ctx, const double* csr_vals_dev, const double* x_dev
 int landau_solve(landau_ctx* ctx, const double* csr_vals_dev, const double* rhs_dev, int batch, double rtol, int max_it,
                  double* x_dev, int* iters_dev, double* relres_dev, void* cuda_stream);
 
+/* Jacobian and operator application from ONE evaluation of the inner integral (what a Newton iteration needs):
+ * out_csr_vals_dev as landau_jacobian, out_rhs_dev as landau_apply. */
+int landau_jacobian_apply(landau_ctx* ctx, const double* batch_f_dev, int batch, double dt, double* out_csr_vals_dev,
+                          double* out_rhs_dev, void* cuda_stream);
+
+/* One backward-Euler step of the implicit collision advance for every batch entry (sec. 2.2), by the
+ * quasi-Newton iteration on the sparse frozen-coefficient Jacobian:
+ *     (M/dt - J[u]) delta = M (u^k - u)/dt + J[u] u,    u <- u + delta,    starting from u = u^k,
+ * until the largest relative update  max over (entry, species) of ||delta|| / ||u||  is <= newton_rtol, at most
+ * max_newton iterations; every linear system is solved by landau_solve(lin_rtol, lin_max_it) from a zero guess.
+ *   u_dev     : dev, layout of batch_f_dev; ON INPUT u^k, on output u^{k+1}
+ *   info_host : host, 4 doubles or NULL: Newton iterations done, last largest relative update, most linear half-steps
+ *               any system took, number of linear solves that missed lin_rtol
+ * Every operator application runs in the kernels of this library; the call synchronises cuda_stream once per Newton
+ * iteration (to read the update norm).  Scratch (the batch's CSR values and four vectors) is grown on demand. */
+int landau_step(landau_ctx* ctx, double* u_dev, int batch, double dt, double newton_rtol, int max_newton, double lin_rtol,
+                int lin_max_it, double* info_host, void* cuda_stream);
+
 /* Host-buffer convenience: same as landau_jacobian / landau_apply with HOST pointers (pageable or pinned); the
  * library stages the copies in internal device buffers and synchronises before returning.  landau_jacobian_host
  * cuts the batch into pieces and copies the CSR values of a finished piece to the host on a second (internal)

@@ -18,7 +18,7 @@ STATUS = {0: "LANDAU_OK", -1: "LANDAU_INVALID_ARG", -2: "LANDAU_UNSUPPORTED", -3
 
 # every symbol include/landau.h declares (tests check that the library exports all of them)
 SYMBOLS = ["landau_create", "landau_destroy", "landau_sizes", "landau_dof_coords", "landau_ip_table",
-           "landau_csr_pattern", "landau_csr_pattern_host", "landau_jacobian", "landau_apply", "landau_spmv", "landau_solve", "landau_jacobian_host",
+           "landau_csr_pattern", "landau_csr_pattern_host", "landau_jacobian", "landau_apply", "landau_spmv", "landau_solve", "landau_jacobian_apply", "landau_step", "landau_jacobian_host",
            "landau_apply_host", "landau_last_coefficients", "landau_tensor_eval", "landau_ellip_eval",
            "landau_fp64_probe", "landau_launch_count", "landau_is_separable", "landau_set_timing", "landau_last_stage_ms",
            "landau_set_inner_kernel", "landau_set_assembly_kernel", "landau_assembly_info", "landau_set_batch_chunk", "landau_last_error"]
@@ -167,6 +167,20 @@ def landau_solve(ctx, csr_vals, rhs, batch, rtol, max_it, x, iters=None, relres=
                                _dev_ptr(x), ip, rp, _stream(stream)), ctx)
 
 
+def landau_jacobian_apply(ctx, batch_f, batch, dt, out_csr_vals, out_rhs, stream=None):
+    _check(load().landau_jacobian_apply(ctx, _dev_ptr(batch_f), C.c_int(batch), C.c_double(dt), _dev_ptr(out_csr_vals),
+                                        _dev_ptr(out_rhs), _stream(stream)), ctx)
+
+
+def landau_step(ctx, u, batch, dt, newton_rtol, max_newton, lin_rtol, lin_max_it, stream=None):
+    """u: u^k in, u^{k+1} out.  Returns dict(newton_its, last_update, lin_half_steps_max, lin_failed)."""
+    info = (C.c_double * 4)()
+    _check(load().landau_step(ctx, _dev_ptr(u), C.c_int(batch), C.c_double(dt), C.c_double(newton_rtol), C.c_int(max_newton),
+                              C.c_double(lin_rtol), C.c_int(lin_max_it), info, _stream(stream)), ctx)
+    return dict(newton_its=int(info[0]), last_update=float(info[1]), lin_half_steps_max=int(info[2]),
+                lin_failed=int(info[3]))
+
+
 def _host_ptr(a):
     """numpy array or CPU (pinned) torch tensor -> pointer."""
     if isinstance(a, np.ndarray):
@@ -313,6 +327,10 @@ class Landau:
         relres = torch.zeros((B, self.S), dtype=torch.float64, device=rhs.device)
         landau_solve(self.ctx, csr_vals, rhs, B, rtol, max_it, x, iters, relres, stream)
         return x, iters, relres
+
+    def step(self, u, dt, newton_rtol=1e-10, max_newton=50, lin_rtol=1e-12, lin_max_it=1000, stream=None):
+        """Backward-Euler step in place (u: [B, f_stride] CUDA float64)."""
+        return landau_step(self.ctx, u, u.shape[0], dt, newton_rtol, max_newton, lin_rtol, lin_max_it, stream)
 
     def last_coefficients(self, batch):
         """list over species of arrays [batch, 5, n_ip]."""

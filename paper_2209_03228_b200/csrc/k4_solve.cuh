@@ -244,4 +244,51 @@ k4_spmv_batch(const K4Grid* __restrict__ grids, const K4Species* __restrict__ sp
           [&](int row, double s) { yy[row] = s; });
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// Small kernels of the backward-Euler quasi-Newton step (landau_step): out = a x + b y, and the update u += delta with
+// the largest relative update over the (entry, species) blocks (positive doubles order like their bit patterns).
+// ------------------------------------------------------------------------------------------------------------
+__global__ void k5_axpby(long long n, double a, const double* __restrict__ x, double b, const double* __restrict__ y,
+                         double* __restrict__ out) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+    out[i] = a * x[i] + b * y[i];
+}
+
+__global__ void __launch_bounds__(256)
+k5_update(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, int n_spec, double* __restrict__ u,
+          const double* __restrict__ delta, long long f_stride, unsigned long long* __restrict__ max_rel_bits) {
+  __shared__ double red[2 * 8];
+  const int sidx = blockIdx.x % n_spec, b = blockIdx.x / n_spec;
+  const K4Species sp = spec[sidx];
+  const int n = grids[sp.grid].n;
+  double* uu = u + (long long)b * f_stride + sp.f_off;
+  const double* dd = delta + (long long)b * f_stride + sp.f_off;
+  double d2 = 0.0, u2 = 0.0;
+  for (int i = threadIdx.x; i < n; i += 256) {
+    const double di = dd[i], ui = uu[i] + di;
+    uu[i] = ui;
+    d2 = fma(di, di, d2);
+    u2 = fma(ui, ui, u2);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    d2 += __shfl_xor_sync(0xffffffffu, d2, o);
+    u2 += __shfl_xor_sync(0xffffffffu, u2, o);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    red[2 * (threadIdx.x >> 5)] = d2;
+    red[2 * (threadIdx.x >> 5) + 1] = u2;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    d2 = u2 = 0.0;
+    for (int w = 0; w < 8; ++w) {
+      d2 += red[2 * w];
+      u2 += red[2 * w + 1];
+    }
+    const double rel = u2 > 0.0 ? sqrt(d2 / u2) : 0.0;
+    atomicMax(max_rel_bits, (unsigned long long)__double_as_longlong(rel));
+  }
+}
+
 }  // namespace landau

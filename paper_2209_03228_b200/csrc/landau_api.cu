@@ -67,6 +67,9 @@ struct landau_ctx {
   size_t k4_smem = 0;
   double* solve_ws = nullptr;
   size_t solve_ws_cap = 0;
+  // landau_step scratch: A values, mass values (one entry, computed once), vectors, iteration counts
+  double *st_A = nullptr, *st_M = nullptr, *st_vec = nullptr, *st_misc = nullptr;
+  size_t st_A_cap = 0, st_M_cap = 0, st_vec_cap = 0, st_misc_cap = 0;
   // scratch (grown on demand)
   double *F = nullptr, *Gp = nullptr, *DK = nullptr, *FL = nullptr, *part_buf = nullptr;
   size_t F_cap = 0, Gp_cap = 0, DK_cap = 0, FL_cap = 0, part_cap = 0;
@@ -590,6 +593,57 @@ int check_call(landau_ctx* ctx, const void* in, int batch, const void* out) {
   return LANDAU_OK;
 }
 
+// a3 + a4 for batch entries [b0, b0 + nbc) from the coefficients in ctx->DK
+int assemble_chunk(landau_ctx* ctx, int b0, int nbc, double inv_dt, double* out_csr_vals_dev, cudaStream_t st) {
+    double* vals = out_csr_vals_dev + (long long)b0 * ctx->v_stride;
+    if (ctx->k3_nspec && ctx->assembly_kernel != 1) {
+      // at least one wave of 4 CTAs per SM; the cell range is cut into segments (each with a recomputed halo) only
+      // when the batch alone gives fewer blocks than that
+      const int ctas = nbc * ctx->k3_nspec, want = 4 * ctx->n_sm;
+      int nseg = 1;
+      if (ctas < want) nseg = std::max(1, std::min(ctx->k3_min_steps, (want + ctas - 1) / ctas));
+      k3_ring<<<ctas * nseg, K3_THREADS, ctx->k3_smem, st>>>(ctx->d_k3grid, ctx->d_k3spec, ctx->k3_nspec, nseg,
+                                                             ctx->d_k3frag, ctx->DK, ctx->dk_stride, inv_dt, vals,
+                                                             ctx->v_stride);
+      ++ctx->launches;
+    }
+    for (int s = 0; s < ctx->S; ++s) {
+      if (ctx->k3_ring_ok[s] && ctx->assembly_kernel != 1) continue;
+      const int g = ctx->species[s].grid;
+      dim3 grid((ctx->hg[g].nnz + 255) / 256, nbc);
+      if (ctx->nb == 9)
+        k3_assemble<9><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, nbc,
+                                             vals, ctx->v_stride, ctx->v_off[s]);
+      else
+        k3_assemble<16><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, nbc,
+                                              vals, ctx->v_stride, ctx->v_off[s]);
+      ++ctx->launches;
+    }
+  return LANDAU_OK;
+}
+
+// a5 for batch entries [b0, b0 + nbc) from the coefficients in ctx->DK
+int apply_chunk(landau_ctx* ctx, const double* batch_f_dev, int b0, int nbc, double* out_rhs_dev, cudaStream_t st) {
+    if (int rc = grow(ctx, &ctx->FL, &ctx->FL_cap, (size_t)ctx->fl_stride * nbc, false)) return rc;
+    for (int s = 0; s < ctx->S; ++s) {
+      const int g = ctx->species[s].grid;
+      dim3 g1(ctx->hg[g].n_cells, (nbc + K1T_BT - 1) / K1T_BT), g2((ctx->hg[g].n_dof + 255) / 256, nbc);
+      if (ctx->nb == 9) {
+        k3_elem_apply<9><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,
+                                             ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);
+        k3_apply_gather<9><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev,
+                                               ctx->f_stride, ctx->f_off[s], b0);
+      } else {
+        k3_elem_apply<16><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,
+                                              ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);
+        k3_apply_gather<16><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev,
+                                                ctx->f_stride, ctx->f_off[s], b0);
+      }
+      ctx->launches += 2;
+    }
+  return LANDAU_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -675,7 +729,8 @@ void landau_destroy(landau_ctx* ctx) {
     cudaDeviceSynchronize();
   }
   for (void* p : ctx->allocs) cudaFree(p);
-  for (double* p : {ctx->F, ctx->Gp, ctx->DK, ctx->FL, ctx->part_buf, ctx->solve_ws, ctx->stage_in, ctx->stage_out})
+  for (double* p : {ctx->F, ctx->Gp, ctx->DK, ctx->FL, ctx->part_buf, ctx->solve_ws, ctx->stage_in, ctx->stage_out, ctx->st_A,
+                    ctx->st_M, ctx->st_vec, ctx->st_misc})
     if (p) cudaFree(p);
   for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
   for (cudaEvent_t e : ctx->copy_ev) cudaEventDestroy(e);
@@ -741,30 +796,7 @@ int landau_jacobian(landau_ctx* ctx, const double* batch_f_dev, int batch, doubl
   for (int b0 = 0; b0 < batch; b0 += ctx->chunk) {
     const int nbc = std::min(ctx->chunk, batch - b0);
     if (int rc = run_coefficients(ctx, batch_f_dev, b0, nbc, st)) return rc;
-    double* vals = out_csr_vals_dev + (long long)b0 * ctx->v_stride;
-    if (ctx->k3_nspec && ctx->assembly_kernel != 1) {
-      // at least one wave of 4 CTAs per SM; the cell range is cut into segments (each with a recomputed halo) only
-      // when the batch alone gives fewer blocks than that
-      const int ctas = nbc * ctx->k3_nspec, want = 4 * ctx->n_sm;
-      int nseg = 1;
-      if (ctas < want) nseg = std::max(1, std::min(ctx->k3_min_steps, (want + ctas - 1) / ctas));
-      k3_ring<<<ctas * nseg, K3_THREADS, ctx->k3_smem, st>>>(ctx->d_k3grid, ctx->d_k3spec, ctx->k3_nspec, nseg,
-                                                             ctx->d_k3frag, ctx->DK, ctx->dk_stride, inv_dt, vals,
-                                                             ctx->v_stride);
-      ++ctx->launches;
-    }
-    for (int s = 0; s < ctx->S; ++s) {
-      if (ctx->k3_ring_ok[s] && ctx->assembly_kernel != 1) continue;
-      const int g = ctx->species[s].grid;
-      dim3 grid((ctx->hg[g].nnz + 255) / 256, nbc);
-      if (ctx->nb == 9)
-        k3_assemble<9><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, nbc,
-                                             vals, ctx->v_stride, ctx->v_off[s]);
-      else
-        k3_assemble<16><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, nbc,
-                                              vals, ctx->v_stride, ctx->v_off[s]);
-      ++ctx->launches;
-    }
+    if (int rc = assemble_chunk(ctx, b0, nbc, inv_dt, out_csr_vals_dev, st)) return rc;
     CUDA_TRY(ctx, cudaGetLastError());
     accumulate_timing(ctx, st);
     ctx->last_batch = nbc;
@@ -780,23 +812,28 @@ int landau_apply(landau_ctx* ctx, const double* batch_f_dev, int batch, double* 
   for (int b0 = 0; b0 < batch; b0 += ctx->chunk) {
     const int nbc = std::min(ctx->chunk, batch - b0);
     if (int rc = run_coefficients(ctx, batch_f_dev, b0, nbc, st)) return rc;
-    if (int rc = grow(ctx, &ctx->FL, &ctx->FL_cap, (size_t)ctx->fl_stride * nbc, false)) return rc;
-    for (int s = 0; s < ctx->S; ++s) {
-      const int g = ctx->species[s].grid;
-      dim3 g1(ctx->hg[g].n_cells, (nbc + K1T_BT - 1) / K1T_BT), g2((ctx->hg[g].n_dof + 255) / 256, nbc);
-      if (ctx->nb == 9) {
-        k3_elem_apply<9><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,
-                                             ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);
-        k3_apply_gather<9><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev,
-                                               ctx->f_stride, ctx->f_off[s], b0);
-      } else {
-        k3_elem_apply<16><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,
-                                              ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);
-        k3_apply_gather<16><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev,
-                                                ctx->f_stride, ctx->f_off[s], b0);
-      }
-      ctx->launches += 2;
-    }
+    if (int rc = apply_chunk(ctx, batch_f_dev, b0, nbc, out_rhs_dev, st)) return rc;
+    CUDA_TRY(ctx, cudaGetLastError());
+    accumulate_timing(ctx, st);
+    ctx->last_batch = nbc;
+  }
+  ctx->last_stream = st;
+  return LANDAU_OK;
+}
+
+int landau_jacobian_apply(landau_ctx* ctx, const double* batch_f_dev, int batch, double dt, double* out_csr_vals_dev,
+                          double* out_rhs_dev, void* cuda_stream) {
+  if (int rc = check_call(ctx, batch_f_dev, batch, out_csr_vals_dev)) return rc;
+  if (batch > 0 && !out_rhs_dev) return fail(ctx, LANDAU_INVALID_ARG, "null buffer");
+  if (!(dt > 0)) return fail(ctx, LANDAU_INVALID_ARG, "dt must be > 0 (use +inf for the unshifted -J)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const double inv_dt = std::isinf(dt) ? 0.0 : 1.0 / dt;
+  ctx->ev_used = 0;
+  for (int b0 = 0; b0 < batch; b0 += ctx->chunk) {
+    const int nbc = std::min(ctx->chunk, batch - b0);
+    if (int rc = run_coefficients(ctx, batch_f_dev, b0, nbc, st)) return rc;  // ONE inner integral for both outputs
+    if (int rc = assemble_chunk(ctx, b0, nbc, inv_dt, out_csr_vals_dev, st)) return rc;
+    if (int rc = apply_chunk(ctx, batch_f_dev, b0, nbc, out_rhs_dev, st)) return rc;
     CUDA_TRY(ctx, cudaGetLastError());
     accumulate_timing(ctx, st);
     ctx->last_batch = nbc;
@@ -898,6 +935,74 @@ int landau_solve(landau_ctx* ctx, const double* csr_vals_dev, const double* rhs_
       iters_dev, relres_dev, ctx->solve_ws, ws_stride, ctx->k4_smem_n);
   ++ctx->launches;
   CUDA_TRY(ctx, cudaGetLastError());
+  return LANDAU_OK;
+}
+
+int landau_step(landau_ctx* ctx, double* u_dev, int batch, double dt, double newton_rtol, int max_newton, double lin_rtol,
+                int lin_max_it, double* info_host, void* cuda_stream) {
+  if (int rc = check_call(ctx, u_dev, batch, u_dev)) return rc;
+  if (!(dt > 0) || std::isinf(dt) || max_newton < 1 || !(lin_rtol > 0) || lin_max_it < 1)
+    return fail(ctx, LANDAU_INVALID_ARG, "landau_step: dt finite > 0, max_newton >= 1, lin_rtol > 0, lin_max_it >= 1");
+  if (info_host) info_host[0] = info_host[1] = info_host[2] = info_host[3] = 0.0;
+  if (batch == 0) return LANDAU_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t nf = (size_t)batch * ctx->f_stride, nsys = (size_t)batch * ctx->S;
+  // mass values (independent of f and of the entry): M = (M/1 - J[0]) since D = K = 0 for f = 0
+  if (!ctx->st_M) {
+    if (int rc = grow(ctx, &ctx->st_M, &ctx->st_M_cap, (size_t)ctx->v_stride + ctx->f_stride, false)) return rc;
+    double* zero_f = ctx->st_M + ctx->v_stride;
+    CUDA_TRY(ctx, cudaMemsetAsync(zero_f, 0, sizeof(double) * ctx->f_stride, st));
+    const bool timing = ctx->timing;
+    ctx->timing = false;
+    const int rc = landau_jacobian(ctx, zero_f, 1, 1.0, ctx->st_M, cuda_stream);
+    ctx->timing = timing;
+    if (rc) return rc;
+  }
+  if (int rc = grow(ctx, &ctx->st_A, &ctx->st_A_cap, (size_t)batch * ctx->v_stride, false)) return rc;
+  if (int rc = grow(ctx, &ctx->st_vec, &ctx->st_vec_cap, 4 * nf, false)) return rc;
+  if (int rc = grow(ctx, &ctx->st_misc, &ctx->st_misc_cap, nsys + 2, false)) return rc;  // iteration counts (int) + scalar
+  double *u0 = ctx->st_vec, *ju = u0 + nf, *rhs = ju + nf, *delta = rhs + nf;
+  int* iters = reinterpret_cast<int*>(ctx->st_misc);
+  unsigned long long* max_rel = reinterpret_cast<unsigned long long*>(ctx->st_misc + (nsys + 1) / 2 + 1);
+  CUDA_TRY(ctx, cudaMemcpyAsync(u0, u_dev, sizeof(double) * nf, cudaMemcpyDeviceToDevice, st));
+  const int eb = (int)std::min<size_t>((nf + 255) / 256, 65535);
+  int it = 0, worst_lin = 0, lin_failed = 0;
+  double rel = 0.0;
+  std::vector<int> h_iters(nsys);
+  for (it = 0; it < max_newton; ++it) {
+    // A = M/dt - J[u], ju = J[u] u from one inner integral
+    if (int rc = landau_jacobian_apply(ctx, u_dev, batch, dt, ctx->st_A, ju, cuda_stream)) return rc;
+    // rhs = M (u0 - u)/dt + J[u] u
+    k5_axpby<<<eb, 256, 0, st>>>((long long)nf, 1.0, u0, -1.0, u_dev, delta);
+    k4_spmv_batch<<<batch * ctx->S, K4_THREADS, 0, st>>>(ctx->d_k4grid, ctx->d_k4spec, ctx->S, ctx->st_M, 0, delta,
+                                                         ctx->f_stride, rhs);
+    k5_axpby<<<eb, 256, 0, st>>>((long long)nf, 1.0 / dt, rhs, 1.0, ju, rhs);
+    ctx->launches += 3;
+    CUDA_TRY(ctx, cudaMemsetAsync(delta, 0, sizeof(double) * nf, st));
+    if (int rc = landau_solve(ctx, ctx->st_A, rhs, batch, lin_rtol, lin_max_it, delta, iters, nullptr, cuda_stream)) return rc;
+    CUDA_TRY(ctx, cudaMemsetAsync(max_rel, 0, sizeof(unsigned long long), st));
+    k5_update<<<batch * ctx->S, 256, 0, st>>>(ctx->d_k4grid, ctx->d_k4spec, ctx->S, u_dev, delta, ctx->f_stride, max_rel);
+    ++ctx->launches;
+    unsigned long long bits = 0;
+    CUDA_TRY(ctx, cudaMemcpyAsync(&bits, max_rel, sizeof(bits), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaMemcpyAsync(h_iters.data(), iters, sizeof(int) * nsys, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    memcpy(&rel, &bits, sizeof(rel));
+    for (int v : h_iters) {
+      worst_lin = std::max(worst_lin, v < 0 ? -v - 1 : v);
+      lin_failed += v < 0;
+    }
+    if (rel <= newton_rtol) {
+      ++it;
+      break;
+    }
+  }
+  if (info_host) {
+    info_host[0] = it;
+    info_host[1] = rel;
+    info_host[2] = worst_lin;
+    info_host[3] = lin_failed;
+  }
   return LANDAU_OK;
 }
 

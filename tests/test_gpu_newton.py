@@ -78,3 +78,54 @@ def test_backward_euler_newton_step(orc, kind):
         assert abs(mom[1, 1] - mom[0, 1]) < 1e-10 * scale[1]              # total energy
         assert np.linalg.norm(got[b] - f0[b]) > 1e-4 * np.linalg.norm(f0[b])  # and the step is not trivial
     L.close()
+
+
+def test_library_step_matches_composed_step_and_relaxes(orc):
+    """landau_step (the same iteration inside the library, one inner integral per Newton iteration) against the oracle
+    step; then several steps of an anisotropic state: densities, momentum and energy stay put while the distribution
+    moves towards equilibrium (the relaxation experiment of PAPER.md sec. 6.1, qualitatively: || J[u] u || decreases)."""
+    import torch
+    from paper_2209_03228_b200 import binding as Bn
+    cfg = W.tiny_config("uniform", 2, batch=2)
+    o = orc.Oracle(cfg["grids"], cfg["species"], cfg["degree"])
+    L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"])
+    f0 = W.make_batch_f(cfg, [o.dof_coords(g) for g in range(o.G)], batch=2)
+    dt = 0.1
+    u = torch.tensor(f0, device="cuda")
+    info = L.step(u, dt, newton_rtol=1e-12, max_newton=60, lin_rtol=1e-13, lin_max_it=500)
+    assert info["lin_failed"] == 0 and info["last_update"] <= 1e-12 and 1 < info["newton_its"] < 60
+    got = u.cpu().numpy()
+    for b in range(2):
+        ref = _oracle_step(o, f0[b], dt, info["newton_its"])
+        for s in range(o.S):
+            sl = slice(o.f_off[s], o.f_off[s + 1])
+            assert np.linalg.norm(got[b, sl] - ref[sl]) < 1e-8 * np.linalg.norm(ref[sl])
+    # a few more steps: invariants and relaxation
+    u0 = torch.tensor(f0, device="cuda")
+    m_vals = (L.jacobian(u0, 1.0) - L.jacobian(u0, float("inf")))
+    def moments(v):
+        mv = L.spmv(m_vals, v).cpu().numpy()
+        out = []
+        for b in range(2):
+            dens, mom, en = [], 0.0, 0.0
+            for s, sp in enumerate(cfg["species"]):
+                rz = o.dof_coords(sp["grid"])
+                blk = mv[b, o.f_off[s]:o.f_off[s + 1]]
+                dens.append(blk.sum())
+                mom += sp["mass"] * (rz[:, 1] @ blk)
+                en += sp["mass"] * ((rz[:, 0] ** 2 + rz[:, 1] ** 2) @ blk)
+            out.append((np.array(dens), mom, en))
+        return out
+    start = moments(u0)
+    norms = [float(L.apply(u).norm())]
+    for k in range(4):
+        info = L.step(u, dt, newton_rtol=1e-12, max_newton=60, lin_rtol=1e-13, lin_max_it=500)
+        assert info["lin_failed"] == 0 and info["last_update"] <= 1e-12
+        norms.append(float(L.apply(u).norm()))
+    end = moments(u)
+    for b in range(2):
+        assert np.abs(end[b][0] - start[b][0]).max() < 1e-10 * np.abs(start[b][0]).max()
+        assert abs(end[b][2] - start[b][2]) < 1e-9 * abs(start[b][2])
+        assert abs(end[b][1] - start[b][1]) < 1e-9 * abs(start[b][2])      # momentum, scaled by the energy
+    assert all(n1 < n0 for n0, n1 in zip(norms, norms[1:])), norms          # || J[u] u || decreases: relaxation
+    L.close()
