@@ -23,8 +23,10 @@
 // Parity pins (tests/test_oracle_*.py): P1 Gauss/Lagrange identities, P2 mass-matrix closed form,
 // P3 tensor identities, P4 closed form vs brute-force azimuthal quadrature of the 3-D tensor and K,E vs
 // std::comp_ellint, P5 Rosenbluth closed forms for a Maxwellian, P6 conservation to round-off,
-// P7 equilibrium trend, P8 brute force on a tiny grid, P9 paper's mesh statistics (14/142/22.2).
-// Unpinned: relaxation *rates* (need a time integrator + solver; out of this path's scope).
+// P7 equilibrium trend, P8 brute force on a tiny grid, P9 paper's mesh statistics (14/142/22.2),
+// P10 / P11 the relaxation rates of PAPER.md Appendix B at t = 0 (bi-Maxwellian isotropisation rate nu_T, two-species
+// thermal equilibration rate nu_bar) from the moments of the applied operator: they fix nu_ab, t0 and the weights.
+// Unpinned: temperature HISTORIES over many collision times (Fig. 5 of the paper: needs its time integrator).
 
 #include <algorithm>
 #include <cmath>
