@@ -129,3 +129,53 @@ def test_library_step_matches_composed_step_and_relaxes(orc):
         assert abs(end[b][1] - start[b][1]) < 1e-9 * abs(start[b][2])      # momentum, scaled by the energy
     assert all(n1 < n0 for n0, n1 in zip(norms, norms[1:])), norms          # || J[u] u || decreases: relaxation
     L.close()
+
+
+def test_anisotropic_relaxation_history_against_nrl():
+    """The relaxation experiment of PAPER.md sec. 6.1-6.2 in small: electrons start bi-Maxwellian (eq. 6.1,
+    alpha = 1.3), 25 backward-Euler steps of landau_step to t = 0.5 t0.  Energy 2 T_perp + T_par is conserved to the
+    nonlinear tolerance, the anisotropy decays monotonically, and its history follows the NRL rate
+    equation of Appendix B -- closely at first, then slightly more slowly because the state stops being bi-Maxwellian
+    (the discrepancy the paper reports under Fig. 5a)."""
+    import math
+    import torch
+    from paper_2209_03228_b200 import binding as Bn
+    grids = [dict(kind=0, r_max=5.0, z_min=-5.0, z_max=5.0, nr=8, nz=16, levels=0)]
+    L = Bn.Landau(grids, [dict(mass=1.0, charge=-1.0, grid=0)], 3)
+    rz = L.dof_coords(0)
+    r, z = rz[:, 0], rz[:, 1]
+    alpha, dt, nsteps = 1.3, 0.02, 25
+    u = torch.tensor(((1 / alpha) * math.pi ** -1.5 * np.exp(-(z ** 2 + r ** 2 / alpha)))[None], device="cuda")
+    m_vals = L.jacobian(u, 1.0) - L.jacobian(u, float("inf"))
+
+    def temps(v):
+        mv = L.spmv(m_vals, v).cpu().numpy()[0]
+        return np.array([(r ** 2) @ mv, 2 * (z ** 2) @ mv]) / mv.sum()
+
+    hist = [temps(u)]
+    for k in range(nsteps):
+        info = L.step(u, dt, newton_rtol=1e-11, max_newton=60, lin_rtol=1e-12, lin_max_it=1000)
+        assert info["lin_failed"] == 0 and info["last_update"] <= 1e-11
+        hist.append(temps(u))
+    h = np.array(hist)
+    energy = 2 * h[:, 0] + h[:, 1]
+    assert np.abs(energy / energy[0] - 1).max() < 1e-10
+    aniso = h[:, 0] - h[:, 1]
+    assert np.all(np.diff(aniso) < 0)
+    # NRL rate equation, RK4 (constant c_iso of tests/golden/nrl_rates.txt)
+    c_iso = 2 ** 1.5 / math.sqrt(math.pi)
+
+    def rate(y):
+        a = y[0] / y[1] - 1
+        nu = c_iso * y[1] ** -1.5 * (-3 + (a + 3) * math.atan(math.sqrt(a)) / math.sqrt(a)) / a ** 2
+        return np.array([-nu * (y[0] - y[1]), 2 * nu * (y[0] - y[1])])
+
+    y, nrl = h[0].copy(), [h[0][0] - h[0][1]]
+    for k in range(nsteps):
+        k1 = rate(y); k2 = rate(y + 0.5 * dt * k1); k3 = rate(y + 0.5 * dt * k2); k4 = rate(y + dt * k3)
+        y = y + dt * (k1 + 2 * k2 + 2 * k3 + k4) / 6
+        nrl.append(y[0] - y[1])
+    nrl = np.array(nrl)
+    assert abs(aniso[1] / nrl[1] - 1) < 5e-3           # first step: the state is still (almost) bi-Maxwellian
+    assert 1.0 < aniso[-1] / nrl[-1] < 1.06            # later: slower than NRL, by a few per cent at t = 0.5 t0
+    L.close()
