@@ -42,7 +42,7 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number 1..5")
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number 1..5 (6: the paper's throughput problem)")
     ap.add_argument("--batch", type=int, default=None, help="batch entries PER GPU (default: the config's)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU time budget of the cpu_baseline sample")
@@ -51,6 +51,8 @@ def parse():
     ap.add_argument("--kernel", type=int, default=0, help="inner-integral kernel: 0 auto, 1 DFMA, 2 DMMA, 3/4 GEMM (32x128 / 16x256 tile)")
     ap.add_argument("--solve", action="store_true", help="also time the batched TFQMR solve of the step's systems "
                     "(reported under \"solve\", not part of value)")
+    ap.add_argument("--advance", type=int, default=0, help="also run this many backward-Euler steps (landau_step) and "
+                    "report the time and Newton iterations under \"advance\" (not part of value)")
     ap.add_argument("--chunk", type=int, default=0, help="batch entries per pass through the stages (0: library default)")
     return ap.parse_args()
 
@@ -299,6 +301,23 @@ def run_ours(args):
                  "not_converged": int((iters < 0).sum()),
                  "max_true_relative_residual": float((res.norm(dim=1) / rhs.norm(dim=1)).max()),
                  "solves_per_s": world * B * L.S / (min(t_solve) * 1e-3)}
+    advance = None
+    if args.advance:
+        # the implicit advance the path belongs to (Table 5): backward-Euler steps of the whole batch
+        u = f_dev[0].clone()
+        Bn.landau_step(L.ctx, u, B, cfg["dt"], 1e-8, 50, 1e-10, 2000)          # warm-up (scratch, mass values)
+        u.copy_(f_dev[0])
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        newton = 0
+        for k in range(args.advance):
+            info = Bn.landau_step(L.ctx, u, B, cfg["dt"], 1e-8, 50, 1e-10, 2000)
+            newton += info["newton_its"]
+        torch.cuda.synchronize()
+        t_adv = time.perf_counter() - t0
+        advance = {"steps": args.advance, "dt": cfg["dt"], "seconds": t_adv, "newton_iterations": newton,
+                   "newton_rtol": 1e-8, "lin_rtol": 1e-10, "last": info,
+                   "newton_iterations_x_batch_per_s": newton * B * world / t_adv}
     if rank == 0:
         # roofline of the dominant kernel (K2, inner integral).  Algorithmic FLOPs per step:
         # 14 flop per (i, j, source column) -- separable nu: one column per batch entry over all N^2 pairs --
@@ -348,7 +367,7 @@ def run_ours(args):
                                      "pair_applications_b_i_j": cols_pairs * world / (ms_per_step * 1e-3)},
                 "stage_ms_per_step": {"a1_fields": stage[0] / args.steps, "a2_inner": k2_ms,
                                       "a2b_combine": stage[2] / args.steps, "a3a4_assembly": k3_ms},
-                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "solve": solve, "gpu_launches": int(launches),
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "solve": solve, "advance": advance, "gpu_launches": int(launches),
                 "clocks": clocks}
         print(json.dumps(line), flush=True)
     L.close()
