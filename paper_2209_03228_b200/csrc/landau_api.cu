@@ -53,6 +53,9 @@ struct landau_ctx {
   std::vector<int> mix_group;         // group of each grid
   std::vector<int> mix_col_in_group;  // first column (per batch entry) of the grid inside its group
   std::vector<CombineTable> comb;     // per species
+  std::vector<CombineTable> comb_resolved;  // with the column bases of the current chunk layout
+  CombineTable* d_comb = nullptr;
+  int comb_key = -1, comb_max_ip = 0;
   // K3 ring kernel: device schedule per grid, species list (only species whose grid has a ring schedule)
   K3Grid* d_k3grid = nullptr;
   K3Species* d_k3spec = nullptr;
@@ -561,20 +564,36 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
     ++ctx->launches;
   }
   mark(ctx, st);
-  // K2b
-  for (int s = 0; s < S; ++s) {
-    CombineTable ct = ctx->comb[s];
-    if (!ctx->separable) {
-      for (int t = 0; t < ct.n_terms; ++t) {
-        const int g = -ct.col_base[t] - 1, q = ctx->mix_group[g];
-        ct.col_base[t] = gcol0[q] + ct.col_stride[t];
-        ct.col_stride[t] = ctx->groups[q].ncb;
+  // K2b: one launch over (IP, entry, species); the resolved tables are re-uploaded only when the column layout changes
+  if (ctx->comb_key != total_cols || !ctx->d_comb) {
+    ctx->comb_resolved = ctx->comb;
+    int max_ip = 0;
+    for (int s = 0; s < S; ++s) {
+      CombineTable& ct = ctx->comb_resolved[s];
+      if (!ctx->separable) {
+        for (int t = 0; t < ct.n_terms; ++t) {
+          const int g = -ct.col_base[t] - 1, q = ctx->mix_group[g];
+          ct.col_base[t] = gcol0[q] + ct.col_stride[t];
+          ct.col_stride[t] = ctx->groups[q].ncb;
+        }
       }
+      const int g = ctx->species[s].grid;
+      ct.ip_off = ctx->ip_off[g];
+      ct.n_ip = ctx->hg[g].n_ip;
+      ct.dk_off = ctx->dk_off[s];
+      max_ip = std::max(max_ip, ct.n_ip);
     }
-    const int g = ctx->species[s].grid;
-    dim3 grid((ctx->hg[g].n_ip + 255) / 256, nbc);
-    k2b_combine<<<grid, 256, 0, st>>>(ct, ctx->Gp, split_stride, nsplit, ctx->n_i_pad, ctx->ip_off[g], ctx->hg[g].n_ip, nbc,
-                                      ctx->DK, ctx->dk_stride, ctx->dk_off[s]);
+    ctx->comb_max_ip = max_ip;
+    if (!ctx->d_comb) {
+      CUDA_TRY(ctx, cudaMalloc(&ctx->d_comb, sizeof(CombineTable) * S));
+      ctx->allocs.push_back(ctx->d_comb);
+    }
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->d_comb, ctx->comb_resolved.data(), sizeof(CombineTable) * S, cudaMemcpyHostToDevice, st));
+    ctx->comb_key = total_cols;
+  }
+  {
+    dim3 grid((ctx->comb_max_ip + 255) / 256, nbc, S);
+    k2b_combine<<<grid, 256, 0, st>>>(ctx->d_comb, ctx->Gp, split_stride, nsplit, ctx->n_i_pad, nbc, ctx->DK, ctx->dk_stride);
     ++ctx->launches;
   }
   mark(ctx, st);

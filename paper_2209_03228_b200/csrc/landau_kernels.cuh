@@ -505,13 +505,19 @@ struct CombineTable {   // per species alpha
   int col_base[16];     // column of batch entry 0
   int col_stride[16];   // columns per batch entry of that group
   double coefD[16], coefK[16];
+  int ip_off, n_ip;     // the species' grid: offset in the concatenated IP arrays, number of IPs
+  long long dk_off;     // offset of the species' block inside one entry of DK
 };
 
+// one launch for all species: blockIdx.z = species
 __global__ void __launch_bounds__(256)
-k2b_combine(CombineTable ct, const double* __restrict__ G, long long g_split_stride, int n_split, int n_i_total,
-            int ip_off, int n_ip, int nbatch, double* __restrict__ DK, long long dk_stride, long long dk_off) {
+k2b_combine(const CombineTable* __restrict__ cts, const double* __restrict__ G, long long g_split_stride, int n_split,
+            int n_i_total, int nbatch, double* __restrict__ DK, long long dk_stride) {
+  const CombineTable& ct = cts[blockIdx.z];
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int b = blockIdx.y;
+  const int ip_off = ct.ip_off, n_ip = ct.n_ip;
+  const long long dk_off = ct.dk_off;
   if (i >= n_ip || b >= nbatch) return;
   double out[5] = {0, 0, 0, 0, 0};
   for (int t = 0; t < ct.n_terms; ++t) {
