@@ -378,9 +378,9 @@ def run_ours(args):
 
 def ncu_traffic(workload):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of this
-    workload (profiles/r1_traffic_v4.json.txt); empty when the workload is another one (traffic = null)."""
+    workload (profiles/r1_traffic.json.txt); empty when the workload is another one (traffic = null)."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r1_traffic_v4.json.txt")) as fh:
+        with open(os.path.join(ROOT, "profiles", "r1_traffic.json.txt")) as fh:
             t = json.load(fh)
         return t if workload.startswith(t["workload"]) else {}
     except (OSError, KeyError, ValueError):
