@@ -24,7 +24,7 @@ struct K4Species {
   long long f_off, v_off;
 };
 
-constexpr int K4_THREADS = 512;
+constexpr int K4_THREADS = 512;  // largest CTA; small systems run with 128 or 256 threads (several CTAs per SM)
 constexpr int K4_NVEC = 7;
 constexpr int K4_RUN_CAP = 600;  // half-steps of one TFQMR run before it is restarted from the current x
 
@@ -44,8 +44,8 @@ __device__ __forceinline__ void k4_block_sum2(double& a, double& b, double* red)
   __syncthreads();
   a = 0.0;
   b = 0.0;
-#pragma unroll
-  for (int wv = 0; wv < K4_THREADS / 32; ++wv) {
+  const int nw = blockDim.x >> 5;
+  for (int wv = 0; wv < nw; ++wv) {
     a += red[2 * wv];
     b += red[2 * wv + 1];
   }
@@ -59,7 +59,7 @@ constexpr int K4_T = 6;  // entries per lane held in registers per row (8 lanes:
 template <class Out>
 __device__ __forceinline__ void k4_spmv(const K4Grid& g, const double* __restrict__ vals, const double* in, Out out) {
   const int l8 = threadIdx.x & 7, sub = (threadIdx.x & 31) >> 3;
-  constexpr int RS = K4_THREADS / 8;  // rows per sweep of the CTA
+  const int RS = blockDim.x >> 3;  // rows per sweep of the CTA
   constexpr int U = 2;                // rows per lane group in flight
   // warp-uniform trip count (the shuffles need all 32 lanes; rows past the end contribute nothing); the row bounds of
   // the next iteration are fetched while the current rows are summed.  All value / index loads of an iteration are
@@ -115,7 +115,7 @@ __device__ __forceinline__ void k4_spmv(const K4Grid& g, const double* __restric
   }
 }
 
-__global__ void __launch_bounds__(K4_THREADS, 1)
+__global__ void __launch_bounds__(K4_THREADS)
 k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, int n_spec, const double* __restrict__ vals,
          long long v_stride, const double* __restrict__ rhs, long long f_stride, double* __restrict__ x, double rtol,
          int max_it, int* __restrict__ iters, double* __restrict__ relres, double* __restrict__ ws, long long ws_stride,
@@ -125,14 +125,14 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
   const int sidx = blockIdx.x % n_spec, b = blockIdx.x / n_spec;
   const K4Species sp = spec[sidx];
   const K4Grid g = grids[sp.grid];
-  const int n = g.n, tid = threadIdx.x;
+  const int n = g.n, tid = threadIdx.x, nthreads = blockDim.x;
   double* vec = n <= smem_n ? k4_smem + 2 * (K4_THREADS / 32) : ws + (long long)blockIdx.x * ws_stride;
   double *rs = vec, *w = vec + n, *u = vec + 2 * n, *v = vec + 3 * n, *d = vec + 4 * n, *au = vec + 5 * n, *idg = vec + 6 * n;
   const double* a = vals + (long long)b * v_stride + sp.v_off;
   const double* bb = rhs + (long long)b * f_stride + sp.f_off;
   double* xx = x + (long long)b * f_stride + sp.f_off;
 
-  for (int i = tid; i < n; i += K4_THREADS) idg[i] = 1.0 / a[g.diag[i]];
+  for (int i = tid; i < n; i += nthreads) idg[i] = 1.0 / a[g.diag[i]];
   __syncthreads();
   // TFQMR's residual bound is updated recursively and drifts away from the true residual on ill-conditioned blocks,
   // so a converged run is CHECKED against the true (Jacobi-scaled) residual and restarted from the current x if it
@@ -152,7 +152,7 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
     });
     __syncthreads();
     double p0 = 0.0, p1 = 0.0;
-    for (int i = tid; i < n; i += K4_THREADS) p0 = fma(rs[i], rs[i], p0);
+    for (int i = tid; i < n; i += nthreads) p0 = fma(rs[i], rs[i], p0);
     k4_block_sum2(p0, p1, red);
     double rho = p0, theta = 0.0, eta = 0.0, alpha = 0.0;
     tau = sqrt(p0);
@@ -173,7 +173,7 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
       const bool even = (k & 1) == 0;
       if (even) {
         double sg = 0.0, z = 0.0;
-        for (int i = tid; i < n; i += K4_THREADS) sg = fma(rs[i], v[i], sg);
+        for (int i = tid; i < n; i += nthreads) sg = fma(rs[i], v[i], sg);
         k4_block_sum2(sg, z, red);
         if (sg == 0.0) {
           status = 2;
@@ -184,7 +184,7 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
       // w -= alpha A u;  d = u + (theta^2 eta / alpha) d;  ||w||^2 and (rs, w)
       const double cd = theta * theta * eta / alpha;
       double ww = 0.0, rw = 0.0;
-      for (int i = tid; i < n; i += K4_THREADS) {
+      for (int i = tid; i < n; i += nthreads) {
         const double wi = fma(-alpha, au[i], w[i]);
         w[i] = wi;
         d[i] = fma(cd, d[i], u[i]);
@@ -196,12 +196,12 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
       const double c = 1.0 / sqrt(1.0 + theta * theta);
       tau = tau * theta * c;
       eta = c * c * alpha;
-      for (int i = tid; i < n; i += K4_THREADS) xx[i] = fma(eta, d[i], xx[i]);
+      for (int i = tid; i < n; i += nthreads) xx[i] = fma(eta, d[i], xx[i]);
       ++m;
       if (tau * sqrt((double)(k + 1)) <= rtol * r0norm) {
         bound_met = true;
       } else if (even) {
-        for (int i = tid; i < n; i += K4_THREADS) u[i] = fma(-alpha, v[i], u[i]);
+        for (int i = tid; i < n; i += nthreads) u[i] = fma(-alpha, v[i], u[i]);
         __syncthreads();
         k4_spmv(g, a, u, [&](int row, double s) { au[row] = idg[row] * s; });
       } else {
@@ -211,7 +211,7 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
         }
         const double beta = rw / rho;
         rho = rw;
-        for (int i = tid; i < n; i += K4_THREADS) u[i] = fma(beta, u[i], w[i]);
+        for (int i = tid; i < n; i += nthreads) u[i] = fma(beta, u[i], w[i]);
         __syncthreads();
         // v = A u_new + beta (A u_old + beta v);  au = A u_new
         k4_spmv(g, a, u, [&](int row, double s) {

@@ -949,7 +949,9 @@ int landau_solve(landau_ctx* ctx, const double* csr_vals_dev, const double* rhs_
     ws_stride = (long long)K4_NVEC * ctx->k4_max_n;
     if (int rc = grow(ctx, &ctx->solve_ws, &ctx->solve_ws_cap, (size_t)ws_stride * batch * ctx->S, false)) return rc;
   }
-  k4_tfqmr<<<batch * ctx->S, K4_THREADS, ctx->k4_smem, (cudaStream_t)cuda_stream>>>(
+  // small systems: fewer threads per system, several systems per SM (the iteration is latency bound)
+  const int threads = ctx->k4_max_n <= 256 ? 128 : ctx->k4_max_n <= 1024 ? 256 : K4_THREADS;
+  k4_tfqmr<<<batch * ctx->S, threads, ctx->k4_smem, (cudaStream_t)cuda_stream>>>(
       ctx->d_k4grid, ctx->d_k4spec, ctx->S, csr_vals_dev, ctx->v_stride, rhs_dev, ctx->f_stride, x_dev, rtol, max_it,
       iters_dev, relres_dev, ctx->solve_ws, ws_stride, ctx->k4_smem_n);
   ++ctx->launches;
