@@ -56,7 +56,16 @@ __device__ __forceinline__ void k4_block_sum2(double& a, double& b, double* red)
 // counts), longer rows (hanging-node rows) finish in a tail loop.
 constexpr int K4_T = 6;  // entries per lane held in registers per row (8 lanes: rows up to 48 entries without a tail)
 
-template <class Out>
+template <bool LDG, class T>
+__device__ __forceinline__ T k4_ld(const T* p) {
+  if constexpr (LDG)
+    return __ldg(p);
+  else
+    return *p;
+}
+
+// LDG: pattern and values in global memory (read-only path); otherwise they may sit in shared memory (plain loads)
+template <bool LDG = true, class Out>
 __device__ __forceinline__ void k4_spmv(const K4Grid& g, const double* __restrict__ vals, const double* in, Out out) {
   const int l8 = threadIdx.x & 7, sub = (threadIdx.x & 31) >> 3;
   const int RS = blockDim.x >> 3;  // rows per sweep of the CTA
@@ -71,8 +80,8 @@ __device__ __forceinline__ void k4_spmv(const K4Grid& g, const double* __restric
     for (int j = 0; j < U; ++j) {
       const int r = row0 + j * RS + sub;
       const bool live = r < g.n;
-      k0[j] = live ? __ldg(g.rowptr + r) : 0;
-      k1[j] = live ? __ldg(g.rowptr + r + 1) : 0;
+      k0[j] = live ? k4_ld<LDG>(g.rowptr + r) : 0;
+      k1[j] = live ? k4_ld<LDG>(g.rowptr + r + 1) : 0;
     }
   };
   bounds(first);
@@ -87,8 +96,8 @@ __device__ __forceinline__ void k4_spmv(const K4Grid& g, const double* __restric
       for (int t = 0; t < K4_T; ++t) {
         const int k = c0[j] + l8 + 8 * t;
         const bool p = k < c1[j];
-        av[j][t] = p ? __ldg(vals + k) : 0.0;
-        ci[j][t] = p ? __ldg(g.colidx + k) : 0;
+        av[j][t] = p ? k4_ld<LDG>(vals + k) : 0.0;
+        ci[j][t] = p ? k4_ld<LDG>(g.colidx + k) : 0;
       }
     }
     if (row0 + U * RS < g.n) bounds(row0 + U * RS);
@@ -98,7 +107,7 @@ __device__ __forceinline__ void k4_spmv(const K4Grid& g, const double* __restric
       double sj = 0.0;
 #pragma unroll
       for (int t = 0; t < K4_T; ++t) sj = fma(av[j][t], in[ci[j][t]], sj);
-      for (int k = c0[j] + l8 + 8 * K4_T; k < c1[j]; k += 8) sj = fma(__ldg(vals + k), in[__ldg(g.colidx + k)], sj);
+      for (int k = c0[j] + l8 + 8 * K4_T; k < c1[j]; k += 8) sj = fma(k4_ld<LDG>(vals + k), in[k4_ld<LDG>(g.colidx + k)], sj);
       sum[j] = sj;
     }
 #pragma unroll
@@ -119,21 +128,43 @@ __global__ void __launch_bounds__(K4_THREADS)
 k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, int n_spec, const double* __restrict__ vals,
          long long v_stride, const double* __restrict__ rhs, long long f_stride, double* __restrict__ x, double rtol,
          int max_it, int* __restrict__ iters, double* __restrict__ relres, double* __restrict__ ws, long long ws_stride,
-         int smem_n) {
+         int smem_n, int mat_nnz) {
   extern __shared__ __align__(16) double k4_smem[];
   double* red = k4_smem;  // [2 * warps]
   const int sidx = blockIdx.x % n_spec, b = blockIdx.x / n_spec;
   const K4Species sp = spec[sidx];
-  const K4Grid g = grids[sp.grid];
+  K4Grid g = grids[sp.grid];
   const int n = g.n, tid = threadIdx.x, nthreads = blockDim.x;
   double* vec = n <= smem_n ? k4_smem + 2 * (K4_THREADS / 32) : ws + (long long)blockIdx.x * ws_stride;
   double *rs = vec, *w = vec + n, *u = vec + 2 * n, *v = vec + 3 * n, *d = vec + 4 * n, *au = vec + 5 * n, *idg = vec + 6 * n;
-  const double* a = vals + (long long)b * v_stride + sp.v_off;
+  const double* a = vals + (long long)b * v_stride + sp.v_off;  // re-pointed to shared memory for small systems
   const double* bb = rhs + (long long)b * f_stride + sp.f_off;
   double* xx = x + (long long)b * f_stride + sp.f_off;
 
   for (int i = tid; i < n; i += nthreads) idg[i] = 1.0 / a[g.diag[i]];
+  // Small systems (mat_nnz > 0: every grid's pattern and one value block fit beside the vectors): the matrix is copied
+  // to shared memory once, and the products of the iteration run from there instead of from L2.
+  const bool mat_smem = mat_nnz > 0;
+  if (mat_smem) {
+    double* sval = k4_smem + 2 * (K4_THREADS / 32) + (long long)K4_NVEC * smem_n;
+    int* scol = reinterpret_cast<int*>(sval + mat_nnz);
+    int* srow = scol + mat_nnz;
+    for (int k = tid; k < g.nnz; k += nthreads) {
+      sval[k] = a[k];
+      scol[k] = g.colidx[k];
+    }
+    for (int i = tid; i <= n; i += nthreads) srow[i] = g.rowptr[i];
+    a = sval;
+    g.colidx = scol;
+    g.rowptr = srow;
+  }
   __syncthreads();
+  auto product = [&](const double* in, auto out) {
+    if (mat_smem)
+      k4_spmv<false>(g, a, in, out);
+    else
+      k4_spmv<true>(g, a, in, out);
+  };
   // TFQMR's residual bound is updated recursively and drifts away from the true residual on ill-conditioned blocks,
   // so a converged run is CHECKED against the true (Jacobi-scaled) residual and restarted from the current x if it
   // misses the tolerance, which stays relative to the first residual.  A run is also restarted after K4_RUN_CAP
@@ -143,7 +174,7 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
   int m = 0, status = 0;  // 1 converged, 2 breakdown, 0 running / not converged
   for (int restart = 0; !status; ++restart) {
     // r = D^-1 (b - A x);  w = u = rs = r, d = 0
-    k4_spmv(g, a, xx, [&](int row, double s) {
+    product(xx, [&](int row, double s) {
       const double r = idg[row] * (bb[row] - s);
       rs[row] = r;
       w[row] = r;
@@ -162,7 +193,7 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
       break;
     }
     if (m >= 2 * max_it) break;
-    k4_spmv(g, a, u, [&](int row, double s) {
+    product(u, [&](int row, double s) {
       const double t = idg[row] * s;
       au[row] = t;
       v[row] = t;
@@ -203,7 +234,7 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
       } else if (even) {
         for (int i = tid; i < n; i += nthreads) u[i] = fma(-alpha, v[i], u[i]);
         __syncthreads();
-        k4_spmv(g, a, u, [&](int row, double s) { au[row] = idg[row] * s; });
+        product(u, [&](int row, double s) { au[row] = idg[row] * s; });
       } else {
         if (rho == 0.0) {
           status = 2;
@@ -214,7 +245,7 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
         for (int i = tid; i < n; i += nthreads) u[i] = fma(beta, u[i], w[i]);
         __syncthreads();
         // v = A u_new + beta (A u_old + beta v);  au = A u_new
-        k4_spmv(g, a, u, [&](int row, double s) {
+        product(u, [&](int row, double s) {
           const double t = idg[row] * s;
           v[row] = fma(beta, fma(beta, v[row], au[row]), t);
           au[row] = t;

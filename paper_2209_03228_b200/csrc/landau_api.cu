@@ -66,7 +66,7 @@ struct landau_ctx {
   // batched solve (k4_solve.cuh)
   K4Grid* d_k4grid = nullptr;
   K4Species* d_k4spec = nullptr;
-  int k4_max_n = 0, k4_smem_n = 0;
+  int k4_max_n = 0, k4_smem_n = 0, k4_mat_nnz = 0;
   size_t k4_smem = 0;
   double* solve_ws = nullptr;
   size_t solve_ws_cap = 0;
@@ -314,6 +314,13 @@ int build_device_side(landau_ctx* ctx) {
     ctx->k4_smem_n = (int)((limit - fixed) / (K4_NVEC * sizeof(double)));
     const int n_in_smem = std::min(ctx->k4_max_n, ctx->k4_smem_n);
     ctx->k4_smem = fixed + (size_t)K4_NVEC * n_in_smem * sizeof(double);
+    // small systems: the pattern and one value block also go to shared memory when everything stays below 56 KB
+    // (four systems per SM)
+    int max_nnz = 0;
+    for (int g = 0; g < G; ++g) max_nnz = std::max(max_nnz, ctx->hg[g].nnz);
+    const size_t mat = (size_t)max_nnz * 12 + (size_t)(ctx->k4_max_n + 2) * 4;
+    ctx->k4_mat_nnz = (ctx->k4_max_n <= ctx->k4_smem_n && ctx->k4_smem + mat <= 56 * 1024) ? max_nnz : 0;
+    if (ctx->k4_mat_nnz) ctx->k4_smem += mat + K4_NVEC * sizeof(double);  // vectors padded to an even length
     CUDA_TRY(ctx, cudaFuncSetAttribute(k4_tfqmr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->k4_smem));
   }
   // source columns: separable nu => one group over all grids, one column per batch entry;
@@ -953,7 +960,8 @@ int landau_solve(landau_ctx* ctx, const double* csr_vals_dev, const double* rhs_
   const int threads = ctx->k4_max_n <= 256 ? 128 : ctx->k4_max_n <= 1024 ? 256 : K4_THREADS;
   k4_tfqmr<<<batch * ctx->S, threads, ctx->k4_smem, (cudaStream_t)cuda_stream>>>(
       ctx->d_k4grid, ctx->d_k4spec, ctx->S, csr_vals_dev, ctx->v_stride, rhs_dev, ctx->f_stride, x_dev, rtol, max_it,
-      iters_dev, relres_dev, ctx->solve_ws, ws_stride, ctx->k4_smem_n);
+      iters_dev, relres_dev, ctx->solve_ws, ws_stride, ctx->k4_mat_nnz ? ((ctx->k4_max_n + 1) & ~1) : ctx->k4_smem_n,
+      ctx->k4_mat_nnz);
   ++ctx->launches;
   CUDA_TRY(ctx, cudaGetLastError());
   return LANDAU_OK;
