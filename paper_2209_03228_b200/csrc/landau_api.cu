@@ -411,7 +411,8 @@ template <int NT>
 int launch_dmma(landau_ctx* ctx, const Group& gr, int ncols, int ncols_pad, int gcol0, int nsplit,
                 long long split_stride, cudaStream_t st) {
   constexpr int CT = 8 * NT;
-  const size_t smem = 2 * (CT * 3 * K2M_LD + 2 * K2M_TJ) * sizeof(double);
+  const size_t smem = (2 * (CT * 3 * K2M_LD + 2 * K2M_TJ) + 4 * LANDAU_ELLIP_TAB_BINADES * (LANDAU_ELLIP_TAB_DEG + 1) * 4) *
+                      sizeof(double);
   // per context (= per device), not per process: the attribute belongs to the device's copy of the function
   if (!(ctx->func_configured & (1u << NT))) {
     CUDA_TRY(ctx, cudaFuncSetAttribute(k2_inner_dmma<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

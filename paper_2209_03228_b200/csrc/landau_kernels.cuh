@@ -413,6 +413,9 @@ k2_inner_dmma(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
   extern __shared__ __align__(16) double smem[];
   // per stage: s_F[CT][3][K2M_LD], s_r[K2M_TJ], s_z[K2M_TJ]
   constexpr int STAGE = CT * 3 * K2M_LD + 2 * K2M_TJ;
+  constexpr int TAB = 4 * LANDAU_ELLIP_TAB_BINADES * (LANDAU_ELLIP_TAB_DEG + 1) * 4;
+  double* sTab = smem + 2 * STAGE;  // elliptic table T, copied once (visible after the first barrier of the tile loop)
+  for (int e = threadIdx.x; e < TAB; e += 256) sTab[e] = g_ellip_tab[e];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int gq = lane >> 2, tq = lane & 3;
   const int i = min((int)(blockIdx.x * 64 + warp * 8 + gq), n_i - 1);
@@ -445,6 +448,7 @@ k2_inner_dmma(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
     cp_async_commit();
   };
 
+  Tensor5 u = {0.0, 0.0, 0.0, 0.0, 0.0};
   if (t0 < t1) issue_tile(t0, 0);
   for (int t = t0; t < t1; ++t) {
     const int stage = (t - t0) & 1;
@@ -458,9 +462,20 @@ k2_inner_dmma(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
     const double* sF = smem + stage * STAGE;
     const double* s_r = sF + CT * 3 * K2M_LD;
     const double* s_z = s_r + K2M_TJ;
-#pragma unroll 1
+    // the tensor of the NEXT four source points is evaluated in stages between the DMMAs of the current four
+    // (PairEval: geometry, three Horner thirds, finish), so that its dependent FP64 chain hides under the DMMA stream;
+    // across a tile boundary the next points' coordinates come from global memory, fetched a whole tile earlier;
+    // only the very first four points are evaluated up front
+    constexpr int D = LANDAU_ELLIP_TAB_DEG, H1 = D - 1 - D / 3, H2 = H1 - D / 3;
+    if (t == t0) u = landau_tensor_2v(r, z, s_r[tq], s_z[tq], sTab);
+    const bool next_tile = t + 1 < t1;
+    const double rn = next_tile ? ip_r[j0 + (t + 1) * K2M_TJ + tq] : 1.0, zn = next_tile ? ip_z[j0 + (t + 1) * K2M_TJ + tq] : 0.0;
+#pragma unroll
     for (int jj = 0; jj < K2M_TJ; jj += 4) {
-      const Tensor5 u = landau_tensor_2v(r, z, s_r[jj + tq], s_z[jj + tq]);
+      const bool inner = jj + 4 < K2M_TJ;
+      const bool more = inner || next_tile;
+      PairEval pe;
+      if (more) pe.geometry(r, z, inner ? s_r[(jj + 4) % K2M_TJ + tq] : rn, inner ? s_z[(jj + 4) % K2M_TJ + tq] : zn, sTab);
 #pragma unroll
       for (int n = 0; n < NT; ++n) {
         const double* col = sF + ((n * 8 + gq) * 3) * K2M_LD + jj + tq;
@@ -472,7 +487,13 @@ k2_inner_dmma(const double* __restrict__ ip_r, const double* __restrict__ ip_z, 
         dmma884(acc[n][3][0], acc[n][3][1], u.UDrz, wfz);
         dmma884(acc[n][4][0], acc[n][4][1], u.UKzr, wfr);
         dmma884(acc[n][4][0], acc[n][4][1], u.UDzz, wfz);
+        if (more) {
+          if (n == (NT - 1) / 4) pe.template steps<D - 1, H1 + 1>();
+          if (n == (NT - 1) / 2) pe.template steps<H1, H2 + 1>();
+          if (n == (3 * (NT - 1)) / 4) pe.template steps<H2, 0>();
+        }
       }
+      if (more) u = pe.finish();
     }
     __syncthreads();
   }
