@@ -15,6 +15,11 @@ inner-integral kernel (K2) against the FP64 pipe peak measured in-process; cpu_b
 stands, on the host cores over a bounded sample of the same workload.
 
 `--impl reference` times the oracle only (no GPU work); under torchrun only rank 0 runs it.
+
+Extras that do not enter `value`: `--solve` times the batched TFQMR solve of the step's backward-Euler systems
+(key "solve"), `--advance N` runs N backward-Euler steps of the batch with landau_step (key "advance": seconds,
+Newton iterations, Newton iterations x batch per second -- the paper's throughput measure, PAPER.md:119);
+`--config 6` is the paper's own throughput problem.
 """
 import argparse
 import json
