@@ -369,6 +369,9 @@ def run_ours(args):
                            "l2": "working set per step (CSR out %.2f GB + scratch) exceeds the 126 MB L2; "
                                  "two input copies alternated" % (csr_bytes / 1e9)},
                 "pair_evals_per_s": {"tensor_evaluations_unique": pairs * world / (ms_per_step * 1e-3),
+                                     # the many-column kernel re-evaluates the tensor once per tile of 256 columns
+                                     "tensor_evaluations_executed": pairs * math.ceil(cols_pairs / pairs / 256.0) * world
+                                     / (ms_per_step * 1e-3) if separable and cols_pairs / pairs > 128 else None,
                                      "pair_applications_b_i_j": cols_pairs * world / (ms_per_step * 1e-3)},
                 "stage_ms_per_step": {"a1_fields": stage[0] / args.steps, "a2_inner": k2_ms,
                                       "a2b_combine": stage[2] / args.steps, "a3a4_assembly": k3_ms},
