@@ -342,3 +342,46 @@ def test_degenerate_cases(orc, Bn, torch_cuda):
                 assert np.linalg.norm(a - r) <= TOL * max(np.linalg.norm(r), 1e-300) or np.abs(r).max() == 0.0
     assert np.all(rhs[1, L.f_off[1]:L.f_off[2]] == 0.0)     # J[f] applied to f = 0 is exactly zero
     L.close()
+
+
+def test_outputs_stay_inside_their_buffers(Bn, torch_cuda):
+    """compute-sanitizer is not available on the pool: every output array is placed between two guard regions filled
+    with a sentinel, and the guards must be untouched after jacobian (ring, gather and stream-mode paths), apply,
+    spmv, solve and step."""
+    torch = torch_cuda
+    G = 4096
+    sentinel = -7.25e300
+
+    def guarded(rows, cols):
+        buf = torch.full((rows * cols + 2 * G,), sentinel, dtype=torch.float64, device="cuda")
+        return buf, buf[G:G + rows * cols].view(rows, cols)
+
+    def intact(buf, rows, cols):
+        return bool((buf[:G] == sentinel).all()) and bool((buf[G + rows * cols:] == sentinel).all())
+
+    for cfg, B in ((W.tiny_config("quadtree", 3, batch=5), 5), (W.config(3), 300)):
+        L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"])
+        f = torch.tensor(W.make_batch_f(cfg, [L.dof_coords(g) for g in range(L.G)], batch=B), device="cuda")
+        for asm in (0, 1):
+            Bn.landau_set_assembly_kernel(L.ctx, asm)
+            vb, vals = guarded(B, L.csr_stride)
+            Bn.landau_jacobian(L.ctx, f, B, cfg["dt"], vals)
+            torch.cuda.synchronize()
+            assert intact(vb, B, L.csr_stride) and bool(torch.isfinite(vals).all())
+        Bn.landau_set_assembly_kernel(L.ctx, 0)
+        rb, rhs = guarded(B, L.f_stride)
+        Bn.landau_apply(L.ctx, f, B, rhs)
+        yb, y = guarded(B, L.f_stride)
+        Bn.landau_spmv(L.ctx, vals, f, B, y)
+        xb, x = guarded(B, L.f_stride)
+        x.zero_()
+        Bn.landau_solve(L.ctx, vals, rhs, B, 1e-8, 100, x)
+        ub, u = guarded(B, L.f_stride)
+        u.copy_(f)
+        Bn.landau_step(L.ctx, u, B, 1e-3, 1e-6, 3, 1e-8, 200)
+        torch.cuda.synchronize()
+        for buf in (rb, yb, xb, ub):
+            assert intact(buf, B, L.f_stride)
+        for t in (rhs, y, x, u):
+            assert bool(torch.isfinite(t).all())
+        L.close()
