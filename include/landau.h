@@ -16,7 +16,9 @@
  *     calls on one context must be serialised by the caller.  Different contexts are independent.
  *   - landau_jacobian / landau_apply are asynchronous on `cuda_stream` (a cudaStream_t passed as void*; NULL =
  *     legacy default stream) and perform no hidden device synchronisation unless their scratch must grow
- *     (first call with a larger batch: one cudaMalloc).
+ *     (first call with a larger batch: one cudaMalloc; landau_reserve pre-sizes it).  Stages are bracketed by NVTX
+ *     ranges ("landau K1 ..", "landau K2 ..", ...).
+ *   - diagnostics, probes and tuning knobs (not part of the product ABI) are declared in landau_debug.h.
  *   - there is no CPU fallback: without a CUDA device landau_create fails with LANDAU_CUDA_ERROR.
  *
  * Units and discretisation (readings A3-A17): velocity coordinates of every grid are in the common
@@ -173,61 +175,13 @@ int landau_jacobian_host(landau_ctx* ctx, const double* batch_f_host, int batch,
                          void* cuda_stream);
 int landau_apply_host(landau_ctx* ctx, const double* batch_f_host, int batch, double* out_rhs_host, void* cuda_stream);
 
-/* Diagnostics -------------------------------------------------------------------------------------------- */
+/* Pre-size every scratch buffer of landau_jacobian / landau_apply / landau_jacobian_apply for calls with
+ * batch <= max_batch (at the current batch chunk), so that those calls neither allocate nor synchronise from the first
+ * one on.  Optional: without it the scratch grows on demand (one cudaMalloc + device synchronisation per growth).
+ * Synchronises the device.  LANDAU_OUT_OF_MEMORY leaves the context usable. */
+int landau_reserve(landau_ctx* ctx, int max_batch);
 
-/* Copy out the frozen coefficients of the LAST landau_jacobian / landau_apply call (synchronises the stream it
- * ran on): dk_host[batch][species a][5][n_ip[grid(a)]] = (Drr, Drz, Dzz, Kr, Kz) at the integration points.
- * Only the last pass is kept, so the call is meaningful when batch <= the batch chunk. */
-int landau_last_coefficients(landau_ctx* ctx, double* dk_host);
-
-/* Evaluate the 2V Landau tensor kernel on the device for n point pairs (dev arrays r,z,rb,zb of n doubles):
- * out_dev[5*n] = (UD_rr, UD_rz, UD_zz, UK_rr, UK_zr) per pair, UK_rz = UD_rz, UK_zz = UD_zz; coincident
- * pairs give zeros.  Same device function as the inner-integral kernel uses. */
-int landau_tensor_eval(const double* r_dev, const double* z_dev, const double* rb_dev, const double* zb_dev, int n,
-                       double* out_dev, void* cuda_stream);
-
-/* Elliptic pieces on the device: for n pairs (m[i], mp[i] = 1-m[i] given separately) out_dev[3*n] =
- * (P0, Dc, Q) = INT_0^{pi/2} {1, cos^2, sin^2 cos^2} (1 - m sin^2)^{-3/2} dtheta. */
-int landau_ellip_eval(const double* m_dev, const double* mp_dev, int n, double* out_dev, void* cuda_stream);
-
-/* FP64 pipe probes used by bench.py for the roofline denominator: run `iters` rounds of register-resident
- * DFMA (kind 0), DMMA m8n8k4 (kind 1) or both interleaved (kind 2) on every SM; *tflops receives the achieved FP64 TFLOP/s
- * (CUDA-event timed on `cuda_stream`, synchronises it). */
-int landau_fp64_probe(int kind, int iters, double* tflops, void* cuda_stream);
-
-/* 1 if the collision-frequency matrix was detected as rank one (nu_ab = a_a b_b: one summed source column per
- * batch entry), 0 if the general per-species-column path is used; negative on error. */
-int landau_is_separable(const landau_ctx* ctx);
-
-/* Number of kernels the library launched on behalf of this context since creation (bench's gpu_launches). */
-long long landau_launch_count(const landau_ctx* ctx);
-
-/* Per-stage device time of the LAST jacobian/apply call in milliseconds, summed over its passes: ms[0] field
- * evaluation, ms[1] inner integral, ms[2] coefficient combination, ms[3] element matrices + assembly (or apply).
- * Recording is enabled with landau_set_timing(ctx, 1): the compute calls then only RECORD CUDA events on their
- * stream (no synchronisation is added to them); landau_last_stage_ms waits for the last event and reads them. */
-int landau_set_timing(landau_ctx* ctx, int enabled);
-int landau_last_stage_ms(landau_ctx* ctx, float* ms4);
-
-/* Choose the inner-integral kernel: 0 auto (by column count), 1 plain DFMA kernel, 2 DMMA kernel with per-warp
- * tensor generation, 3 / 4 DMMA GEMM kernel with the tensor tile evaluated once per CTA and shared by its warps
- * (TMA-staged source tiles; 32 x 128 / 16 x 256 CTA tile: 4 is the default for more than 128 source columns). */
-int landau_set_inner_kernel(landau_ctx* ctx, int which);
-
-/* Choose the element-matrix + assembly kernel: 0 auto (k3_ring: DMMA sum-factorised element matrices kept in a
- * shared-memory ring, CSR slots gathered from it; used for every grid whose ring fits in shared memory),
- * 1 force the general slot-gather kernel (k3_assemble: one thread per CSR slot, scalar FP64). */
-int landau_set_assembly_kernel(landau_ctx* ctx, int which);
-
-/* Schedule of the ring assembly kernel for grid g (host query, works on host-only contexts): ring_cells = element
- * matrices kept in shared memory (0: the ring does not fit, the slot-gather kernel is used for this grid),
- * n_steps = panels of 16 cells, n_simple_slots = CSR slots fed by exactly one element-matrix entry with weight 1. */
-int landau_assembly_info(const landau_ctx* ctx, int grid, int* ring_cells, int* n_steps, int* n_simple_slots);
-
-/* Batch entries pushed through the stages per pass (default 1024); scratch is sized for one pass, so that the
- * intermediates (source fields, partial sums, D/K) of a pass stay L2-resident.  chunk >= 1. */
-int landau_set_batch_chunk(landau_ctx* ctx, int chunk);
-
+/* Message of the last failure of `ctx` (ctx == NULL: of the last failed landau_create); owned by the library. */
 const char* landau_last_error(const landau_ctx* ctx);
 
 #ifdef __cplusplus

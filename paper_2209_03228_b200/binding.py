@@ -16,12 +16,16 @@ LANDAU_OK = 0
 STATUS = {0: "LANDAU_OK", -1: "LANDAU_INVALID_ARG", -2: "LANDAU_UNSUPPORTED", -3: "LANDAU_OUT_OF_MEMORY",
           -4: "LANDAU_CUDA_ERROR"}
 
-# every symbol include/landau.h declares (tests check that the library exports all of them)
+# every symbol include/landau.h (the product ABI) and include/landau_debug.h (diagnostics, probes, tuning knobs)
+# declare; tests check that the headers and these lists agree and that the library exports all of them
 SYMBOLS = ["landau_create", "landau_destroy", "landau_sizes", "landau_dof_coords", "landau_ip_table",
-           "landau_csr_pattern", "landau_csr_pattern_host", "landau_jacobian", "landau_apply", "landau_spmv", "landau_solve", "landau_jacobian_apply", "landau_step", "landau_jacobian_host",
-           "landau_apply_host", "landau_last_coefficients", "landau_tensor_eval", "landau_ellip_eval",
-           "landau_fp64_probe", "landau_launch_count", "landau_is_separable", "landau_set_timing", "landau_last_stage_ms",
-           "landau_set_inner_kernel", "landau_set_assembly_kernel", "landau_assembly_info", "landau_set_batch_chunk", "landau_last_error"]
+           "landau_csr_pattern", "landau_csr_pattern_host", "landau_jacobian", "landau_apply", "landau_spmv",
+           "landau_solve", "landau_jacobian_apply", "landau_step", "landau_jacobian_host", "landau_apply_host",
+           "landau_reserve", "landau_last_error"]
+DEBUG_SYMBOLS = ["landau_last_coefficients", "landau_tensor_eval", "landau_ellip_eval", "landau_fp64_probe",
+                 "landau_launch_count", "landau_is_separable", "landau_set_timing", "landau_last_stage_ms",
+                 "landau_set_inner_kernel", "landau_set_assembly_kernel", "landau_assembly_info",
+                 "landau_set_batch_chunk"]
 
 
 class LandauError(RuntimeError):
@@ -201,10 +205,15 @@ def landau_apply_host(ctx, batch_f_host, batch, out_rhs_host, stream=None):
                                     _stream(stream)), ctx)
 
 
-def landau_last_coefficients(ctx, n_doubles):
-    out = np.zeros(n_doubles)
-    _check(load().landau_last_coefficients(ctx, _np(out)), ctx)
+def landau_last_coefficients(ctx, n_entries, dk_stride):
+    """Coefficients of the first `n_entries` entries of the last pass: array [n_entries * dk_stride]."""
+    out = np.zeros(int(n_entries) * int(dk_stride))
+    _check(load().landau_last_coefficients(ctx, _np(out), C.c_int(n_entries)), ctx)
     return out
+
+
+def landau_reserve(ctx, max_batch):
+    _check(load().landau_reserve(ctx, C.c_int(max_batch)), ctx)
 
 
 def landau_tensor_eval(r, z, rb, zb, out, stream=None):
@@ -334,7 +343,7 @@ class Landau:
 
     def last_coefficients(self, batch):
         """list over species of arrays [batch, 5, n_ip]."""
-        raw = landau_last_coefficients(self.ctx, batch * self.dk_stride).reshape(batch, self.dk_stride)
+        raw = landau_last_coefficients(self.ctx, batch, self.dk_stride).reshape(batch, self.dk_stride)
         out, o = [], 0
         for g in self.sgrid:
             n = 5 * int(self.n_ip[g])

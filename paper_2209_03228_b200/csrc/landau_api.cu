@@ -7,7 +7,10 @@
 #include <string>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "../../include/landau.h"
+#include "../../include/landau_debug.h"
 #include "host_setup.hpp"
 #include "landau_kernels.cuh"
 #include "k3_ring.cuh"
@@ -126,7 +129,9 @@ int upload(landau_ctx* ctx, const std::vector<T>& h, const T** out) {
   return LANDAU_OK;
 }
 
-int grow(landau_ctx* ctx, double** p, size_t* cap, size_t need, bool zero) {
+// Scratch growth.  `zero` clears the new block ON `st` (the stream the consumer kernels run on: a cudaMemset on the
+// legacy stream is not ordered with a cudaStreamNonBlocking stream).
+int grow(landau_ctx* ctx, double** p, size_t* cap, size_t need, bool zero, cudaStream_t st = nullptr) {
   if (need <= *cap) return LANDAU_OK;
   if (*p) {
     CUDA_TRY(ctx, cudaDeviceSynchronize());
@@ -135,12 +140,37 @@ int grow(landau_ctx* ctx, double** p, size_t* cap, size_t need, bool zero) {
     *cap = 0;
   }
   CUDA_TRY(ctx, cudaMalloc(p, need * sizeof(double)));
-  if (zero) CUDA_TRY(ctx, cudaMemset(*p, 0, need * sizeof(double)));
+  if (zero) CUDA_TRY(ctx, cudaMemsetAsync(*p, 0, need * sizeof(double), st));
   *cap = need;
   return LANDAU_OK;
 }
 
 int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+// NVTX range around the launches of one stage (visible in Nsight Systems / ncu --nvtx; free when no tool is attached)
+struct NvtxRange {
+  bool open = true;
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  void end() {
+    if (open) nvtxRangePop();
+    open = false;
+  }
+  ~NvtxRange() { end(); }
+};
+
+// Dynamic shared-memory limit of a kernel whose need depends on the context (k3_ring: ring size, k4_tfqmr: system size).
+// The attribute belongs to the device's copy of the function, not to a context: keep a per-device high-water mark and
+// only ever raise it, so that two live contexts of different sizes on one GPU can be used alternately.
+constexpr int MAX_DEVICES = 64;
+size_t g_k3_smem_set[MAX_DEVICES] = {0}, g_k4_smem_set[MAX_DEVICES] = {0};
+template <class F>
+int raise_smem_limit(landau_ctx* ctx, F func, size_t* table, size_t bytes) {
+  size_t* cur = ctx->device >= 0 && ctx->device < MAX_DEVICES ? &table[ctx->device] : nullptr;
+  if (cur && bytes <= *cur) return LANDAU_OK;
+  CUDA_TRY(ctx, cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  if (cur) *cur = bytes;
+  return LANDAU_OK;
+}
 
 // stage timing: events are only recorded here (no synchronisation); landau_last_stage_ms resolves them
 void mark(landau_ctx* ctx, cudaStream_t st) {
@@ -290,7 +320,7 @@ int build_device_side(landau_ctx* ctx) {
     ctx->d_k3grid = const_cast<K3Grid*>(tg);
     ctx->d_k3spec = const_cast<K3Species*>(tsp);
     if (ctx->k3_nspec)
-      CUDA_TRY(ctx, cudaFuncSetAttribute(k3_ring, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->k3_smem));
+      if (int rc = raise_smem_limit(ctx, k3_ring, g_k3_smem_set, ctx->k3_smem)) return rc;
   }
   // batched solve: pattern views per grid, block offsets per species
   {
@@ -321,7 +351,7 @@ int build_device_side(landau_ctx* ctx) {
     const size_t mat = (size_t)max_nnz * 12 + (size_t)(ctx->k4_max_n + 2) * 4;
     ctx->k4_mat_nnz = (ctx->k4_max_n <= ctx->k4_smem_n && ctx->k4_smem + mat <= 56 * 1024) ? max_nnz : 0;
     if (ctx->k4_mat_nnz) ctx->k4_smem += mat + K4_NVEC * sizeof(double);  // vectors padded to an even length
-    CUDA_TRY(ctx, cudaFuncSetAttribute(k4_tfqmr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->k4_smem));
+    if (int rc = raise_smem_limit(ctx, k4_tfqmr, g_k4_smem_set, ctx->k4_smem)) return rc;
   }
   // source columns: separable nu => one group over all grids, one column per batch entry;
   // general nu => one group per grid, one column per species of the grid.
@@ -431,6 +461,26 @@ constexpr int K2BIG_TC = K2Big::TC;
 // wide variant: 16 x 256 CTA tile (one tensor pair per thread per source tile), 2 B stages
 using K2Wide = K2G<2, 4, 1, 8, 2>;
 
+// Stream mode of the many-column kernel (k2_gemm.cuh): persistent CTAs, one per SM, when the tiles do not fill whole
+// waves.  It needs every CTA to own at least one (tile, source tile) step of the partial wave: with
+// R = (T mod P) njt < P some shares [R p / P, R (p+1) / P) would be empty and the kernel's part count (which counts CTAs
+// first..last) would never be reached -- such shapes run in grid mode.
+template <class C>
+bool gemm_stream_mode(const landau_ctx* ctx, const Group& gr, int ncols, int nsplit) {
+  const int n_it = (ctx->n_i_pad + C::TI - 1) / C::TI, n_ct = (ncols + C::TC - 1) / C::TC, T = n_it * n_ct, P = ctx->n_sm;
+  return ctx->stream_k && nsplit == 1 && T >= P && T % P != 0 && (long long)(T % P) * (gr.nj_pad / K2G_TJ) >= P;
+}
+// doubles of part_buf a stream-mode launch needs (accumulator dumps of the cut tiles + their arrival counters)
+template <class C>
+size_t gemm_part_need(const landau_ctx* ctx, const Group& gr, int ncols, int nsplit, int* part_stride_out = nullptr) {
+  if (!gemm_stream_mode<C>(ctx, gr, ncols, nsplit)) return 0;
+  const int n_it = (ctx->n_i_pad + C::TI - 1) / C::TI, n_ct = (ncols + C::TC - 1) / C::TC;
+  const int T = n_it * n_ct, P = ctx->n_sm, r = T % P;
+  const int part_stride = (P + r - 1) / r + 2;  // parts per cut tile, upper bound
+  if (part_stride_out) *part_stride_out = part_stride;
+  return (size_t)r * part_stride * C::ACC_PER_THREAD * C::NTHREADS + (size_t)(P + 1) / 2 + 1;
+}
+
 template <int WI_T, int WC_T, int WGI, int WGC, int NST>
 int launch_gemm_t(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nsplit, long long split_stride,
                   cudaStream_t st) {
@@ -442,15 +492,14 @@ int launch_gemm_t(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int ns
     ctx->func_configured |= bit;
   }
   const int n_it = (ctx->n_i_pad + C::TI - 1) / C::TI, n_ct = (ncols + C::TC - 1) / C::TC;
-  const bool stream = ctx->stream_k && nsplit == 1 && n_it * n_ct >= ctx->n_sm && (n_it * n_ct) % ctx->n_sm != 0;
-  if (stream) {
-    // persistent CTAs, one per SM: whole tiles for the full waves, the tiles of the last partial wave cut evenly over all
-    // CTAs; parts of a cut tile meet in part_buf and are added in part order by the last CTA to arrive (k2_gemm.cuh)
+  if (gemm_stream_mode<C>(ctx, gr, ncols, nsplit)) {
+    // whole tiles for the full waves, the tiles of the last partial wave cut evenly over all CTAs; parts of a cut tile
+    // meet in part_buf and are added in part order by the last CTA to arrive (k2_gemm.cuh)
     const int T = n_it * n_ct, P = ctx->n_sm, r = T % P;
-    const int part_stride = (P + r - 1) / r + 2;  // parts per cut tile, upper bound
+    int part_stride = 0;
+    const size_t need = gemm_part_need<C>(ctx, gr, ncols, nsplit, &part_stride);
+    if (int rc = grow(ctx, &ctx->part_buf, &ctx->part_cap, need, false)) return rc;
     const size_t per_part = (size_t)C::ACC_PER_THREAD * C::NTHREADS;
-    if (int rc = grow(ctx, &ctx->part_buf, &ctx->part_cap, (size_t)r * part_stride * per_part + (size_t)(P + 1) / 2 + 1, false))
-      return rc;
     int* part_count = reinterpret_cast<int*>(ctx->part_buf + (size_t)r * part_stride * per_part);
     CUDA_TRY(ctx, cudaMemsetAsync(part_count, 0, sizeof(int) * P, st));
     k2_inner_gemm<WI_T, WC_T, WGI, WGC, NST><<<dim3(P, 1, 1), C::NTHREADS, C::SMEM_BYTES, st>>>(
@@ -481,54 +530,82 @@ int pick_kernel(const landau_ctx* ctx, int ncols) {
   return ncols > 128 ? 4 : ncols > 96 ? 3 : (ncols >= 8 ? 2 : 1);  // crossovers measured on config 2 (N = 4096)
 }
 
+// Column layout, kernel choice, j-split and scratch needs of one pass over `nbc` batch entries.
+struct ChunkPlan {
+  std::vector<int> gcol0, ncols, ncols_pad, kern;
+  std::vector<long long> f_off;
+  long long f_doubles = 0, split_stride = 0, layout_key = 0;
+  int total_cols = 0, nsplit = 1;
+  size_t part_doubles = 0;
+};
+
+ChunkPlan plan_chunk(const landau_ctx* ctx, int nbc) {
+  ChunkPlan pl;
+  const size_t nq = ctx->groups.size();
+  pl.gcol0.resize(nq);
+  pl.ncols.resize(nq);
+  pl.ncols_pad.resize(nq);
+  pl.kern.resize(nq);
+  pl.f_off.resize(nq);
+  for (size_t q = 0; q < nq; ++q) {
+    const Group& gr = ctx->groups[q];
+    pl.ncols[q] = nbc * gr.ncb;
+    pl.kern[q] = pick_kernel(ctx, pl.ncols[q]);
+    pl.ncols_pad[q] = round_up(pl.ncols[q], pl.kern[q] >= 3 ? kern_tc(pl.kern[q]) : 64);
+    pl.layout_key = pl.layout_key * 1000003 + pl.ncols_pad[q] * 4 + pl.kern[q];
+    pl.f_off[q] = pl.f_doubles;
+    pl.f_doubles += (long long)pl.ncols_pad[q] * 3 * gr.nj_pad;
+    pl.gcol0[q] = pl.total_cols;
+    pl.total_cols += pl.ncols[q];
+  }
+  // j-split so that small problems still fill the machine
+  int max_blocks = 1 << 30;
+  for (size_t q = 0; q < nq; ++q) {
+    const int k = pl.kern[q];
+    const int blocks = k >= 3   ? ((ctx->n_i_pad + kern_ti(k) - 1) / kern_ti(k)) * (pl.ncols_pad[q] / kern_tc(k))
+                       : k == 2 ? ((ctx->n_i_pad + 63) / 64) * ((pl.ncols[q] + 63) / 64)
+                                : ((ctx->n_i_pad + 127) / 128) * ((pl.ncols[q] + 3) / 4);
+    if (blocks < max_blocks) max_blocks = blocks;
+  }
+  const int want = 2 * ctx->n_sm;
+  if (max_blocks < want) {
+    pl.nsplit = (want + max_blocks - 1) / max_blocks;
+    int min_tiles = 1 << 30;
+    for (const Group& gr : ctx->groups) min_tiles = std::min(min_tiles, gr.nj_pad / K2M_TJ);
+    pl.nsplit = std::max(1, std::min(std::min(pl.nsplit, min_tiles), 64));
+  }
+  pl.split_stride = (long long)pl.total_cols * 5 * ctx->n_i_pad;
+  for (size_t q = 0; q < nq; ++q) {
+    size_t need = 0;
+    if (pl.kern[q] == 4) need = gemm_part_need<K2Wide>(ctx, ctx->groups[q], pl.ncols[q], pl.nsplit);
+    if (pl.kern[q] == 3) need = gemm_part_need<K2Big>(ctx, ctx->groups[q], pl.ncols[q], pl.nsplit);
+    pl.part_doubles = std::max(pl.part_doubles, need);
+  }
+  return pl;
+}
+
 // stages a1..a2b for batch entries [b0, b0+nbc): leaves D,K in ctx->DK
 int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cudaStream_t st) {
   const int G = ctx->G, S = ctx->S;
-  // column bookkeeping for this chunk
-  long long foff = 0;
-  int total_cols = 0;
-  std::vector<int> gcol0(ctx->groups.size()), ncols(ctx->groups.size()), ncols_pad(ctx->groups.size()),
-      kern(ctx->groups.size());
-  long long layout_key = 0;
-  for (size_t q = 0; q < ctx->groups.size(); ++q) {
-    Group& gr = ctx->groups[q];
-    ncols[q] = nbc * gr.ncb;
-    kern[q] = pick_kernel(ctx, ncols[q]);
-    ncols_pad[q] = round_up(ncols[q], kern[q] >= 3 ? kern_tc(kern[q]) : 64);
-    layout_key = layout_key * 1000003 + ncols_pad[q] * 4 + kern[q];
-    gr.f_off = foff;
-    foff += (long long)ncols_pad[q] * 3 * gr.nj_pad;
-    gcol0[q] = total_cols;
-    total_cols += ncols[q];
-  }
-  // j-split so that small problems still fill the machine
-  int max_blocks = 1 << 30, nsplit = 1;
-  for (size_t q = 0; q < ctx->groups.size(); ++q) {
-    const int blocks = kern[q] >= 3   ? ((ctx->n_i_pad + kern_ti(kern[q]) - 1) / kern_ti(kern[q])) * (ncols_pad[q] / kern_tc(kern[q]))
-                       : kern[q] == 2 ? ((ctx->n_i_pad + 63) / 64) * ((ncols[q] + 63) / 64)
-                                      : ((ctx->n_i_pad + 127) / 128) * ((ncols[q] + 3) / 4);
-    if (blocks < max_blocks) max_blocks = blocks;
-  }
-  if (max_blocks < 296) {
-    nsplit = (296 + max_blocks - 1) / max_blocks;
-    int min_tiles = 1 << 30;
-    for (const Group& gr : ctx->groups) min_tiles = std::min(min_tiles, gr.nj_pad / K2M_TJ);
-    nsplit = std::max(1, std::min(std::min(nsplit, min_tiles), 64));
-  }
-  const long long split_stride = (long long)total_cols * 5 * ctx->n_i_pad;
+  const ChunkPlan pl = plan_chunk(ctx, nbc);
+  const std::vector<int>&gcol0 = pl.gcol0, &ncols = pl.ncols, &ncols_pad = pl.ncols_pad, &kern = pl.kern;
+  const int total_cols = pl.total_cols, nsplit = pl.nsplit;
+  const long long split_stride = pl.split_stride;
+  for (size_t q = 0; q < ctx->groups.size(); ++q) ctx->groups[q].f_off = pl.f_off[q];
   {
     const size_t cap0 = ctx->F_cap;
-    if (int rc = grow(ctx, &ctx->F, &ctx->F_cap, (size_t)foff, true)) return rc;
+    if (int rc = grow(ctx, &ctx->F, &ctx->F_cap, (size_t)pl.f_doubles, true, st)) return rc;
     // padding columns / padding source points must read as zero: re-zero when the layout changes
-    if (layout_key != ctx->f_layout_key && cap0 == ctx->F_cap)
-      CUDA_TRY(ctx, cudaMemsetAsync(ctx->F, 0, (size_t)foff * sizeof(double), st));
-    ctx->f_layout_key = layout_key;
+    if (pl.layout_key != ctx->f_layout_key && cap0 == ctx->F_cap)
+      CUDA_TRY(ctx, cudaMemsetAsync(ctx->F, 0, (size_t)pl.f_doubles * sizeof(double), st));
+    ctx->f_layout_key = pl.layout_key;
   }
   if (int rc = grow(ctx, &ctx->Gp, &ctx->Gp_cap, (size_t)split_stride * nsplit, false)) return rc;
   if (int rc = grow(ctx, &ctx->DK, &ctx->DK_cap, (size_t)ctx->dk_stride * nbc, false)) return rc;
 
   mark(ctx, st);
   // K1
+  nvtxRangePushA("landau K1 fields (a1)");
   for (int g = 0; g < G; ++g) {
     const int q = ctx->mix_group[g];
     const Group& gr = ctx->groups[q];
@@ -542,8 +619,10 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
                                                ctx->F + gr.f_off, gr.nj_pad, joff, 0, kern_tc(kern[q]));
     ++ctx->launches;
   }
+  nvtxRangePop();
   mark(ctx, st);
   // K2
+  NvtxRange k2_range("landau K2 inner integral (a2)");
   for (size_t q = 0; q < ctx->groups.size(); ++q) {
     const Group& gr = ctx->groups[q];
     if (kern[q] == 4) {
@@ -571,7 +650,9 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
     }
     ++ctx->launches;
   }
+  k2_range.end();
   mark(ctx, st);
+  NvtxRange k2b_range("landau K2b combine (a2)");
   // K2b: one launch over (IP, entry, species); the resolved tables are re-uploaded only when the column layout changes
   if (ctx->comb_key != total_cols || !ctx->d_comb) {
     ctx->comb_resolved = ctx->comb;
@@ -622,6 +703,7 @@ int check_call(landau_ctx* ctx, const void* in, int batch, const void* out) {
 
 // a3 + a4 for batch entries [b0, b0 + nbc) from the coefficients in ctx->DK
 int assemble_chunk(landau_ctx* ctx, int b0, int nbc, double inv_dt, double* out_csr_vals_dev, cudaStream_t st) {
+    NvtxRange range("landau K3 element matrices + assembly (a3+a4)");
     double* vals = out_csr_vals_dev + (long long)b0 * ctx->v_stride;
     if (ctx->k3_nspec && ctx->assembly_kernel != 1) {
       // at least one wave of 4 CTAs per SM; the cell range is cut into segments (each with a recomputed halo) only
@@ -651,6 +733,7 @@ int assemble_chunk(landau_ctx* ctx, int b0, int nbc, double inv_dt, double* out_
 
 // a5 for batch entries [b0, b0 + nbc) from the coefficients in ctx->DK
 int apply_chunk(landau_ctx* ctx, const double* batch_f_dev, int b0, int nbc, double* out_rhs_dev, cudaStream_t st) {
+    NvtxRange range("landau K3' apply (a5)");
     if (int rc = grow(ctx, &ctx->FL, &ctx->FL_cap, (size_t)ctx->fl_stride * nbc, false)) return rc;
     for (int s = 0; s < ctx->S; ++s) {
       const int g = ctx->species[s].grid;
@@ -810,6 +893,34 @@ int landau_csr_pattern_host(const landau_ctx* ctx, int grid, int* rowptr_host, i
   const HostGrid& h = ctx->hg[grid];
   memcpy(rowptr_host, h.rowptr.data(), sizeof(int) * h.rowptr.size());
   memcpy(colidx_host, h.colidx.data(), sizeof(int) * h.colidx.size());
+  return LANDAU_OK;
+}
+
+int landau_reserve(landau_ctx* ctx, int max_batch) {
+  if (!ctx || max_batch < 1) return ctx ? fail(ctx, LANDAU_INVALID_ARG, "landau_reserve: max_batch >= 1") : LANDAU_INVALID_ARG;
+  if (ctx->device < 0) return fail(ctx, LANDAU_CUDA_ERROR, "host-only context (cuda_device < 0): no compute, no CPU fallback");
+  CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+  // the needs are not monotone in the pass size (small passes split the source range over more planes): take the
+  // largest need over every pass size a call with batch <= max_batch can produce
+  const int top = std::min(ctx->chunk, max_batch);
+  size_t f = 0, gp = 0, part = 0;
+  for (int nbc = 1; nbc <= top; ++nbc) {
+    const ChunkPlan pl = plan_chunk(ctx, nbc);
+    f = std::max(f, (size_t)pl.f_doubles);
+    gp = std::max(gp, (size_t)pl.split_stride * pl.nsplit);
+    part = std::max(part, pl.part_doubles);
+  }
+  if (int rc = grow(ctx, &ctx->F, &ctx->F_cap, f, true)) return rc;
+  ctx->f_layout_key = -1;
+  if (int rc = grow(ctx, &ctx->Gp, &ctx->Gp_cap, gp, false)) return rc;
+  if (int rc = grow(ctx, &ctx->part_buf, &ctx->part_cap, part, false)) return rc;
+  if (int rc = grow(ctx, &ctx->DK, &ctx->DK_cap, (size_t)ctx->dk_stride * top, false)) return rc;
+  if (int rc = grow(ctx, &ctx->FL, &ctx->FL_cap, (size_t)ctx->fl_stride * top, false)) return rc;
+  if (!ctx->d_comb) {
+    CUDA_TRY(ctx, cudaMalloc(&ctx->d_comb, sizeof(CombineTable) * ctx->S));
+    ctx->allocs.push_back(ctx->d_comb);
+  }
+  CUDA_TRY(ctx, cudaDeviceSynchronize());
   return LANDAU_OK;
 }
 
@@ -1036,12 +1147,15 @@ int landau_step(landau_ctx* ctx, double* u_dev, int batch, double dt, double new
   return LANDAU_OK;
 }
 
-int landau_last_coefficients(landau_ctx* ctx, double* dk_host) {
-  if (!ctx || !dk_host) return LANDAU_INVALID_ARG;
+int landau_last_coefficients(landau_ctx* ctx, double* dk_host, int n_entries) {
+  if (!ctx || !dk_host || n_entries < 1) return LANDAU_INVALID_ARG;
   if (ctx->device < 0 || ctx->last_batch == 0 || !ctx->DK) return fail(ctx, LANDAU_INVALID_ARG, "no previous jacobian/apply call");
+  if (n_entries > ctx->last_batch)
+    return fail(ctx, LANDAU_INVALID_ARG, "landau_last_coefficients: only the last pass is kept (" +
+                                             std::to_string(ctx->last_batch) + " entries), " + std::to_string(n_entries) + " asked");
   CUDA_TRY(ctx, cudaSetDevice(ctx->device));
   CUDA_TRY(ctx, cudaStreamSynchronize(ctx->last_stream));
-  CUDA_TRY(ctx, cudaMemcpy(dk_host, ctx->DK, sizeof(double) * ctx->dk_stride * ctx->last_batch, cudaMemcpyDeviceToHost));
+  CUDA_TRY(ctx, cudaMemcpy(dk_host, ctx->DK, sizeof(double) * ctx->dk_stride * n_entries, cudaMemcpyDeviceToHost));
   return LANDAU_OK;
 }
 

@@ -20,20 +20,36 @@ def lib():
     return Bn.load()
 
 
-def _declared_symbols():
-    text = open(os.path.join(ROOT, "include", "landau.h")).read()
+def _declared_symbols(header):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(landau_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_library_exports_every_declared_symbol(lib):
-    names = _declared_symbols()
-    assert "landau_create" in names and "landau_jacobian" in names and "landau_apply" in names
-    for n in names:
+    names = _declared_symbols("landau.h")
+    # the calls SURVEY 8(b) lists are in the product header
+    for n in ("landau_create", "landau_destroy", "landau_sizes", "landau_dof_coords", "landau_csr_pattern",
+              "landau_jacobian", "landau_apply", "landau_last_error"):
+        assert n in names
+    debug = _declared_symbols("landau_debug.h")
+    assert not set(names) & set(debug)
+    for n in names + debug:
         assert hasattr(lib, n), "liblandau_b200.so does not export %s" % n
     assert sorted(Bn.SYMBOLS) == names, "binding.SYMBOLS out of date with include/landau.h"
-    for n in names:  # the binding carries the same names
+    assert sorted(Bn.DEBUG_SYMBOLS) == debug, "binding.DEBUG_SYMBOLS out of date with include/landau_debug.h"
+    for n in names + debug:  # the binding carries the same names
         assert hasattr(Bn, n), "binding lacks %s" % n
+
+
+def test_reserve_refuses_without_device(lib):
+    cfg = W.tiny_config("uniform", 2, batch=1)
+    ctx = Bn.landau_create(cfg["grids"], cfg["species"], cfg["degree"], cuda_device=-1)
+    with pytest.raises(Bn.LandauError, match="no CPU fallback"):
+        Bn.landau_reserve(ctx, 4)
+    with pytest.raises(Bn.LandauError):
+        Bn.landau_reserve(ctx, 0)
+    Bn.landau_destroy(ctx)
 
 
 def test_no_cpu_fallback_compute_refuses_without_device(lib):

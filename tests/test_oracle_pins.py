@@ -255,13 +255,48 @@ def test_P6_conservation_to_roundoff(orc, kind, degree):
         assert np.abs(colsum).max() < 1e-13 * colabs.max()
 
 
-def test_P6_shift_is_mass_over_dt(orc):
-    cfg = W.tiny_config("quadtree", 2, two_species=False)
-    o = orc.Oracle(cfg["grids"], cfg["species"], 2)
-    f = W.make_batch_f(cfg, [o.dof_coords(0)], batch=1)[0]
-    a = o.jacobian(f, 0.25)
-    b = o.jacobian(f, float("inf"))
-    assert np.allclose(a - b, o.mass(0) / 0.25, rtol=0, atol=1e-13 * np.abs(a).max())
+def _csr_bilinear(rp, ci, vals, p, q):
+    """p^T A q for a CSR matrix."""
+    return float(sum(p[i] * np.dot(vals[rp[i]:rp[i + 1]], q[ci[rp[i]:rp[i + 1]]]) for i in range(len(rp) - 1)))
+
+
+@pytest.mark.parametrize("grid", [dict(kind=1, r_max=5.0, z_min=-5.0, z_max=5.0, nr=2, nz=4, levels=1),
+                                  dict(kind=1, r_max=3.0, z_min=-1.0, z_max=5.0, nr=4, nz=8, levels=3)],
+                         ids=["14cells", "104cells"])
+@pytest.mark.parametrize("degree", [2, 3])
+def test_P6_shift_and_mass_closed_forms_on_quadtree(orc, grid, degree):
+    """The shift of the output matrix (M/dt - J) - (-J) is M/dt, and M on a QUADTREE grid is pinned by closed forms (not by
+    the oracle's own mass()): with nodal vectors p, q of polynomials of degree <= k per direction, p^T M q = INT p q r dr dz
+    exactly (the hanging-node fold P_e^T M_e P_e reproduces polynomials; Gauss rule exact to degree 2k+1)."""
+    R, z0, z1 = grid["r_max"], grid["z_min"], grid["z_max"]
+    o = orc.Oracle([grid], [dict(mass=1.0, charge=-1.0, grid=0)], degree)
+    rz = o.dof_coords(0)
+    f = W.sample_state(1.0, 1.0, 1.0, 0.1, 1.0, rz)
+    dt = 0.25
+    shift = (o.jacobian(f, dt) - o.jacobian(f, float("inf"))) * dt
+    M = o.mass(0)
+    rp, ci = o.pattern(0)
+    scale = np.abs(M).max()
+    assert np.abs(shift - M).max() < 1e-12 * max(scale, np.abs(o.jacobian(f, dt)).max() * dt)
+
+    def mono_int(a, b):  # INT_0^R r^a r dr * INT_z0^z1 z^b dz
+        return R ** (a + 2) / (a + 2) * (z1 ** (b + 1) - z0 ** (b + 1)) / (b + 1)
+
+    for vals in (M, shift):
+        assert abs(vals.sum() - mono_int(0, 0)) < 1e-11 * mono_int(0, 0)
+        for (a1, b1, a2, b2) in [(1, 0, 0, 1), (degree, 0, degree, 0), (0, degree, 0, degree), (1, degree, degree, 1),
+                                 (degree, degree, degree, degree)]:
+            pvec = rz[:, 0] ** a1 * rz[:, 1] ** b1
+            qvec = rz[:, 0] ** a2 * rz[:, 1] ** b2
+            exact = mono_int(a1 + a2, b1 + b2)
+            size = R ** (a1 + a2 + 2) * (abs(z1) ** (b1 + b2 + 1) + abs(z0) ** (b1 + b2 + 1))
+            got = _csr_bilinear(rp, ci, vals, pvec, qvec)
+            assert abs(got - exact) < 1e-11 * size, (a1, b1, a2, b2)
+    # M is symmetric
+    dense = np.zeros((o.n_dof[0], o.n_dof[0]))
+    for i in range(o.n_dof[0]):
+        dense[i, ci[rp[i]:rp[i + 1]]] = M[rp[i]:rp[i + 1]]
+    assert np.abs(dense - dense.T).max() < 1e-14 * scale
 
 
 # ------------------------------------------------------------------ P7 equilibrium trend
@@ -364,6 +399,161 @@ def test_P8_brute_force_dense_jacobian(orc):
         for i in range(n):
             dense[i, ci[rp[i]:rp[i + 1]]] = v[rp[i]:rp[i + 1]]
         assert np.linalg.norm(dense - A) < 1e-11 * np.linalg.norm(A)
+
+
+def _lagrange_eq(k, x):
+    """values and derivatives of the k+1 equispaced Lagrange polynomials on [-1, 1] at x (plain product formula)."""
+    nodes = -1.0 + 2.0 * np.arange(k + 1) / k
+    val, der = np.zeros(k + 1), np.zeros(k + 1)
+    for a in range(k + 1):
+        others = [b for b in range(k + 1) if b != a]
+        val[a] = np.prod([(x - nodes[b]) / (nodes[a] - nodes[b]) for b in others])
+        der[a] = sum(np.prod([(x - nodes[b]) / (nodes[a] - nodes[b]) for b in others if b != e]) / (nodes[a] - nodes[e])
+                     for e in others)
+    return val, der
+
+
+def _amr_global_basis(R, z0, z1, nr, nz, k):
+    """Independent (geometric) construction of the nonconforming Qk space on an nr x nz base grid with ONE quadtree
+    level about the origin (reading A12: refine base cells inside [0, R/2] x [zc - zh/2, zc + zh/2]).
+
+    Returns (ip [nq_tot, 2], w [nq_tot], PH, PR, PZ [nq_tot, n_dof], dof coordinates [n_dof, 2]) where column I of PH/PR/PZ is
+    the GLOBAL shape function of free node I (and its r, z derivatives) at the integration points.  A hanging node
+    (a node of a refined cell lying on an edge of an unrefined neighbour without being one of its nodes) carries no dof:
+    the value there is the unrefined neighbour's own interpolant -- that is what continuity means."""
+    hr, hz = R / nr, (z1 - z0) / nz
+    zc, zh = 0.5 * (z0 + z1), 0.5 * (z1 - z0)
+    cells = []  # (r0, z0, hr, hz, level)
+    for cz in range(nz):
+        for cr in range(nr):
+            r_lo, z_lo = cr * hr, z0 + cz * hz
+            inside = r_lo + hr <= R / 2 + 1e-12 and z_lo >= zc - zh / 2 - 1e-12 and z_lo + hz <= zc + zh / 2 + 1e-12
+            if inside:
+                for bz in range(2):
+                    for br in range(2):
+                        cells.append((r_lo + br * hr / 2, z_lo + bz * hz / 2, hr / 2, hz / 2, 1))
+            else:
+                cells.append((r_lo, z_lo, hr, hz, 0))
+    key = lambda r, z: (round(r / hr * 4 * k), round((z - z0) / hz * 4 * k))   # exact integer lattice of all nodes
+    node_pos = {}
+    for (r0, zz0, h1, h2, lev) in cells:
+        for a2 in range(k + 1):
+            for a1 in range(k + 1):
+                node_pos[key(r0 + a1 * h1 / k, zz0 + a2 * h2 / k)] = (r0 + a1 * h1 / k, zz0 + a2 * h2 / k)
+    coarse = [c for c in cells if c[4] == 0]
+    own = lambda c: {key(c[0] + a1 * c[2] / k, c[1] + a2 * c[3] / k) for a1 in range(k + 1) for a2 in range(k + 1)}
+    hanging = {}   # key -> coarse cell whose edge carries it
+    for (r0, zz0, h1, h2, lev) in cells:
+        if lev == 0:
+            continue
+        for a2 in range(k + 1):
+            for a1 in range(k + 1):
+                r, z = r0 + a1 * h1 / k, zz0 + a2 * h2 / k
+                for c in coarse:
+                    on = c[0] - 1e-12 <= r <= c[0] + c[2] + 1e-12 and c[1] - 1e-12 <= z <= c[1] + c[3] + 1e-12
+                    if on and key(r, z) not in own(c):
+                        hanging[key(r, z)] = c
+    free = sorted((kk for kk in node_pos if kk not in hanging), key=lambda kk: (kk[1], kk[0]))   # (z, r) order
+    dof = {kk: n for n, kk in enumerate(free)}
+    gx, gw = np.polynomial.legendre.leggauss(k + 1)
+
+    def nodal_rows(c):
+        """[nb, n_dof]: value of every global shape function at the local nodes of cell c."""
+        rows = np.zeros(((k + 1) ** 2, len(free)))
+        for a2 in range(k + 1):
+            for a1 in range(k + 1):
+                r, z = c[0] + a1 * c[2] / k, c[1] + a2 * c[3] / k
+                kk = key(r, z)
+                if kk in dof:
+                    rows[a1 + (k + 1) * a2, dof[kk]] = 1.0
+                else:          # trace of the unrefined neighbour's interpolant at (r, z)
+                    cc = hanging[kk]
+                    v1, _ = _lagrange_eq(k, -1 + 2 * (r - cc[0]) / cc[2])
+                    v2, _ = _lagrange_eq(k, -1 + 2 * (z - cc[1]) / cc[3])
+                    for b2 in range(k + 1):
+                        for b1 in range(k + 1):
+                            wgt = v1[b1] * v2[b2]
+                            if abs(wgt) > 1e-15:
+                                rows[a1 + (k + 1) * a2, dof[key(cc[0] + b1 * cc[2] / k, cc[1] + b2 * cc[3] / k)]] += wgt
+        return rows
+
+    ip, w, PH, PR, PZ = [], [], [], [], []
+    for c in cells:
+        N = nodal_rows(c)
+        for q2 in range(k + 1):
+            for q1 in range(k + 1):
+                v1, d1 = _lagrange_eq(k, gx[q1])
+                v2, d2 = _lagrange_eq(k, gx[q2])
+                r = c[0] + c[2] * (1 + gx[q1]) / 2
+                ip.append((r, c[1] + c[3] * (1 + gx[q2]) / 2))
+                w.append(gw[q1] * gw[q2] * c[2] * c[3] / 4 * r)
+                PH.append(np.outer(v2, v1).ravel() @ N)
+                PR.append((2 / c[2]) * np.outer(v2, d1).ravel() @ N)
+                PZ.append((2 / c[3]) * np.outer(d2, v1).ravel() @ N)
+    coords = np.array([node_pos[kk] for kk in free])
+    return np.array(ip), np.array(w), np.array(PH), np.array(PR), np.array(PZ), coords
+
+
+def test_P8_brute_force_dense_jacobian_with_hanging_nodes(orc):
+    """P8 on a one-level quadtree grid (2 x 4 base cells, 14 Q2 cells, hanging nodes on three coarse edges) coupled to a
+    uniform 2 x 2 grid: dense Jacobian from global shape functions built geometrically (continuity across hanging edges),
+    azimuthal-quadrature tensor and a plain double loop -- pins the fold P_e^T A_e P_e of assemble_species, the
+    constrained field evaluation and the cross-grid inner integral."""
+    k, dt = 2, 0.7
+    ext = [(2.0, -2.0, 2.0, 2, 4, 1), (1.0, -1.0, 1.0, 2, 2, 0)]
+    species = [dict(mass=1.0, charge=-1.0, grid=0), dict(mass=9.0, charge=2.0, grid=1)]
+    grids = [dict(kind=1 if e[5] else 0, r_max=e[0], z_min=e[1], z_max=e[2], nr=e[3], nz=e[4], levels=e[5]) for e in ext]
+    o = orc.Oracle(grids, species, k)
+    ip, wt, PH, PR, PZ = [], [], [], [], []
+    for g, (R, z0, z1, nr, nz, lev) in enumerate(ext):
+        # (the 2 x 2 grid goes through the same construction: the box test refines none of its cells)
+        a = _amr_global_basis(R, z0, z1, nr, nz, k)
+        assert a[5].shape[0] == o.n_dof[g] and np.abs(a[5] - o.dof_coords(g)).max() < 1e-13   # same dofs, same order
+        assert len(a[1]) == o.n_ip[g] and abs(a[2].sum(1) - 1).max() < 1e-13                   # partition of unity
+        ip.append(a[0]); wt.append(a[1]); PH.append(a[2]); PR.append(a[3]); PZ.append(a[4])
+    assert o.n_cells[0] == 14 and o.n_dof[0] < 14 * 9
+    cfg = dict(index=78, species=species, state="shifted", alpha=[1.0, 1.0], batch=1)
+    f = W.make_batch_f(cfg, [o.dof_coords(g) for g in range(2)], batch=1)[0]
+    fs = [f[o.f_off[s]:o.f_off[s + 1]] for s in range(2)]
+    vals = o.jacobian(f, dt)
+    rhs = o.apply(f)
+    for a, spa in enumerate(species):
+        ga = spa["grid"]
+        nq = len(ip[ga])
+        D = np.zeros((nq, 2, 2)); K = np.zeros((nq, 2))
+        for b, spb in enumerate(species):
+            gb = spb["grid"]
+            nu = spa["charge"] ** 2 * spb["charge"] ** 2
+            fj, frj, fzj = PH[gb] @ fs[b], PR[gb] @ fs[b], PZ[gb] @ fs[b]
+            for i in range(nq):
+                for j in range(len(ip[gb])):
+                    if ga == gb and i == j:
+                        continue
+                    U = orc.tensor_quadrature(ip[ga][i, 0], ip[ga][i, 1], ip[gb][j, 0], ip[gb][j, 1], 1500)
+                    UD = np.array([[U[0], U[1]], [U[7], U[2]]])
+                    UK = np.array([[U[3], U[4]], [U[5], U[6]]])
+                    D[i] += nu / spa["mass"] ** 2 * wt[gb][j] * fj[j] * UD
+                    K[i] += nu / (spa["mass"] * spb["mass"]) * wt[gb][j] * (UK @ np.array([frj[j], fzj[j]]))
+        n = PH[ga].shape[1]
+        A = np.zeros((n, n))
+        for q in range(nq):
+            gphi = np.stack([PR[ga][q], PZ[ga][q]], 0)
+            A += wt[ga][q] * (np.outer(PH[ga][q], PH[ga][q]) / dt + gphi.T @ D[q] @ gphi
+                              - np.outer(gphi.T @ K[q], PH[ga][q]))
+        rp, ci = o.pattern(ga)
+        dense = np.zeros((n, n))
+        v = vals[o.v_off[a]:o.v_off[a + 1]]
+        for i in range(n):
+            dense[i, ci[rp[i]:rp[i + 1]]] = v[rp[i]:rp[i + 1]]
+        assert np.linalg.norm(dense - A) < 1e-11 * np.linalg.norm(A)
+        assert np.abs(dense - A).max() < 1e-11 * np.abs(A).max()
+        # the structural pattern holds every coupling the brute force produces
+        assert np.all((np.abs(A) > 1e-13 * np.abs(A).max()) <= (dense != 0))
+        # operator application from the same dense pieces: rhs = J f = (M/dt - A) f
+        Mq = sum(wt[ga][q] * np.outer(PH[ga][q], PH[ga][q]) for q in range(nq))
+        ref_rhs = (Mq / dt - A) @ fs[a]
+        blk = rhs[o.f_off[a]:o.f_off[a + 1]]
+        assert np.linalg.norm(blk - ref_rhs) < 1e-10 * np.linalg.norm(ref_rhs)
 
 
 # ------------------------------------------------------------------ P9 mesh statistics printed by the paper
