@@ -405,6 +405,9 @@ def test_non_blocking_stream_and_reserve(orc, Bn, torch_cuda):
     ref = o.jacobian_batch(f[[0, 39]], cfg["dt"])
     assert _block_errors(L, vals[[0, 39]].cpu().numpy(), ref, L.v_off).max() < TOL
     assert _block_errors(L, rhs[[0, 39]].cpu().numpy(), o.apply_batch(f[[0, 39]]), L.f_off).max() < TOL
+    for B in (7, 1, 23):      # load every kernel variant the sizes below take (CUDA loads modules lazily)
+        L.jacobian(fd[:B].contiguous(), cfg["dt"])
+    torch.cuda.synchronize()
     L.close()
     L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"])
     Bn.landau_reserve(L.ctx, 40)
@@ -423,3 +426,134 @@ def test_non_blocking_stream_and_reserve(orc, Bn, torch_cuda):
         assert _block_errors(L, out[:1].cpu().numpy(), ref[:1], L.v_off).max() < TOL
         assert _block_errors(L, r[:1].cpu().numpy(), o.apply_batch(f[:1]), L.f_off).max() < TOL
     L.close()
+
+
+def test_config4_quadtree_bimaxwellian(orc, Bn, torch_cuda):
+    _config_parity(orc, Bn, torch_cuda, W.config(4), 256, _sample_entries(256, 4)[:5])
+
+
+def test_config5_bench_launch_configuration(orc, Bn, torch_cuda):
+    """Full size of the bench workload (B = 1024, default chunking), sampled entries against the oracle."""
+    _config_parity(orc, Bn, torch_cuda, W.config(5), 1024, [0, 517, 1023], check_apply=False)
+
+
+def test_stream_mode_reproducible_and_batch_independent(Bn, torch_cuda):
+    """Many-column K2 in persistent stream mode (config 3, B = 512: 384 tiles on 148 SMs): the same call gives the same
+    bits, and an entry's Jacobian does not depend on the rest of the batch beyond summation order."""
+    torch = torch_cuda
+    cfg = W.config(3)
+    L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"])
+    coords = [L.dof_coords(g) for g in range(L.G)]
+    fd = torch.tensor(W.make_batch_f(cfg, coords, batch=512), device="cuda")
+    a = L.jacobian(fd, cfg["dt"])
+    b = L.jacobian(fd, cfg["dt"])
+    assert torch.equal(a, b)
+    c = L.jacobian(fd[:300].contiguous(), cfg["dt"])
+    num = (c - a[:300]).norm(dim=1)
+    assert float((num / a[:300].norm(dim=1)).max()) < 1e-13
+    L.close()
+
+
+def test_config5_maximum_batch(orc, Bn, torch_cuda):
+    """BASELINE.json's largest size (config 5, B = 4096: 5.8 GB of CSR values, four passes of the default chunk): the
+    first and the last entry against the oracle, every block's column sums, and the first pass bit-identical to a
+    stand-alone run of the same 1024 entries."""
+    torch = torch_cuda
+    cfg = W.config(5)
+    B = 4096
+    o, L = _make(orc, Bn, cfg)
+    coords = [L.dof_coords(g) for g in range(L.G)]
+    f = W.make_batch_f(cfg, coords, batch=B)
+    fd = torch.tensor(f, device="cuda")
+    vals = L.jacobian(fd, cfg["dt"])
+    entries = [0, B - 1]
+    ref = np.stack([o.jacobian(f[b], cfg["dt"]) for b in entries])
+    assert _block_errors(L, vals[entries].cpu().numpy(), ref, L.v_off).max() < TOL
+    first = L.jacobian(fd[:1024].contiguous(), cfg["dt"])
+    assert torch.equal(first, vals[:1024])
+    del first
+    vals.copy_(L.jacobian(fd, float("inf")))
+    for s in range(L.S):
+        g = L.sgrid[s]
+        _, ci = L.pattern(g)
+        cid = torch.tensor(ci.astype(np.int64), device="cuda")
+        worst = 0.0
+        for b0 in range(0, B, 512):
+            blk = vals[b0:b0 + 512, L.v_off[s]:L.v_off[s + 1]]
+            colsum = torch.zeros((blk.shape[0], int(L.n_dof[g])), dtype=torch.float64, device="cuda").index_add_(1, cid, blk)
+            colabs = torch.zeros((blk.shape[0], int(L.n_dof[g])), dtype=torch.float64, device="cuda").index_add_(1, cid, blk.abs())
+            worst = max(worst, float(colsum.abs().max() / colabs.max()))
+        assert worst < 1e-12
+    L.close()
+
+
+def test_degenerate_cases(orc, Bn, torch_cuda):
+    """Degenerate inputs of the method: (a) two species on two IDENTICAL grids -- every integration point of one grid
+    coincides with one of the other, so the coincident-pair rule (reading A2) is exercised across grids; (b) a grid of
+    a single cell; (c) a species that is absent (f = 0): its block must reduce to M/dt plus the field of the others."""
+    torch = torch_cuda
+    same = dict(kind=0, r_max=4.0, z_min=-4.0, z_max=4.0, nr=3, nz=5, levels=0)
+    one = dict(kind=0, r_max=2.0, z_min=-2.0, z_max=2.0, nr=1, nz=1, levels=0)
+    cfg = dict(name="degenerate", index=97, grids=[same, dict(same), one],
+               species=[dict(mass=1.0, charge=-1.0, grid=0), dict(mass=2.0, charge=1.0, grid=1),
+                        dict(mass=4.0, charge=2.0, grid=2)],
+               degree=2, dt=0.3, batch=2, state="shifted", alpha=[1.0, 1.0, 1.0])
+    o, L = _make(orc, Bn, cfg)
+    f = W.make_batch_f(cfg, [o.dof_coords(g) for g in range(o.G)], batch=2)
+    f[1, L.f_off[1]:L.f_off[2]] = 0.0                      # (c): species 1 absent in entry 1
+    fd = torch.tensor(f, device="cuda")
+    for kernel in (1, 2):
+        Bn.landau_set_inner_kernel(L.ctx, kernel)
+        vals = L.jacobian(fd, cfg["dt"]).cpu().numpy()
+        assert _block_errors(L, vals, o.jacobian_batch(f, cfg["dt"]), L.v_off).max() < TOL
+        rhs = L.apply(fd).cpu().numpy()
+        ref = o.apply_batch(f)
+        for b in range(2):
+            for s in range(L.S):
+                a, r = rhs[b, L.f_off[s]:L.f_off[s + 1]], ref[b, L.f_off[s]:L.f_off[s + 1]]
+                assert np.linalg.norm(a - r) <= TOL * max(np.linalg.norm(r), 1e-300) or np.abs(r).max() == 0.0
+    assert np.all(rhs[1, L.f_off[1]:L.f_off[2]] == 0.0)     # J[f] applied to f = 0 is exactly zero
+    L.close()
+
+
+def test_outputs_stay_inside_their_buffers(Bn, torch_cuda):
+    """compute-sanitizer is not available on the pool: every output array is placed between two guard regions filled
+    with a sentinel, and the guards must be untouched after jacobian (ring, gather and stream-mode paths), apply,
+    spmv, solve and step."""
+    torch = torch_cuda
+    G = 4096
+    sentinel = -7.25e300
+
+    def guarded(rows, cols):
+        buf = torch.full((rows * cols + 2 * G,), sentinel, dtype=torch.float64, device="cuda")
+        return buf, buf[G:G + rows * cols].view(rows, cols)
+
+    def intact(buf, rows, cols):
+        return bool((buf[:G] == sentinel).all()) and bool((buf[G + rows * cols:] == sentinel).all())
+
+    for cfg, B in ((W.tiny_config("quadtree", 3, batch=5), 5), (W.config(3), 300)):
+        L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"])
+        f = torch.tensor(W.make_batch_f(cfg, [L.dof_coords(g) for g in range(L.G)], batch=B), device="cuda")
+        for asm in (0, 1):
+            Bn.landau_set_assembly_kernel(L.ctx, asm)
+            vb, vals = guarded(B, L.csr_stride)
+            Bn.landau_jacobian(L.ctx, f, B, cfg["dt"], vals)
+            torch.cuda.synchronize()
+            assert intact(vb, B, L.csr_stride) and bool(torch.isfinite(vals).all())
+        Bn.landau_set_assembly_kernel(L.ctx, 0)
+        rb, rhs = guarded(B, L.f_stride)
+        Bn.landau_apply(L.ctx, f, B, rhs)
+        yb, y = guarded(B, L.f_stride)
+        Bn.landau_spmv(L.ctx, vals, f, B, y)
+        xb, x = guarded(B, L.f_stride)
+        x.zero_()
+        Bn.landau_solve(L.ctx, vals, rhs, B, 1e-8, 100, x)
+        ub, u = guarded(B, L.f_stride)
+        u.copy_(f)
+        Bn.landau_step(L.ctx, u, B, 1e-3, 1e-6, 3, 1e-8, 200)
+        torch.cuda.synchronize()
+        for buf in (rb, yb, xb, ub):
+            assert intact(buf, B, L.f_stride)
+        for t in (rhs, y, x, u):
+            assert bool(torch.isfinite(t).all())
+        L.close()
