@@ -58,6 +58,7 @@ def parse():
                     "(reported under \"solve\", not part of value)")
     ap.add_argument("--advance", type=int, default=0, help="also run this many backward-Euler steps (landau_step) and "
                     "report the time and Newton iterations under \"advance\" (not part of value)")
+    ap.add_argument("--assembly", type=int, default=0, help="assembly kernel build (landau_set_assembly_kernel; 0: default)")
     ap.add_argument("--chunk", type=int, default=0, help="batch entries per pass through the stages (0: library default)")
     return ap.parse_args()
 
@@ -198,6 +199,8 @@ def run_ours(args):
     B = args.batch or cfg["batch"]
     L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"], device=local)
     Bn.landau_set_inner_kernel(L.ctx, args.kernel)
+    if args.assembly:
+        Bn.landau_set_assembly_kernel(L.ctx, args.assembly)
     if args.chunk:
         Bn.landau_set_batch_chunk(L.ctx, args.chunk)
     coords = [L.dof_coords(g) for g in range(L.G)]

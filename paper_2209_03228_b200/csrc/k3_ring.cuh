@@ -63,15 +63,22 @@ __device__ __forceinline__ double k3_lds(unsigned addr) {
 __host__ __device__ constexpr size_t k3_smem_bytes(int rc) { return ((size_t)rc * K3_RS + 8 + 16 * 32) * sizeof(double); }
 
 __global__ void __launch_bounds__(K3_THREADS, 4)
-k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, int n_spec, int nseg,
+k3_ring(const K3Grid* __restrict__ grids, const K3Species* __restrict__ spec, int n_spec, int n_whole, int nseg,
         const double* __restrict__ frag, const double* __restrict__ DK, long long dk_stride, double inv_dt,
         double* __restrict__ vals, long long v_stride) {
   extern __shared__ __align__(16) double ring[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int gq = lane >> 2, tq = lane & 3;
-  int bid = blockIdx.x;
-  const int seg = bid % nseg;
-  bid /= nseg;
+  // blocks [0, n_whole): one (entry, species) block each; later blocks: the remaining (entry, species) blocks cut into
+  // nseg segments of steps each (landau_api.cu, assemble_chunk: fills the last wave / small batches)
+  int bid = blockIdx.x, seg = 0;
+  if (bid >= n_whole) {
+    const int j = bid - n_whole;
+    seg = j % nseg;
+    bid = n_whole + j / nseg;
+  } else {
+    nseg = 1;
+  }
   const int sidx = bid % n_spec, b = bid / n_spec;
   const K3Species sp = spec[sidx];
   const K3Grid* __restrict__ g = grids + sp.grid;

@@ -63,7 +63,8 @@ struct landau_ctx {
   K3Grid* d_k3grid = nullptr;
   K3Species* d_k3spec = nullptr;
   const double* d_k3frag = nullptr;
-  int k3_nspec = 0, k3_min_steps = 0;
+  int k3_nspec = 0, k3_min_steps = 0, k3_ctas_per_sm = 4;
+  bool k3_tail_split = true;
   size_t k3_smem = 0;
   std::vector<char> k3_ring_ok;  // per species
   // batched solve (k4_solve.cuh)
@@ -320,7 +321,12 @@ int build_device_side(landau_ctx* ctx) {
     ctx->d_k3grid = const_cast<K3Grid*>(tg);
     ctx->d_k3spec = const_cast<K3Species*>(tsp);
     if (ctx->k3_nspec)
+    {
       if (int rc = raise_smem_limit(ctx, k3_ring, g_k3_smem_set, ctx->k3_smem)) return rc;
+      int per_sm = 0;
+      CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k3_ring, K3_THREADS, ctx->k3_smem));
+      ctx->k3_ctas_per_sm = std::max(1, per_sm);
+    }
   }
   // batched solve: pattern views per grid, block offsets per species
   {
@@ -706,14 +712,24 @@ int assemble_chunk(landau_ctx* ctx, int b0, int nbc, double inv_dt, double* out_
     NvtxRange range("landau K3 element matrices + assembly (a3+a4)");
     double* vals = out_csr_vals_dev + (long long)b0 * ctx->v_stride;
     if (ctx->k3_nspec && ctx->assembly_kernel != 1) {
-      // at least one wave of 4 CTAs per SM; the cell range is cut into segments (each with a recomputed halo) only
-      // when the batch alone gives fewer blocks than that
-      const int ctas = nbc * ctx->k3_nspec, want = 4 * ctx->n_sm;
-      int nseg = 1;
-      if (ctas < want) nseg = std::max(1, std::min(ctx->k3_min_steps, (want + ctas - 1) / ctas));
-      k3_ring<<<ctas * nseg, K3_THREADS, ctx->k3_smem, st>>>(ctx->d_k3grid, ctx->d_k3spec, ctx->k3_nspec, nseg,
-                                                             ctx->d_k3frag, ctx->DK, ctx->dk_stride, inv_dt, vals,
-                                                             ctx->v_stride);
+      // One CTA per (entry, species) block; blocks are cut into segments of steps (each with a recomputed halo) where that
+      // fills the machine: every block when the batch alone gives less than one wave of resident CTAs, otherwise just
+      // enough of the LAST blocks (cut in two) to bring the CTA count up to whole waves -- 2048 blocks on 148 x 4 slots
+      // were 3.46 waves and took the time of 4; the short CTAs are launched last and fill the tail.
+      const int ctas = nbc * ctx->k3_nspec, want = ctx->k3_ctas_per_sm * ctx->n_sm;
+      int n_whole = ctas, nseg = 1;
+      if (ctas < want) {
+        n_whole = 0;
+        nseg = std::max(1, std::min(ctx->k3_min_steps, (want + ctas - 1) / ctas));
+      } else if (ctas % want != 0 && ctx->k3_min_steps >= 8 && ctx->k3_tail_split) {
+        const int extra = want - ctas % want;  // cut `extra` blocks in two
+        n_whole = ctas - std::min(extra, ctas);
+        nseg = 2;
+      }
+      const int grid = n_whole + (ctas - n_whole) * nseg;
+      k3_ring<<<grid, K3_THREADS, ctx->k3_smem, st>>>(ctx->d_k3grid, ctx->d_k3spec, ctx->k3_nspec, n_whole, nseg,
+                                                      ctx->d_k3frag, ctx->DK, ctx->dk_stride, inv_dt, vals,
+                                                      ctx->v_stride);
       ++ctx->launches;
     }
     for (int s = 0; s < ctx->S; ++s) {
@@ -1250,8 +1266,9 @@ int landau_set_inner_kernel(landau_ctx* ctx, int which) {
 }
 
 int landau_set_assembly_kernel(landau_ctx* ctx, int which) {
-  if (!ctx || which < 0 || which > 1) return LANDAU_INVALID_ARG;
-  ctx->assembly_kernel = which;
+  if (!ctx || which < 0 || which > 2) return LANDAU_INVALID_ARG;
+  ctx->k3_tail_split = which != 2;  // 2: ring kernel without the tail cut (one CTA per block), for A/B measurements
+  ctx->assembly_kernel = which == 1 ? 1 : 0;
   return LANDAU_OK;
 }
 
