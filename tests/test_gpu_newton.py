@@ -179,3 +179,102 @@ def test_anisotropic_relaxation_history_against_nrl():
     assert abs(aniso[1] / nrl[1] - 1) < 5e-3           # first step: the state is still (almost) bi-Maxwellian
     assert 1.0 < aniso[-1] / nrl[-1] < 1.06            # later: slower than NRL, by a few per cent at t = 0.5 t0
     L.close()
+
+
+def test_two_species_anisotropic_relaxation_against_nrl(orc):
+    """The paper's verification experiment (sec. 6.1-6.2, Fig. 5a; App. B) with both species: a deuterium
+    plasma, e- and D+ bi-Maxwellian by eq. (6.1) with alpha = 1.3 and T_e,par = 300, T_e,perp = 390, T_i,par = 200,
+    T_i,perp = 260 eV (in units T0 = 300 eV), no shift, on quadtree-AMR Q3 grids of config-4 shape (4 x 8 base cells, 3
+    levels towards the origin), each grid scaled to 5 initial parallel thermal speeds of its species.
+    50 backward-Euler steps of landau_step to t = t0; the four temperatures (tests/temperature_moments.py) are compared
+    with an RK4 integration of the coupled NRL equations: isotropisation of each species + thermal equilibration.
+
+    * invariants: total energy to the nonlinear tolerance, density of each species to round-off (PAPER.md:278);
+    * ions (like-particle collisions dominate, electrons only heat them): anisotropy and heating follow NRL to 3 %;
+    * electrons: at t = 0 the rate from the applied operator of the ORACLE (exact for this bi-Maxwellian state) is
+      reproduced by the first step; the history is FASTER than the like-particle NRL rate because electron-ion
+      pitch-angle scattering isotropises the electrons as well (Z = 1: comparable to e-e), and it stays monotone;
+    * the first steps agree with the same steps on the oracle (direct solves) to 1e-8."""
+    import math
+    import os
+    import torch
+    import temperature_moments as TM
+    from paper_2209_03228_b200 import binding as Bn
+    g = TM.golden_rates(os.path.join(os.path.dirname(__file__), "golden", "nrl_rates.txt"))
+    alpha, mi = 1.3, 3670.0
+    mass, tau_par = [1.0, mi], [1.0, 200.0 / 300.0]
+    theta = [tau_par[s] / mass[s] for s in range(2)]
+    grids = [dict(kind=1, r_max=5.0 * math.sqrt(th), z_min=-5.0 * math.sqrt(th), z_max=5.0 * math.sqrt(th), nr=4, nz=8,
+                  levels=3) for th in theta]
+    species = [dict(mass=1.0, charge=-1.0, grid=0), dict(mass=mi, charge=1.0, grid=1)]
+    L = Bn.Landau(grids, species, 3)
+    o = orc.Oracle(grids, species, 3)
+    rz = [L.dof_coords(s) for s in range(2)]
+    f0 = np.concatenate([(1 / alpha) * (math.pi * theta[s]) ** -1.5 *
+                         np.exp(-(rz[s][:, 1] ** 2 + rz[s][:, 0] ** 2 / alpha) / theta[s]) for s in range(2)])
+    u = torch.tensor(f0[None], device="cuda")
+    m_vals = L.jacobian(u, 1.0) - L.jacobian(u, float("inf"))
+
+    def temps(v):
+        mv = L.spmv(m_vals, v).cpu().numpy()[0]
+        out = []
+        for s in range(2):
+            out += list(TM.temperatures(mv[L.f_off[s]:L.f_off[s + 1]], rz[s][:, 0], rz[s][:, 1], mass[s]))
+        return np.array(out)                      # n_e, Te_perp, Te_par, n_i, Ti_perp, Ti_par
+
+    dt, nsteps, n_oracle = 0.02, 50, 2
+    hist, states = [temps(u)], []
+    for k in range(nsteps):
+        info = L.step(u, dt, newton_rtol=1e-11, max_newton=80, lin_rtol=1e-12, lin_max_it=2000)
+        assert info["lin_failed"] == 0 and info["last_update"] <= 1e-11
+        hist.append(temps(u))
+        if k < n_oracle:
+            states.append((u.cpu().numpy()[0].copy(), info["newton_its"]))
+    h = np.array(hist)
+    assert abs(h[0, 1] - 1.3) < 5e-3 and abs(h[0, 2] - 1.0) < 2e-3            # 390 / 300 eV, 300 / 300 eV
+    assert abs(h[0, 4] - 260 / 300) < 5e-3 and abs(h[0, 5] - 200 / 300) < 2e-3
+    # invariants
+    energy = h[:, 0] * (2 * h[:, 1] + h[:, 2]) + h[:, 3] * (2 * h[:, 4] + h[:, 5])
+    assert np.abs(energy / energy[0] - 1).max() < 1e-10
+    assert np.abs(h[:, 0] / h[0, 0] - 1).max() < 1e-11 and np.abs(h[:, 3] / h[0, 3] - 1).max() < 1e-11
+    # the same first steps on the oracle
+    ref = f0
+    for k in range(n_oracle):
+        ref = _oracle_step(o, ref, dt, states[k][1])
+        for s in range(2):
+            sl = slice(o.f_off[s], o.f_off[s + 1])
+            assert np.linalg.norm(states[k][0][sl] - ref[sl]) < 1e-8 * np.linalg.norm(ref[sl])
+    # coupled NRL equations (App. B), y = (Te_perp, Te_par, Ti_perp, Ti_par), densities n = 1
+    def rate(y):
+        te, ti = (2 * y[0] + y[1]) / 3, (2 * y[2] + y[3]) / 3
+        nub = TM.nrl_equilibration_rate(g["c_eq"], 1.0, 1.0, 1.0, mass[0], mass[1], te, ti)
+        ne = TM.nrl_isotropization_rate(g["c_iso"], 1.0, mass[0], y[0], y[1])
+        ni = TM.nrl_isotropization_rate(g["c_iso"], 1.0, mass[1], y[2], y[3])
+        return np.array([-ne * (y[0] - y[1]) + nub * (ti - te), 2 * ne * (y[0] - y[1]) + nub * (ti - te),
+                         -ni * (y[2] - y[3]) + nub * (te - ti), 2 * ni * (y[2] - y[3]) + nub * (te - ti)])
+    nrl = TM.rk4(rate, h[0, [1, 2, 4, 5]], dt, nsteps)
+    # ions
+    ai, ai_nrl = h[:, 4] - h[:, 5], nrl[:, 2] - nrl[:, 3]
+    assert np.all(np.diff(ai) < 0)
+    assert np.abs((ai - ai[0])[1:] / (ai_nrl - ai[0])[1:] - 1).max() < 0.03
+    ti, ti_nrl = (2 * h[:, 4] + h[:, 5]) / 3, (2 * nrl[:, 2] + nrl[:, 3]) / 3
+    assert np.all(np.diff(ti) > 0)                                           # heated by the hotter electrons
+    assert np.abs((ti - ti[0])[1:] / (ti_nrl - ti[0])[1:] - 1).max() < 0.03
+    # electrons
+    ae, ae_nrl = h[:, 1] - h[:, 2], nrl[:, 0] - nrl[:, 1]
+    assert np.all(np.diff(ae) < 0)
+    assert np.all(ae[1:] < ae_nrl[1:]) and ae[-1] > 0.4 * ae_nrl[-1]          # faster than like-particle NRL (e-i scattering)
+    rhs0 = o.apply(f0)                                                      # exact initial rates from the oracle's operator
+    rp, ci = o.pattern(0)
+    mf = np.add.reduceat(o.mass(0) * f0[:o.f_off[1]][ci], rp[:-1])
+    dperp, dpar = TM.temperature_rates(mf, rhs0[:o.f_off[1]], rz[0][:, 0], rz[0][:, 1], 1.0)
+    assert dperp - dpar < -3 * TM.nrl_isotropization_rate(g["c_iso"], 1.0, 1.0, h[0, 1], h[0, 2]) * ae[0]   # e-e + e-i
+    # backward Euler: M (u1 - u0)/dt = J[u1] u1, so the difference quotient of any moment IS that moment of the operator
+    # applied to the new state (to the nonlinear tolerance), and it lies within 15 % of the initial rate
+    rhs1 = L.apply(torch.tensor(states[0][0][None], device="cuda")).cpu().numpy()[0]
+    mf1 = L.spmv(m_vals, torch.tensor(states[0][0][None], device="cuda")).cpu().numpy()[0]
+    d1perp, d1par = TM.temperature_rates(mf1[:L.f_off[1]], rhs1[:L.f_off[1]], rz[0][:, 0], rz[0][:, 1], 1.0)
+    fd = (ae[1] - ae[0]) / dt
+    assert abs(fd / (d1perp - d1par) - 1) < 1e-7
+    assert (dperp - dpar) < fd < 0 and abs(fd / (dperp - dpar) - 1) < 0.15
+    L.close()

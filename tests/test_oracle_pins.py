@@ -10,6 +10,7 @@ import numpy as np
 import pytest
 from scipy import special
 
+import temperature_moments as TM
 from paper_2209_03228_b200 import workloads as W
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "paper_mesh_stats.txt")
@@ -629,25 +630,17 @@ def test_splitmix_is_counter_based():
 
 # ------------------------------------------------------------------------------------------------ P10, P11: dynamics
 def _golden_rates():
-    vals = {}
-    for line in open(os.path.join(os.path.dirname(__file__), "golden", "nrl_rates.txt")):
-        if line.strip() and not line.startswith("#"):
-            k, v = line.split()[:2]
-            vals[k] = float(v)
-    return vals
+    return TM.golden_rates(os.path.join(os.path.dirname(__file__), "golden", "nrl_rates.txt"))
 
 
 def _moment_rates(o, s, f, rhs, mass_s):
-    """(n, T_perp, T_par, dT_perp/dt, dT_par/dt) of species s in units T0: since M df/dt = rhs, the time derivative of any
-    moment psi^T M f is psi^T rhs -- no solve.  T_perp = m <r^2>, T_par = 2 m <z^2> (theta = T/m, reading A8)."""
+    """(n, T_perp, T_par, dT_perp/dt, dT_par/dt) of species s in units T0 (tests/temperature_moments.py): since
+    M df/dt = rhs, the time derivative of any moment psi^T M f is psi^T rhs -- no solve."""
     rz = o.dof_coords(o.sgrid[s])
     sl = slice(o.f_off[s], o.f_off[s + 1])
     rp, ci = o.pattern(o.sgrid[s])
     mf = np.add.reduceat(o.mass(o.sgrid[s]) * f[sl][ci], rp[:-1])
-    n = mf.sum()
-    r2, z2 = rz[:, 0] ** 2, rz[:, 1] ** 2
-    return (2 * math.pi * n, mass_s * (r2 @ mf) / n, 2 * mass_s * (z2 @ mf) / n,
-            mass_s * (r2 @ rhs[sl]) / n, 2 * mass_s * (z2 @ rhs[sl]) / n)
+    return TM.temperatures(mf, rz[:, 0], rz[:, 1], mass_s) + TM.temperature_rates(mf, rhs[sl], rz[:, 0], rz[:, 1], mass_s)
 
 
 @pytest.mark.parametrize("alpha", [1.05, 1.3])
@@ -663,8 +656,7 @@ def test_P10_isotropization_rate_matches_appendix_B(orc, alpha):
     n, tperp, tpar, dperp, dpar = _moment_rates(o, 0, f, o.apply(f), 1.0)
     assert abs(n - 1.0) < 1e-3 and abs(tperp / tpar - alpha) < 2e-3
     assert abs(dperp + 0.5 * dpar) < 1e-12 * abs(dperp)                     # energy: 2 T_perp + T_par constant
-    A = tperp / tpar - 1.0
-    nu_t = c_iso * n * tpar ** -1.5 * (-3.0 + (A + 3.0) * math.atan(math.sqrt(A)) / math.sqrt(A)) / A ** 2
+    nu_t = TM.nrl_isotropization_rate(c_iso, n, 1.0, tperp, tpar)
     assert abs(-dperp / (tperp - tpar) - nu_t) < 3e-3 * nu_t
 
 
@@ -687,5 +679,5 @@ def test_P11_thermal_equilibration_rate_matches_appendix_B(orc):
     for s, (m, t, n_other, m_other, t_other) in enumerate(((ma, ta, nb, mb, tb), (mb, tb, na, ma, ta))):
         n, tperp, tpar, dperp, dpar = _moment_rates(o, s, f, rhs, m)
         dT = (2 * dperp + dpar) / 3.0                                       # T = (2 T_perp + T_par)/3
-        nu_bar = g["c_eq"] * qb ** 2 * n_other * math.sqrt(m * m_other) / (m * t_other + m_other * t) ** 1.5
+        nu_bar = TM.nrl_equilibration_rate(g["c_eq"], 1.0, qb, n_other, m, m_other, t, t_other)
         assert abs(dT - nu_bar * (t_other - t)) < 5e-3 * abs(nu_bar * (t_other - t))
