@@ -155,3 +155,57 @@ def make_batch_f(cfg, dof_coords, batch=None, entries=None):
             parts.append(sample_state(sp["mass"], n[row, s], T[row, s], u[row, s], al[row, s], dof_coords[sp["grid"]]))
         out.append(np.concatenate(parts))
     return np.ascontiguousarray(np.stack(out))
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# 3V workloads (Table 6): Q2 hexahedra on cubes [-half, half]^3
+# ------------------------------------------------------------------------------------------------------------------
+def _grid3(half, n, levels=0):
+    return dict(half=half, n=n, levels=levels)
+
+
+def config3v(name="paper", batch=None):
+    """3V problem descriptions.
+
+    "paper": the paper's 3V throughput problem (Table 6: batch 32) -- the ten species of config 3
+             (electrons, deuterium, eight heavier ions) on three grids of 120 Q2 cells each (4 x 4 x 4 base cells, one
+             refinement level about the origin: 1,045 equations per species), each grid scaled to 5 thermal speeds of
+             its lightest species;
+    "eD":    e- / D+ on two such grids (the 3V analogue of config 2), shifted Maxwellians;
+    "tiny" / "tiny_uniform": two species on small grids (3^3 base cells with the centre cell refined + 2^3 cells;
+             uniform 3^3 + 2^3) for fast tests.
+    The `state` recipes are those of the 2V configs (species_state); a drift is along z.
+    """
+    if name == "paper":
+        c3 = config(3)
+        lightest = {0: 1.0, 1: c3["species"][1]["mass"], 2: c3["species"][4]["mass"]}
+        grids = [_grid3(5.0 / math.sqrt(lightest[g]), 4, 1) for g in range(3)]
+        return dict(name="paper_3V_10species_3x120Q2", index=7, dim=3, grids=grids, species=c3["species"], dt=1e-3,
+                    batch=batch or 32, state="maxwellian_nT", alpha=[1.0] * 10)
+    if name == "eD":
+        md = 3670.0
+        return dict(name="3V_eD_2x120Q2", index=8, dim=3, grids=[_grid3(5.0, 4, 1), _grid3(5.0 / math.sqrt(md), 4, 1)],
+                    species=[dict(mass=1.0, charge=-1.0, grid=0), dict(mass=md, charge=1.0, grid=1)], dt=1.0,
+                    batch=batch or 32, state="shifted", alpha=[1.0, 1.0])
+    if name in ("tiny", "tiny_uniform"):
+        lev = 1 if name == "tiny" else 0
+        return dict(name="3V_" + name, index=95 + lev, dim=3, grids=[_grid3(4.0, 3, lev), _grid3(4.0 / 3.0, 2, 0)],
+                    species=[dict(mass=1.0, charge=-1.0, grid=0), dict(mass=9.0, charge=2.0, grid=1)], dt=0.5,
+                    batch=batch or 3, state="shifted", alpha=[1.0, 1.0])
+    raise ValueError("unknown 3V config %r" % (name,))
+
+
+def sample_state3v(mass, n, T, u, alpha, xyz):
+    """The state of sample_state in Cartesian coordinates: r^2 = x^2 + y^2, z parallel."""
+    theta = T / mass
+    return (n / alpha) * (math.pi * theta) ** -1.5 * np.exp(-((xyz[:, 2] - u) ** 2 + (xyz[:, 0] ** 2 + xyz[:, 1] ** 2) / alpha) / theta)
+
+
+def make_batch_f3v(cfg, dof_coords, batch=None, entries=None):
+    """Nodal interpolant of the seeded states on 3V grids: dof_coords[g] = [n_dof_g, 3] (x, y, z)."""
+    n, T, u, al = species_state(cfg, batch, entries)
+    out = []
+    for row in range(n.shape[0]):
+        out.append(np.concatenate([sample_state3v(sp["mass"], n[row, s], T[row, s], u[row, s], al[row, s], dof_coords[sp["grid"]])
+                                   for s, sp in enumerate(cfg["species"])]))
+    return np.ascontiguousarray(np.stack(out))
