@@ -15,7 +15,8 @@ LandauError = _b.LandauError
 SYMBOLS = ["landau3v_create", "landau3v_destroy", "landau3v_sizes", "landau3v_dof_coords", "landau3v_ip_table",
            "landau3v_csr_pattern", "landau3v_csr_pattern_host", "landau3v_jacobian", "landau3v_apply",
            "landau3v_jacobian_host", "landau3v_last_coefficients", "landau3v_set_timing", "landau3v_last_stage_ms",
-           "landau3v_launch_count", "landau3v_set_inner_kernel", "landau3v_set_batch_chunk", "landau3v_last_error"]
+           "landau3v_launch_count", "landau3v_set_inner_kernel", "landau3v_set_assembly_kernel", "landau3v_set_batch_chunk",
+           "landau3v_last_error"]
 
 
 class GridDesc3(C.Structure):
@@ -133,6 +134,10 @@ def landau3v_launch_count(ctx):
 
 def landau3v_set_inner_kernel(ctx, which):
     _check(load().landau3v_set_inner_kernel(ctx, C.c_int(which)), ctx)
+
+
+def landau3v_set_assembly_kernel(ctx, which):
+    _check(load().landau3v_set_assembly_kernel(ctx, C.c_int(which)), ctx)
 
 
 def landau3v_set_batch_chunk(ctx, chunk):

@@ -11,6 +11,7 @@
 #include "host_setup3v.hpp"
 #include "landau3v_kernels.cuh"
 #include "landau3v_dmma.cuh"
+#include "landau3v_k3.cuh"
 
 using namespace landau3v;
 
@@ -38,6 +39,12 @@ struct landau3v_ctx {
   std::vector<Mix3> mix;
   Ranges3 ranges;
   Combine3* d_comb = nullptr;
+  double* EM = nullptr;
+  size_t EM_cap = 0;
+  std::vector<long long> em_off;
+  long long em_stride = 0;
+  int assembly_kernel = 0;  // 0: element matrices on the MMA pipe + gather, 1: per-slot quadrature (first version)
+  bool k3e_configured = false;
   double *F = nullptr, *Gs = nullptr, *DK = nullptr, *FE = nullptr, *stage_in = nullptr, *stage_out = nullptr;
   size_t F_cap = 0, G_cap = 0, DK_cap = 0, FE_cap = 0, stage_in_cap = 0, stage_out_cap = 0;
   int f_nbc = -1;
@@ -313,11 +320,30 @@ int run_coefficients(landau3v_ctx* ctx, const double* batch_f, int b0, int nbc, 
 int assemble_chunk(landau3v_ctx* ctx, int b0, int nbc, double inv_dt, double* out, cudaStream_t st) {
   nvtxRangePushA("landau3v K3 element matrices + assembly (a3+a4)");
   double* vals = out + (long long)b0 * ctx->v_stride;
-  for (int s = 0; s < ctx->S; ++s) {
-    const int g = ctx->species[s].grid;
-    k3v_assemble<<<dim3((ctx->hg[g].nnz + 127) / 128, nbc), 128, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s],
-                                                                          inv_dt, vals, ctx->v_stride, ctx->v_off[s]);
-    ++ctx->launches;
+  if (ctx->assembly_kernel == 1) {
+    for (int s = 0; s < ctx->S; ++s) {
+      const int g = ctx->species[s].grid;
+      k3v_assemble<<<dim3((ctx->hg[g].nnz + 127) / 128, nbc), 128, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride,
+                                                                            ctx->dk_off[s], inv_dt, vals, ctx->v_stride, ctx->v_off[s]);
+      ++ctx->launches;
+    }
+  } else {
+    if (int rc = grow(ctx, &ctx->EM, &ctx->EM_cap, (size_t)ctx->em_stride * nbc)) {
+      nvtxRangePop();
+      return rc;
+    }
+    if (!ctx->k3e_configured) {
+      cudaFuncSetAttribute(k3v_elem_matrix, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K3E_SMEM);
+      ctx->k3e_configured = true;
+    }
+    for (int s = 0; s < ctx->S; ++s) {
+      const int g = ctx->species[s].grid;
+      k3v_elem_matrix<<<dim3((ctx->hg[g].n_cells + K3E_WARPS - 1) / K3E_WARPS, nbc), K3E_WARPS * 32, K3E_SMEM, st>>>(
+          ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, ctx->EM, ctx->em_stride, ctx->em_off[s]);
+      k3v_gather<<<dim3((ctx->hg[g].nnz + 255) / 256, nbc), 256, 0, st>>>(ctx->dg[g], ctx->EM, ctx->em_stride, ctx->em_off[s], vals,
+                                                                          ctx->v_stride, ctx->v_off[s]);
+      ctx->launches += 2;
+    }
   }
   nvtxRangePop();
   return LANDAU_OK;
@@ -380,6 +406,7 @@ int landau3v_create(const landau3v_grid_desc* grids, int n_grids, const landau_s
       ctx->v_off.push_back(vo);
       ctx->dk_off.push_back(dko);
       ctx->fe_off.push_back(feo);
+      ctx->em_off.push_back(feo * NB);
       fo += h.n_dof;
       vo += h.nnz;
       dko += 9LL * h.n_ip;
@@ -389,6 +416,7 @@ int landau3v_create(const landau3v_grid_desc* grids, int n_grids, const landau_s
     ctx->v_stride = vo;
     ctx->dk_stride = dko;
     ctx->fe_stride = feo;
+    ctx->em_stride = feo * NB;
   } catch (const std::bad_alloc&) {
     return bail(LANDAU_OUT_OF_MEMORY, "host allocation failed");
   }
@@ -415,7 +443,7 @@ void landau3v_destroy(landau3v_ctx* ctx) {
     cudaDeviceSynchronize();
   }
   for (void* p : ctx->allocs) cudaFree(p);
-  for (double* p : {ctx->F, ctx->Gs, ctx->DK, ctx->FE, ctx->stage_in, ctx->stage_out})
+  for (double* p : {ctx->F, ctx->Gs, ctx->DK, ctx->FE, ctx->EM, ctx->stage_in, ctx->stage_out})
     if (p) cudaFree(p);
   for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
   delete ctx;
@@ -552,6 +580,12 @@ long long landau3v_launch_count(const landau3v_ctx* ctx) { return ctx ? ctx->lau
 int landau3v_set_inner_kernel(landau3v_ctx* ctx, int which) {
   if (!ctx || which < 0 || which > 2) return LANDAU_INVALID_ARG;
   ctx->inner_kernel = which;
+  return LANDAU_OK;
+}
+
+int landau3v_set_assembly_kernel(landau3v_ctx* ctx, int which) {
+  if (!ctx || which < 0 || which > 1) return LANDAU_INVALID_ARG;
+  ctx->assembly_kernel = which;
   return LANDAU_OK;
 }
 
