@@ -43,6 +43,7 @@ struct landau3v_ctx {
   size_t EM_cap = 0;
   std::vector<long long> em_off;
   long long em_stride = 0;
+  int dmma_ctas_per_sm[5] = {0, 0, 0, 0, 0};
   int assembly_kernel = 0;  // 0: element matrices on the MMA pipe + gather, 1: per-slot quadrature (first version)
   bool k3e_configured = false;
   double *F = nullptr, *Gs = nullptr, *DK = nullptr, *FE = nullptr, *stage_in = nullptr, *stage_out = nullptr;
@@ -264,7 +265,9 @@ int run_coefficients(landau3v_ctx* ctx, const double* batch_f, int b0, int nbc, 
     const long long items = (long long)(ctx->n_pad / (K2D_WARPS * 8)) * NCL * ((nbc + ncol - 1) / ncol);
     int min_tiles = 1 << 30;
     for (int c = 0; c < NCL; ++c) min_tiles = std::min(min_tiles, (ctx->ranges.j1[c] - ctx->ranges.j0[c]) / K2D_TJ);
-    nsplit = (int)std::max(1LL, std::min<long long>(std::min(min_tiles, 32), (4LL * ctx->n_sm + items - 1) / items));
+    const int nt = inner_dmma_nt(nbc);
+    if (ctx->dmma_ctas_per_sm[nt] == 0) ctx->dmma_ctas_per_sm[nt] = inner_dmma_ctas_per_sm(nt);
+    nsplit = inner_dmma_split(items, (long long)ctx->dmma_ctas_per_sm[nt] * ctx->n_sm, std::max(1, std::min(min_tiles / 4, 32)));
   }
   const long long split_stride = (long long)NCL * nbc * 9 * ctx->n_pad;
   const size_t f_need = (size_t)NCL * nbc * 4 * ctx->n_pad, g_need = (size_t)split_stride * nsplit;

@@ -22,13 +22,17 @@ __device__ __forceinline__ void dmma3(double& d0, double& d1, double a, double b
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
+__device__ __forceinline__ void cp8_3v(double* smem, const double* gmem) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
+}
+
 template <int NT>
 __global__ void __launch_bounds__(K2D_WARPS * 32) k3v_inner_dmma(const double* __restrict__ px, const double* __restrict__ py,
                                                                 const double* __restrict__ pz, int n_pad, Ranges3 rg, int nbc,
                                                                 int nsplit, const double* __restrict__ F, double* __restrict__ G,
                                                                 long long split_stride) {
-  constexpr int NCOL = 8 * NT;
-  __shared__ double sF[NCOL * 4 * K2D_LD], sxyz[3][K2D_TJ];
+  constexpr int NCOL = 8 * NT, TILE = NCOL * 4 * K2D_LD + 3 * K2D_TJ;  // doubles per stage: F rows, then x, y, z
+  __shared__ double stage[2][TILE];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
   const int tiles_per_class = (nbc + NCOL - 1) / NCOL;
   const int cls = blockIdx.y / tiles_per_class, bfirst = (blockIdx.y % tiles_per_class) * NCOL;
@@ -44,19 +48,32 @@ __global__ void __launch_bounds__(K2D_WARPS * 32) k3v_inner_dmma(const double* _
   const int t0 = rg.j0[cls] / K2D_TJ, t1 = rg.j1[cls] / K2D_TJ;
   const int ta = t0 + (int)((long long)(t1 - t0) * blockIdx.z / nsplit), tb = t0 + (int)((long long)(t1 - t0) * (blockIdx.z + 1) / nsplit);
   const double* Fc = F + ((long long)cls * nbc + bfirst) * 4 * n_pad;
-  for (int jt = ta; jt < tb; ++jt) {
+  const int nrows = min(NCOL, nbc - bfirst) * 4;  // rows (column, component) that exist; the others stay zero
+  for (int e = tid; e < 2 * TILE; e += K2D_WARPS * 32) (&stage[0][0])[e] = 0.0;
+  __syncthreads();
+  // a source tile travels global -> shared memory by 8-byte async copies, one tile ahead of its use
+  auto fetch = [&](int jt) {
+    double* st = stage[jt & 1];
     const int j0 = jt * K2D_TJ;
-    __syncthreads();
-    if (tid < 3 * K2D_TJ) sxyz[tid / K2D_TJ][tid % K2D_TJ] = (tid < K2D_TJ ? px : tid < 2 * K2D_TJ ? py : pz)[j0 + tid % K2D_TJ];
-    for (int e = tid; e < NCOL * 4 * K2D_TJ; e += K2D_WARPS * 32) {
-      const int row = e / K2D_TJ, j = e % K2D_TJ;  // row = col * 4 + comp
-      sF[row * K2D_LD + j] = bfirst + row / 4 < nbc ? Fc[(long long)row * n_pad + j0 + j] : 0.0;
+    for (int e = tid; e < nrows * K2D_TJ; e += K2D_WARPS * 32) {
+      const int row = e / K2D_TJ, j = e % K2D_TJ;
+      cp8_3v(st + row * K2D_LD + j, Fc + (long long)row * n_pad + j0 + j);
     }
-    __syncthreads();
+    if (tid < 3 * K2D_TJ) cp8_3v(st + NCOL * 4 * K2D_LD + tid, (tid < K2D_TJ ? px : tid < 2 * K2D_TJ ? py : pz) + j0 + tid % K2D_TJ);
+  };
+  if (ta < tb) fetch(ta);
+  asm volatile("cp.async.commit_group;");
+  for (int jt = ta; jt < tb; ++jt) {
+    asm volatile("cp.async.wait_group 0;");
+    __syncthreads();  // tile jt has landed for everybody, and everybody has finished tile jt - 1 (whose buffer is refilled now)
+    if (jt + 1 < tb) fetch(jt + 1);
+    asm volatile("cp.async.commit_group;");
+    const double* sF = stage[jt & 1];
+    const double* sxyz = sF + NCOL * 4 * K2D_LD;
 #pragma unroll
     for (int ks = 0; ks < 4; ++ks) {
       const int j = ks * 4 + t;
-      const Tensor6 U = landau_tensor_3v(xi, yi, zi, ri2, sxyz[0][j], sxyz[1][j], sxyz[2][j]);
+      const Tensor6 U = landau_tensor_3v(xi, yi, zi, ri2, sxyz[j], sxyz[K2D_TJ + j], sxyz[2 * K2D_TJ + j]);
 #pragma unroll
       for (int n = 0; n < NT; ++n) {
         const double* fr = sF + (n * 8 + g) * 4 * K2D_LD + j;
@@ -94,17 +111,52 @@ __global__ void __launch_bounds__(K2D_WARPS * 32) k3v_inner_dmma(const double* _
     }
 }
 
-// returns 0 or a landau_status; *nsplit_out = parts the source range was cut into (K2b adds them)
+template <int NT>
+inline void launch_inner_dmma_t(const double* px, const double* py, const double* pz, int n_pad, const Ranges3& rg, int n_classes,
+                                int nbc, int nsplit, const double* F, double* G, long long split_stride, cudaStream_t st) {
+  const dim3 grid(n_pad / (K2D_WARPS * 8), n_classes * ((nbc + 8 * NT - 1) / (8 * NT)), nsplit);
+  k3v_inner_dmma<NT><<<grid, K2D_WARPS * 32, 0, st>>>(px, py, pz, n_pad, rg, nbc, nsplit, F, G, split_stride);
+}
+inline int inner_dmma_nt(int nbc) { return nbc > 16 ? 4 : nbc > 8 ? 2 : 1; }
+
+// CTAs of the variant that fit on one SM (registers / shared memory), queried once per variant
+inline int inner_dmma_ctas_per_sm(int nt) {
+  int n = 0;
+  if (nt == 4)
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k3v_inner_dmma<4>, K2D_WARPS * 32, 0);
+  else if (nt == 2)
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k3v_inner_dmma<2>, K2D_WARPS * 32, 0);
+  else
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k3v_inner_dmma<1>, K2D_WARPS * 32, 0);
+  return n > 0 ? n : 1;
+}
+
+// Parts to cut the source range into: the smallest count for which the CTAs fill at least 95 % of the waves they take
+// (304 field tiles on 148 x 2 slots are 1.03 waves and would take the time of 2), else the best one found.
+inline int inner_dmma_split(long long items, long long slots, int max_split) {
+  int best = 1;
+  double best_eff = 0.0;
+  for (int n = 1; n <= max_split; ++n) {
+    const long long ctas = items * n, waves = (ctas + slots - 1) / slots;
+    const double eff = (double)ctas / (double)(waves * slots);
+    if (eff > best_eff + 1e-9) {
+      best_eff = eff;
+      best = n;
+    }
+    if (eff >= 0.95) return n;
+  }
+  return best;
+}
+
 inline int launch_inner_dmma(const double* px, const double* py, const double* pz, int n_pad, const Ranges3& rg, int n_classes,
                              int nbc, int nsplit, const double* F, double* G, long long split_stride, cudaStream_t st) {
-  const int nt = nbc > 16 ? 4 : nbc > 8 ? 2 : 1, ncol = 8 * nt;
-  const dim3 grid(n_pad / (K2D_WARPS * 8), n_classes * ((nbc + ncol - 1) / ncol), nsplit);
+  const int nt = inner_dmma_nt(nbc);
   if (nt == 4)
-    k3v_inner_dmma<4><<<grid, K2D_WARPS * 32, 0, st>>>(px, py, pz, n_pad, rg, nbc, nsplit, F, G, split_stride);
+    launch_inner_dmma_t<4>(px, py, pz, n_pad, rg, n_classes, nbc, nsplit, F, G, split_stride, st);
   else if (nt == 2)
-    k3v_inner_dmma<2><<<grid, K2D_WARPS * 32, 0, st>>>(px, py, pz, n_pad, rg, nbc, nsplit, F, G, split_stride);
+    launch_inner_dmma_t<2>(px, py, pz, n_pad, rg, n_classes, nbc, nsplit, F, G, split_stride, st);
   else
-    k3v_inner_dmma<1><<<grid, K2D_WARPS * 32, 0, st>>>(px, py, pz, n_pad, rg, nbc, nsplit, F, G, split_stride);
+    launch_inner_dmma_t<1>(px, py, pz, n_pad, rg, n_classes, nbc, nsplit, F, G, split_stride, st);
   return 0;
 }
 
