@@ -8,18 +8,23 @@ a3+a4 element matrices + assembly into the batched CSR of M/dt - J) over one bat
 distribution functions.  Default workload: BASELINE.json configs[4] ("large-batch
 throughput ... Jacobian build + assembly timed end to end"), e-/D+ on uniform 14x28 Q3 grids, batch 1024 per GPU
 (DESIGN.md "Measurement" says why this one and not configs[1]; `--config 2 --batch 64` runs configs[1]).
+`--config 6` is the paper's own 2V throughput problem, `--config 7` the paper's 3V problem (ten species, three grids of
+120 Q2 hexahedra, batch 32; Table 6), `--config 8` e-/D+ on two such 3V grids.
 
 Prints ONE JSON line (rank 0): value = Landau Jacobians/s of the whole job, device-resident inputs; e2e = same
 metric through landau_jacobian_host (pinned HOST buffers, H2D + D2H inside the timed region); roofline = the
-inner-integral kernel (K2) against the FP64 pipe peak measured in-process; cpu_baseline = the oracle, as it
-stands, on the host cores over a bounded sample of the same workload.
+inner-integral kernel (K2) against the FP64 pipe peak measured in-process (nominal figure beside it), with the assembly
+kernel (K3) against the measured HBM bandwidth under "assembly"; cpu_baseline = the oracle, as it stands, on the host
+cores over a bounded sample of the same workload.  Extras that do not enter `value`:
+  other_configs  short runs (3 steps) of the other BASELINE.json configs and of the paper's 3V problem: Jacobians/s, stage
+                 times, K2 and K3 roofline fractions (skip with --no-other-configs)
+  solve          the batched TFQMR + Jacobi solve of the step's backward-Euler systems on a bounded sub-batch
+                 (148 entries; the whole batch with --solve)
+  advance        `--advance N`: N backward-Euler steps with landau_step (Newton iterations x batch per second)
 
+`--gpus N` without a torchrun environment starts N ranks itself (one per GPU; NCCL for the barrier and the max-reduce
+only: batch entries are independent); `--dry-run` exercises that plumbing without a GPU (gloo).
 `--impl reference` times the oracle only (no GPU work); under torchrun only rank 0 runs it.
-
-Extras that do not enter `value`: `--solve` times the batched TFQMR solve of the step's backward-Euler systems
-(key "solve"), `--advance N` runs N backward-Euler steps of the batch with landau_step (key "advance": seconds,
-Newton iterations, Newton iterations x batch per second -- the paper's throughput measure, PAPER.md:119);
-`--config 6` is the paper's own throughput problem.
 """
 import argparse
 import json
@@ -38,8 +43,13 @@ import numpy as np  # noqa: E402
 
 METRIC = "landau_jacobians_per_s"
 UNIT = "Jacobians/s"
-FLOP_PER_PAIR_COLUMN = 14.0   # 7 FP64 FMA per (i, j, source column): DESIGN.md "Algorithmic work"
-TENSOR_FLOP_PER_PAIR = 250.0  # one evaluation of the 5 tensor components (counted from SASS)
+# Algorithmic FP64 work of the inner integral: FMAs x 2 per (i, j, source column), plus ONE
+# tensor evaluation per pair.  The cost of an evaluation comes from the ncu instruction totals of the committed capture
+# (profiles/r2_traffic.json.txt: thread-level dfma / dmul / dadd counts of K2 divided by the evaluations it executed);
+# the constants below are only the fall-back when that file does not cover the kernel.
+FLOP_PER_PAIR_COLUMN = {2: 14.0, 3: 30.0}
+TENSOR_FLOP_FALLBACK = {2: 140.0, 3: 40.0}
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FMA/clk x 2 x 1.965 GHz (guide: unit counts, max clock)
 
 
 def parse():
@@ -47,63 +57,168 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number 1..5 (6: the paper's throughput problem)")
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number 1..5 (6: the paper's 2V throughput "
+                    "problem, 7: the paper's 3V problem, 8: e-/D+ in 3V)")
     ap.add_argument("--batch", type=int, default=None, help="batch entries PER GPU (default: the config's)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU time budget of the cpu_baseline sample")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the short runs of the other configs")
+    ap.add_argument("--no-solve", action="store_true", help="skip the bounded TFQMR solve")
     ap.add_argument("--kernel", type=int, default=0, help="inner-integral kernel: 0 auto, 1 DFMA, 2 DMMA, 3/4 GEMM (32x128 / 16x256 tile)")
-    ap.add_argument("--solve", action="store_true", help="also time the batched TFQMR solve of the step's systems "
-                    "(reported under \"solve\", not part of value)")
+    ap.add_argument("--solve", action="store_true", help="time the batched TFQMR solve on the WHOLE batch (default: 148 entries)")
     ap.add_argument("--advance", type=int, default=0, help="also run this many backward-Euler steps (landau_step) and "
                     "report the time and Newton iterations under \"advance\" (not part of value)")
     ap.add_argument("--assembly", type=int, default=0, help="assembly kernel build (landau_set_assembly_kernel; 0: default)")
     ap.add_argument("--chunk", type=int, default=0, help="batch entries per pass through the stages (0: library default)")
+    ap.add_argument("--dry-run", action="store_true", help="rank plumbing only (gloo, no GPU work): the CPU test of --gpus N")
     return ap.parse_args()
 
 
+def load_config(index, batch=None):
+    """(cfg, dim): BASELINE.json configs 1..5, the paper's 2V problem (6) and the 3V problems (7, 8)."""
+    from paper_2209_03228_b200 import workloads as W
+    if index in (7, 8):
+        return W.config3v("paper" if index == 7 else "eD", batch), 3
+    return W.config(index, batch), 2
+
+
 def workload_name(cfg, B):
-    return "%s batch=%d/GPU (BASELINE.json configs[%d])" % (cfg["name"], B, cfg["index"] - 1)
+    if cfg["index"] <= 5:
+        return "%s batch=%d/GPU (BASELINE.json configs[%d])" % (cfg["name"], B, cfg["index"] - 1)
+    return "%s batch=%d/GPU (the paper's own problem, PAPER.md:125)" % (cfg["name"], B)
+
+
+def profile_data():
+    """Per-launch ncu figures of the committed `ncu --set full` captures (profiles/r2_traffic.json.txt)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.json.txt")) as fh:
+            return json.load(fh)
+    except (OSError, ValueError):
+        return {}
+
+
+def hbm_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "MEASURED_PEAKS.json"
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class Problem:
+    """One context (2V: binding.Landau, 3V: binding3v.Landau3V) behind the calls the measurement needs."""
+
+    def __init__(self, cfg, dim, device, kernel=0, assembly=0, chunk=0):
+        from paper_2209_03228_b200 import workloads as W
+        self.cfg, self.dim = cfg, dim
+        if dim == 2:
+            from paper_2209_03228_b200 import binding as Bn
+            self.Bn = Bn
+            self.L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"], device=device)
+            Bn.landau_set_inner_kernel(self.L.ctx, kernel)
+            if assembly:
+                Bn.landau_set_assembly_kernel(self.L.ctx, assembly)
+            if chunk:
+                Bn.landau_set_batch_chunk(self.L.ctx, chunk)
+            self.separable = bool(Bn.landau_is_separable(self.L.ctx))
+            self.make_f = W.make_batch_f
+        else:
+            from paper_2209_03228_b200 import binding3v as B3
+            self.Bn = B3
+            self.L = B3.Landau3V(cfg["grids"], cfg["species"], device=device)
+            if kernel:
+                B3.landau3v_set_inner_kernel(self.L.ctx, min(kernel, 2))
+            if assembly:
+                B3.landau3v_set_assembly_kernel(self.L.ctx, 1 if assembly == 1 else 0)
+            if chunk:
+                B3.landau3v_set_batch_chunk(self.L.ctx, chunk)
+            self.separable = True   # nu = q_a^2 q_b^2 is rank one
+            self.make_f = W.make_batch_f3v
+        self.N = int(sum(self.L.n_ip))
+        self.csr_stride, self.dk_stride, self.f_stride = int(self.L.csr_stride), int(self.L.dk_stride), int(self.L.f_stride)
+
+    def coords(self):
+        return [self.L.dof_coords(g) for g in range(self.L.G)]
+
+    def jacobian(self, f, B, out):
+        (self.Bn.landau_jacobian if self.dim == 2 else self.Bn.landau3v_jacobian)(self.L.ctx, f, B, self.cfg["dt"], out)
+
+    def jacobian_host(self, f_host, B, out_host):
+        (self.Bn.landau_jacobian_host if self.dim == 2 else self.Bn.landau3v_jacobian_host)(
+            self.L.ctx, f_host, B, self.cfg["dt"], out_host)
+
+    def set_timing(self, on):
+        (self.Bn.landau_set_timing if self.dim == 2 else self.Bn.landau3v_set_timing)(self.L.ctx, 1 if on else 0)
+
+    def stage_ms(self):
+        return np.array((self.Bn.landau_last_stage_ms if self.dim == 2 else self.Bn.landau3v_last_stage_ms)(self.L.ctx))
+
+    def launches(self):
+        return (self.Bn.landau_launch_count if self.dim == 2 else self.Bn.landau3v_launch_count)(self.L.ctx)
+
+    def pair_work(self, B):
+        """(unique tensor pairs, (i, j, column) products) of one step of B entries."""
+        pairs = float(self.N) * float(self.N)
+        if self.separable:
+            return pairs, pairs * B
+        sizes = [int(x) for x in self.L.n_ip]
+        per_grid = [sum(1 for s in self.L.sgrid if s == g) for g in range(self.L.G)]
+        return pairs, float(self.N) * sum(sizes[g] * per_grid[g] for g in range(self.L.G)) * B
+
+    def mass_block_sum(self):
+        """sum of all entries of the first species' block of M/dt - J = (1/dt) 1^T M 1 (since 1^T J = 0): the grid's measure."""
+        g0 = self.cfg["grids"][self.L.sgrid[0]]
+        vol = (2 * g0["half"]) ** 3 if self.dim == 3 else g0["r_max"] ** 2 * (g0["z_max"] - g0["z_min"]) / 2.0
+        return vol / self.cfg["dt"], int(self.L.nnz[self.L.sgrid[0]])
+
+    def close(self):
+        self.L.close()
 
 
 # ----------------------------------------------------------------------------------------------------------------
 # the oracle arm: cpu_baseline leg and --impl reference
 # ----------------------------------------------------------------------------------------------------------------
-def oracle_sample(cfg, seconds, min_entries=1, max_entries=64):
+def open_oracle(cfg, dim):
+    """(oracle object, make_batch_f) for a 2V or a 3V problem."""
+    from paper_2209_03228_b200 import workloads as W
+    if dim == 3:
+        from oracle import oracle3v as O3
+        O3.build()
+        return O3.Oracle3V(cfg["grids"], cfg["species"]), W.make_batch_f3v
+    from oracle import oracle as O
+    O.build()
+    return O.Oracle(cfg["grids"], cfg["species"], cfg["degree"]), W.make_batch_f
+
+
+def oracle_sample(cfg, dim, seconds, min_entries=1, max_entries=64):
     """Time the oracle (as it stands, OpenMP over field points) on entries 0, 1, ... of the workload until
     `seconds` of wall time are used.  Returns (Jacobians/s, entries done, threads, per-entry seconds)."""
-    from oracle import oracle as O
-    from paper_2209_03228_b200 import workloads as W
-    O.build()
-    o = O.Oracle(cfg["grids"], cfg["species"], cfg["degree"])
+    o, make_f = open_oracle(cfg, dim)
     coords = [o.dof_coords(g) for g in range(o.G)]
     times = []
     t_start = time.perf_counter()
     b = 0
     while b < max_entries and (b < min_entries or time.perf_counter() - t_start < seconds):
-        f = W.make_batch_f(cfg, coords, entries=[b])[0]
+        f = make_f(cfg, coords, entries=[b])[0]
         t0 = time.perf_counter()
         o.jacobian(f, cfg["dt"])
         times.append(time.perf_counter() - t0)
         b += 1
-    total = sum(times)
-    return len(times) / total, len(times), o.threads, times
+    return len(times) / sum(times), len(times), o.threads, times
 
 
 def run_reference(args):
-    from paper_2209_03228_b200 import workloads as W
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    cfg = W.config(args.config)
+    cfg, dim = load_config(args.config)
     B = args.batch or cfg["batch"]
     # a step = a bounded sample: ONE Jacobian (entry s mod B) of the workload on all host cores
-    from oracle import oracle as O
-    O.build()
-    o = O.Oracle(cfg["grids"], cfg["species"], cfg["degree"])
+    o, make_f = open_oracle(cfg, dim)
     coords = [o.dof_coords(g) for g in range(o.G)]
-    fs = [W.make_batch_f(cfg, coords, entries=[s % B])[0] for s in range(args.steps + args.warmup)]
+    fs = [make_f(cfg, coords, entries=[s % B])[0] for s in range(args.steps + args.warmup)]
     for s in range(args.warmup):
         o.jacobian(fs[s], cfg["dt"])
     t0 = time.perf_counter()
@@ -174,20 +289,207 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(sel)}
 
 
+
+
 # ----------------------------------------------------------------------------------------------------------------
 # our arm
 # ----------------------------------------------------------------------------------------------------------------
+def tensor_flop(dim, prof):
+    """FP64 FLOP of one tensor evaluation: ncu thread-instruction totals of K2 (2 x dfma + dmul + dadd; the DMMA
+    accumulation is a separate op class) divided by the evaluations the captured launch executed."""
+    key = "k2" if dim == 2 else "k2_3v"
+    try:
+        ev = float(prof[key + "_tensor_evaluations_executed"])
+        return (2.0 * prof[key + "_thread_inst_dfma"] + prof[key + "_thread_inst_dmul"] + prof[key + "_thread_inst_dadd"]) / ev, \
+            "ncu (profiles/r2_traffic.json.txt)"
+    except (KeyError, TypeError, ZeroDivisionError):
+        return TENSOR_FLOP_FALLBACK[dim], "fall-back constant"
+
+
+def rooflines(P, B, stage_ms, fp64_peak, prof, workload):
+    """Roofline objects of K2 (inner integral, FP64 pipe) and K3 (assembly, HBM) from the stage times of one step."""
+    pairs, cols_pairs = P.pair_work(B)
+    flop_u, flop_src = tensor_flop(P.dim, prof)
+    alg_flop = cols_pairs * FLOP_PER_PAIR_COLUMN[P.dim] + pairs * flop_u
+    k2_ms, k3_ms = float(stage_ms[1]), float(stage_ms[3])
+    achieved = alg_flop / (k2_ms * 1e-3) / 1e12
+    hbm, hbm_src = hbm_peak()
+    alg_bytes = float(B) * (P.csr_stride + P.dk_stride) * 8
+    tag = "" if P.dim == 2 else "_3v"
+    same = str(prof.get("workload" + tag, "")) and workload.startswith(str(prof.get("workload" + tag, "")))
+    k2 = {"kernel": "K2 inner integral (%s)" % ("k2_inner_*" if P.dim == 2 else "k3v_inner_*"), "bound": "alu",
+          "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s", "frac": achieved / fp64_peak,
+          "traffic": prof.get("k2%s_dram_bytes_per_launch" % tag) if same else None,
+          "k2_ms_per_step": k2_ms, "share_of_step": k2_ms / float(sum(stage_ms)), "algorithmic_flop_per_step": alg_flop,
+          "tensor_flop_per_evaluation": flop_u, "tensor_flop_source": flop_src}
+    k3 = {"kernel": "K3 element matrices + assembly (%s)" % ("k3_ring" if P.dim == 2 else "k3v_elem_matrix + k3v_gather"),
+          "bound": "hbm", "achieved": alg_bytes / (k3_ms * 1e-3) / 1e9, "peak": hbm, "peak_source": hbm_src, "unit": "GB/s",
+          "frac": alg_bytes / (k3_ms * 1e-3) / 1e9 / hbm, "k3_ms_per_step": k3_ms, "algorithmic_bytes_per_step": alg_bytes,
+          "traffic": prof.get("k3%s_dram_bytes_per_launch" % tag) if same else None}
+    return k2, k3
+
+
+def measure(P, B, steps, warmup, f_dev, out_dev, world, dev, sharding, sampler_index=None):
+    """`warmup` untimed + `steps` timed steps (CUDA events on the launching stream, barrier + synchronize on both sides, max
+    over ranks).  Returns (ms per step, stage ms per step, launches in the timed region, clocks summary or None)."""
+    import torch
+    stream = torch.cuda.current_stream()
+    for i in range(warmup):
+        P.jacobian(f_dev[i & 1], B, out_dev)
+    P.set_timing(True)
+    sampler = ClockSampler(sampler_index) if sampler_index is not None else None
+    sharding.barrier(world)
+    torch.cuda.synchronize()
+    launches0 = P.launches()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_wall0 = time.perf_counter()
+    e0.record(stream)
+    stage = np.zeros(4)
+    for i in range(steps):
+        P.jacobian(f_dev[i & 1], B, out_dev)
+        if i == steps - 1:
+            e1.record(stream)
+        stage += P.stage_ms()  # waits for this step's last event (host only)
+    torch.cuda.synchronize()
+    sharding.barrier(world)
+    t_wall1 = time.perf_counter()
+    ms_total = sharding.max_over_ranks(e0.elapsed_time(e1), world, dev)
+    launches = P.launches() - launches0
+    P.set_timing(False)
+    clocks = None
+    if sampler is not None:
+        sampler.stop()
+        clocks = sampler.summary(t_wall0, t_wall1)
+    return ms_total / steps, stage / steps, int(launches), clocks
+
+
+def sanity(P, out_dev):
+    expect, n0 = P.mass_block_sum()
+    got = float(out_dev[0, :n0].sum())
+    if not (math.isfinite(got) and abs(got - expect) < 1e-8 * abs(expect)):
+        raise SystemExit("bench sanity failed: sum(M/dt - J) = %r, expected %r" % (got, expect))
+
+
+def other_config_runs(local, dev, fp64_peak, prof, skip):
+    """Short runs of the configs BASELINE.json lists besides the headline one, and of the paper's 3V problem."""
+    import torch
+    from paper_2209_03228_b200 import sharding
+    rows = []
+    plan = [(1, 1), (2, 64), (3, 1), (3, 16), (3, 64), (3, 256), (3, 512), (4, 256), (5, 1024), (5, 4096), (7, 32)]
+    probs = {}
+    for index, B in plan:
+        if (index, B) == skip:
+            continue
+        try:
+            if index not in probs:
+                for P in probs.values():
+                    P.close()
+                probs = {}
+                cfg, dim = load_config(index)
+                probs[index] = Problem(cfg, dim, local)
+            P = probs[index]
+            f = torch.from_numpy(P.make_f(P.cfg, P.coords(), batch=B)).to(dev)
+            out = torch.empty((B, P.csr_stride), dtype=torch.float64, device=dev)
+            ms, stage, launches, _ = measure(P, B, 3, 2, [f, f], out, 1, dev, sharding)
+            sanity(P, out)
+            k2, k3 = rooflines(P, B, stage, fp64_peak, prof, "")
+            rows.append({"workload": workload_name(P.cfg, B), "jacobians_per_s": B / (ms * 1e-3), "ms_per_step": ms,
+                         "stage_ms": {"a1": stage[0], "a2": stage[1], "a2b": stage[2], "a3a4": stage[3]},
+                         "k2_tflops": k2["achieved"], "k2_frac": k2["frac"], "k3_gbs": k3["achieved"], "k3_frac": k3["frac"],
+                         "launches_per_step": launches / 3})
+            del f, out
+        except Exception as e:  # a failing extra must not take the headline number with it
+            rows.append({"workload": "config %d batch %d" % (index, B), "error": repr(e)[:200]})
+    for P in probs.values():
+        P.close()
+    torch.cuda.empty_cache()
+    return rows
+
+
+def solve_run(P, B, f_dev0, out_dev, dev, whole):
+    """The step after the hot path: backward-Euler systems (M/dt - J) x = (M/dt) f of a bounded
+    sub-batch, TFQMR + Jacobi, one system per CTA."""
+    import torch
+    Bn, L, cfg = P.Bn, P.L, P.cfg
+    nb = B if whole else min(B, 148)
+    f = f_dev0[:nb].contiguous()
+    a = torch.empty((nb, P.csr_stride), dtype=torch.float64, device=dev)
+    a_inf = torch.empty_like(a)
+    Bn.landau_jacobian(L.ctx, f, nb, float("inf"), a_inf)
+    Bn.landau_jacobian(L.ctx, f, nb, cfg["dt"], a)
+    rhs = torch.empty_like(f)
+    Bn.landau_spmv(L.ctx, a - a_inf, f, nb, rhs)
+    del a_inf
+    x = torch.zeros_like(rhs)
+    iters = torch.zeros((nb, L.S), dtype=torch.int32, device=dev)
+    stream = torch.cuda.current_stream()
+    t_solve = []
+    for rep in range(3):
+        x.zero_()
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record(stream)
+        Bn.landau_solve(L.ctx, a, rhs, nb, 1e-8, 2000, x, iters)
+        s1.record(stream)
+        torch.cuda.synchronize()
+        t_solve.append(s0.elapsed_time(s1))
+    res = rhs - L.spmv(a, x)
+    ms = min(t_solve)
+    # bytes one half-step of one system moves through the SM (one SpMV: values + column indices, plus ~10 vector passes)
+    half = iters.abs().to(torch.float64).cpu().numpy()
+    byts = 0.0
+    for s in range(L.S):
+        g = L.sgrid[s]
+        byts += float(half[:, s].sum()) * (12.0 * float(L.nnz[g]) + 10 * 8.0 * float(L.n_dof[g]))
+    return {"ms_per_batch": ms, "entries": int(nb), "systems": int(nb * L.S), "rtol": 1e-8,
+            "half_steps_mean": float(half.mean()), "half_steps_max": int(half.max()),
+            "not_converged": int((iters < 0).sum()),
+            "max_true_relative_residual": float((res.norm(dim=1) / rhs.norm(dim=1)).max()),
+            "solves_per_s": nb * L.S / (ms * 1e-3),
+            "roofline": {"kernel": "K4 batched TFQMR (k4_tfqmr)", "bound": "l2", "achieved": byts / (ms * 1e-3) / 1e9,
+                         "unit": "GB/s", "peak": None,
+                         "note": "matrix + vector bytes per half-step from L2 / shared memory; the guides state no L2 "
+                                 "bandwidth figure, ncu shows the kernel at 71 % of the L1TEX throughput (DESIGN.md K4)"}}
+
+
+def run_dry(args):
+    """--dry-run: the N-rank plumbing without a GPU (gloo): shards, barrier, max over ranks, one JSON line from rank 0."""
+    import torch
+    import torch.distributed as dist
+    from paper_2209_03228_b200 import sharding
+    rank, world, local = sharding.env_rank()
+    if world > 1:
+        dist.init_process_group("gloo")
+    cfg, dim = load_config(args.config)
+    B = args.batch or cfg["batch"]
+    entries = sharding.shard_entries(rank, world, B * world, mode="weak")
+    sharding.barrier(world)
+    ms = sharding.max_over_ranks(1.0 + rank, world, torch.device("cpu"))
+    counts = [None] * world
+    if world > 1:
+        dist.all_gather_object(counts, (rank, entries[0], entries[-1]))
+    else:
+        counts = [(0, entries[0], entries[-1])]
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": None, "unit": UNIT, "n_gpus": world, "dry_run": True,
+                          "max_over_ranks_ms": ms, "shards": counts,
+                          "config": {"workload": workload_name(cfg, B), "parallelism": "batch shards, no collective (dp%d)" % world}}),
+              flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_ours(args):
     import torch
     from paper_2209_03228_b200 import binding as Bn
     from paper_2209_03228_b200 import sharding
-    from paper_2209_03228_b200 import workloads as W
 
     rank, world, local = sharding.env_rank()
-    if world != args.gpus and world > 1:
+    if world != args.gpus:
         raise SystemExit("--gpus %d but WORLD_SIZE=%d" % (args.gpus, world))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    if local >= torch.cuda.device_count():
+        raise SystemExit("rank %d has no GPU (%d visible)" % (rank, torch.cuda.device_count()))
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
@@ -195,131 +497,71 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
     Bn.load()
 
-    cfg = W.config(args.config)
+    cfg, dim = load_config(args.config)
     B = args.batch or cfg["batch"]
-    L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"], device=local)
-    Bn.landau_set_inner_kernel(L.ctx, args.kernel)
-    if args.assembly:
-        Bn.landau_set_assembly_kernel(L.ctx, args.assembly)
-    if args.chunk:
-        Bn.landau_set_batch_chunk(L.ctx, args.chunk)
-    coords = [L.dof_coords(g) for g in range(L.G)]
+    P = Problem(cfg, dim, local, args.kernel, args.assembly, args.chunk)
     # weak scaling: rank r owns the global batch entries [r*B, (r+1)*B) -- independent problems, no collective
     entries = sharding.shard_entries(rank, world, B * world, mode="weak")
-    f_host = torch.from_numpy(W.make_batch_f(cfg, coords, batch=B * world, entries=entries)).pin_memory()
-    out_host = torch.empty((B, L.csr_stride), dtype=torch.float64).pin_memory()
+    f_host = torch.from_numpy(P.make_f(cfg, P.coords(), batch=B * world, entries=entries)).pin_memory()
+    out_host = torch.empty((B, P.csr_stride), dtype=torch.float64).pin_memory()
     f_dev = [f_host.to(dev), f_host.to(dev).clone()]  # two input copies, alternated
-    out_dev = torch.empty((B, L.csr_stride), dtype=torch.float64, device=dev)
-    stream = torch.cuda.current_stream()
-    N = int(sum(L.n_ip))
-    pairs = float(N) * float(N)
+    out_dev = torch.empty((B, P.csr_stride), dtype=torch.float64, device=dev)
+    pairs, cols_pairs = P.pair_work(B)
 
     # FP64 pipe peaks measured in-process (roofline denominator): plain DFMA and DMMA m8n8k4
     peak_dfma = Bn.landau_fp64_probe(0, 20000)
     peak_dmma = Bn.landau_fp64_probe(1, 20000)
     peak = max(peak_dfma, peak_dmma)
+    prof = profile_data()
 
-    def step(i):
-        Bn.landau_jacobian(L.ctx, f_dev[i & 1], B, cfg["dt"], out_dev)
-
-    for i in range(args.warmup):
-        step(i)
-    Bn.landau_set_timing(L.ctx, 1)
-    sampler = ClockSampler(local) if rank == 0 else None
-    sharding.barrier(world)
-    torch.cuda.synchronize()
-    launches0 = Bn.landau_launch_count(L.ctx)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t_wall0 = time.perf_counter()
-    e0.record(stream)
-    stage = np.zeros(4)
-    for i in range(args.steps):
-        step(i)
-        if i == args.steps - 1:
-            e1.record(stream)
-        stage += np.array(Bn.landau_last_stage_ms(L.ctx))  # waits for this step's last event (host only)
-    torch.cuda.synchronize()
-    sharding.barrier(world)
-    t_wall1 = time.perf_counter()
-    ms_total = sharding.max_over_ranks(e0.elapsed_time(e1), world, dev)
-    launches = Bn.landau_launch_count(L.ctx) - launches0
-    Bn.landau_set_timing(L.ctx, 0)
-    clocks = None
-    if sampler is not None:
-        sampler.stop()
-        clocks = sampler.summary(t_wall0, t_wall1)
-    ms_per_step = ms_total / args.steps
+    ms_per_step, stage, launches, clocks = measure(P, B, args.steps, args.warmup, f_dev, out_dev, world, dev, sharding,
+                                                   local if rank == 0 else None)
     value = world * B / (ms_per_step * 1e-3)
-
-    # sanity on the result of the timed steps: finite, and 1^T J = 0 cannot be checked with the shift, so
-    # check the mass identity instead: sum of all entries of M/dt - J block = (1/dt) 1^T M 1 (since 1^T J = 0)
-    blk = out_dev[0, :int(L.nnz[L.sgrid[0]])]
-    g0 = cfg["grids"][L.sgrid[0]]
-    expect = g0["r_max"] ** 2 * (g0["z_max"] - g0["z_min"]) / 2.0 / cfg["dt"]
-    got = float(blk.sum())
-    if not (math.isfinite(got) and abs(got - expect) < 1e-8 * abs(expect)):
-        raise SystemExit("bench sanity failed: sum(M/dt - J) = %r, expected %r" % (got, expect))
+    per_rank = None
+    if world > 1:
+        import torch.distributed as dist
+        mine = torch.tensor([B / (ms_per_step * 1e-3)], dtype=torch.float64, device=dev)
+        allv = [torch.zeros_like(mine) for _ in range(world)]
+        dist.all_gather(allv, mine)
+        per_rank = [float(v.item()) for v in allv]
+    sanity(P, out_dev)
 
     # end to end through the C ABI with HOST buffers (H2D of f and D2H of the CSR values inside the timed region)
     e2e = None
     if not args.no_e2e:
         for i in range(2):
-            Bn.landau_jacobian_host(L.ctx, f_host, B, cfg["dt"], out_host)
+            P.jacobian_host(f_host, B, out_host)
         sharding.barrier(world)
         torch.cuda.synchronize()
         n_e2e = max(2, min(args.steps, 5))
         t0 = time.perf_counter()
         for i in range(n_e2e):
-            Bn.landau_jacobian_host(L.ctx, f_host, B, cfg["dt"], out_host)  # synchronous
+            P.jacobian_host(f_host, B, out_host)  # synchronous
         torch.cuda.synchronize()
         t_e2e = sharding.max_over_ranks((time.perf_counter() - t0) * 1e3, world, dev) / n_e2e
         # same values up to summation order: the host path runs the batch in pieces, and the persistent K2 cuts the
         # source range of a few tiles at piece-dependent places (K2 stream mode)
-        if (args.steps - 1) & 1 == 0:
-            a, b = out_host[0].numpy(), out_dev[0].cpu().numpy()
-            if not np.linalg.norm(a - b) <= 1e-13 * np.linalg.norm(b):
-                raise SystemExit("bench sanity failed: host-buffer path differs from device path")
+        a, b = out_host[0].numpy(), out_dev[0].cpu().numpy()
+        if not np.linalg.norm(a - b) <= 1e-13 * np.linalg.norm(b):
+            raise SystemExit("bench sanity failed: host-buffer path differs from device path")
         e2e = {"value": world * B / (t_e2e * 1e-3), "unit": UNIT, "ms_per_step": t_e2e,
                "h2d_bytes_per_step": int(f_host.numel() * 8), "d2h_bytes_per_step": int(out_host.numel() * 8),
-               "steps": n_e2e, "api": "landau_jacobian_host (pinned host buffers)"}
+               "steps": n_e2e, "api": "landau%s_jacobian_host (pinned host buffers)" % ("" if dim == 2 else "3v")}
 
     solve = None
-    if args.solve:
-        # the step after the hot path: backward-Euler systems (M/dt - J) x = (M/dt) f, TFQMR + Jacobi
-        a_inf = torch.empty_like(out_dev)
-        Bn.landau_jacobian(L.ctx, f_dev[0], B, float("inf"), a_inf)
-        Bn.landau_jacobian(L.ctx, f_dev[0], B, cfg["dt"], out_dev)
-        rhs = torch.empty_like(f_dev[0])
-        Bn.landau_spmv(L.ctx, out_dev - a_inf, f_dev[0], B, rhs)
-        del a_inf
-        x = torch.zeros_like(rhs)
-        iters = torch.zeros((B, L.S), dtype=torch.int32, device=dev)
-        t_solve = []
-        for rep in range(3):
-            x.zero_()
-            s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            s0.record(stream)
-            Bn.landau_solve(L.ctx, out_dev, rhs, B, 1e-8, 2000, x, iters)
-            s1.record(stream)
-            torch.cuda.synchronize()
-            t_solve.append(s0.elapsed_time(s1))
-        res = rhs - L.spmv(out_dev, x)
-        solve = {"ms_per_batch": min(t_solve), "systems": int(B * L.S), "rtol": 1e-8,
-                 "half_steps_mean": float(iters.float().abs().mean()), "half_steps_max": int(iters.abs().max()),
-                 "not_converged": int((iters < 0).sum()),
-                 "max_true_relative_residual": float((res.norm(dim=1) / rhs.norm(dim=1)).max()),
-                 "solves_per_s": world * B * L.S / (min(t_solve) * 1e-3)}
+    if dim == 2 and not args.no_solve and rank == 0:
+        solve = solve_run(P, B, f_dev[0], out_dev, dev, args.solve)
     advance = None
-    if args.advance:
+    if args.advance and dim == 2:
         # the implicit advance the path belongs to (Table 5): backward-Euler steps of the whole batch
         u = f_dev[0].clone()
-        Bn.landau_step(L.ctx, u, B, cfg["dt"], 1e-8, 50, 1e-10, 2000)          # warm-up (scratch, mass values)
+        Bn.landau_step(P.L.ctx, u, B, cfg["dt"], 1e-8, 50, 1e-10, 2000)          # warm-up (scratch, mass values)
         u.copy_(f_dev[0])
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         newton = 0
         for k in range(args.advance):
-            info = Bn.landau_step(L.ctx, u, B, cfg["dt"], 1e-8, 50, 1e-10, 2000)
+            info = Bn.landau_step(P.L.ctx, u, B, cfg["dt"], 1e-8, 50, 1e-10, 2000)
             newton += info["newton_its"]
         torch.cuda.synchronize()
         t_adv = time.perf_counter() - t0
@@ -327,89 +569,70 @@ def run_ours(args):
                    "newton_rtol": 1e-8, "lin_rtol": 1e-10, "last": info,
                    "newton_iterations_x_batch_per_s": newton * B * world / t_adv}
     if rank == 0:
-        # roofline of the dominant kernel (K2, inner integral).  Algorithmic FLOPs per step:
-        # 14 flop per (i, j, source column) -- separable nu: one column per batch entry over all N^2 pairs --
-        # plus ONE tensor evaluation per pair (the tensor does not depend on the batch entry).
-        cols_pairs = 0.0
-        sizes = [int(x) for x in L.n_ip]
-        sp_per_grid = [sum(1 for s in L.sgrid if s == g) for g in range(L.G)]
-        separable = Bn.landau_is_separable(L.ctx)
-        if separable:
-            cols_pairs = pairs * B
-        else:
-            cols_pairs = float(N) * sum(sizes[g] * sp_per_grid[g] for g in range(L.G)) * B
-        flop_u = TENSOR_FLOP_PER_PAIR
-        alg_flop = cols_pairs * FLOP_PER_PAIR_COLUMN + pairs * flop_u
-        k2_ms = stage[1] / args.steps
-        achieved = alg_flop / (k2_ms * 1e-3) / 1e12
-        k3_ms = stage[3] / args.steps
-        csr_bytes = float(B) * L.csr_stride * 8
-        dk_bytes = float(B) * L.dk_stride * 8
-        traffic = ncu_traffic(workload_name(cfg, B))
-        roofline = {"kernel": "K2 inner integral (k2_inner_*)", "bound": "alu", "achieved": achieved, "peak": peak,
-                    "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic.get("k2_dram_bytes_per_launch"),
-                    "traffic_source": traffic.get("source"),
-                    "peak_source": "in-process FP64 probe (DFMA %.2f, DMMA m8n8k4 %.2f TFLOP/s), max taken"
-                                   % (peak_dfma, peak_dmma),
-                    "k2_ms_per_step": k2_ms, "share_of_step": k2_ms / (sum(stage) / args.steps),
-                    "algorithmic_flop_per_step": alg_flop,
-                    "assembly": {"kernel": "K3 element matrices + assembly (k3_*)", "bound": "hbm",
-                                 "achieved": (csr_bytes + dk_bytes) / (k3_ms * 1e-3) / 1e9, "peak": hbm_peak(),
-                                 "unit": "GB/s", "frac": (csr_bytes + dk_bytes) / (k3_ms * 1e-3) / 1e9 / hbm_peak(),
-                                 "k3_ms_per_step": k3_ms, "algorithmic_bytes_per_step": csr_bytes + dk_bytes,
-                                 "traffic": traffic.get("k3_dram_bytes_per_launch")}}
+        name = workload_name(cfg, B)
+        k2, k3 = rooflines(P, B, stage, peak, prof, name)
+        k2.update({"peak_probe": peak, "peak_nominal": FP64_NOMINAL_TFLOPS,
+                   "peak_source": "in-process FP64 probe (DFMA %.2f, DMMA m8n8k4 %.2f TFLOP/s), max taken; nominal "
+                                  "148 SM x 64 FMA/clk x 2 x 1.965 GHz = %.2f" % (peak_dfma, peak_dmma, FP64_NOMINAL_TFLOPS),
+                   "traffic_source": prof.get("source"), "assembly": k3})
         cpu = None
         if not args.no_cpu_baseline and world == 1:
-            v, n_done, threads, times = oracle_sample(cfg, args.cpu_seconds)
+            v, n_done, threads, times = oracle_sample(cfg, dim, args.cpu_seconds)
             cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
                    "sample": "%d Jacobian(s) (batch entries 0..%d) of the workload, %.1f s" % (n_done, n_done - 1, sum(times))}
+        csr_bytes = float(B) * P.csr_stride * 8
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": {"workload": workload_name(cfg, B), "species": L.S, "grids": L.G, "n_ip": N,
-                           "pairs_per_jacobian": pairs, "csr_bytes_per_jacobian": int(L.csr_stride * 8),
+                "config": {"workload": name, "species": P.L.S, "grids": P.L.G, "n_ip": P.N,
+                           "pairs_per_jacobian": pairs, "csr_bytes_per_jacobian": int(P.csr_stride * 8),
                            "parallelism": "batch shards, no collective (dp%d)" % world,
-                           "l2": "working set per step (CSR out %.2f GB + scratch) exceeds the 126 MB L2; "
-                                 "two input copies alternated" % (csr_bytes / 1e9)},
+                           "l2": "working set per step (CSR out %.2f GB + scratch) %s the 126 MB L2; two input copies "
+                                 "alternated" % (csr_bytes / 1e9, "exceeds" if csr_bytes > 126e6 else "is below")},
                 "pair_evals_per_s": {"tensor_evaluations_unique": pairs * world / (ms_per_step * 1e-3),
-                                     # the many-column kernel re-evaluates the tensor once per tile of 256 columns
-                                     "tensor_evaluations_executed": pairs * math.ceil(cols_pairs / pairs / 256.0) * world
-                                     / (ms_per_step * 1e-3) if separable and cols_pairs / pairs > 128 else None,
+                                     # the many-column 2V kernel re-evaluates the tensor once per tile of 256 columns, the 3V
+                                     # kernel once per tile of 32
+                                     "tensor_evaluations_executed": pairs * math.ceil(cols_pairs / pairs / (256.0 if dim == 2 else 32.0))
+                                     * world / (ms_per_step * 1e-3) if P.separable and (dim == 3 or cols_pairs / pairs > 128) else None,
                                      "pair_applications_b_i_j": cols_pairs * world / (ms_per_step * 1e-3)},
-                "stage_ms_per_step": {"a1_fields": stage[0] / args.steps, "a2_inner": k2_ms,
-                                      "a2b_combine": stage[2] / args.steps, "a3a4_assembly": k3_ms},
-                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "solve": solve, "advance": advance, "gpu_launches": int(launches),
-                "clocks": clocks}
+                "stage_ms_per_step": {"a1_fields": stage[0], "a2_inner": stage[1], "a2b_combine": stage[2], "a3a4_assembly": stage[3]},
+                "roofline": k2, "cpu_baseline": cpu, "e2e": e2e, "solve": solve, "advance": advance,
+                "gpu_launches": int(launches), "clocks": clocks}
+        if per_rank is not None:
+            line["per_rank_jacobians_per_s"] = per_rank
+    # the context of the headline run is released before the extras so that config 5 at batch 4096 (5.8 GB of CSR) fits
+    del f_dev, out_dev
+    P.close()
+    torch.cuda.empty_cache()
+    if rank == 0:
+        if not args.no_other_configs and world == 1:
+            line["other_configs"] = other_config_runs(local, dev, peak, prof, (args.config, B))
         print(json.dumps(line), flush=True)
-    L.close()
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
 
 
-def ncu_traffic(workload):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of this
-    workload (profiles/r1_traffic.json.txt); empty when the workload is another one (traffic = null)."""
-    try:
-        with open(os.path.join(ROOT, "profiles", "r1_traffic.json.txt")) as fh:
-            t = json.load(fh)
-        return t if workload.startswith(t["workload"]) else {}
-    except (OSError, KeyError, ValueError):
-        return {}
-
-
-def hbm_peak():
-    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    try:
-        with open(p) as fh:
-            return float(json.load(fh)["hbm_gbs"])
-    except (OSError, KeyError, ValueError):
-        return 6650.0  # B200_PROFILING.md fallback
+def spawn_ranks(args):
+    """`--gpus N` outside a torchrun environment: start N ranks of this script (one per GPU) the way the driver would and
+    pass their output through.  Rank 0 prints the JSON line."""
+    import socket
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
 
 
 if __name__ == "__main__":
     a = parse()
+    if a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(a)
     if a.impl == "reference":
         run_reference(a)
+    elif a.dry_run:
+        run_dry(a)
     else:
         run_ours(a)

@@ -71,3 +71,22 @@ def test_world2_gloo_shards_and_reductions():
         assert p.exitcode == 0
     tag, m, same = q.get(timeout=10)
     assert tag == "ok" and m == 11.0 and same
+
+
+def test_bench_gpus_n_starts_n_ranks():
+    """`python bench.py --gpus 2` outside a torchrun environment must really run two ranks (here: --dry-run, gloo, no GPU work)
+    and say so in its line -- it used to benchmark one GPU silently."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--dry-run", "--config", "2", "--batch", "8"],
+                         capture_output=True, text=True, env=env, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1                                   # rank 0 alone prints
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["dry_run"] is True
+    assert line["shards"] == [[0, 0, 7], [1, 8, 15]]          # weak scaling: rank r owns entries [8 r, 8 r + 8)
+    assert line["max_over_ranks_ms"] == 2.0                   # max over ranks of (1 + rank)
