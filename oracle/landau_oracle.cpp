@@ -14,6 +14,8 @@
 //   * PAPER.md:92 (sec. 2.3)     -- 2V cylindrical coordinates; the tensor is the azimuthal average of the
 //                                   3-D Landau tensor (the paper only cites [12] App. A; derivation in DESIGN.md)
 //   * PAPER.md:125               -- quadtree AMR grid with hanging nodes, no essential BCs (14 cells/142 eqs pin)
+//   * PAPER.md:225-229 (sec. 5.2) -- unstructured grids of quadrilateral (tensor) cells: straight-sided cells, bilinear
+//                                   reference map, gradient transformation J^-T per integration point (orc_create_meshes)
 //
 // Step by step, in the order of DESIGN.md "oracle steps" O1..O10.  No blocking, fusion or reordering:
 // every batch entry recomputes every tensor.  Inner sums accumulate in long double; the tensor itself is
@@ -261,6 +263,12 @@ struct Grid {
   std::vector<int> rowptr, colidx;
   // integration points, cell-major: ip = cell*nq + q
   std::vector<ld> ip_r, ip_z, ip_w;
+  // unstructured straight-sided quadrilaterals (sec. 5.2): the reference-to-physical map is bilinear, so
+  // the gradient transformation differs from point to point.  gm[ip] = J^-T, (d/dr, d/dz) = gm (d/dxi, d/deta);
+  // rectangular grids keep the two scale factors 2/hr, 2/hz of their cell.
+  bool unstructured = false;
+  std::vector<ld> gm;            // [ip][4]: m00 m01 m10 m11
+  std::vector<ld> node_r, node_z;  // dof coordinates (unstructured grids)
   int n_ip() const { return (int)ip_r.size(); }
 };
 
@@ -443,6 +451,126 @@ void cell_sizes(const Grid& g, int e, ld* hr, ld* hz) {
   *hz = g.k * s * g.uz;
 }
 
+// physical gradient of a function with reference gradient (dxi, deta) at integration point q of cell e
+inline void grad_phys(const Grid& g, int e, int ip, ld dxi, ld deta, ld* pr, ld* pz) {
+  if (g.unstructured) {
+    const ld* m = &g.gm[4 * (size_t)ip];
+    *pr = m[0] * dxi + m[1] * deta;
+    *pz = m[2] * dxi + m[3] * deta;
+  } else {
+    ld hr, hz;
+    cell_sizes(g, e, &hr, &hz);
+    *pr = (2 / hr) * dxi;
+    *pz = (2 / hz) * deta;
+  }
+}
+
+// O3' + O4' unstructured conforming mesh of straight-sided quadrilaterals (vertices (r, z), cells = 4 vertex ids,
+// counter-clockwise).  Qk nodes sit at the images of the equispaced reference nodes under the cell's bilinear map; nodes
+// of neighbouring cells that coincide are one dof (found geometrically: equal coordinates on a grid of 2^-30 of the mesh
+// extent); dofs are ordered by (z, r) on that grid; no constraints.  Integration points: the images of the Gauss points,
+// w = gw gw det(J) r with J the Jacobian of the bilinear map at the point.
+bool build_unstructured(const Problem& pb, Grid& g, int nv, const double* verts, int nc, const int* cells) {
+  const int k = pb.k, n1 = k + 1;
+  g.unstructured = true;
+  g.L = 0;
+  g.cells.assign(nc, Cell{0, 0, 0});
+  ld scale = 0;
+  for (int v = 0; v < 2 * nv; v++) scale = std::max(scale, fabsl((ld)verts[v]));
+  const ld quantum = scale / (ld)(1L << 30);
+  auto bilinear = [&](int e, ld xi, ld eta, ld* r, ld* z, ld* J) {
+    const ld N[4] = {(1 - xi) * (1 - eta) / 4, (1 + xi) * (1 - eta) / 4, (1 + xi) * (1 + eta) / 4, (1 - xi) * (1 + eta) / 4};
+    const ld Nx[4] = {-(1 - eta) / 4, (1 - eta) / 4, (1 + eta) / 4, -(1 + eta) / 4};
+    const ld Ne[4] = {-(1 - xi) / 4, -(1 + xi) / 4, (1 + xi) / 4, (1 - xi) / 4};
+    *r = *z = 0;
+    if (J) J[0] = J[1] = J[2] = J[3] = 0;
+    for (int v = 0; v < 4; v++) {
+      const ld vr = verts[2 * cells[4 * e + v]], vz = verts[2 * cells[4 * e + v] + 1];
+      *r += N[v] * vr;
+      *z += N[v] * vz;
+      if (J) {
+        J[0] += Nx[v] * vr;  // dr/dxi
+        J[1] += Ne[v] * vr;  // dr/deta
+        J[2] += Nx[v] * vz;  // dz/dxi
+        J[3] += Ne[v] * vz;  // dz/deta
+      }
+    }
+  };
+  std::map<Key, int> node_id;  // (quantised z, quantised r) -> provisional id
+  std::vector<Key> keys;
+  std::vector<ld> nr, nz;
+  std::vector<int> cell_node((size_t)nc * n1 * n1);
+  for (int e = 0; e < nc; e++)
+    for (int a2 = 0; a2 <= k; a2++)
+      for (int a1 = 0; a1 <= k; a1++) {
+        ld r, z;
+        bilinear(e, -1 + 2 * (ld)a1 / k, -1 + 2 * (ld)a2 / k, &r, &z, nullptr);
+        const Key key((long)llroundl(z / quantum), (long)llroundl(r / quantum));
+        auto it = node_id.find(key);
+        int id;
+        if (it == node_id.end()) {
+          id = (int)keys.size();
+          node_id[key] = id;
+          keys.push_back(key);
+          nr.push_back(r);
+          nz.push_back(z);
+        } else {
+          id = it->second;
+        }
+        cell_node[((size_t)e * n1 + a2) * n1 + a1] = id;
+      }
+  std::vector<int> order(keys.size());
+  for (size_t i = 0; i < order.size(); i++) order[i] = (int)i;
+  std::sort(order.begin(), order.end(), [&](int a, int b) { return keys[a] < keys[b]; });
+  std::vector<int> dof_of(keys.size());
+  g.n_dof = (int)keys.size();
+  g.node_r.resize(g.n_dof);
+  g.node_z.resize(g.n_dof);
+  for (int I = 0; I < g.n_dof; I++) {
+    dof_of[order[I]] = I;
+    g.node_r[I] = nr[order[I]];
+    g.node_z[I] = nz[order[I]];
+  }
+  g.P.assign(nc, std::vector<std::vector<std::pair<int, ld>>>(n1 * n1));
+  for (int e = 0; e < nc; e++)
+    for (int a = 0; a < n1 * n1; a++) g.P[e][a].push_back(std::make_pair(dof_of[cell_node[(size_t)e * n1 * n1 + a]], (ld)1));
+  std::vector<std::vector<int>> rows(g.n_dof);
+  for (int e = 0; e < nc; e++) {
+    std::vector<int> touched;
+    for (const auto& row : g.P[e])
+      for (const auto& dw : row) touched.push_back(dw.first);
+    std::sort(touched.begin(), touched.end());
+    touched.erase(std::unique(touched.begin(), touched.end()), touched.end());
+    for (int I : touched)
+      for (int J : touched) rows[I].push_back(J);
+  }
+  g.rowptr.assign(g.n_dof + 1, 0);
+  g.colidx.clear();
+  for (int I = 0; I < g.n_dof; I++) {
+    std::sort(rows[I].begin(), rows[I].end());
+    rows[I].erase(std::unique(rows[I].begin(), rows[I].end()), rows[I].end());
+    g.rowptr[I + 1] = g.rowptr[I] + (int)rows[I].size();
+    g.colidx.insert(g.colidx.end(), rows[I].begin(), rows[I].end());
+  }
+  for (int e = 0; e < nc; e++)
+    for (int q2 = 0; q2 < pb.nq1; q2++)
+      for (int q1 = 0; q1 < pb.nq1; q1++) {
+        ld r, z, J[4];
+        bilinear(e, pb.gx[q1], pb.gx[q2], &r, &z, J);
+        const ld det = J[0] * J[3] - J[1] * J[2];
+        if (!(det > 0)) return false;  // inverted or clockwise cell
+        g.ip_r.push_back(r);
+        g.ip_z.push_back(z);
+        g.ip_w.push_back(pb.gw[q1] * pb.gw[q2] * det * r);
+        // J^-1 = 1/det [ dz/deta, -dr/deta ; -dz/dxi, dr/dxi ] (rows: xi_r xi_z ; eta_r eta_z); gm = J^-T
+        g.gm.push_back(J[3] / det);
+        g.gm.push_back(-J[2] / det);
+        g.gm.push_back(-J[1] / det);
+        g.gm.push_back(J[0] / det);
+      }
+  return true;
+}
+
 // O5  field values at the integration points of one species: f, df/dr, df/dz.
 void fields_at_ips(const Problem& pb, const Grid& g, const double* fdof, std::vector<ld>& f,
                    std::vector<ld>& fr, std::vector<ld>& fz) {
@@ -451,8 +579,6 @@ void fields_at_ips(const Problem& pb, const Grid& g, const double* fdof, std::ve
   fr.assign(nip, 0);
   fz.assign(nip, 0);
   for (size_t e = 0; e < g.cells.size(); e++) {
-    ld hr, hz;
-    cell_sizes(g, (int)e, &hr, &hz);
     std::vector<ld> fe(pb.nb, 0);  // (P_e f)_a
     for (int a = 0; a < pb.nb; a++)
       for (const auto& dw : g.P[e][a]) fe[a] += dw.second * (ld)fdof[dw.first];
@@ -464,8 +590,7 @@ void fields_at_ips(const Problem& pb, const Grid& g, const double* fdof, std::ve
         ve += pb.dBeta[q * pb.nb + a] * fe[a];
       }
       f[e * pb.nq + q] = v;
-      fr[e * pb.nq + q] = (2 / hr) * vx;
-      fz[e * pb.nq + q] = (2 / hz) * ve;
+      grad_phys(g, (int)e, (int)(e * pb.nq + q), vx, ve, &fr[e * pb.nq + q], &fz[e * pb.nq + q]);
     }
   }
 }
@@ -547,16 +672,16 @@ void assemble_species(const Problem& pb, const Grid& g, const DK* dk, ld inv_dt,
   std::vector<ld> acc(g.colidx.size(), 0);
   const int nb = pb.nb, nq = pb.nq;
   for (size_t e = 0; e < g.cells.size(); e++) {
-    ld hr, hz;
-    cell_sizes(g, (int)e, &hr, &hz);
     std::vector<ld> Ae(nb * nb, 0);
     for (int q = 0; q < nq; q++) {
       int ip = (int)e * nq + q;
       ld w = g.ip_w[ip];
       for (int a = 0; a < nb; a++) {
-        ld pa = pb.B[q * nb + a], par = (2 / hr) * pb.dBxi[q * nb + a], paz = (2 / hz) * pb.dBeta[q * nb + a];
+        ld pa = pb.B[q * nb + a], par, paz;
+        grad_phys(g, (int)e, ip, pb.dBxi[q * nb + a], pb.dBeta[q * nb + a], &par, &paz);
         for (int c = 0; c < nb; c++) {
-          ld pc = pb.B[q * nb + c], pcr = (2 / hr) * pb.dBxi[q * nb + c], pcz = (2 / hz) * pb.dBeta[q * nb + c];
+          ld pc = pb.B[q * nb + c], pcr, pcz;
+          grad_phys(g, (int)e, ip, pb.dBxi[q * nb + c], pb.dBeta[q * nb + c], &pcr, &pcz);
           ld v = inv_dt * pa * pc;
           if (with_operator) {
             v += par * (dk->Drr[ip] * pcr + dk->Drz[ip] * pcz) + paz * (dk->Drz[ip] * pcr + dk->Dzz[ip] * pcz);
@@ -581,13 +706,12 @@ void apply_species(const Problem& pb, const Grid& g, const DK& dk, const double*
   std::vector<ld> acc(g.n_dof, 0);
   const int nb = pb.nb, nq = pb.nq;
   for (size_t e = 0; e < g.cells.size(); e++) {
-    ld hr, hz;
-    cell_sizes(g, (int)e, &hr, &hz);
     for (int a = 0; a < nb; a++) {
       ld s = 0;
       for (int q = 0; q < nq; q++) {
         int ip = (int)e * nq + q;
-        ld par = (2 / hr) * pb.dBxi[q * nb + a], paz = (2 / hz) * pb.dBeta[q * nb + a];
+        ld par, paz;
+        grad_phys(g, (int)e, ip, pb.dBxi[q * nb + a], pb.dBeta[q * nb + a], &par, &paz);
         ld flux_r = dk.Drr[ip] * fr[ip] + dk.Drz[ip] * fz[ip] - dk.Kr[ip] * f[ip];
         ld flux_z = dk.Drz[ip] * fr[ip] + dk.Dzz[ip] * fz[ip] - dk.Kz[ip] * f[ip];
         s -= g.ip_w[ip] * (par * flux_r + paz * flux_z);
@@ -654,8 +778,7 @@ void orc_tensor_quadrature(double r, double z, double rb, double zb, int nphi, d
   for (int k = 0; k < 8; k++) out[k] = (double)o[k];
 }
 
-void* orc_create(const GridDesc* grids, int n_grids, const SpeciesDesc* species, int n_species, int degree,
-                 const double* nu, int threads) {
+static Problem* new_problem(int degree, int threads) {
   Problem* pb = new Problem();
   pb->k = degree;
   pb->nq1 = degree + 1;
@@ -682,13 +805,10 @@ void* orc_create(const GridDesc* grids, int n_grids, const SpeciesDesc* species,
           pb->dBeta[q * pb->nb + a] = v1[a1] * d2[a2];
         }
     }
-  pb->grids.resize(n_grids);
-  for (int g = 0; g < n_grids; g++) {
-    pb->grids[g].desc = grids[g];
-    pb->grids[g].k = degree;
-    build_mesh(pb->grids[g]);
-    build_ips(*pb, pb->grids[g]);
-  }
+  return pb;
+}
+
+static void finish_problem(Problem* pb, const SpeciesDesc* species, int n_species, const double* nu) {
   pb->species.assign(species, species + n_species);
   pb->nu.resize((size_t)n_species * n_species);
   for (int a = 0; a < n_species; a++)
@@ -705,6 +825,39 @@ void* orc_create(const GridDesc* grids, int n_grids, const SpeciesDesc* species,
   }
   pb->f_stride = fo;
   pb->v_stride = vo;
+}
+
+void* orc_create(const GridDesc* grids, int n_grids, const SpeciesDesc* species, int n_species, int degree,
+                 const double* nu, int threads) {
+  Problem* pb = new_problem(degree, threads);
+  pb->grids.resize(n_grids);
+  for (int g = 0; g < n_grids; g++) {
+    pb->grids[g].desc = grids[g];
+    pb->grids[g].k = degree;
+    build_mesh(pb->grids[g]);
+    build_ips(*pb, pb->grids[g]);
+  }
+  finish_problem(pb, species, n_species, nu);
+  return pb;
+}
+
+// Unstructured quadrilateral grids: grid g has n_vertices[g] vertices (vertices[g]: (r, z) pairs) and
+// n_cells[g] cells (cells[g]: 4 counter-clockwise vertex ids each).  Returns NULL for an inverted cell.
+void* orc_create_meshes(int n_grids, const int* n_vertices, const double* const* vertices, const int* n_cells,
+                        const int* const* cells, const SpeciesDesc* species, int n_species, int degree, const double* nu,
+                        int threads) {
+  Problem* pb = new_problem(degree, threads);
+  pb->grids.resize(n_grids);
+  for (int g = 0; g < n_grids; g++) {
+    memset(&pb->grids[g].desc, 0, sizeof(GridDesc));
+    pb->grids[g].desc.kind = 2;
+    pb->grids[g].k = degree;
+    if (!build_unstructured(*pb, pb->grids[g], n_vertices[g], vertices[g], n_cells[g], cells[g])) {
+      delete pb;
+      return nullptr;
+    }
+  }
+  finish_problem(pb, species, n_species, nu);
   return pb;
 }
 
@@ -724,6 +877,13 @@ void orc_sizes(void* h, int* n_dof, int* nnz, int* n_ip, int* n_cells, long long
 
 void orc_dof_coords(void* h, int g, double* rz) {
   const Grid& G = ((Problem*)h)->grids[g];
+  if (G.unstructured) {
+    for (int i = 0; i < G.n_dof; i++) {
+      rz[2 * i] = (double)G.node_r[i];
+      rz[2 * i + 1] = (double)G.node_z[i];
+    }
+    return;
+  }
   for (int i = 0; i < G.n_dof; i++) {
     rz[2 * i] = (double)(G.dof_ix[i] * G.ur);
     rz[2 * i + 1] = (double)((ld)G.desc.z_min + G.dof_iz[i] * G.uz);

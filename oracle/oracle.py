@@ -105,6 +105,10 @@ class Oracle:
             nu_p = _p(self._nu)
         self.h = C.c_void_p(L.orc_create(g_arr, C.c_int(self.G), s_arr, C.c_int(self.S), C.c_int(degree), nu_p,
                                          C.c_int(self.threads)))
+        self._sizes(species)
+
+    def _sizes(self, species):
+        L = lib()
         n_dof = np.zeros(self.G, np.int32)
         nnz = np.zeros(self.G, np.int32)
         n_ip = np.zeros(self.G, np.int32)
@@ -118,6 +122,35 @@ class Oracle:
         self.f_off = np.concatenate([[0], np.cumsum([n_dof[g] for g in self.sgrid])]).astype(np.int64)
         self.v_off = np.concatenate([[0], np.cumsum([nnz[g] for g in self.sgrid])]).astype(np.int64)
         self.ip_off = np.concatenate([[0], np.cumsum([n_ip[g] for g in self.sgrid])]).astype(np.int64)
+
+    @classmethod
+    def from_meshes(cls, meshes, species, degree, nu=None, threads=None):
+        """Unstructured quadrilateral grids: meshes = list of (vertices [nv, 2] (r, z), cells [nc, 4] counter-clockwise)."""
+        self = cls.__new__(cls)
+        L = lib()
+        L.orc_create_meshes.restype = C.c_void_p
+        self.G, self.S, self.degree = len(meshes), len(species), degree
+        self.species = [dict(s) for s in species]
+        self.grids = [dict(kind=2) for _ in meshes]
+        self._v = [np.ascontiguousarray(m[0], dtype=np.float64) for m in meshes]
+        self._c = [np.ascontiguousarray(m[1], dtype=np.int32) for m in meshes]
+        nv = np.array([len(v) for v in self._v], dtype=np.int32)
+        nc = np.array([len(c) for c in self._c], dtype=np.int32)
+        vp = (C.c_void_p * self.G)(*[v.ctypes.data for v in self._v])
+        cp = (C.c_void_p * self.G)(*[c.ctypes.data for c in self._c])
+        s_arr = (SpeciesDesc * self.S)(*[SpeciesDesc(float(s["mass"]), float(s["charge"]), int(s["grid"])) for s in species])
+        self.threads = int(threads) if threads else (os.cpu_count() or 1)
+        nu_p = None
+        if nu is not None:
+            self._nu = np.ascontiguousarray(nu, dtype=np.float64)
+            nu_p = _p(self._nu)
+        h = L.orc_create_meshes(C.c_int(self.G), _p(nv), vp, _p(nc), cp, s_arr, C.c_int(self.S), C.c_int(degree), nu_p,
+                                C.c_int(self.threads))
+        if not h:
+            raise RuntimeError("orc_create_meshes failed (inverted cell)")
+        self.h = C.c_void_p(h)
+        self._sizes(species)
+        return self
 
     def __del__(self):
         try:

@@ -209,3 +209,51 @@ def make_batch_f3v(cfg, dof_coords, batch=None, entries=None):
         out.append(np.concatenate([sample_state3v(sp["mass"], n[row, s], T[row, s], u[row, s], al[row, s], dof_coords[sp["grid"]])
                                    for s, sp in enumerate(cfg["species"])]))
     return np.ascontiguousarray(np.stack(out))
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# unstructured quadrilateral meshes (sec. 5.2, Fig. 4: "semi-circular grids ... with
+# tensor elements").  The paper's mesh files are not available; this generator stands in for them.
+# ------------------------------------------------------------------------------------------------------------------
+def semicircle_mesh(radius, n=2, m=2, core=0.5):
+    """Straight-sided quadrilateral mesh of the half disc r >= 0, r^2 + z^2 <= radius^2 (polygonal boundary): a core
+    rectangle [0, a] x [-a, a], a = core * radius / sqrt(2), of n x 2n cells, and a ring of 4n x m cells between its
+    three outer sides and the circle (an O-grid).  n = 2, m = 2 gives 24 cells -- with Q3 the 384 integration points of the
+    paper's Table 13.  Returns (vertices [nv, 2] as (r, z), cells [nc, 4] counter-clockwise vertex ids).
+    Input description only: no arithmetic of the method lives here."""
+    a = core * radius / math.sqrt(2.0)
+    verts, index = [], {}
+
+    def vid(key, r, z):
+        if key not in index:
+            index[key] = len(verts)
+            verts.append((r, z))
+        return index[key]
+
+    h = a / n
+    for j in range(2 * n + 1):
+        for i in range(n + 1):
+            vid(("c", i, j), i * h, -a + j * h)
+    cells = []
+    for j in range(2 * n):
+        for i in range(n):
+            cells.append((index[("c", i, j)], index[("c", i + 1, j)], index[("c", i + 1, j + 1)], index[("c", i, j + 1)]))
+    # perimeter of the core from (0, -a) along the bottom, up the right side and back along the top to (0, a)
+    per = [("c", i, 0) for i in range(n + 1)] + [("c", n, j) for j in range(1, 2 * n + 1)] + [("c", i, 2 * n) for i in range(n - 1, -1, -1)]
+    K = len(per) - 1   # 4 n edges
+    for k, key in enumerate(per):
+        p = verts[index[key]]
+        th = -0.5 * math.pi + math.pi * k / K
+        c = (radius * math.cos(th) if 0 < k < K else 0.0, radius * math.sin(th))
+        for l in range(1, m + 1):
+            t = l / m
+            vid(("r", k, l), p[0] + t * (c[0] - p[0]), p[1] + t * (c[1] - p[1]))
+
+    def ring(k, l):
+        return index[per[k]] if l == 0 else index[("r", k, l)]
+
+    for k in range(K):
+        for l in range(m):
+            # (k, l) -> (k, l+1) -> (k+1, l+1) -> (k+1, l) runs counter-clockwise in the (r, z) plane
+            cells.append((ring(k, l), ring(k, l + 1), ring(k + 1, l + 1), ring(k + 1, l)))
+    return np.array(verts, dtype=np.float64), np.array(cells, dtype=np.int32)
