@@ -83,6 +83,26 @@ typedef struct {
 int landau_create(const landau_grid_desc* grids, int n_grids, const landau_species_desc* species, int n_species,
                   const landau_quadrature_desc* quadrature, const double* nu, int cuda_device, landau_ctx** out);
 
+/* One unstructured velocity-space grid of straight-sided quadrilaterals on the (r, z) half plane (PAPER.md:225-229
+ * sec. 5.2, "unstructured grids with ... tensor elements").  The mesh must be conforming (no hanging
+ * nodes); every cell lists its four vertices counter-clockwise (positive Jacobian).  The cell geometry is the bilinear
+ * map of the reference square, so the gradient transformation J^-T and det J differ from point to point; Qk nodes are
+ * the images of the equispaced reference nodes. */
+typedef struct {
+  int n_vertices;
+  const double* vertices_rz; /* host, n_vertices x 2: (r, z) in units of v0 */
+  int n_cells;
+  const int* cells;          /* host, n_cells x 4 vertex indices */
+} landau_mesh_desc;
+
+/* landau_create for unstructured quadrilateral grids: meshes[n_grids] (host, read during the call) take the place of the
+ * grid descriptors, everything else as above.  Dofs are ordered by (z, r) of their coordinates (on a grid of 2^-30 of the
+ * mesh extent), exposed through landau_dof_coords; all other entry points work unchanged on such a context.
+ * landau_last_coefficients (landau_debug.h) returns the coefficients pulled back to the reference cell on these grids.
+ * Extra errors: LANDAU_INVALID_ARG for a cell with a missing vertex or a non-positive Jacobian. */
+int landau_create_meshes(const landau_mesh_desc* meshes, int n_grids, const landau_species_desc* species, int n_species,
+                         const landau_quadrature_desc* quadrature, const double* nu, int cuda_device, landau_ctx** out);
+
 /* Frees every host and device resource of the context (synchronises the device first).  NULL is a no-op. */
 void landau_destroy(landau_ctx* ctx);
 

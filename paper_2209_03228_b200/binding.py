@@ -18,7 +18,7 @@ STATUS = {0: "LANDAU_OK", -1: "LANDAU_INVALID_ARG", -2: "LANDAU_UNSUPPORTED", -3
 
 # every symbol include/landau.h (the product ABI) and include/landau_debug.h (diagnostics, probes, tuning knobs)
 # declare; tests check that the headers and these lists agree and that the library exports all of them
-SYMBOLS = ["landau_create", "landau_destroy", "landau_sizes", "landau_dof_coords", "landau_ip_table",
+SYMBOLS = ["landau_create", "landau_create_meshes", "landau_destroy", "landau_sizes", "landau_dof_coords", "landau_ip_table",
            "landau_csr_pattern", "landau_csr_pattern_host", "landau_jacobian", "landau_apply", "landau_spmv",
            "landau_solve", "landau_jacobian_apply", "landau_step", "landau_jacobian_host", "landau_apply_host",
            "landau_reserve", "landau_last_error"]
@@ -109,6 +109,29 @@ def landau_create(grids, species, quadrature, nu=None, cuda_device=0):
     ctx = C.c_void_p()
     rc = lib.landau_create(g_arr, C.c_int(len(grids)), s_arr, C.c_int(len(species)), C.byref(qd),
                            None if nu_arr is None else _np(nu_arr), C.c_int(cuda_device), C.byref(ctx))
+    _check(rc, None)
+    return ctx
+
+
+class MeshDesc(C.Structure):
+    _fields_ = [("n_vertices", C.c_int), ("vertices_rz", C.c_void_p), ("n_cells", C.c_int), ("cells", C.c_void_p)]
+
+
+def landau_create_meshes(meshes, species, quadrature, nu=None, cuda_device=0):
+    """meshes: list of (vertices [nv, 2] (r, z), cells [nc, 4] counter-clockwise vertex ids); otherwise as landau_create."""
+    lib = load()
+    if isinstance(quadrature, int):
+        quadrature = dict(degree=quadrature, n_gauss_1d=quadrature + 1)
+    vs = [np.ascontiguousarray(m[0], dtype=np.float64) for m in meshes]
+    cs = [np.ascontiguousarray(m[1], dtype=np.int32) for m in meshes]
+    m_arr = (MeshDesc * len(meshes))(*[MeshDesc(len(v), v.ctypes.data, len(c), c.ctypes.data) for v, c in zip(vs, cs)])
+    s_arr = (SpeciesDesc * len(species))(*[SpeciesDesc(float(s["mass"]), float(s["charge"]), int(s["grid"]))
+                                           for s in species])
+    qd = QuadratureDesc(int(quadrature["degree"]), int(quadrature["n_gauss_1d"]))
+    nu_arr = None if nu is None else np.ascontiguousarray(nu, dtype=np.float64)
+    ctx = C.c_void_p()
+    rc = lib.landau_create_meshes(m_arr, C.c_int(len(meshes)), s_arr, C.c_int(len(species)), C.byref(qd),
+                                  None if nu_arr is None else _np(nu_arr), C.c_int(cuda_device), C.byref(ctx))
     _check(rc, None)
     return ctx
 
@@ -278,6 +301,19 @@ class Landau:
         self.species = [dict(s) for s in species]
         self.sgrid = [int(s["grid"]) for s in species]
         self.ctx = landau_create(grids, species, degree, nu, device)
+        self._sizes()
+
+    @classmethod
+    def from_meshes(cls, meshes, species, degree, nu=None, device=0):
+        """Unstructured quadrilateral grids (landau_create_meshes)."""
+        self = cls.__new__(cls)
+        self.G, self.S, self.degree = len(meshes), len(species), degree
+        self.sgrid = [int(s["grid"]) for s in species]
+        self.ctx = landau_create_meshes(meshes, species, degree, nu, device)
+        self._sizes()
+        return self
+
+    def _sizes(self):
         sz = landau_sizes(self.ctx, self.G)
         self.n_dof, self.nnz, self.n_ip, self.n_cells = sz["n_dof"], sz["nnz"], sz["n_ip"], sz["n_cells"]
         self.f_stride, self.csr_stride = sz["f_stride"], sz["csr_stride"]

@@ -4,7 +4,9 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstring>
 #include <map>
+#include <string>
 #include <tuple>
 #include <unordered_map>
 
@@ -295,6 +297,15 @@ int build_grid(const landau_grid_desc& d, const HostTables& t, HostGrid* g, std:
         g->ip_w[ip] = t.gauss_w[q1] * t.gauss_w[q2] * 0.25 * hr * hz * r;
       }
   }
+  return finish_grid(t, g, msg);
+}
+
+// Everything that follows from the rows of P_e (en_ptr / en_dof / en_w): CSR pattern, assembly and apply gather tables,
+// the K3 ring schedule.  Shared by the rectangular / quadtree grids and the unstructured meshes.
+int finish_grid(const HostTables& t, HostGrid* g, std::string* msg) {
+  (void)msg;
+  const int k = t.k, n1 = k + 1, nb = t.nb;
+  (void)k;
   // ---- CSR pattern ----------------------------------------------------------------------------------------------
   std::vector<std::vector<int>> rows(g->n_dof);
   std::vector<int> touched;
@@ -462,6 +473,140 @@ int build_grid(const landau_grid_desc& d, const HostTables& t, HostGrid* g, std:
       }
   }
   return LANDAU_OK;
+}
+
+// ---- unstructured conforming meshes of straight-sided quadrilaterals (sec. 5.2) -------------------------
+// Nodes are identified by topology, not geometry: a corner node by its vertex id, an edge node by (lower vertex id, higher
+// vertex id, position counted from the lower one), an interior node by (cell, a1, a2).  Dofs are then ordered by their
+// coordinates on a grid of 2^-30 of the mesh extent, z-major.
+int build_mesh_grid(const landau_mesh_desc& m, const HostTables& t, HostGrid* g, std::string* msg) {
+  if (m.n_vertices < 4 || m.n_cells < 1 || !m.vertices_rz || !m.cells) {
+    *msg = "bad mesh: at least 4 vertices and 1 cell";
+    return LANDAU_INVALID_ARG;
+  }
+  const int k = t.k, n1 = k + 1, nb = t.nb, nq = t.nq, nc = m.n_cells;
+  memset(&g->desc, 0, sizeof(g->desc));
+  g->desc.kind = 2;
+  g->k = k;
+  g->nb = nb;
+  g->nq = nq;
+  g->n_cells = nc;
+  for (int e = 0; e < 4 * nc; ++e)
+    if (m.cells[e] < 0 || m.cells[e] >= m.n_vertices) {
+      *msg = "mesh cell refers to a missing vertex";
+      return LANDAU_INVALID_ARG;
+    }
+  double scale = 0.0;
+  for (int v = 0; v < 2 * m.n_vertices; ++v) scale = std::max(scale, std::fabs(m.vertices_rz[v]));
+  const double quantum = scale / 1073741824.0;
+  auto vert = [&](int e, int c, int d) { return m.vertices_rz[2 * m.cells[4 * e + c] + d]; };
+  // bilinear map of cell e and its Jacobian [dr/dxi, dr/deta, dz/dxi, dz/deta]
+  auto map_point = [&](int e, double xi, double eta, double* x, double* J) {
+    const double N[4] = {0.25 * (1 - xi) * (1 - eta), 0.25 * (1 + xi) * (1 - eta), 0.25 * (1 + xi) * (1 + eta), 0.25 * (1 - xi) * (1 + eta)};
+    const double Nx[4] = {-0.25 * (1 - eta), 0.25 * (1 - eta), 0.25 * (1 + eta), -0.25 * (1 + eta)};
+    const double Ne[4] = {-0.25 * (1 - xi), -0.25 * (1 + xi), 0.25 * (1 + xi), 0.25 * (1 - xi)};
+    x[0] = x[1] = 0.0;
+    if (J) J[0] = J[1] = J[2] = J[3] = 0.0;
+    for (int c = 0; c < 4; ++c) {
+      x[0] += N[c] * vert(e, c, 0);
+      x[1] += N[c] * vert(e, c, 1);
+      if (J) {
+        J[0] += Nx[c] * vert(e, c, 0);
+        J[1] += Ne[c] * vert(e, c, 0);
+        J[2] += Nx[c] * vert(e, c, 1);
+        J[3] += Ne[c] * vert(e, c, 1);
+      }
+    }
+  };
+  typedef std::tuple<int, int, int, int> NodeKey;  // (kind, i, j, l)
+  std::map<NodeKey, int> node_of;
+  std::vector<double> nr, nz;
+  std::vector<int> cell_node((size_t)nc * nb);
+  auto edge_key = [&](int va, int vb, int tpos) { return va < vb ? NodeKey(1, va, vb, tpos) : NodeKey(1, vb, va, k - tpos); };
+  for (int e = 0; e < nc; ++e) {
+    const int* cv = &m.cells[4 * e];
+    for (int a2 = 0; a2 <= k; ++a2)
+      for (int a1 = 0; a1 <= k; ++a1) {
+        NodeKey key;
+        const bool x0 = a1 == 0, x1 = a1 == k, y0 = a2 == 0, y1 = a2 == k;
+        if ((x0 || x1) && (y0 || y1))
+          key = NodeKey(0, cv[y0 ? (x0 ? 0 : 1) : (x0 ? 3 : 2)], 0, 0);
+        else if (y0)
+          key = edge_key(cv[0], cv[1], a1);
+        else if (x1)
+          key = edge_key(cv[1], cv[2], a2);
+        else if (y1)
+          key = edge_key(cv[3], cv[2], a1);
+        else if (x0)
+          key = edge_key(cv[0], cv[3], a2);
+        else
+          key = NodeKey(2, e, a1, a2);
+        auto it = node_of.find(key);
+        int id;
+        if (it == node_of.end()) {
+          id = (int)nr.size();
+          node_of[key] = id;
+          double x[2];
+          map_point(e, -1.0 + 2.0 * a1 / k, -1.0 + 2.0 * a2 / k, x, nullptr);
+          nr.push_back(x[0]);
+          nz.push_back(x[1]);
+        } else {
+          id = it->second;
+        }
+        cell_node[(size_t)e * nb + a1 + n1 * a2] = id;
+      }
+  }
+  const int nn = (int)nr.size();
+  std::vector<std::pair<std::pair<long long, long long>, int>> order(nn);
+  for (int i = 0; i < nn; ++i) order[i] = std::make_pair(std::make_pair(std::llround(nz[i] / quantum), std::llround(nr[i] / quantum)), i);
+  std::sort(order.begin(), order.end());
+  std::vector<int> dof_of(nn);
+  g->n_dof = nn;
+  g->dof_r.resize(nn);
+  g->dof_z.resize(nn);
+  for (int I = 0; I < nn; ++I) {
+    dof_of[order[I].second] = I;
+    g->dof_r[I] = nr[order[I].second];
+    g->dof_z[I] = nz[order[I].second];
+  }
+  g->en_ptr.assign(1, 0);
+  g->en_dof.clear();
+  g->en_w.clear();
+  for (int ea = 0; ea < nc * nb; ++ea) {
+    g->en_dof.push_back(dof_of[cell_node[ea]]);
+    g->en_w.push_back(1.0);
+    g->en_ptr.push_back((int)g->en_dof.size());
+  }
+  // the kernels work in reference coordinates on these grids: unit scale factors, J^-T per point (ip_gm)
+  g->cell_r0.assign(nc, 0.0);
+  g->cell_z0.assign(nc, 0.0);
+  g->cell_hr.assign(nc, 2.0);
+  g->cell_hz.assign(nc, 2.0);
+  g->n_ip = nc * nq;
+  g->ip_r.resize(g->n_ip);
+  g->ip_z.resize(g->n_ip);
+  g->ip_w.resize(g->n_ip);
+  g->ip_gm.resize(4 * (size_t)g->n_ip);
+  for (int e = 0; e < nc; ++e)
+    for (int q2 = 0; q2 < n1; ++q2)
+      for (int q1 = 0; q1 < n1; ++q1) {
+        const int ip = e * nq + q1 + n1 * q2;
+        double x[2], J[4];
+        map_point(e, t.gauss_x[q1], t.gauss_x[q2], x, J);
+        const double det = J[0] * J[3] - J[1] * J[2];
+        if (!(det > 0.0)) {
+          *msg = "mesh cell " + std::to_string(e) + " is inverted or clockwise";
+          return LANDAU_INVALID_ARG;
+        }
+        g->ip_r[ip] = x[0];
+        g->ip_z[ip] = x[1];
+        g->ip_w[ip] = t.gauss_w[q1] * t.gauss_w[q2] * det * x[0];
+        g->ip_gm[4 * (size_t)ip] = J[3] / det;       // (d/dr, d/dz) = gm (d/dxi, d/deta)
+        g->ip_gm[4 * (size_t)ip + 1] = -J[2] / det;
+        g->ip_gm[4 * (size_t)ip + 2] = -J[1] / det;
+        g->ip_gm[4 * (size_t)ip + 3] = J[0] / det;
+      }
+  return finish_grid(t, g, msg);
 }
 
 }  // namespace landau

@@ -32,6 +32,8 @@ struct HostGrid {
   std::vector<double> cell_r0, cell_z0, cell_hr, cell_hz;
   // integration points, cell-major (ip = cell*nq + q, q = q1 + (k+1) q2)
   std::vector<double> ip_r, ip_z, ip_w;
+  // unstructured meshes only: J^-T at every integration point, [ip][4], (d/dr, d/dz) = gm (d/dxi, d/deta); empty otherwise
+  std::vector<double> ip_gm;
   std::vector<double> dof_r, dof_z;
   // element-node -> dof expansion (rows of P_e): entries en_ptr[cell*nb+a] .. en_ptr[cell*nb+a+1]
   std::vector<int> en_ptr, en_dof;
@@ -75,5 +77,9 @@ bool build_tables(int k, HostTables* t, std::string* msg);
 
 // Builds one grid.  status: 0 ok, LANDAU_INVALID_ARG / LANDAU_UNSUPPORTED with msg.
 int build_grid(const landau_grid_desc& d, const HostTables& t, HostGrid* g, std::string* msg);
+// Builds one unstructured quadrilateral mesh grid (include/landau.h, landau_mesh_desc).
+int build_mesh_grid(const landau_mesh_desc& m, const HostTables& t, HostGrid* g, std::string* msg);
+// CSR pattern, gather tables and K3 schedule from the element expansions (called by both builders).
+int finish_grid(const HostTables& t, HostGrid* g, std::string* msg);
 
 }  // namespace landau

@@ -255,6 +255,8 @@ int build_device_side(landau_ctx* ctx) {
     rc = rc ? rc : upload(ctx, sr, &d.cell_sr);
     rc = rc ? rc : upload(ctx, sz, &d.cell_sz);
     rc = rc ? rc : upload(ctx, h.ip_w, &d.ip_w);
+    d.ip_gm = nullptr;
+    if (!h.ip_gm.empty()) rc = rc ? rc : upload(ctx, h.ip_gm, &d.ip_gm);
     rc = rc ? rc : upload(ctx, h.en_ptr, &d.en_ptr);
     rc = rc ? rc : upload(ctx, h.en_dof, &d.en_dof);
     rc = rc ? rc : upload(ctx, h.en_w, &d.en_w);
@@ -676,6 +678,7 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
       ct.ip_off = ctx->ip_off[g];
       ct.n_ip = ctx->hg[g].n_ip;
       ct.dk_off = ctx->dk_off[s];
+      ct.ip_gm = ctx->dg[g].ip_gm;
       max_ip = std::max(max_ip, ct.n_ip);
     }
     ctx->comb_max_ip = max_ip;
@@ -774,9 +777,13 @@ int apply_chunk(landau_ctx* ctx, const double* batch_f_dev, int b0, int nbc, dou
 
 extern "C" {
 
-int landau_create(const landau_grid_desc* grids, int n_grids, const landau_species_desc* species, int n_species,
-                  const landau_quadrature_desc* quadrature, const double* nu, int cuda_device, landau_ctx** out) {
-  if (!grids || !species || !quadrature || !out || n_grids < 1 || n_species < 1)
+}  // extern "C"
+
+namespace {
+// landau_create / landau_create_meshes: exactly one of grids / meshes is given
+int create_any(const landau_grid_desc* grids, const landau_mesh_desc* meshes, int n_grids, const landau_species_desc* species,
+               int n_species, const landau_quadrature_desc* quadrature, const double* nu, int cuda_device, landau_ctx** out) {
+  if ((!grids && !meshes) || !species || !quadrature || !out || n_grids < 1 || n_species < 1)
     return fail(nullptr, LANDAU_INVALID_ARG, "null argument or empty grid/species list");
   if (quadrature->n_gauss_1d != quadrature->degree + 1)
     return fail(nullptr, LANDAU_UNSUPPORTED, "n_gauss_1d must be degree + 1");
@@ -796,7 +803,7 @@ int landau_create(const landau_grid_desc* grids, int n_grids, const landau_speci
     ctx->S = n_species;
     ctx->hg.resize(n_grids);
     for (int g = 0; g < n_grids; ++g) {
-      int rc = build_grid(grids[g], ctx->ht, &ctx->hg[g], &msg);
+      int rc = grids ? build_grid(grids[g], ctx->ht, &ctx->hg[g], &msg) : build_mesh_grid(meshes[g], ctx->ht, &ctx->hg[g], &msg);
       if (rc) return bail(rc, msg);
     }
     ctx->species.assign(species, species + n_species);
@@ -846,6 +853,21 @@ int landau_create(const landau_grid_desc* grids, int n_grids, const landau_speci
   }
   *out = ctx;
   return LANDAU_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int landau_create(const landau_grid_desc* grids, int n_grids, const landau_species_desc* species, int n_species,
+                  const landau_quadrature_desc* quadrature, const double* nu, int cuda_device, landau_ctx** out) {
+  if (!grids) return fail(nullptr, LANDAU_INVALID_ARG, "null argument or empty grid/species list");
+  return create_any(grids, nullptr, n_grids, species, n_species, quadrature, nu, cuda_device, out);
+}
+
+int landau_create_meshes(const landau_mesh_desc* meshes, int n_grids, const landau_species_desc* species, int n_species,
+                         const landau_quadrature_desc* quadrature, const double* nu, int cuda_device, landau_ctx** out) {
+  if (!meshes) return fail(nullptr, LANDAU_INVALID_ARG, "null argument or empty grid/species list");
+  return create_any(nullptr, meshes, n_grids, species, n_species, quadrature, nu, cuda_device, out);
 }
 
 void landau_destroy(landau_ctx* ctx) {

@@ -205,6 +205,7 @@ struct DevGrid {
   const double* cell_sr;  // 2/hr per cell
   const double* cell_sz;  // 2/hz per cell
   const double* ip_w;     // [n_ip]
+  const double* ip_gm;    // unstructured meshes: J^-T per point, [n_ip][4]; nullptr on rectangular grids (cell_sr / cell_sz)
   const int* en_ptr;      // [n_cells*nb + 1]
   const int* en_dof;
   const double* en_w;
@@ -299,7 +300,13 @@ k1_fields(DevGrid g, const DevTables* __restrict__ tab, MixTable mix, const doub
         vy = fma(sT[2][a][lo], fk, vy);
       }
       const long long col = col0 + (long long)b * mix.ncb + c;
-      const double o0 = w * v, o1 = w * (vx * sr), o2 = w * (vy * sz);
+      double gr = vx * sr, gz = vy * sz;
+      if (g.ip_gm) {  // non-affine cell: (d/dr, d/dz) = J^-T (d/dxi, d/deta) at this point
+        const double* m = g.ip_gm + 4 * (long long)j;
+        gr = fma(m[0], vx, m[1] * vy);
+        gz = fma(m[2], vx, m[3] * vy);
+      }
+      const double o0 = w * v, o1 = w * gr, o2 = w * gz;
       if (tiled_tc) {
         const int njt = (int)(nj_pad >> 4), jg = j_off_in_group + j;
         F[k2g_f_offset(tiled_tc, njt, (int)col, 0, jg)] = o0;
@@ -528,6 +535,7 @@ struct CombineTable {   // per species alpha
   double coefD[16], coefK[16];
   int ip_off, n_ip;     // the species' grid: offset in the concatenated IP arrays, number of IPs
   long long dk_off;     // offset of the species' block inside one entry of DK
+  const double* ip_gm;  // the grid's J^-T per point (unstructured meshes) or nullptr
 };
 
 // one launch for all species: blockIdx.z = species
@@ -554,6 +562,18 @@ k2b_combine(const CombineTable* __restrict__ cts, const double* __restrict__ G, 
     out[2] = fma(ct.coefD[t], s[2], out[2]);
     out[3] = fma(ct.coefK[t], s[3], out[3]);
     out[4] = fma(ct.coefK[t], s[4], out[4]);
+  }
+  if (ct.ip_gm) {
+    // unstructured mesh: K3 and K3' work in reference coordinates there, so D and K are pulled back,
+    // D~ = M^T D M, K~ = M^T K with M = J^-T of this point (grad phi = M grad_ref phi)
+    const double* m = ct.ip_gm + 4 * (long long)i;
+    const double m00 = m[0], m01 = m[1], m10 = m[2], m11 = m[3];
+    const double drr = out[0], drz = out[1], dzz = out[2], kr = out[3], kz = out[4];
+    out[0] = m00 * (m00 * drr + m10 * drz) + m10 * (m00 * drz + m10 * dzz);
+    out[1] = m01 * (m00 * drr + m10 * drz) + m11 * (m00 * drz + m10 * dzz);
+    out[2] = m01 * (m01 * drr + m11 * drz) + m11 * (m01 * drz + m11 * dzz);
+    out[3] = m00 * kr + m10 * kz;
+    out[4] = m01 * kr + m11 * kz;
   }
   double* dst = DK + (long long)b * dk_stride + dk_off + i;
 #pragma unroll

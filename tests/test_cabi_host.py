@@ -133,3 +133,33 @@ def test_ring_assembly_schedule_exists_for_every_baseline_config(lib, c):
         assert info["n_steps"] == (int(sz["n_cells"][g]) + 7) // 8
         assert 0.7 * sz["nnz"][g] < info["n_simple_slots"] <= sz["nnz"][g]
     Bn.landau_destroy(ctx)
+
+
+def test_unstructured_host_setup_matches_oracle(lib, orc):
+    """landau_create_meshes (topological node identification, own bilinear geometry) against the oracle's geometric
+    construction: same dofs, same pattern, same integration points and weights."""
+    for k, (n, m) in ((3, (2, 2)), (2, (3, 2))):
+        mesh = W.semicircle_mesh(5.0, n, m)
+        species = [dict(mass=1.0, charge=-1.0, grid=0)]
+        L = Bn.Landau.from_meshes([mesh], species, k, device=-1)
+        o = orc.Oracle.from_meshes([mesh], species, k)
+        assert L.n_dof[0] == o.n_dof[0] and L.nnz[0] == o.nnz[0] and L.n_ip[0] == o.n_ip[0] and L.n_cells[0] == o.n_cells[0]
+        assert np.abs(L.dof_coords(0) - o.dof_coords(0)).max() < 1e-13      # same order on this mesh
+        rp, ci = L.pattern(0)
+        rp2, ci2 = o.pattern(0)
+        assert np.array_equal(rp, rp2) and np.array_equal(ci, ci2)
+        a, b = np.stack(L.ip_table(0), 1), np.stack(o.ip_table(0), 1)
+        pa = np.array([int(np.argmin(((a[:, :2] - x) ** 2).sum(1))) for x in b[:, :2]])   # IP order is implementation-private
+        assert len(set(pa)) == len(pa) and np.abs(a[pa] - b).max() < 1e-13
+        L.close()
+    # Table 13 (PAPER.md:311): 24 Q3 cells <-> 384 integration points, from the product side
+    L = Bn.Landau.from_meshes([W.semicircle_mesh(5.0, 2, 2)], [dict(mass=1.0, charge=-1.0, grid=0)], 3, device=-1)
+    assert L.n_cells[0] == 24 and L.n_ip[0] == 384
+    L.close()
+    v, c = W.semicircle_mesh(5.0, 2, 2)
+    with pytest.raises(Bn.LandauError, match="inverted"):
+        Bn.Landau.from_meshes([(v, c[:, ::-1].copy())], [dict(mass=1.0, charge=-1.0, grid=0)], 3, device=-1)
+    bad = c.copy()
+    bad[0, 0] = 99
+    with pytest.raises(Bn.LandauError, match="missing vertex"):
+        Bn.Landau.from_meshes([(v, bad)], [dict(mass=1.0, charge=-1.0, grid=0)], 3, device=-1)
