@@ -414,6 +414,8 @@ struct Problem {
   std::vector<SpeciesDesc> species;
   std::vector<ld> nu;  // S x S
   std::vector<ld> gx, gw;
+  bool simplex = false;            // triangles: reference quadrature points / weights below, nodes (i/k, j/k)
+  std::vector<ld> sx, se, sw;
   // basis tabulation at the Gauss points of the reference cell:
   // B[q][a], dBxi[q][a], dBeta[q][a]; q = q1 + nq1*q2, a = a1 + (k+1)*a2
   std::vector<ld> B, dBxi, dBeta;
@@ -465,12 +467,101 @@ inline void grad_phys(const Grid& g, int e, int ip, ld dxi, ld deta, ld* pr, ld*
   }
 }
 
+// O3'' + O4'' the same for triangles: affine map x = v0 + (v1 - v0) xi + (v2 - v0) eta, constant J per cell.
+bool build_unstructured_simplex(const Problem& pb, Grid& g, int nv, const double* verts, int nc, const int* cells) {
+  const int k = pb.k, nb = pb.nb;
+  g.unstructured = true;
+  g.L = 0;
+  g.cells.assign(nc, Cell{0, 0, 0});
+  ld scale = 0;
+  for (int v = 0; v < 2 * nv; v++) scale = std::max(scale, fabsl((ld)verts[v]));
+  const ld quantum = scale / (ld)(1L << 30);
+  auto vr = [&](int e, int c) { return (ld)verts[2 * cells[3 * e + c]]; };
+  auto vz = [&](int e, int c) { return (ld)verts[2 * cells[3 * e + c] + 1]; };
+  std::map<Key, int> node_id;
+  std::vector<Key> keys;
+  std::vector<ld> nr, nz;
+  std::vector<int> cell_node((size_t)nc * nb);
+  for (int e = 0; e < nc; e++) {
+    int a = 0;
+    for (int j = 0; j <= k; j++)
+      for (int i = 0; i <= k - j; i++, a++) {
+        const ld xi = (ld)i / k, eta = (ld)j / k;
+        const ld r = vr(e, 0) + (vr(e, 1) - vr(e, 0)) * xi + (vr(e, 2) - vr(e, 0)) * eta;
+        const ld z = vz(e, 0) + (vz(e, 1) - vz(e, 0)) * xi + (vz(e, 2) - vz(e, 0)) * eta;
+        const Key key((long)llroundl(z / quantum), (long)llroundl(r / quantum));
+        auto it = node_id.find(key);
+        int id;
+        if (it == node_id.end()) {
+          id = (int)keys.size();
+          node_id[key] = id;
+          keys.push_back(key);
+          nr.push_back(r);
+          nz.push_back(z);
+        } else {
+          id = it->second;
+        }
+        cell_node[(size_t)e * nb + a] = id;
+      }
+  }
+  std::vector<int> order(keys.size());
+  for (size_t i = 0; i < order.size(); i++) order[i] = (int)i;
+  std::sort(order.begin(), order.end(), [&](int a, int b) { return keys[a] < keys[b]; });
+  std::vector<int> dof_of(keys.size());
+  g.n_dof = (int)keys.size();
+  g.node_r.resize(g.n_dof);
+  g.node_z.resize(g.n_dof);
+  for (int I = 0; I < g.n_dof; I++) {
+    dof_of[order[I]] = I;
+    g.node_r[I] = nr[order[I]];
+    g.node_z[I] = nz[order[I]];
+  }
+  g.P.assign(nc, std::vector<std::vector<std::pair<int, ld>>>(nb));
+  for (int e = 0; e < nc; e++)
+    for (int a = 0; a < nb; a++) g.P[e][a].push_back(std::make_pair(dof_of[cell_node[(size_t)e * nb + a]], (ld)1));
+  std::vector<std::vector<int>> rows(g.n_dof);
+  for (int e = 0; e < nc; e++) {
+    std::vector<int> touched;
+    for (const auto& row : g.P[e])
+      for (const auto& dw : row) touched.push_back(dw.first);
+    std::sort(touched.begin(), touched.end());
+    touched.erase(std::unique(touched.begin(), touched.end()), touched.end());
+    for (int I : touched)
+      for (int J : touched) rows[I].push_back(J);
+  }
+  g.rowptr.assign(g.n_dof + 1, 0);
+  g.colidx.clear();
+  for (int I = 0; I < g.n_dof; I++) {
+    std::sort(rows[I].begin(), rows[I].end());
+    rows[I].erase(std::unique(rows[I].begin(), rows[I].end()), rows[I].end());
+    g.rowptr[I + 1] = g.rowptr[I] + (int)rows[I].size();
+    g.colidx.insert(g.colidx.end(), rows[I].begin(), rows[I].end());
+  }
+  for (int e = 0; e < nc; e++) {
+    const ld J[4] = {vr(e, 1) - vr(e, 0), vr(e, 2) - vr(e, 0), vz(e, 1) - vz(e, 0), vz(e, 2) - vz(e, 0)};
+    const ld det = J[0] * J[3] - J[1] * J[2];
+    if (!(det > 0)) return false;
+    for (int q = 0; q < pb.nq; q++) {
+      const ld r = vr(e, 0) + J[0] * pb.sx[q] + J[1] * pb.se[q], z = vz(e, 0) + J[2] * pb.sx[q] + J[3] * pb.se[q];
+      g.ip_r.push_back(r);
+      g.ip_z.push_back(z);
+      g.ip_w.push_back(pb.sw[q] * det * r);
+      g.gm.push_back(J[3] / det);
+      g.gm.push_back(-J[2] / det);
+      g.gm.push_back(-J[1] / det);
+      g.gm.push_back(J[0] / det);
+    }
+  }
+  return true;
+}
+
 // O3' + O4' unstructured conforming mesh of straight-sided quadrilaterals (vertices (r, z), cells = 4 vertex ids,
 // counter-clockwise).  Qk nodes sit at the images of the equispaced reference nodes under the cell's bilinear map; nodes
 // of neighbouring cells that coincide are one dof (found geometrically: equal coordinates on a grid of 2^-30 of the mesh
 // extent); dofs are ordered by (z, r) on that grid; no constraints.  Integration points: the images of the Gauss points,
 // w = gw gw det(J) r with J the Jacobian of the bilinear map at the point.
 bool build_unstructured(const Problem& pb, Grid& g, int nv, const double* verts, int nc, const int* cells) {
+  if (pb.simplex) return build_unstructured_simplex(pb, g, nv, verts, nc, cells);
   const int k = pb.k, n1 = k + 1;
   g.unstructured = true;
   g.L = 0;
@@ -569,6 +660,61 @@ bool build_unstructured(const Problem& pb, Grid& g, int nv, const double* verts,
         g.gm.push_back(J[0] / det);
       }
   return true;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Simplex cells (sec. 5.1, Tables 11-12: P2 / P3 / P4 triangles with 6 / 12 / 16 integration points
+// per cell -- 864/144, 816/68, 384/24).  Reference triangle (0,0), (1,0), (0,1); Lagrange basis of degree k on the
+// equispaced lattice (i/k, j/k), i + j <= k, local order j-major: phi = P_i(xi) P_j(eta) P_l(1 - xi - eta), l = k - i - j,
+// P_n(t) = prod_{m<n} (k t - m)/(m + 1).  Quadrature: the symmetric rules of degree 4, 6, 8 with exactly those point counts
+// (Dunavant 1985), weights normalised to the reference area 1/2.
+// ---------------------------------------------------------------------------------------------
+void simplex_p(int k, int n, ld t, ld* v, ld* d) {
+  ld val = 1, der = 0;
+  for (int m = 0; m < n; m++) {
+    // product rule, factor (k t - m)/(m + 1)
+    der = der * (k * t - m) / (m + 1) + val * k / (ld)(m + 1);
+    val = val * (k * t - m) / (m + 1);
+  }
+  *v = val;
+  *d = der;
+}
+
+void simplex_rule(int k, std::vector<ld>& xi, std::vector<ld>& eta, std::vector<ld>& w) {
+  auto orbit3 = [&](ld a, ld wt) {  // (a, a, 1 - 2a) and permutations
+    const ld b = 1 - 2 * a;
+    const ld p[3][2] = {{a, a}, {a, b}, {b, a}};
+    for (int i = 0; i < 3; i++) {
+      xi.push_back(p[i][0]);
+      eta.push_back(p[i][1]);
+      w.push_back(wt / 2);
+    }
+  };
+  auto orbit6 = [&](ld a, ld b, ld wt) {
+    const ld c = 1 - a - b;
+    const ld p[6][2] = {{a, b}, {b, a}, {a, c}, {c, a}, {b, c}, {c, b}};
+    for (int i = 0; i < 6; i++) {
+      xi.push_back(p[i][0]);
+      eta.push_back(p[i][1]);
+      w.push_back(wt / 2);
+    }
+  };
+  if (k == 2) {  // degree 4, 6 points
+    orbit3(0.445948490915965L, 0.223381589678011L);
+    orbit3(0.091576213509771L, 0.109951743655322L);
+  } else if (k == 3) {  // degree 6, 12 points
+    orbit3(0.249286745170910L, 0.116786275726379L);
+    orbit3(0.063089014491502L, 0.050844906370207L);
+    orbit6(0.053145049844817L, 0.310352451033784L, 0.082851075618374L);
+  } else {  // degree 8, 16 points
+    xi.push_back(1 / (ld)3);
+    eta.push_back(1 / (ld)3);
+    w.push_back(0.144315607677787L / 2);
+    orbit3(0.459292588292723L, 0.095091634267285L);
+    orbit3(0.170569307751760L, 0.103217370534718L);
+    orbit3(0.050547228317031L, 0.032458497623198L);
+    orbit6(0.008394777409958L, 0.263112829634638L, 0.027230314174435L);
+  }
 }
 
 // O5  field values at the integration points of one species: f, df/dr, df/dz.
@@ -808,6 +954,35 @@ static Problem* new_problem(int degree, int threads) {
   return pb;
 }
 
+static Problem* new_problem_simplex(int degree, int threads) {
+  Problem* pb = new Problem();
+  pb->k = degree;
+  pb->nq1 = 0;
+  pb->simplex = true;
+  pb->nb = (degree + 1) * (degree + 2) / 2;
+  simplex_rule(degree, pb->sx, pb->se, pb->sw);
+  pb->nq = (int)pb->sw.size();
+  pb->threads = threads > 0 ? threads : 1;
+  pb->B.resize(pb->nq * pb->nb);
+  pb->dBxi.resize(pb->nq * pb->nb);
+  pb->dBeta.resize(pb->nq * pb->nb);
+  for (int q = 0; q < pb->nq; q++) {
+    const ld xi = pb->sx[q], eta = pb->se[q], lam = 1 - xi - eta;
+    int a = 0;
+    for (int j = 0; j <= degree; j++)
+      for (int i = 0; i <= degree - j; i++, a++) {
+        ld pi, di, pj, dj, pl, dl;
+        simplex_p(degree, i, xi, &pi, &di);
+        simplex_p(degree, j, eta, &pj, &dj);
+        simplex_p(degree, degree - i - j, lam, &pl, &dl);
+        pb->B[q * pb->nb + a] = pi * pj * pl;
+        pb->dBxi[q * pb->nb + a] = di * pj * pl - pi * pj * dl;
+        pb->dBeta[q * pb->nb + a] = pi * dj * pl - pi * pj * dl;
+      }
+  }
+  return pb;
+}
+
 static void finish_problem(Problem* pb, const SpeciesDesc* species, int n_species, const double* nu) {
   pb->species.assign(species, species + n_species);
   pb->nu.resize((size_t)n_species * n_species);
@@ -841,12 +1016,14 @@ void* orc_create(const GridDesc* grids, int n_grids, const SpeciesDesc* species,
   return pb;
 }
 
-// Unstructured quadrilateral grids: grid g has n_vertices[g] vertices (vertices[g]: (r, z) pairs) and
-// n_cells[g] cells (cells[g]: 4 counter-clockwise vertex ids each).  Returns NULL for an inverted cell.
+// Unstructured grids: grid g has n_vertices[g] vertices (vertices[g]: (r, z) pairs) and n_cells[g] cells
+// (cells[g]: vertices_per_cell counter-clockwise vertex ids each; 4: quadrilaterals Qk, 3: triangles Pk).  Returns NULL for an
+// inverted cell.
 void* orc_create_meshes(int n_grids, const int* n_vertices, const double* const* vertices, const int* n_cells,
-                        const int* const* cells, const SpeciesDesc* species, int n_species, int degree, const double* nu,
-                        int threads) {
-  Problem* pb = new_problem(degree, threads);
+                        const int* const* cells, int vertices_per_cell, const SpeciesDesc* species, int n_species,
+                        int degree, const double* nu, int threads) {
+  if ((vertices_per_cell != 3 && vertices_per_cell != 4) || degree < 2 || degree > 4) return nullptr;
+  Problem* pb = vertices_per_cell == 3 ? new_problem_simplex(degree, threads) : new_problem(degree, threads);
   pb->grids.resize(n_grids);
   for (int g = 0; g < n_grids; g++) {
     memset(&pb->grids[g].desc, 0, sizeof(GridDesc));

@@ -125,7 +125,7 @@ class Oracle:
 
     @classmethod
     def from_meshes(cls, meshes, species, degree, nu=None, threads=None):
-        """Unstructured quadrilateral grids: meshes = list of (vertices [nv, 2] (r, z), cells [nc, 4] counter-clockwise)."""
+        """Unstructured grids: meshes = list of (vertices [nv, 2] (r, z), cells [nc, 4] or [nc, 3] counter-clockwise)."""
         self = cls.__new__(cls)
         L = lib()
         L.orc_create_meshes.restype = C.c_void_p
@@ -144,8 +144,10 @@ class Oracle:
         if nu is not None:
             self._nu = np.ascontiguousarray(nu, dtype=np.float64)
             nu_p = _p(self._nu)
-        h = L.orc_create_meshes(C.c_int(self.G), _p(nv), vp, _p(nc), cp, s_arr, C.c_int(self.S), C.c_int(degree), nu_p,
-                                C.c_int(self.threads))
+        vpc = int(self._c[0].shape[1])
+        assert all(c.shape[1] == vpc for c in self._c)
+        h = L.orc_create_meshes(C.c_int(self.G), _p(nv), vp, _p(nc), cp, C.c_int(vpc), s_arr, C.c_int(self.S), C.c_int(degree),
+                                nu_p, C.c_int(self.threads))
         if not h:
             raise RuntimeError("orc_create_meshes failed (inverted cell)")
         self.h = C.c_void_p(h)

@@ -257,3 +257,14 @@ def semicircle_mesh(radius, n=2, m=2, core=0.5):
             # (k, l) -> (k, l+1) -> (k+1, l+1) -> (k+1, l) runs counter-clockwise in the (r, z) plane
             cells.append((ring(k, l), ring(k, l + 1), ring(k + 1, l + 1), ring(k + 1, l)))
     return np.array(verts, dtype=np.float64), np.array(cells, dtype=np.int32)
+
+
+def semicircle_triangles(radius, n=2, m=2, core=0.5):
+    """The cells of semicircle_mesh cut along a diagonal: a conforming triangle mesh of the same half disc (stand-in for the
+    paper's Simmetrix meshes, sec. 5.1).  Returns (vertices [nv, 2], cells [2 nc, 3] counter-clockwise)."""
+    v, q = semicircle_mesh(radius, n, m, core)
+    tri = []
+    for c in q:
+        tri.append((c[0], c[1], c[2]))
+        tri.append((c[0], c[2], c[3]))
+    return v, np.array(tri, dtype=np.int32)
