@@ -92,14 +92,19 @@ typedef struct {
   int n_vertices;
   const double* vertices_rz; /* host, n_vertices x 2: (r, z) in units of v0 */
   int n_cells;
-  const int* cells;          /* host, n_cells x 4 vertex indices */
+  const int* cells;          /* host, n_cells x vertices_per_cell vertex indices, counter-clockwise */
+  int vertices_per_cell;     /* 4: quadrilaterals (Qk, k = 2, 3); 3: triangles (Pk, k = 2, 3, 4; sec. 5.1) */
 } landau_mesh_desc;
 
 /* landau_create for unstructured quadrilateral grids: meshes[n_grids] (host, read during the call) take the place of the
  * grid descriptors, everything else as above.  Dofs are ordered by (z, r) of their coordinates (on a grid of 2^-30 of the
  * mesh extent), exposed through landau_dof_coords; all other entry points work unchanged on such a context.
  * landau_last_coefficients (landau_debug.h) returns the coefficients pulled back to the reference cell on these grids.
- * Extra errors: LANDAU_INVALID_ARG for a cell with a missing vertex or a non-positive Jacobian. */
+ * Triangles: Lagrange Pk on the equispaced lattice of the cell, the symmetric quadrature rule of degree 2k with 6 / 12 / 16
+ * points (the point counts of the paper's Tables 11-12), affine geometry; `quadrature->n_gauss_1d` must still be degree + 1
+ * and is otherwise ignored; all meshes of a context must have the same cell type.
+ * Extra errors: LANDAU_INVALID_ARG for a cell with a missing vertex or a non-positive Jacobian, LANDAU_UNSUPPORTED for
+ * mixed cell types or a degree the cell type does not have. */
 int landau_create_meshes(const landau_mesh_desc* meshes, int n_grids, const landau_species_desc* species, int n_species,
                          const landau_quadrature_desc* quadrature, const double* nu, int cuda_device, landau_ctx** out);
 

@@ -114,17 +114,20 @@ def landau_create(grids, species, quadrature, nu=None, cuda_device=0):
 
 
 class MeshDesc(C.Structure):
-    _fields_ = [("n_vertices", C.c_int), ("vertices_rz", C.c_void_p), ("n_cells", C.c_int), ("cells", C.c_void_p)]
+    _fields_ = [("n_vertices", C.c_int), ("vertices_rz", C.c_void_p), ("n_cells", C.c_int), ("cells", C.c_void_p),
+                ("vertices_per_cell", C.c_int)]
 
 
 def landau_create_meshes(meshes, species, quadrature, nu=None, cuda_device=0):
-    """meshes: list of (vertices [nv, 2] (r, z), cells [nc, 4] counter-clockwise vertex ids); otherwise as landau_create."""
+    """meshes: list of (vertices [nv, 2] (r, z), cells [nc, 4] (quadrilaterals) or [nc, 3] (triangles), counter-clockwise
+    vertex ids); otherwise as landau_create."""
     lib = load()
     if isinstance(quadrature, int):
         quadrature = dict(degree=quadrature, n_gauss_1d=quadrature + 1)
     vs = [np.ascontiguousarray(m[0], dtype=np.float64) for m in meshes]
     cs = [np.ascontiguousarray(m[1], dtype=np.int32) for m in meshes]
-    m_arr = (MeshDesc * len(meshes))(*[MeshDesc(len(v), v.ctypes.data, len(c), c.ctypes.data) for v, c in zip(vs, cs)])
+    m_arr = (MeshDesc * len(meshes))(*[MeshDesc(len(v), v.ctypes.data, len(c), c.ctypes.data, int(c.shape[1]))
+                                       for v, c in zip(vs, cs)])
     s_arr = (SpeciesDesc * len(species))(*[SpeciesDesc(float(s["mass"]), float(s["charge"]), int(s["grid"]))
                                            for s in species])
     qd = QuadratureDesc(int(quadrature["degree"]), int(quadrature["n_gauss_1d"]))

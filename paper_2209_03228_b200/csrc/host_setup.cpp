@@ -8,6 +8,7 @@
 #include <map>
 #include <string>
 #include <tuple>
+#include <tuple>
 #include <unordered_map>
 
 namespace landau {
@@ -107,6 +108,81 @@ bool build_tables(int k, HostTables* t, std::string* msg) {
           t->dBxi[q * t->nb + a] = d[q1 * n1 + a1] * v[q2 * n1 + a2];
           t->dBeta[q * t->nb + a] = v[q1 * n1 + a1] * d[q2 * n1 + a2];
         }
+  return true;
+}
+
+bool build_tables_simplex(int k, HostTables* t, std::string* msg) {
+  if (k < 2 || k > 4) {
+    *msg = "triangle degree must be 2, 3 or 4";
+    return false;
+  }
+  t->k = k;
+  t->nq1 = 0;
+  t->simplex = true;
+  t->nb = (k + 1) * (k + 2) / 2;
+  t->sx.clear();
+  t->se.clear();
+  t->sw.clear();
+  // symmetric rules on the reference triangle, barycentric orbits (a, a, 1 - 2a) and (a, b, 1 - a - b); weights sum to 1/2
+  struct Orbit {
+    int n;
+    double a, b, w;
+  };
+  static const Orbit deg4[] = {{3, 0.445948490915965, 0, 0.223381589678011}, {3, 0.091576213509771, 0, 0.109951743655322}};
+  static const Orbit deg6[] = {{3, 0.249286745170910, 0, 0.116786275726379},
+                               {3, 0.063089014491502, 0, 0.050844906370207},
+                               {6, 0.053145049844817, 0.310352451033784, 0.082851075618374}};
+  static const Orbit deg8[] = {{1, 1.0 / 3.0, 0, 0.144315607677787},
+                               {3, 0.459292588292723, 0, 0.095091634267285},
+                               {3, 0.170569307751760, 0, 0.103217370534718},
+                               {3, 0.050547228317031, 0, 0.032458497623198},
+                               {6, 0.008394777409958, 0.263112829634638, 0.027230314174435}};
+  const Orbit* rule = k == 2 ? deg4 : k == 3 ? deg6 : deg8;
+  const int n_orbits = k == 2 ? 2 : k == 3 ? 3 : 5;
+  for (int o = 0; o < n_orbits; ++o) {
+    const Orbit& r = rule[o];
+    const double c3 = 1.0 - 2.0 * r.a, c6 = 1.0 - r.a - r.b;
+    // the orbit's points (lambda_1, lambda_2) = (xi, eta): 1 (centroid), 3 ((a, a, c) permuted) or 6 ((a, b, c) permuted)
+    const double p1[1][2] = {{r.a, r.a}};
+    const double p3[3][2] = {{r.a, r.a}, {r.a, c3}, {c3, r.a}};
+    const double p6[6][2] = {{r.a, r.b}, {r.b, r.a}, {r.a, c6}, {c6, r.a}, {r.b, c6}, {c6, r.b}};
+    const double(*pts)[2] = r.n == 1 ? p1 : r.n == 3 ? p3 : p6;
+    for (int p = 0; p < r.n; ++p) {
+      t->sx.push_back(pts[p][0]);
+      t->se.push_back(pts[p][1]);
+      t->sw.push_back(0.5 * r.w);
+    }
+  }
+  t->nq = (int)t->sw.size();
+  // Lagrange basis of the lattice node (i, j, l = k - i - j): product over the three barycentric coordinates of
+  // N_n(lambda) = prod_{m < n} (k lambda - m) / (m + 1); local order j-major, i fastest
+  auto factor = [&](int n, double lam, double* v, double* d) {
+    double val = 1.0, der = 0.0;
+    for (int m = 0; m < n; ++m) {
+      const double f = (k * lam - m) / (m + 1.0);
+      der = der * f + val * (k / (m + 1.0));
+      val *= f;
+    }
+    *v = val;
+    *d = der;
+  };
+  t->B.assign((size_t)t->nq * t->nb, 0.0);
+  t->dBxi.assign((size_t)t->nq * t->nb, 0.0);
+  t->dBeta.assign((size_t)t->nq * t->nb, 0.0);
+  for (int q = 0; q < t->nq; ++q) {
+    const double xi = t->sx[q], eta = t->se[q], lam0 = 1.0 - xi - eta;
+    int a = 0;
+    for (int j = 0; j <= k; ++j)
+      for (int i = 0; i <= k - j; ++i, ++a) {
+        double vi, di, vj, dj, vl, dl;
+        factor(i, xi, &vi, &di);
+        factor(j, eta, &vj, &dj);
+        factor(k - i - j, lam0, &vl, &dl);
+        t->B[(size_t)q * t->nb + a] = vi * vj * vl;
+        t->dBxi[(size_t)q * t->nb + a] = di * vj * vl - vi * vj * dl;   // d lam0 / d xi = -1
+        t->dBeta[(size_t)q * t->nb + a] = vi * dj * vl - vi * vj * dl;
+      }
+  }
   return true;
 }
 
@@ -360,8 +436,8 @@ int finish_grid(const HostTables& t, HostGrid* g, std::string* msg) {
       ++fill[en.slot];
     }
   }
-  // ---- K3 ring schedule --------------------------------------------------------------------------------------------
-  {
+  // ---- K3 ring schedule (tensor-product cells only: the ring kernel is sum-factorised) ----------------------------------
+  if (!t.simplex) {
     const int nb2 = nb * nb;
     g->k3_nsteps = (g->n_cells + K3_PC - 1) / K3_PC;
     // emission step of every CSR slot = step of its last contributing cell; an element matrix stays in the ring from
@@ -479,11 +555,130 @@ int finish_grid(const HostTables& t, HostGrid* g, std::string* msg) {
 // Nodes are identified by topology, not geometry: a corner node by its vertex id, an edge node by (lower vertex id, higher
 // vertex id, position counted from the lower one), an interior node by (cell, a1, a2).  Dofs are then ordered by their
 // coordinates on a grid of 2^-30 of the mesh extent, z-major.
+// triangles: the same topological identification (vertex / edge / interior keys), affine geometry
+static int build_triangle_grid(const landau_mesh_desc& m, const HostTables& t, HostGrid* g, std::string* msg) {
+  const int k = t.k, nb = t.nb, nq = t.nq, nc = m.n_cells;
+  memset(&g->desc, 0, sizeof(g->desc));
+  g->desc.kind = 3;
+  g->k = k;
+  g->nb = nb;
+  g->nq = nq;
+  g->n_cells = nc;
+  for (int e = 0; e < 3 * nc; ++e)
+    if (m.cells[e] < 0 || m.cells[e] >= m.n_vertices) {
+      *msg = "mesh cell refers to a missing vertex";
+      return LANDAU_INVALID_ARG;
+    }
+  double scale = 0.0;
+  for (int v = 0; v < 2 * m.n_vertices; ++v) scale = std::max(scale, std::fabs(m.vertices_rz[v]));
+  const double quantum = scale / 1073741824.0;
+  typedef std::tuple<int, int, int, int> NodeKey;
+  std::map<NodeKey, int> node_of;
+  std::vector<double> nr, nz;
+  std::vector<int> cell_node((size_t)nc * nb);
+  auto edge_key = [&](int va, int vb, int tpos) { return va < vb ? NodeKey(1, va, vb, tpos) : NodeKey(1, vb, va, k - tpos); };
+  for (int e = 0; e < nc; ++e) {
+    const int* cv = &m.cells[3 * e];
+    const double* P0 = &m.vertices_rz[2 * cv[0]];
+    const double* P1 = &m.vertices_rz[2 * cv[1]];
+    const double* P2 = &m.vertices_rz[2 * cv[2]];
+    int a = 0;
+    for (int j = 0; j <= k; ++j)
+      for (int i = 0; i <= k - j; ++i, ++a) {
+        const int l = k - i - j;
+        NodeKey key;
+        if (i == k)
+          key = NodeKey(0, cv[1], 0, 0);
+        else if (j == k)
+          key = NodeKey(0, cv[2], 0, 0);
+        else if (l == k)
+          key = NodeKey(0, cv[0], 0, 0);
+        else if (j == 0)
+          key = edge_key(cv[0], cv[1], i);  // on v0 -> v1, i steps from v0
+        else if (l == 0)
+          key = edge_key(cv[1], cv[2], j);  // on v1 -> v2, j steps from v1
+        else if (i == 0)
+          key = edge_key(cv[0], cv[2], j);  // on v0 -> v2, j steps from v0
+        else
+          key = NodeKey(2, e, i, j);
+        auto it = node_of.find(key);
+        int id;
+        if (it == node_of.end()) {
+          id = (int)nr.size();
+          node_of[key] = id;
+          const double xi = (double)i / k, eta = (double)j / k;
+          nr.push_back(P0[0] + (P1[0] - P0[0]) * xi + (P2[0] - P0[0]) * eta);
+          nz.push_back(P0[1] + (P1[1] - P0[1]) * xi + (P2[1] - P0[1]) * eta);
+        } else {
+          id = it->second;
+        }
+        cell_node[(size_t)e * nb + a] = id;
+      }
+  }
+  const int nn = (int)nr.size();
+  std::vector<std::pair<std::pair<long long, long long>, int>> order(nn);
+  for (int i = 0; i < nn; ++i) order[i] = std::make_pair(std::make_pair(std::llround(nz[i] / quantum), std::llround(nr[i] / quantum)), i);
+  std::sort(order.begin(), order.end());
+  std::vector<int> dof_of(nn);
+  g->n_dof = nn;
+  g->dof_r.resize(nn);
+  g->dof_z.resize(nn);
+  for (int I = 0; I < nn; ++I) {
+    dof_of[order[I].second] = I;
+    g->dof_r[I] = nr[order[I].second];
+    g->dof_z[I] = nz[order[I].second];
+  }
+  g->en_ptr.assign(1, 0);
+  g->en_dof.clear();
+  g->en_w.clear();
+  for (int ea = 0; ea < nc * nb; ++ea) {
+    g->en_dof.push_back(dof_of[cell_node[ea]]);
+    g->en_w.push_back(1.0);
+    g->en_ptr.push_back((int)g->en_dof.size());
+  }
+  g->cell_r0.assign(nc, 0.0);
+  g->cell_z0.assign(nc, 0.0);
+  g->cell_hr.assign(nc, 2.0);
+  g->cell_hz.assign(nc, 2.0);
+  g->n_ip = nc * nq;
+  g->ip_r.resize(g->n_ip);
+  g->ip_z.resize(g->n_ip);
+  g->ip_w.resize(g->n_ip);
+  g->ip_gm.resize(4 * (size_t)g->n_ip);
+  for (int e = 0; e < nc; ++e) {
+    const int* cv = &m.cells[3 * e];
+    const double* P0 = &m.vertices_rz[2 * cv[0]];
+    const double J[4] = {m.vertices_rz[2 * cv[1]] - P0[0], m.vertices_rz[2 * cv[2]] - P0[0], m.vertices_rz[2 * cv[1] + 1] - P0[1],
+                         m.vertices_rz[2 * cv[2] + 1] - P0[1]};
+    const double det = J[0] * J[3] - J[1] * J[2];
+    if (!(det > 0.0)) {
+      *msg = "mesh cell " + std::to_string(e) + " is inverted or clockwise";
+      return LANDAU_INVALID_ARG;
+    }
+    for (int q = 0; q < nq; ++q) {
+      const int ip = e * nq + q;
+      g->ip_r[ip] = P0[0] + J[0] * t.sx[q] + J[1] * t.se[q];
+      g->ip_z[ip] = P0[1] + J[2] * t.sx[q] + J[3] * t.se[q];
+      g->ip_w[ip] = t.sw[q] * det * g->ip_r[ip];
+      g->ip_gm[4 * (size_t)ip] = J[3] / det;
+      g->ip_gm[4 * (size_t)ip + 1] = -J[2] / det;
+      g->ip_gm[4 * (size_t)ip + 2] = -J[1] / det;
+      g->ip_gm[4 * (size_t)ip + 3] = J[0] / det;
+    }
+  }
+  return finish_grid(t, g, msg);
+}
+
 int build_mesh_grid(const landau_mesh_desc& m, const HostTables& t, HostGrid* g, std::string* msg) {
   if (m.n_vertices < 4 || m.n_cells < 1 || !m.vertices_rz || !m.cells) {
     *msg = "bad mesh: at least 4 vertices and 1 cell";
     return LANDAU_INVALID_ARG;
   }
+  if ((m.vertices_per_cell == 3) != t.simplex || (m.vertices_per_cell != 3 && m.vertices_per_cell != 4)) {
+    *msg = "mesh cell type does not match the context's element tables (all meshes must have the same vertices_per_cell, 3 or 4)";
+    return LANDAU_UNSUPPORTED;
+  }
+  if (t.simplex) return build_triangle_grid(m, t, g, msg);
   const int k = t.k, n1 = k + 1, nb = t.nb, nq = t.nq, nc = m.n_cells;
   memset(&g->desc, 0, sizeof(g->desc));
   g->desc.kind = 2;

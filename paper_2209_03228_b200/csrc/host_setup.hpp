@@ -64,6 +64,8 @@ struct HostGrid {
 
 struct HostTables {
   int k = 0, nq1 = 0, nb = 0, nq = 0;
+  bool simplex = false;                  // triangles: nb = (k+1)(k+2)/2, reference points (sx, se) and weights sw (sum 1/2)
+  std::vector<double> sx, se, sw;
   std::vector<double> gauss_x, gauss_w;  // on [-1,1]
   std::vector<double> B, dBxi, dBeta;    // [q][a]
   std::vector<double> lag_v, lag_d;      // 1-D Lagrange values / derivatives at the Gauss points, [q1][c]
@@ -74,6 +76,8 @@ struct HostTables {
 
 // Fills tables for degree k (2 or 3).  Returns false with msg on unsupported degree.
 bool build_tables(int k, HostTables* t, std::string* msg);
+// Tables of the Pk triangle (k = 2, 3, 4): basis on the equispaced lattice, symmetric rule of degree 2k.
+bool build_tables_simplex(int k, HostTables* t, std::string* msg);
 
 // Builds one grid.  status: 0 ok, LANDAU_INVALID_ARG / LANDAU_UNSUPPORTED with msg.
 int build_grid(const landau_grid_desc& d, const HostTables& t, HostGrid* g, std::string* msg);

@@ -148,6 +148,23 @@ int grow(landau_ctx* ctx, double** p, size_t* cap, size_t need, bool zero, cudaS
 
 int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
+// kernels templated on (basis functions, integration points) per cell: Q2, Q3 quadrilaterals, P2, P3, P4 triangles
+#define LANDAU_ELEM_DISPATCH(ctx, CALL)                  \
+  do {                                                   \
+    const int nb_ = (ctx)->nb, nq_ = (ctx)->nq;          \
+    if (nb_ == 9 && nq_ == 9) {                          \
+      CALL(9, 9);                                        \
+    } else if (nb_ == 16 && nq_ == 16) {                 \
+      CALL(16, 16);                                      \
+    } else if (nb_ == 6 && nq_ == 6) {                   \
+      CALL(6, 6);                                        \
+    } else if (nb_ == 10 && nq_ == 12) {                 \
+      CALL(10, 12);                                      \
+    } else {                                             \
+      CALL(15, 16);                                      \
+    }                                                    \
+  } while (0)
+
 // NVTX range around the launches of one stage (visible in Nsight Systems / ncu --nvtx; free when no tool is attached)
 struct NvtxRange {
   bool open = true;
@@ -619,12 +636,11 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
     const Group& gr = ctx->groups[q];
     dim3 grid(ctx->hg[g].n_cells, (nbc + K1T_BT - 1) / K1T_BT);
     const int joff = ctx->ip_off[g] - gr.j0;
-    if (ctx->nb == 9)
-      k1_fields<9><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->mix[g], batch_f, ctx->f_stride, b0, nbc,
-                                              ctx->F + gr.f_off, gr.nj_pad, joff, 0, kern_tc(kern[q]));
-    else
-      k1_fields<16><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->mix[g], batch_f, ctx->f_stride, b0, nbc,
-                                               ctx->F + gr.f_off, gr.nj_pad, joff, 0, kern_tc(kern[q]));
+#define K1_CALL(NB_, NQ_)                                                                                                 \
+  k1_fields<NB_, NQ_><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->mix[g], batch_f, ctx->f_stride, b0, nbc, ctx->F + gr.f_off, \
+                                            gr.nj_pad, joff, 0, kern_tc(kern[q]))
+    LANDAU_ELEM_DISPATCH(ctx, K1_CALL);
+#undef K1_CALL
     ++ctx->launches;
   }
   nvtxRangePop();
@@ -739,12 +755,11 @@ int assemble_chunk(landau_ctx* ctx, int b0, int nbc, double inv_dt, double* out_
       if (ctx->k3_ring_ok[s] && ctx->assembly_kernel != 1) continue;
       const int g = ctx->species[s].grid;
       dim3 grid((ctx->hg[g].nnz + 255) / 256, nbc);
-      if (ctx->nb == 9)
-        k3_assemble<9><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, nbc,
-                                             vals, ctx->v_stride, ctx->v_off[s]);
-      else
-        k3_assemble<16><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, nbc,
-                                              vals, ctx->v_stride, ctx->v_off[s]);
+#define K3_CALL(NB_, NQ_)                                                                                                 \
+  k3_assemble<NB_, NQ_><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, nbc, vals, \
+                                              ctx->v_stride, ctx->v_off[s])
+      LANDAU_ELEM_DISPATCH(ctx, K3_CALL);
+#undef K3_CALL
       ++ctx->launches;
     }
   return LANDAU_OK;
@@ -757,17 +772,13 @@ int apply_chunk(landau_ctx* ctx, const double* batch_f_dev, int b0, int nbc, dou
     for (int s = 0; s < ctx->S; ++s) {
       const int g = ctx->species[s].grid;
       dim3 g1(ctx->hg[g].n_cells, (nbc + K1T_BT - 1) / K1T_BT), g2((ctx->hg[g].n_dof + 255) / 256, nbc);
-      if (ctx->nb == 9) {
-        k3_elem_apply<9><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,
-                                             ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);
-        k3_apply_gather<9><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev,
-                                               ctx->f_stride, ctx->f_off[s], b0);
-      } else {
-        k3_elem_apply<16><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,
-                                              ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);
-        k3_apply_gather<16><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev,
-                                                ctx->f_stride, ctx->f_off[s], b0);
-      }
+#define K3A_CALL(NB_, NQ_)                                                                                                \
+  k3_elem_apply<NB_, NQ_><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,    \
+                                              ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);    \
+  k3_apply_gather<NB_><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev, ctx->f_stride, \
+                                           ctx->f_off[s], b0)
+      LANDAU_ELEM_DISPATCH(ctx, K3A_CALL);
+#undef K3A_CALL
       ctx->launches += 2;
     }
   return LANDAU_OK;
@@ -795,7 +806,9 @@ int create_any(const landau_grid_desc* grids, const landau_mesh_desc* meshes, in
     return fail(nullptr, code, m);
   };
   try {
-    if (!build_tables(quadrature->degree, &ctx->ht, &msg)) return bail(LANDAU_UNSUPPORTED, msg);
+    const bool triangles = meshes && meshes[0].vertices_per_cell == 3;
+    if (!(triangles ? build_tables_simplex(quadrature->degree, &ctx->ht, &msg) : build_tables(quadrature->degree, &ctx->ht, &msg)))
+      return bail(LANDAU_UNSUPPORTED, msg);
     ctx->k = quadrature->degree;
     ctx->nb = ctx->ht.nb;
     ctx->nq = ctx->ht.nq;

@@ -254,7 +254,8 @@ __host__ __device__ __forceinline__ long long k2g_f_offset(int TC, int njt, int 
 // ------------------------------------------------------------------------------------------------------------
 constexpr int K1T_BT = 16;
 
-template <int NB>
+// NB basis functions, NQ integration points per cell (equal on tensor cells; 10 / 12 and 15 / 16 on P3 / P4 triangles)
+template <int NB, int NQ = NB>
 __global__ void __launch_bounds__(256)
 k1_fields(DevGrid g, const DevTables* __restrict__ tab, MixTable mix, const double* __restrict__ batch_f,
                long long f_stride, int b0, int nbatch, double* __restrict__ F, long long nj_pad, int j_off_in_group,
@@ -263,15 +264,15 @@ k1_fields(DevGrid g, const DevTables* __restrict__ tab, MixTable mix, const doub
   __shared__ double sD[NB][K1T_BT], sK[NB][K1T_BT];
   const int tid = threadIdx.x, lo = tid & 15, bl = tid >> 4;
   const int cell = blockIdx.x, b = blockIdx.y * K1T_BT + bl;
-  for (int e = tid; e < NB * NB; e += 256) {
+  for (int e = tid; e < NQ * NB; e += 256) {
     const int q = e / NB, a = e - q * NB;
     sT[0][a][q] = tab->B[e];
     sT[1][a][q] = tab->dBxi[e];
     sT[2][a][q] = tab->dBeta[e];
   }
   const double sr = g.cell_sr[cell], sz = g.cell_sz[cell];
-  const int j = cell * NB + lo;
-  const double w = lo < NB ? g.ip_w[j] : 0.0;
+  const int j = cell * NQ + lo;
+  const double w = lo < NQ ? g.ip_w[j] : 0.0;
   const bool live = b < nbatch;
   const double* fb = batch_f + (long long)(b0 + (live ? b : 0)) * f_stride;
   for (int c = 0; c < mix.ncb; ++c) {
@@ -290,7 +291,7 @@ k1_fields(DevGrid g, const DevTables* __restrict__ tab, MixTable mix, const doub
       sK[lo][bl] = fK;
     }
     __syncthreads();
-    if (lo < NB && live) {  // lo = quadrature point q
+    if (lo < NQ && live) {  // lo = quadrature point q
       double v = 0.0, vx = 0.0, vy = 0.0;
 #pragma unroll
       for (int a = 0; a < NB; ++a) {
@@ -586,12 +587,12 @@ k2b_combine(const CombineTable* __restrict__ cts, const double* __restrict__ G, 
 // (eq. 2.4 with the sparse Jacobian of PAPER.md:73), weighted by the constraint products P[a][I] P[c][J].
 // Every CSR value is written exactly once, coalesced along the slot index; no atomics.
 // ------------------------------------------------------------------------------------------------------------
-template <int NB>
+template <int NB, int NQ = NB>
 __global__ void __launch_bounds__(256)
 k3_assemble(DevGrid g, const DevTables* __restrict__ tab, const double* __restrict__ DK, long long dk_stride,
             long long dk_off, double inv_dt, int nbatch, double* __restrict__ vals, long long v_stride, long long v_off) {
-  __shared__ double sB[NB * NB], sX[NB * NB], sY[NB * NB];
-  for (int e = threadIdx.x; e < NB * NB; e += blockDim.x) {
+  __shared__ double sB[NQ * NB], sX[NQ * NB], sY[NQ * NB];
+  for (int e = threadIdx.x; e < NQ * NB; e += blockDim.x) {
     sB[e] = tab->B[e];
     sX[e] = tab->dBxi[e];
     sY[e] = tab->dBeta[e];
@@ -608,8 +609,8 @@ k3_assemble(DevGrid g, const DevTables* __restrict__ tab, const double* __restri
     const double sr = g.cell_sr[cell], sz = g.cell_sz[cell];
     double s = 0.0;
 #pragma unroll 4
-    for (int q = 0; q < NB; ++q) {
-      const int ip = cell * NB + q;
+    for (int q = 0; q < NQ; ++q) {
+      const int ip = cell * NQ + q;
       const double w = g.ip_w[ip];
       const double Drr = dk[ip], Drz = dk[g.n_ip + ip], Dzz = dk[2 * g.n_ip + ip], Kr = dk[3 * g.n_ip + ip],
                    Kz = dk[4 * g.n_ip + ip];
@@ -634,17 +635,17 @@ k3_assemble(DevGrid g, const DevTables* __restrict__ tab, const double* __restri
 //   k3_apply_gather: one thread per (dof, entry) sums its element-vector entries (constraint weights), coalesced along
 //     the dof index.
 // ------------------------------------------------------------------------------------------------------------
-template <int NB>
+template <int NB, int NQ = NB>
 __global__ void __launch_bounds__(256)
 k3_elem_apply(DevGrid g, const DevTables* __restrict__ tab, const double* __restrict__ batch_f, long long f_stride,
               long long f_off, int b0, const double* __restrict__ DK, long long dk_stride, long long dk_off, int nbatch,
               double* __restrict__ RE, long long re_stride, long long re_off) {
   __shared__ double sT[3][NB][16];  // B, dBxi, dBeta as [a][q]
-  __shared__ double sF[NB][K1T_BT], sFl[2][NB][K1T_BT];
+  __shared__ double sF[NB][K1T_BT], sFl[2][NQ][K1T_BT];
   const int tid = threadIdx.x, lo = tid & 15, bl = tid >> 4;
   const int cell = blockIdx.x, b = blockIdx.y * K1T_BT + bl;
   const bool live = b < nbatch;
-  for (int e = tid; e < NB * NB; e += 256) {
+  for (int e = tid; e < NQ * NB; e += 256) {
     const int q = e / NB, a = e - q * NB;
     sT[0][a][q] = tab->B[e];
     sT[1][a][q] = tab->dBxi[e];
@@ -658,7 +659,7 @@ k3_elem_apply(DevGrid g, const DevTables* __restrict__ tab, const double* __rest
     sF[lo][bl] = fa;
   }
   __syncthreads();
-  if (lo < NB) {  // lo = quadrature point q
+  if (lo < NQ) {  // lo = quadrature point q
     double v = 0.0, vx = 0.0, vy = 0.0;
 #pragma unroll
     for (int a = 0; a < NB; ++a) {
@@ -667,7 +668,7 @@ k3_elem_apply(DevGrid g, const DevTables* __restrict__ tab, const double* __rest
       vx = fma(sT[1][a][lo], fa, vx);
       vy = fma(sT[2][a][lo], fa, vy);
     }
-    const int j = cell * NB + lo;
+    const int j = cell * NQ + lo;
     const double fr = vx * sr, fz = vy * sz, w = g.ip_w[j];
     const double* dk = DK + (long long)(live ? b : 0) * dk_stride + dk_off;
     const double Drr = dk[j], Drz = dk[g.n_ip + j], Dzz = dk[2 * g.n_ip + j], Kr = dk[3 * g.n_ip + j], Kz = dk[4 * g.n_ip + j];
@@ -678,7 +679,7 @@ k3_elem_apply(DevGrid g, const DevTables* __restrict__ tab, const double* __rest
   if (lo < NB && live) {  // lo = basis function a again
     double r = 0.0;
 #pragma unroll
-    for (int q = 0; q < NB; ++q) {
+    for (int q = 0; q < NQ; ++q) {
       r = fma(sT[1][lo][q] * sr, sFl[0][q][bl], r);
       r = fma(sT[2][lo][q] * sz, sFl[1][q][bl], r);
     }

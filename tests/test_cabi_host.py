@@ -163,3 +163,28 @@ def test_unstructured_host_setup_matches_oracle(lib, orc):
     bad[0, 0] = 99
     with pytest.raises(Bn.LandauError, match="missing vertex"):
         Bn.Landau.from_meshes([(v, bad)], [dict(mass=1.0, charge=-1.0, grid=0)], 3, device=-1)
+
+
+@pytest.mark.parametrize("k,per_cell", [(2, 6), (3, 12), (4, 16)])
+def test_triangle_host_setup_matches_oracle(lib, orc, k, per_cell):
+    """Triangles P2 - P4 (landau_mesh_desc.vertices_per_cell = 3): the product's tables and topological node identification
+    against the oracle's; point counts per cell as in the paper's Tables 11-12 (864/144, 816/68, 384/24)."""
+    mesh = W.semicircle_triangles(5.0, 2, 2)
+    species = [dict(mass=1.0, charge=-1.0, grid=0)]
+    L = Bn.Landau.from_meshes([mesh], species, k, device=-1)
+    o = orc.Oracle.from_meshes([mesh], species, k)
+    assert L.n_ip[0] == L.n_cells[0] * per_cell == o.n_ip[0]
+    assert L.n_dof[0] == o.n_dof[0] and L.nnz[0] == o.nnz[0]
+    assert np.abs(L.dof_coords(0) - o.dof_coords(0)).max() < 1e-13
+    rp, ci = L.pattern(0)
+    rp2, ci2 = o.pattern(0)
+    assert np.array_equal(rp, rp2) and np.array_equal(ci, ci2)
+    a, b = np.stack(L.ip_table(0), 1), np.stack(o.ip_table(0), 1)
+    pa = np.array([int(np.argmin(((a[:, :2] - x) ** 2).sum(1))) for x in b[:, :2]])
+    assert len(set(pa)) == len(pa) and np.abs(a[pa] - b).max() < 1e-13
+    L.close()
+    quads = W.semicircle_mesh(5.0, 2, 2)
+    with pytest.raises(Bn.LandauError, match="cell type"):               # one cell type per context
+        Bn.Landau.from_meshes([mesh, quads], [dict(mass=1.0, charge=-1.0, grid=0), dict(mass=2.0, charge=1.0, grid=1)], 3, device=-1)
+    with pytest.raises(Bn.LandauError):                                  # Q4 quadrilaterals are not built
+        Bn.Landau.from_meshes([quads], species, 4, device=-1)
