@@ -51,12 +51,14 @@ int landau_last_stage_ms(landau_ctx* ctx, float* ms4);
 
 /* Choose the inner-integral kernel: 0 auto (by column count), 1 plain DFMA kernel, 2 DMMA kernel with per-warp
  * tensor generation, 3 / 4 DMMA GEMM kernel with the tensor tile evaluated once per CTA and shared by its warps
- * (TMA-staged source tiles; 32 x 128 / 16 x 256 CTA tile: 4 is the default for more than 128 source columns). */
+ * (TMA-staged source tiles; 32 x 128 / 16 x 256 CTA tile: 4 is the default for more than 128 source columns), 5 the same
+ * with a 16 x 64 tile (default for 49 .. 64 columns when the field tiles fill the machine). */
 int landau_set_inner_kernel(landau_ctx* ctx, int which);
 
 /* Choose the element-matrix + assembly kernel: 0 auto (k3_ring: DMMA sum-factorised element matrices kept in a
  * shared-memory ring, CSR slots gathered from it; used for every grid whose ring fits in shared memory),
- * 1 force the general slot-gather kernel (k3_assemble: one thread per CSR slot, scalar FP64). */
+ * 1 force the general slot-gather kernel (k3_assemble: one thread per CSR slot, scalar FP64), 2 the ring kernel without the
+ * tail cut (one CTA per (entry, species) block; for A/B measurements). */
 int landau_set_assembly_kernel(landau_ctx* ctx, int which);
 
 /* Schedule of the ring assembly kernel for grid g (host query, works on host-only contexts): ring_cells = element

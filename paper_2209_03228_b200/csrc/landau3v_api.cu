@@ -39,6 +39,9 @@ struct landau3v_ctx {
   std::vector<Mix3> mix;
   Ranges3 ranges;
   Combine3* d_comb = nullptr;
+  DevGrid3* d_grids = nullptr;
+  Spec3* d_spec = nullptr;
+  int max_cells = 0, max_nnz = 0;
   double* EM = nullptr;
   size_t EM_cap = 0;
   std::vector<long long> em_off;
@@ -242,6 +245,18 @@ int build_device_side(landau3v_ctx* ctx) {
   const Combine3* dc;
   if (int rc = upload(ctx, comb, &dc)) return rc;
   ctx->d_comb = const_cast<Combine3*>(dc);
+  std::vector<Spec3> specs(S);
+  for (int s = 0; s < S; ++s) {
+    specs[s] = Spec3{ctx->species[s].grid, ctx->dk_off[s], ctx->em_off[s], ctx->v_off[s]};
+    ctx->max_cells = std::max(ctx->max_cells, ctx->hg[ctx->species[s].grid].n_cells);
+    ctx->max_nnz = std::max(ctx->max_nnz, ctx->hg[ctx->species[s].grid].nnz);
+  }
+  const Spec3* dsp;
+  const DevGrid3* dgr;
+  if (int rc = upload(ctx, specs, &dsp)) return rc;
+  if (int rc = upload(ctx, ctx->dg, &dgr)) return rc;
+  ctx->d_spec = const_cast<Spec3*>(dsp);
+  ctx->d_grids = const_cast<DevGrid3*>(dgr);
   return LANDAU_OK;
 }
 
@@ -339,14 +354,11 @@ int assemble_chunk(landau3v_ctx* ctx, int b0, int nbc, double inv_dt, double* ou
       cudaFuncSetAttribute(k3v_elem_matrix, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K3E_SMEM);
       ctx->k3e_configured = true;
     }
-    for (int s = 0; s < ctx->S; ++s) {
-      const int g = ctx->species[s].grid;
-      k3v_elem_matrix<<<dim3((ctx->hg[g].n_cells + K3E_WARPS - 1) / K3E_WARPS, nbc), K3E_WARPS * 32, K3E_SMEM, st>>>(
-          ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, ctx->EM, ctx->em_stride, ctx->em_off[s]);
-      k3v_gather<<<dim3((ctx->hg[g].nnz + 255) / 256, nbc), 256, 0, st>>>(ctx->dg[g], ctx->EM, ctx->em_stride, ctx->em_off[s], vals,
-                                                                          ctx->v_stride, ctx->v_off[s]);
-      ctx->launches += 2;
-    }
+    k3v_elem_matrix<<<dim3((ctx->max_cells + K3E_WARPS - 1) / K3E_WARPS, nbc, ctx->S), K3E_WARPS * 32, K3E_SMEM, st>>>(
+        ctx->d_grids, ctx->d_spec, ctx->d_tab, ctx->DK, ctx->dk_stride, inv_dt, ctx->EM, ctx->em_stride);
+    k3v_gather<<<dim3((ctx->max_nnz + 255) / 256, nbc, ctx->S), 256, 0, st>>>(ctx->d_grids, ctx->d_spec, ctx->EM, ctx->em_stride, vals,
+                                                                              ctx->v_stride);
+    ctx->launches += 2;
   }
   nvtxRangePop();
   return LANDAU_OK;

@@ -18,15 +18,24 @@
 
 namespace landau3v {
 
+// one launch covers every species: blockIdx.z picks the species, its grid comes from a device table
+struct Spec3 {
+  int grid;
+  long long dk_off, em_off, v_off;
+};
+
 constexpr int K3E_WARPS = 4;
 // dynamic shared memory of k3v_elem_matrix: tab4 [27][32][4] | rfrag [27][4][32] | coef [warps][27][4][4]
 constexpr size_t K3E_SMEM = (27 * 32 * 4 + 27 * 4 * 32 + K3E_WARPS * 27 * 16) * sizeof(double);
 
-// grid (ceil(n_cells / K3E_WARPS), nbc), K3E_WARPS warps, one cell per warp
-__global__ void __launch_bounds__(K3E_WARPS * 32) k3v_elem_matrix(DevGrid3 g, const Tables3* __restrict__ tab,
-                                                                 const double* __restrict__ DK, long long dk_stride,
-                                                                 long long dk_off, double inv_dt, double* __restrict__ EM,
-                                                                 long long em_stride, long long em_off) {
+// grid (ceil(max n_cells / K3E_WARPS), nbc, S), K3E_WARPS warps, one cell per warp
+__global__ void __launch_bounds__(K3E_WARPS * 32) k3v_elem_matrix(const DevGrid3* __restrict__ grids, const Spec3* __restrict__ spec,
+                                                                 const Tables3* __restrict__ tab, const double* __restrict__ DK,
+                                                                 long long dk_stride, double inv_dt, double* __restrict__ EM,
+                                                                 long long em_stride) {
+  const Spec3 sp = spec[blockIdx.z];
+  const DevGrid3& g = grids[sp.grid];
+  const long long dk_off = sp.dk_off, em_off = sp.em_off;
   extern __shared__ __align__(16) double sm3[];
   double* tab4 = sm3;                      // [q][a (32, zero padded)][B, dBx, dBy, dBz]
   double* rfrag = tab4 + 27 * 32 * 4;      // [q][nt][lane]: R[(q, t)][8 nt + g]
@@ -115,9 +124,13 @@ __global__ void __launch_bounds__(K3E_WARPS * 32) k3v_elem_matrix(DevGrid3 g, co
   }
 }
 
-// grid (ceil(nnz / 256), nbc): one thread per CSR slot
-__global__ void __launch_bounds__(256) k3v_gather(DevGrid3 g, const double* __restrict__ EM, long long em_stride, long long em_off,
-                                                  double* __restrict__ vals, long long v_stride, long long v_off) {
+// grid (ceil(max nnz / 256), nbc, S): one thread per CSR slot
+__global__ void __launch_bounds__(256) k3v_gather(const DevGrid3* __restrict__ grids, const Spec3* __restrict__ spec,
+                                                  const double* __restrict__ EM, long long em_stride, double* __restrict__ vals,
+                                                  long long v_stride) {
+  const Spec3 sp = spec[blockIdx.z];
+  const DevGrid3& g = grids[sp.grid];
+  const long long em_off = sp.em_off, v_off = sp.v_off;
   const int n = blockIdx.x * 256 + threadIdx.x, b = blockIdx.y;
   if (n >= g.nnz) return;
   const double* em = EM + (long long)b * em_stride + em_off;

@@ -486,6 +486,9 @@ constexpr int K2BIG_TC = K2Big::TC;
 // wide variant: 16 x 256 CTA tile (one tensor pair per thread per source tile), 2 B stages
 using K2Wide = K2G<2, 4, 1, 8, 2>;
 
+// narrow variant for 33 .. 96 columns: 16 x 64 CTA tile, 4 warps of 16 x 16, two tensor pairs per thread per source tile
+using K2Narrow = K2G<2, 2, 1, 4, 3>;
+
 // Stream mode of the many-column kernel (k2_gemm.cuh): persistent CTAs, one per SM, when the tiles do not fill whole
 // waves.  It needs every CTA to own at least one (tile, source tile) step of the partial wave: with
 // R = (T mod P) njt < P some shares [R p / P, R (p+1) / P) would be empty and the kernel's part count (which counts CTAs
@@ -510,7 +513,7 @@ template <int WI_T, int WC_T, int WGI, int WGC, int NST>
 int launch_gemm_t(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nsplit, long long split_stride,
                   cudaStream_t st) {
   using C = K2G<WI_T, WC_T, WGI, WGC, NST>;
-  constexpr unsigned bit = 1u << (16 + WGC);
+  constexpr unsigned bit = 1u << (WC_T == 2 ? 28 : 16 + WGC);  // one flag per instantiation (32x128: 20, 16x256: 24, 16x64: 28)
   if (!(ctx->func_configured & bit)) {
     CUDA_TRY(ctx, cudaFuncSetAttribute(k2_inner_gemm<WI_T, WC_T, WGI, WGC, NST>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
@@ -545,14 +548,17 @@ int launch_gemm(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nspl
 }
 
 // column-tile width of the tiled F layout a kernel reads (0: plain layout), field points per CTA
-int kern_tc(int kern) { return kern == 3 ? K2BIG_TC : kern == 4 ? K2Wide::TC : 0; }
-int kern_ti(int kern) { return kern == 3 ? K2Big::TI : kern == 4 ? K2Wide::TI : 0; }
+int kern_tc(int kern) { return kern == 3 ? K2BIG_TC : kern == 4 ? K2Wide::TC : kern == 5 ? K2Narrow::TC : 0; }
+int kern_ti(int kern) { return kern == 3 ? K2Big::TI : kern == 4 ? K2Wide::TI : kern == 5 ? K2Narrow::TI : 0; }
 
-// which inner-integral kernel a group of `ncols` columns takes: 1 DFMA, 2 DMMA (per-warp tensor), 3 / 4 GEMM with the
-// tensor tile shared by the CTA (32 x 128 / 16 x 256 CTA tile)
+// which inner-integral kernel a group of `ncols` columns takes: 1 DFMA, 2 DMMA (per-warp tensor), 3 / 4 / 5 GEMM with the
+// tensor tile shared by the CTA (32 x 128 / 16 x 256 / 16 x 64 CTA tile)
 int pick_kernel(const landau_ctx* ctx, int ncols) {
   if (ctx->inner_kernel) return ctx->inner_kernel;
-  return ncols > 128 ? 4 : ncols > 96 ? 3 : (ncols >= 8 ? 2 : 1);  // crossovers measured on config 2 (N = 4096)
+  // crossovers measured on config 2 (N = 4096).  The 16 x 64 tile pays when its single column tile is full enough and the
+  // field tiles fill the machine (config 2, B = 64: 0.90 -> 0.74 ms; config 3, B = 64 with 192 tiles on 148 SMs: slower)
+  if (ncols > 48 && ncols <= 64 && (ctx->n_i_pad + K2Narrow::TI - 1) / K2Narrow::TI >= (17 * ctx->n_sm) / 10) return 5;
+  return ncols > 128 ? 4 : ncols > 96 ? 3 : (ncols >= 8 ? 2 : 1);
 }
 
 // Column layout, kernel choice, j-split and scratch needs of one pass over `nbc` batch entries.
@@ -604,6 +610,7 @@ ChunkPlan plan_chunk(const landau_ctx* ctx, int nbc) {
     size_t need = 0;
     if (pl.kern[q] == 4) need = gemm_part_need<K2Wide>(ctx, ctx->groups[q], pl.ncols[q], pl.nsplit);
     if (pl.kern[q] == 3) need = gemm_part_need<K2Big>(ctx, ctx->groups[q], pl.ncols[q], pl.nsplit);
+    if (pl.kern[q] == 5) need = gemm_part_need<K2Narrow>(ctx, ctx->groups[q], pl.ncols[q], pl.nsplit);
     pl.part_doubles = std::max(pl.part_doubles, need);
   }
   return pl;
@@ -651,6 +658,8 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
     const Group& gr = ctx->groups[q];
     if (kern[q] == 4) {
       if (int rc = launch_gemm_t<2, 4, 1, 8, 2>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
+    } else if (kern[q] == 5) {
+      if (int rc = launch_gemm_t<2, 2, 1, 4, 3>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
     } else if (kern[q] == 3) {
       if (int rc = launch_gemm(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
     } else if (kern[q] == 2) {
@@ -1295,7 +1304,7 @@ int landau_last_stage_ms(landau_ctx* ctx, float* ms4) {
 }
 
 int landau_set_inner_kernel(landau_ctx* ctx, int which) {
-  if (!ctx || which < 0 || which > 4) return LANDAU_INVALID_ARG;
+  if (!ctx || which < 0 || which > 5) return LANDAU_INVALID_ARG;
   ctx->inner_kernel = which;
   return LANDAU_OK;
 }

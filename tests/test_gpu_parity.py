@@ -95,7 +95,7 @@ def test_tensor_device_vs_oracle(orc, Bn, torch_cuda):
 
 # ------------------------------------------------------------------------------------------------ small, full batch
 @pytest.mark.parametrize("kind,degree", [("uniform", 2), ("uniform", 3), ("quadtree", 2), ("quadtree", 3)])
-@pytest.mark.parametrize("kernel", [1, 2, 3, 4])
+@pytest.mark.parametrize("kernel", [1, 2, 3, 4, 5])
 def test_tiny_jacobian_apply_and_coefficients(orc, Bn, torch_cuda, kind, degree, kernel):
     torch = torch_cuda
     cfg = W.tiny_config(kind, degree, batch=3)
@@ -157,7 +157,7 @@ def test_general_nu_matrix_path(orc, Bn, torch_cuda):
     o, L = _make(orc, Bn, cfg, nu=nu)
     f = W.make_batch_f(cfg, [o.dof_coords(g) for g in range(o.G)], batch=2)
     fd = torch.tensor(f, device="cuda")
-    for kernel in (1, 2, 3, 4):
+    for kernel in (1, 2, 3, 4, 5):
         Bn.landau_set_inner_kernel(L.ctx, kernel)
         vals = L.jacobian(fd, 0.3).cpu().numpy()
         assert _block_errors(L, vals, o.jacobian_batch(f, 0.3), L.v_off).max() < TOL
@@ -263,7 +263,7 @@ def test_config3_ten_species(orc, Bn, torch_cuda, B):
     _config_parity(orc, Bn, torch_cuda, W.config(3), B, _sample_entries(B, 3)[:4], check_apply=(B in (16, 256)))
 
 
-@pytest.mark.parametrize("kernel", [2, 3, 4])
+@pytest.mark.parametrize("kernel", [2, 3, 4, 5])
 @pytest.mark.parametrize("general_nu", [False, True])
 def test_several_species_on_one_grid_forced_kernels(orc, Bn, torch_cuda, kernel, general_nu):
     """Three species on ONE grid + one on a second grid, forced through the tiled-F layouts of the many-column kernels
