@@ -49,6 +49,7 @@ struct landau3v_ctx {
   int dmma_ctas_per_sm[5] = {0, 0, 0, 0, 0};
   int assembly_kernel = 0;  // 0: element matrices on the MMA pipe + gather, 1: per-slot quadrature (first version)
   bool k3e_configured = false;
+  int k3e_ctas_per_sm = 0;
   double *F = nullptr, *Gs = nullptr, *DK = nullptr, *FE = nullptr, *stage_in = nullptr, *stage_out = nullptr;
   size_t F_cap = 0, G_cap = 0, DK_cap = 0, FE_cap = 0, stage_in_cap = 0, stage_out_cap = 0;
   int f_nbc = -1;
@@ -354,8 +355,17 @@ int assemble_chunk(landau3v_ctx* ctx, int b0, int nbc, double inv_dt, double* ou
       cudaFuncSetAttribute(k3v_elem_matrix, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K3E_SMEM);
       ctx->k3e_configured = true;
     }
-    k3v_elem_matrix<<<dim3((ctx->max_cells + K3E_WARPS - 1) / K3E_WARPS, nbc, ctx->S), K3E_WARPS * 32, K3E_SMEM, st>>>(
-        ctx->d_grids, ctx->d_spec, ctx->d_tab, ctx->DK, ctx->dk_stride, inv_dt, ctx->EM, ctx->em_stride);
+    {
+      if (ctx->k3e_ctas_per_sm == 0) {
+        int n = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k3v_elem_matrix, K3E_WARPS * 32, K3E_SMEM);
+        ctx->k3e_ctas_per_sm = n > 0 ? n : 1;
+      }
+      const long long items = (long long)ctx->S * nbc * ctx->max_cells;
+      const int grid = (int)std::max(1LL, std::min<long long>((items + K3E_WARPS - 1) / K3E_WARPS, (long long)ctx->k3e_ctas_per_sm * ctx->n_sm));
+      k3v_elem_matrix<<<grid, K3E_WARPS * 32, K3E_SMEM, st>>>(ctx->d_grids, ctx->d_spec, ctx->S, nbc, ctx->max_cells, ctx->d_tab, ctx->DK,
+                                                              ctx->dk_stride, inv_dt, ctx->EM, ctx->em_stride);
+    }
     k3v_gather<<<dim3((ctx->max_nnz + 255) / 256, nbc, ctx->S), 256, 0, st>>>(ctx->d_grids, ctx->d_spec, ctx->EM, ctx->em_stride, vals,
                                                                               ctx->v_stride);
     ctx->launches += 2;

@@ -25,21 +25,20 @@ struct Spec3 {
 };
 
 constexpr int K3E_WARPS = 4;
-// dynamic shared memory of k3v_elem_matrix: tab4 [27][32][4] | rfrag [27][4][32] | coef [warps][27][4][4]
-constexpr size_t K3E_SMEM = (27 * 32 * 4 + 27 * 4 * 32 + K3E_WARPS * 27 * 16) * sizeof(double);
+// dynamic shared memory of k3v_elem_matrix: tab4 [27][32][4] | coef [warps][27][4][4]
+constexpr size_t K3E_SMEM = (27 * 32 * 4 + K3E_WARPS * 27 * 16) * sizeof(double);
 
-// grid (ceil(max n_cells / K3E_WARPS), nbc, S), K3E_WARPS warps, one cell per warp
+// Persistent grid: every warp strides through the (species, entry, cell) items; the basis table is loaded once per CTA.
+// (The first version started one CTA per four cells and reloaded 55 KB of tables each time.)
 __global__ void __launch_bounds__(K3E_WARPS * 32) k3v_elem_matrix(const DevGrid3* __restrict__ grids, const Spec3* __restrict__ spec,
+                                                                 int n_spec, int nbc, int max_cells,
                                                                  const Tables3* __restrict__ tab, const double* __restrict__ DK,
                                                                  long long dk_stride, double inv_dt, double* __restrict__ EM,
                                                                  long long em_stride) {
-  const Spec3 sp = spec[blockIdx.z];
-  const DevGrid3& g = grids[sp.grid];
-  const long long dk_off = sp.dk_off, em_off = sp.em_off;
   extern __shared__ __align__(16) double sm3[];
-  double* tab4 = sm3;                      // [q][a (32, zero padded)][B, dBx, dBy, dBz]
-  double* rfrag = tab4 + 27 * 32 * 4;      // [q][nt][lane]: R[(q, t)][8 nt + g]
-  double* coef = rfrag + 27 * 4 * 32;      // [warp][q][t][4]
+  double* tab4 = sm3;                  // [q][a (32, zero padded)][B, dBx, dBy, dBz]; also the R fragments: R[(q, t)][8 nt + g]
+                                       // = tab4[q][8 nt + g][t] = tab4[q * 128 + nt * 32 + lane]
+  double* coef = tab4 + 27 * 32 * 4;   // [warp][q][t][4]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gq = lane >> 2, t = lane & 3;
   for (int e = tid; e < 27 * 32; e += K3E_WARPS * 32) {
     const int q = e / 32, a = e % 32;
@@ -49,77 +48,78 @@ __global__ void __launch_bounds__(K3E_WARPS * 32) k3v_elem_matrix(const DevGrid3
     tab4[e * 4 + 2] = ok ? tab->dBy[q * 27 + a] : 0.0;
     tab4[e * 4 + 3] = ok ? tab->dBz[q * 27 + a] : 0.0;
   }
-  for (int e = tid; e < 27 * 4 * 32; e += K3E_WARPS * 32) {
-    const int q = e / 128, nt = (e / 32) % 4, l = e % 32, c = 8 * nt + (l >> 2), k = l & 3;
-    const double* src = k == 0 ? tab->B : k == 1 ? tab->dBx : k == 2 ? tab->dBy : tab->dBz;
-    rfrag[e] = c < 27 ? src[q * 27 + c] : 0.0;
-  }
   __syncthreads();
-  const int cell = blockIdx.x * K3E_WARPS + warp, b = blockIdx.y;
-  if (cell >= g.n_cells) return;
-  // per-cell coefficients: lane q < 27 loads the point's weight, D and K
   double* cw = coef + warp * 27 * 16;
-  if (lane < 27) {
-    const long long N = g.n_ip;
-    const int ip = cell * 27 + lane;
-    const double* dk = DK + (long long)b * dk_stride + dk_off + ip;
-    const double sc = 2.0 / g.cell_h[cell], w = g.ip_w[ip], ws = w * sc, wss = ws * sc;
-    const double dxx = wss * dk[0], dxy = wss * dk[N], dxz = wss * dk[2 * N], dyy = wss * dk[3 * N], dyz = wss * dk[4 * N],
-                 dzz = wss * dk[5 * N];
-    double* c = cw + lane * 16;
-    c[0] = w * inv_dt;
-    c[1] = -ws * dk[6 * N];
-    c[2] = -ws * dk[7 * N];
-    c[3] = -ws * dk[8 * N];
-    c[4] = 0.0;
-    c[5] = dxx;
-    c[6] = dxy;
-    c[7] = dxz;
-    c[8] = 0.0;
-    c[9] = dxy;
-    c[10] = dyy;
-    c[11] = dyz;
-    c[12] = 0.0;
-    c[13] = dxz;
-    c[14] = dyz;
-    c[15] = dzz;
-  }
-  __syncwarp();
-  double acc[4][4][2];
+  const long long n_items = (long long)n_spec * nbc * max_cells;
+  for (long long item = (long long)blockIdx.x * K3E_WARPS + warp; item < n_items; item += (long long)gridDim.x * K3E_WARPS) {
+    const int cell = (int)(item % max_cells), b = (int)((item / max_cells) % nbc), sidx = (int)(item / ((long long)max_cells * nbc));
+    const Spec3 sp = spec[sidx];
+    const DevGrid3& g = grids[sp.grid];
+    if (cell >= g.n_cells) continue;
+    __syncwarp();
+    // per-cell coefficients: lane q < 27 loads the point's weight, D and K
+    if (lane < 27) {
+      const long long N = g.n_ip;
+      const int ip = cell * 27 + lane;
+      const double* dk = DK + (long long)b * dk_stride + sp.dk_off + ip;
+      const double sc = 2.0 / g.cell_h[cell], w = g.ip_w[ip], ws = w * sc, wss = ws * sc;
+      const double dxx = wss * dk[0], dxy = wss * dk[N], dxz = wss * dk[2 * N], dyy = wss * dk[3 * N], dyz = wss * dk[4 * N],
+                   dzz = wss * dk[5 * N];
+      double* c = cw + lane * 16;
+      c[0] = w * inv_dt;
+      c[1] = -ws * dk[6 * N];
+      c[2] = -ws * dk[7 * N];
+      c[3] = -ws * dk[8 * N];
+      c[4] = 0.0;
+      c[5] = dxx;
+      c[6] = dxy;
+      c[7] = dxz;
+      c[8] = 0.0;
+      c[9] = dxy;
+      c[10] = dyy;
+      c[11] = dyz;
+      c[12] = 0.0;
+      c[13] = dxz;
+      c[14] = dyz;
+      c[15] = dzz;
+    }
+    __syncwarp();
+    double acc[4][4][2];
 #pragma unroll
-  for (int mt = 0; mt < 4; ++mt)
+    for (int mt = 0; mt < 4; ++mt)
 #pragma unroll
-    for (int nt = 0; nt < 4; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+      for (int nt = 0; nt < 4; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
 #pragma unroll 1
-  for (int q = 0; q < 27; ++q) {
-    const double2 c01 = *reinterpret_cast<const double2*>(cw + q * 16 + t * 4), c23 = *reinterpret_cast<const double2*>(cw + q * 16 + t * 4 + 2);
-    double l[4];
+    for (int q = 0; q < 27; ++q) {
+      const double2 c01 = *reinterpret_cast<const double2*>(cw + q * 16 + t * 4), c23 = *reinterpret_cast<const double2*>(cw + q * 16 + t * 4 + 2);
+      double l[4];
+#pragma unroll
+      for (int mt = 0; mt < 4; ++mt) {
+        const double* tp = tab4 + (q * 32 + 8 * mt + gq) * 4;
+        const double2 t01 = *reinterpret_cast<const double2*>(tp), t23 = *reinterpret_cast<const double2*>(tp + 2);
+        l[mt] = fma(c01.x, t01.x, fma(c01.y, t01.y, fma(c23.x, t23.x, c23.y * t23.y)));
+      }
+#pragma unroll
+      for (int nt = 0; nt < 4; ++nt) {
+        const double r = tab4[q * 128 + nt * 32 + lane];
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt) dmma3(acc[mt][nt][0], acc[mt][nt][1], l[mt], r);
+      }
+    }
+    // C fragment: lane (g, t) holds A[8 mt + g][8 nt + 2 t + h]
+    double* dst = EM + (long long)b * em_stride + sp.em_off + (long long)cell * 729;
 #pragma unroll
     for (int mt = 0; mt < 4; ++mt) {
-      const double* tp = tab4 + (q * 32 + 8 * mt + gq) * 4;
-      const double2 t01 = *reinterpret_cast<const double2*>(tp), t23 = *reinterpret_cast<const double2*>(tp + 2);
-      l[mt] = fma(c01.x, t01.x, fma(c01.y, t01.y, fma(c23.x, t23.x, c23.y * t23.y)));
-    }
+      const int a = 8 * mt + gq;
+      if (a < 27) {
 #pragma unroll
-    for (int nt = 0; nt < 4; ++nt) {
-      const double r = rfrag[(q * 4 + nt) * 32 + lane];
+        for (int nt = 0; nt < 4; ++nt)
 #pragma unroll
-      for (int mt = 0; mt < 4; ++mt) dmma3(acc[mt][nt][0], acc[mt][nt][1], l[mt], r);
-    }
-  }
-  // C fragment: lane (g, t) holds A[8 mt + g][8 nt + 2 t + h]
-  double* dst = EM + (long long)b * em_stride + em_off + (long long)cell * 729;
-#pragma unroll
-  for (int mt = 0; mt < 4; ++mt) {
-    const int a = 8 * mt + gq;
-    if (a < 27) {
-#pragma unroll
-      for (int nt = 0; nt < 4; ++nt)
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          const int c = 8 * nt + 2 * t + h;
-          if (c < 27) dst[a * 27 + c] = acc[mt][nt][h];
-        }
+          for (int h = 0; h < 2; ++h) {
+            const int c = 8 * nt + 2 * t + h;
+            if (c < 27) dst[a * 27 + c] = acc[mt][nt][h];
+          }
+      }
     }
   }
 }

@@ -160,3 +160,30 @@ def test_ten_species_three_grids(o3, B3):
     rhs = L.apply(fd).cpu().numpy()
     assert _block_errors(L, rhs, o.apply_batch(f), L.f_off).max() < TOL
     L.close()
+
+
+def test_two_levels_and_general_nu_with_shared_grid(o3, B3):
+    """Two nested refinement levels (constraint rows through two shells) and a non-rank-one nu with two species sharing a grid
+    (one source column per (entry, species), zero outside the species' own grid), both inner-integral kernels."""
+    import torch
+    grids = [dict(half=3.0, n=2, levels=2), dict(half=1.0, n=3, levels=1)]
+    species = [dict(mass=1.0, charge=-1.0, grid=0), dict(mass=4.0, charge=1.0, grid=1), dict(mass=9.0, charge=2.0, grid=1)]
+    nu = np.array([[1.0, 2.0, 0.5], [2.0, 3.0, 1.5], [0.5, 1.5, 4.0]])
+    cfg = dict(index=97, species=species, state="shifted", alpha=[1.0] * 3, batch=9, dt=0.4)
+    L = B3.Landau3V(grids, species, nu=nu)
+    o = o3.Oracle3V(grids, species, nu=nu)
+    assert L.n_cells[0] == 120                                          # 8 -> 64 -> 64 - 8 + 64
+    f = W.make_batch_f3v(cfg, [o.dof_coords(g) for g in range(2)], batch=9)
+    fd = torch.tensor(f, device="cuda")
+    pick = [0, 8]
+    ref, ref_rhs = o.jacobian_batch(f[pick], cfg["dt"]), o.apply_batch(f[pick])
+    for kernel in (1, 2):
+        B3.landau3v_set_inner_kernel(L.ctx, kernel)
+        vals, rhs = L.jacobian(fd, cfg["dt"]).cpu().numpy(), L.apply(fd).cpu().numpy()
+        assert _block_errors(L, vals[pick], ref, L.v_off).max() < TOL
+        assert _block_errors(L, rhs[pick], ref_rhs, L.f_off).max() < TOL
+    # the first assembly version (every slot integrates its own entries) agrees with the default one
+    B3.landau3v_set_assembly_kernel(L.ctx, 1)
+    vals1 = L.jacobian(fd, cfg["dt"]).cpu().numpy()
+    assert np.abs(vals1 - vals).max() < 1e-12 * np.abs(vals).max()
+    L.close()
