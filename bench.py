@@ -20,7 +20,8 @@ cores over a bounded sample of the same workload.  Extras that do not enter `val
                  times, K2 and K3 roofline fractions (skip with --no-other-configs)
   solve          the batched TFQMR + Jacobi solve of the step's backward-Euler systems on a bounded sub-batch
                  (148 entries; the whole batch with --solve)
-  advance        `--advance N`: N backward-Euler steps with landau_step (Newton iterations x batch per second)
+  advance        three backward-Euler steps (landau_step) of the paper's 2V throughput problem, Newton iterations x batch per
+                 second; `--advance N`: N steps of the headline workload instead
 
 `--gpus N` without a torchrun environment starts N ranks itself (one per GPU; NCCL for the barrier and the max-reduce
 only: batch entries are independent); `--dry-run` exercises that plumbing without a GPU (gloo).
@@ -406,6 +407,33 @@ def other_config_runs(local, dev, fp64_peak, prof, skip):
     return rows
 
 
+def advance_run(local, dev, steps=3):
+    """The implicit advance the path belongs to, bounded: `steps` backward-Euler steps (landau_step: quasi-Newton on the
+    sparse Jacobian, batched TFQMR) of the paper's own 2V throughput problem (config 6: ten species, three grids of 14 Q3
+    cells, batch 256; Table 5).  Newton iterations x batch per second is the paper's throughput measure
+    (PAPER.md:119)."""
+    import torch
+    cfg, dim = load_config(6)
+    B = cfg["batch"]
+    P = Problem(cfg, dim, local)
+    Bn = P.Bn
+    f = torch.from_numpy(P.make_f(cfg, P.coords(), batch=B)).to(dev)
+    u = f.clone()
+    Bn.landau_step(P.L.ctx, u, B, cfg["dt"], 1e-8, 50, 1e-10, 2000)          # warm-up (scratch, mass values)
+    u.copy_(f)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    newton, info = 0, None
+    for k in range(steps):
+        info = Bn.landau_step(P.L.ctx, u, B, cfg["dt"], 1e-8, 50, 1e-10, 2000)
+        newton += info["newton_its"]
+    torch.cuda.synchronize()
+    t_adv = time.perf_counter() - t0
+    P.close()
+    return {"workload": workload_name(cfg, B), "steps": steps, "dt": cfg["dt"], "seconds": t_adv, "newton_iterations": newton,
+            "newton_rtol": 1e-8, "lin_rtol": 1e-10, "last": info, "newton_iterations_x_batch_per_s": newton * B / t_adv}
+
+
 def solve_run(P, B, f_dev0, out_dev, dev, whole):
     """The step after the hot path: backward-Euler systems (M/dt - J) x = (M/dt) f of a bounded
     sub-batch, TFQMR + Jacobi, one system per CTA."""
@@ -607,6 +635,11 @@ def run_ours(args):
     if rank == 0:
         if not args.no_other_configs and world == 1:
             line["other_configs"] = other_config_runs(local, dev, peak, prof, (args.config, B))
+            if line["advance"] is None:
+                try:
+                    line["advance"] = advance_run(local, dev)
+                except Exception as e:  # an extra must not take the headline number with it
+                    line["advance"] = {"error": repr(e)[:200]}
         print(json.dumps(line), flush=True)
     if world > 1:
         import torch.distributed as dist
