@@ -67,7 +67,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="skip the short runs of the other configs")
     ap.add_argument("--no-solve", action="store_true", help="skip the bounded TFQMR solve")
-    ap.add_argument("--kernel", type=int, default=0, help="inner-integral kernel: 0 auto, 1 DFMA, 2 DMMA, 3/4 GEMM (32x128 / 16x256 tile)")
+    ap.add_argument("--kernel", type=int, default=0, help="inner-integral kernel: 0 auto, 1 DFMA, 2 DMMA, 3/4/5 GEMM (16x128 / 16x256 / 16x64 tile)")
     ap.add_argument("--solve", action="store_true", help="time the batched TFQMR solve on the WHOLE batch (default: 148 entries)")
     ap.add_argument("--advance", type=int, default=0, help="also run this many backward-Euler steps (landau_step) and "
                     "report the time and Newton iterations under \"advance\" (not part of value)")

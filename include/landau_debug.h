@@ -51,8 +51,9 @@ int landau_last_stage_ms(landau_ctx* ctx, float* ms4);
 
 /* Choose the inner-integral kernel: 0 auto (by column count), 1 plain DFMA kernel, 2 DMMA kernel with per-warp
  * tensor generation, 3 / 4 DMMA GEMM kernel with the tensor tile evaluated once per CTA and shared by its warps
- * (TMA-staged source tiles; 32 x 128 / 16 x 256 CTA tile: 4 is the default for more than 128 source columns), 5 the same
- * with a 16 x 64 tile (default for 49 .. 64 columns when the field tiles fill the machine). */
+ * (TMA-staged source tiles; 16 x 128 / 16 x 256 CTA tile: defaults for 65 .. 128 and for more than 128 source columns), 5 the
+ * same with a 16 x 64 tile (default for 49 .. 64 columns).  The three run as persistent CTAs that cut the tiles of the last
+ * partial wave along the source range whenever the tile count is not a multiple of the resident CTAs. */
 int landau_set_inner_kernel(landau_ctx* ctx, int which);
 
 /* Choose the element-matrix + assembly kernel: 0 auto (k3_ring: DMMA sum-factorised element matrices kept in a

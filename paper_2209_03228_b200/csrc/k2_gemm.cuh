@@ -44,6 +44,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 
 template <int WI_T, int WC_T, int WGI, int WGC, int NST>
 struct K2G {
+  static constexpr int P_WI_T = WI_T, P_WC_T = WC_T, P_WGI = WGI, P_WGC = WGC, P_NST = NST;
   static constexpr int NTHREADS = 32 * WGI * WGC;
   static constexpr int TI = 8 * WI_T * WGI;
   static constexpr int TC = 8 * WC_T * WGC;

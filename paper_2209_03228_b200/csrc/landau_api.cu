@@ -479,31 +479,50 @@ int launch_dmma(landau_ctx* ctx, const Group& gr, int ncols, int ncols_pad, int 
   return LANDAU_OK;
 }
 
-// many-column kernel (k2_gemm.cuh): TI=32 x TC=128 CTA tile, 8 warps of 16 x 32
-using K2Big = K2G<2, 4, 2, 4, 3>;
+// many-column kernel (k2_gemm.cuh): TI=16 x TC=128 CTA tile, 8 warps of 16 x 16 (one tensor pair per thread per source tile)
+#ifndef K2BIG_ARGS
+#define K2BIG_ARGS 2, 2, 1, 8, 3
+#endif
+using K2Big = K2G<K2BIG_ARGS>;
 constexpr int K2BIG_TC = K2Big::TC;
 
 // wide variant: 16 x 256 CTA tile (one tensor pair per thread per source tile), 2 B stages
 using K2Wide = K2G<2, 4, 1, 8, 2>;
 
-// narrow variant for 33 .. 96 columns: 16 x 64 CTA tile, 4 warps of 16 x 16, two tensor pairs per thread per source tile
-using K2Narrow = K2G<2, 2, 1, 4, 3>;
+// narrow variant for 49 .. 64 columns: 16 x 64 CTA tile, 4 warps of 16 x 16, two tensor pairs per thread per source tile; two CTAs per SM
+#ifndef K2NARROW_ARGS
+#define K2NARROW_ARGS 2, 2, 1, 4, 3
+#endif
+using K2Narrow = K2G<K2NARROW_ARGS>;
 
-// Stream mode of the many-column kernel (k2_gemm.cuh): persistent CTAs, one per SM, when the tiles do not fill whole
+// Stream mode of the many-column kernel (k2_gemm.cuh): persistent CTAs, as many as are resident, when the tiles do not fill whole
 // waves.  It needs every CTA to own at least one (tile, source tile) step of the partial wave: with
 // R = (T mod P) njt < P some shares [R p / P, R (p+1) / P) would be empty and the kernel's part count (which counts CTAs
 // first..last) would never be reached -- such shapes run in grid mode.
+// persistent CTAs of a stream-mode launch: as many as are resident at once (registers / shared memory of the variant)
+template <class C>
+int gemm_stream_ctas(const landau_ctx* ctx) {
+  static int per_sm[64] = {0};
+  int& n = per_sm[ctx->device & 63];
+  if (!n) {
+    auto* kern = k2_inner_gemm<C::P_WI_T, C::P_WC_T, C::P_WGI, C::P_WGC, C::P_NST>;
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, C::NTHREADS, C::SMEM_BYTES) != cudaSuccess || n < 1) n = 1;
+  }
+  return n * ctx->n_sm;
+}
 template <class C>
 bool gemm_stream_mode(const landau_ctx* ctx, const Group& gr, int ncols, int nsplit) {
-  const int n_it = (ctx->n_i_pad + C::TI - 1) / C::TI, n_ct = (ncols + C::TC - 1) / C::TC, T = n_it * n_ct, P = ctx->n_sm;
-  return ctx->stream_k && nsplit == 1 && T >= P && T % P != 0 && (long long)(T % P) * (gr.nj_pad / K2G_TJ) >= P;
+  const int n_it = (ctx->n_i_pad + C::TI - 1) / C::TI, n_ct = (ncols + C::TC - 1) / C::TC, T = n_it * n_ct;
+  const int P = gemm_stream_ctas<C>(ctx);
+  return ctx->stream_k && nsplit == 1 && T % P != 0 && (long long)(T % P) * (gr.nj_pad / K2G_TJ) >= P;
 }
 // doubles of part_buf a stream-mode launch needs (accumulator dumps of the cut tiles + their arrival counters)
 template <class C>
 size_t gemm_part_need(const landau_ctx* ctx, const Group& gr, int ncols, int nsplit, int* part_stride_out = nullptr) {
   if (!gemm_stream_mode<C>(ctx, gr, ncols, nsplit)) return 0;
   const int n_it = (ctx->n_i_pad + C::TI - 1) / C::TI, n_ct = (ncols + C::TC - 1) / C::TC;
-  const int T = n_it * n_ct, P = ctx->n_sm, r = T % P;
+  const int T = n_it * n_ct, P = gemm_stream_ctas<C>(ctx), r = T % P;
   const int part_stride = (P + r - 1) / r + 2;  // parts per cut tile, upper bound
   if (part_stride_out) *part_stride_out = part_stride;
   return (size_t)r * part_stride * C::ACC_PER_THREAD * C::NTHREADS + (size_t)(P + 1) / 2 + 1;
@@ -513,17 +532,19 @@ template <int WI_T, int WC_T, int WGI, int WGC, int NST>
 int launch_gemm_t(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nsplit, long long split_stride,
                   cudaStream_t st) {
   using C = K2G<WI_T, WC_T, WGI, WGC, NST>;
-  constexpr unsigned bit = 1u << (WC_T == 2 ? 28 : 16 + WGC);  // one flag per instantiation (32x128: 20, 16x256: 24, 16x64: 28)
-  if (!(ctx->func_configured & bit)) {
+  // the limit belongs to the device's copy of this instantiation and its size is fixed: raise it once per device
+  static unsigned long long configured_devices = 0;
+  const unsigned long long bit = 1ull << (ctx->device & 63);
+  if (!(configured_devices & bit)) {
     CUDA_TRY(ctx, cudaFuncSetAttribute(k2_inner_gemm<WI_T, WC_T, WGI, WGC, NST>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
-    ctx->func_configured |= bit;
+    configured_devices |= bit;
   }
   const int n_it = (ctx->n_i_pad + C::TI - 1) / C::TI, n_ct = (ncols + C::TC - 1) / C::TC;
   if (gemm_stream_mode<C>(ctx, gr, ncols, nsplit)) {
     // whole tiles for the full waves, the tiles of the last partial wave cut evenly over all CTAs; parts of a cut tile
     // meet in part_buf and are added in part order by the last CTA to arrive (k2_gemm.cuh)
-    const int T = n_it * n_ct, P = ctx->n_sm, r = T % P;
+    const int T = n_it * n_ct, P = gemm_stream_ctas<C>(ctx), r = T % P;
     int part_stride = 0;
     const size_t need = gemm_part_need<C>(ctx, gr, ncols, nsplit, &part_stride);
     if (int rc = grow(ctx, &ctx->part_buf, &ctx->part_cap, need, false)) return rc;
@@ -544,7 +565,7 @@ int launch_gemm_t(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int ns
 
 int launch_gemm(landau_ctx* ctx, const Group& gr, int ncols, int gcol0, int nsplit, long long split_stride,
                 cudaStream_t st) {
-  return launch_gemm_t<2, 4, 2, 4, 3>(ctx, gr, ncols, gcol0, nsplit, split_stride, st);
+  return launch_gemm_t<K2BIG_ARGS>(ctx, gr, ncols, gcol0, nsplit, split_stride, st);
 }
 
 // column-tile width of the tiled F layout a kernel reads (0: plain layout), field points per CTA
@@ -552,13 +573,15 @@ int kern_tc(int kern) { return kern == 3 ? K2BIG_TC : kern == 4 ? K2Wide::TC : k
 int kern_ti(int kern) { return kern == 3 ? K2Big::TI : kern == 4 ? K2Wide::TI : kern == 5 ? K2Narrow::TI : 0; }
 
 // which inner-integral kernel a group of `ncols` columns takes: 1 DFMA, 2 DMMA (per-warp tensor), 3 / 4 / 5 GEMM with the
-// tensor tile shared by the CTA (32 x 128 / 16 x 256 / 16 x 64 CTA tile)
+// tensor tile shared by the CTA (16 x 128 / 16 x 256 / 16 x 64 CTA tile)
 int pick_kernel(const landau_ctx* ctx, int ncols) {
   if (ctx->inner_kernel) return ctx->inner_kernel;
-  // crossovers measured on config 2 (N = 4096).  The 16 x 64 tile pays when its single column tile is full enough and the
-  // field tiles fill the machine (config 2, B = 64: 0.90 -> 0.74 ms; config 3, B = 64 with 192 tiles on 148 SMs: slower)
-  if (ncols > 48 && ncols <= 64 && (ctx->n_i_pad + K2Narrow::TI - 1) / K2Narrow::TI >= (17 * ctx->n_sm) / 10) return 5;
-  return ncols > 128 ? 4 : ncols > 96 ? 3 : (ncols >= 8 ? 2 : 1);
+  // crossovers measured on configs 2-5 at B = 32 .. 256 (profiles/r2_launches.md): a CTA-shared tensor tile pays as soon as
+  // its column tile is three quarters full
+  if (ncols > 128) return 4;
+  if (ncols > 64) return 3;
+  if (ncols > 48) return 5;
+  return ncols >= 8 ? 2 : 1;
 }
 
 // Column layout, kernel choice, j-split and scratch needs of one pass over `nbc` batch entries.
@@ -589,10 +612,15 @@ ChunkPlan plan_chunk(const landau_ctx* ctx, int nbc) {
     pl.gcol0[q] = pl.total_cols;
     pl.total_cols += pl.ncols[q];
   }
-  // j-split so that small problems still fill the machine
+  // j-split so that small problems still fill the machine (groups whose kernel runs in stream mode cut their tiles
+  // along j themselves and need none)
   int max_blocks = 1 << 30;
   for (size_t q = 0; q < nq; ++q) {
     const int k = pl.kern[q];
+    const Group& gr = ctx->groups[q];
+    if ((k == 3 && gemm_stream_mode<K2Big>(ctx, gr, pl.ncols[q], 1)) || (k == 4 && gemm_stream_mode<K2Wide>(ctx, gr, pl.ncols[q], 1)) ||
+        (k == 5 && gemm_stream_mode<K2Narrow>(ctx, gr, pl.ncols[q], 1)))
+      continue;
     const int blocks = k >= 3   ? ((ctx->n_i_pad + kern_ti(k) - 1) / kern_ti(k)) * (pl.ncols_pad[q] / kern_tc(k))
                        : k == 2 ? ((ctx->n_i_pad + 63) / 64) * ((pl.ncols[q] + 63) / 64)
                                 : ((ctx->n_i_pad + 127) / 128) * ((pl.ncols[q] + 3) / 4);
@@ -659,7 +687,7 @@ int run_coefficients(landau_ctx* ctx, const double* batch_f, int b0, int nbc, cu
     if (kern[q] == 4) {
       if (int rc = launch_gemm_t<2, 4, 1, 8, 2>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
     } else if (kern[q] == 5) {
-      if (int rc = launch_gemm_t<2, 2, 1, 4, 3>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
+      if (int rc = launch_gemm_t<K2NARROW_ARGS>(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
     } else if (kern[q] == 3) {
       if (int rc = launch_gemm(ctx, gr, ncols[q], gcol0[q], nsplit, split_stride, st)) return rc;
     } else if (kern[q] == 2) {

@@ -267,7 +267,7 @@ def test_config3_ten_species(orc, Bn, torch_cuda, B):
 @pytest.mark.parametrize("general_nu", [False, True])
 def test_several_species_on_one_grid_forced_kernels(orc, Bn, torch_cuda, kernel, general_nu):
     """Three species on ONE grid + one on a second grid, forced through the tiled-F layouts of the many-column kernels
-    (3: 32 x 128, 4: 16 x 256) and the plain layout (2): the species mix of K1 (rank-one nu) and the per-species columns
+    (3: 16 x 128, 4: 16 x 256) and the plain layout (2): the species mix of K1 (rank-one nu) and the per-species columns
     (general nu) in every F layout, full batch against the oracle."""
     torch = torch_cuda
     cfg = W.tiny_config("quadtree", 3, batch=5)
@@ -363,6 +363,14 @@ def test_many_column_kernel_partial_wave_smaller_than_the_machine(orc, Bn, torch
     ref = np.stack([o.jacobian(f[b], 0.5) for b in entries])
     assert _block_errors(L, vals[entries].cpu().numpy(), ref, L.v_off).max() < TOL
     L.close()
+
+
+@pytest.mark.parametrize("cfg_no,B", [(4, 64), (4, 128), (3, 64), (2, 128)])
+def test_stream_mode_with_fewer_tiles_than_resident_ctas(orc, Bn, torch_cuda, cfg_no, B):
+    """The persistent many-column kernels cut their tiles along the source range also when there are FEWER tiles than
+    resident CTAs (config 4: 208 field tiles on 2 x 148 CTAs of the 16 x 64 kernel, every tile is shared by two or three
+    CTAs whose parts are added in part order) -- sampled entries against the oracle."""
+    _config_parity(orc, Bn, torch_cuda, W.config(cfg_no), B, _sample_entries(B, cfg_no)[:3], check_apply=False)
 
 
 def test_two_contexts_of_different_sizes_alternate(orc, Bn, torch_cuda):
