@@ -66,6 +66,23 @@ int landau3v_jacobian(landau3v_ctx* ctx, const double* batch_f_dev, int batch, d
                       void* cuda_stream);
 /* rhs = J[f] f  (M df/dt = rhs). */
 int landau3v_apply(landau3v_ctx* ctx, const double* batch_f_dev, int batch, double* out_rhs_dev, void* cuda_stream);
+/* Both from ONE evaluation of the inner integral (what a Newton iteration needs). */
+int landau3v_jacobian_apply(landau3v_ctx* ctx, const double* batch_f_dev, int batch, double dt, double* out_csr_vals_dev,
+                            double* out_rhs_dev, void* cuda_stream);
+
+/* The steps after the path, as for the 2V variant (landau.h: landau_spmv, landau_solve, landau_step; PAPER.md:75-77,
+ * 115-117) on the 3V patterns -- same kernels, same argument meaning: y = A x per (entry, species) block; Jacobi-
+ * preconditioned TFQMR, one system per CTA and one launch for the batch (x_dev: initial guess on input; iters_dev /
+ * relres_dev: [batch][species] or NULL, negative count = tolerance missed); one backward-Euler step
+ * (M/dt - J[u]) delta = M (u^k - u)/dt + J[u] u, u <- u + delta by the quasi-Newton iteration, info_host = 4 doubles or
+ * NULL (Newton iterations, last largest relative update, most half-steps of any system, unconverged solves). */
+int landau3v_spmv(landau3v_ctx* ctx, const double* csr_vals_dev, const double* x_dev, int batch, double* y_dev,
+                  void* cuda_stream);
+int landau3v_solve(landau3v_ctx* ctx, const double* csr_vals_dev, const double* rhs_dev, int batch, double rtol, int max_it,
+                   double* x_dev, int* iters_dev, double* relres_dev, void* cuda_stream);
+int landau3v_step(landau3v_ctx* ctx, double* u_dev, int batch, double dt, double newton_rtol, int max_newton,
+                  double lin_rtol, int lin_max_it, double* info_host, void* cuda_stream);
+
 /* Same with HOST buffers (copies inside the call, synchronous on return). */
 int landau3v_jacobian_host(landau3v_ctx* ctx, const double* batch_f_host, int batch, double dt, double* out_csr_vals_host,
                            void* cuda_stream);

@@ -14,7 +14,8 @@ LandauError = _b.LandauError
 # every symbol include/landau3v.h declares (tests check the header, this list and the library's exports against each other)
 SYMBOLS = ["landau3v_create", "landau3v_destroy", "landau3v_sizes", "landau3v_dof_coords", "landau3v_ip_table",
            "landau3v_csr_pattern", "landau3v_csr_pattern_host", "landau3v_jacobian", "landau3v_apply",
-           "landau3v_jacobian_host", "landau3v_last_coefficients", "landau3v_set_timing", "landau3v_last_stage_ms",
+           "landau3v_jacobian_host", "landau3v_jacobian_apply", "landau3v_spmv", "landau3v_solve", "landau3v_step",
+           "landau3v_last_coefficients", "landau3v_set_timing", "landau3v_last_stage_ms",
            "landau3v_launch_count", "landau3v_set_inner_kernel", "landau3v_set_assembly_kernel", "landau3v_set_batch_chunk",
            "landau3v_last_error"]
 
@@ -102,6 +103,32 @@ def landau3v_jacobian(ctx, batch_f, batch, dt, out, stream=None):
 
 def landau3v_apply(ctx, batch_f, batch, out, stream=None):
     _check(load().landau3v_apply(ctx, _b._dev_ptr(batch_f), C.c_int(batch), _b._dev_ptr(out), _b._stream(stream)), ctx)
+
+
+def landau3v_jacobian_apply(ctx, batch_f, batch, dt, out_csr_vals, out_rhs, stream=None):
+    _check(load().landau3v_jacobian_apply(ctx, _b._dev_ptr(batch_f), C.c_int(batch), C.c_double(dt), _b._dev_ptr(out_csr_vals),
+                                          _b._dev_ptr(out_rhs), _b._stream(stream)), ctx)
+
+
+def landau3v_spmv(ctx, csr_vals, x, batch, y, stream=None):
+    _check(load().landau3v_spmv(ctx, _b._dev_ptr(csr_vals), _b._dev_ptr(x), C.c_int(batch), _b._dev_ptr(y), _b._stream(stream)), ctx)
+
+
+def landau3v_solve(ctx, csr_vals, rhs, batch, rtol, max_it, x, iters=None, relres=None, stream=None):
+    """x: initial guess in, solution out.  iters (int32 CUDA tensor [batch, S]) / relres (float64) optional."""
+    ip = C.c_void_p(iters.data_ptr()) if iters is not None else None
+    rp = C.c_void_p(relres.data_ptr()) if relres is not None else None
+    _check(load().landau3v_solve(ctx, _b._dev_ptr(csr_vals), _b._dev_ptr(rhs), C.c_int(batch), C.c_double(rtol), C.c_int(max_it),
+                                 _b._dev_ptr(x), ip, rp, _b._stream(stream)), ctx)
+
+
+def landau3v_step(ctx, u, batch, dt, newton_rtol, max_newton, lin_rtol, lin_max_it, stream=None):
+    """u: u^k in, u^{k+1} out.  Returns dict(newton_its, last_update, lin_half_steps_max, lin_failed)."""
+    info = (C.c_double * 4)()
+    _check(load().landau3v_step(ctx, _b._dev_ptr(u), C.c_int(batch), C.c_double(dt), C.c_double(newton_rtol), C.c_int(max_newton),
+                                C.c_double(lin_rtol), C.c_int(lin_max_it), info, _b._stream(stream)), ctx)
+    return dict(newton_its=int(info[0]), last_update=float(info[1]), lin_half_steps_max=int(info[2]),
+                lin_failed=int(info[3]))
 
 
 def landau3v_jacobian_host(ctx, batch_f_host, batch, dt, out_host, stream=None):
@@ -198,6 +225,34 @@ class Landau3V:
             out = torch.empty((B, self.f_stride), dtype=torch.float64, device=batch_f.device)
         landau3v_apply(self.ctx, batch_f, B, out, stream)
         return out
+
+    def jacobian_apply(self, batch_f, dt, stream=None):
+        import torch
+        B = batch_f.shape[0]
+        vals = torch.empty((B, self.csr_stride), dtype=torch.float64, device=batch_f.device)
+        rhs = torch.empty((B, self.f_stride), dtype=torch.float64, device=batch_f.device)
+        landau3v_jacobian_apply(self.ctx, batch_f, B, dt, vals, rhs, stream)
+        return vals, rhs
+
+    def spmv(self, csr_vals, x, stream=None):
+        import torch
+        y = torch.empty_like(x)
+        landau3v_spmv(self.ctx, csr_vals, x, x.shape[0], y, stream)
+        return y
+
+    def solve(self, csr_vals, rhs, rtol=1e-10, max_it=200, x0=None, stream=None):
+        """Returns (x, half-steps [B, S] int32, residual bounds [B, S])."""
+        import torch
+        B = rhs.shape[0]
+        x = torch.zeros_like(rhs) if x0 is None else x0.clone()
+        iters = torch.zeros((B, self.S), dtype=torch.int32, device=rhs.device)
+        relres = torch.zeros((B, self.S), dtype=torch.float64, device=rhs.device)
+        landau3v_solve(self.ctx, csr_vals, rhs, B, rtol, max_it, x, iters, relres, stream)
+        return x, iters, relres
+
+    def step(self, u, dt, newton_rtol=1e-10, max_newton=50, lin_rtol=1e-12, lin_max_it=1000, stream=None):
+        """Backward-Euler step in place (u: [B, f_stride] CUDA float64)."""
+        return landau3v_step(self.ctx, u, u.shape[0], dt, newton_rtol, max_newton, lin_rtol, lin_max_it, stream)
 
     def last_coefficients(self, batch):
         """list over species of arrays [batch, 9, n_ip]."""

@@ -5,8 +5,8 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblandau_b200.so")
-SOURCES = ["landau_api.cu", "host_setup.cpp", "landau3v_api.cu", "host_setup3v.cpp"]
-DEPS = SOURCES + ["landau3v_kernels.cuh", "landau3v_dmma.cuh", "landau3v_k3.cuh", "host_setup3v.hpp", os.path.join("..", "..", "include", "landau3v.h"), "landau_kernels.cuh", "k2_gemm.cuh", "k3_ring.cuh", "k4_solve.cuh", "host_setup.hpp", "ellip_coeffs.h", os.path.join("..", "..", "include", "landau.h"),
+SOURCES = ["landau_api.cu", "host_setup.cpp", "landau3v_api.cu", "host_setup3v.cpp", "batch_solver.cu"]
+DEPS = SOURCES + ["batch_solver.hpp", "landau3v_kernels.cuh", "landau3v_dmma.cuh", "landau3v_k3.cuh", "host_setup3v.hpp", os.path.join("..", "..", "include", "landau3v.h"), "landau_kernels.cuh", "k2_gemm.cuh", "k3_ring.cuh", "k4_solve.cuh", "host_setup.hpp", "ellip_coeffs.h", os.path.join("..", "..", "include", "landau.h"),
         os.path.join("..", "..", "include", "landau_debug.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
               "-shared", "-ldl"]

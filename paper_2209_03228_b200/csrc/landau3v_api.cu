@@ -8,6 +8,7 @@
 #include <nvtx3/nvToolsExt.h>
 
 #include "../../include/landau3v.h"
+#include "batch_solver.hpp"
 #include "host_setup3v.hpp"
 #include "landau3v_kernels.cuh"
 #include "landau3v_dmma.cuh"
@@ -59,6 +60,10 @@ struct landau3v_ctx {
   std::vector<cudaEvent_t> ev;
   int ev_used = 0;
   long long launches = 0;
+  // batched solve and implicit step (batch_solver.hpp); mass values of one entry, computed at the first landau3v_step
+  landau::BatchSolver solver;
+  double* st_M = nullptr;
+  size_t st_M_cap = 0;
   std::string err;
 };
 
@@ -258,6 +263,14 @@ int build_device_side(landau3v_ctx* ctx) {
   if (int rc = upload(ctx, ctx->dg, &dgr)) return rc;
   ctx->d_spec = const_cast<Spec3*>(dsp);
   ctx->d_grids = const_cast<DevGrid3*>(dgr);
+  // batched solve: pattern views per grid, block offsets per species
+  std::vector<landau::SolverGridView> gv(ctx->G);
+  for (int g = 0; g < ctx->G; ++g)
+    gv[g] = landau::SolverGridView{ctx->hg[g].n_dof, ctx->hg[g].nnz, ctx->d_rowptr[g], ctx->d_colidx[g], ctx->hg[g].diag.data()};
+  std::vector<landau::SolverSpeciesView> sv(S);
+  for (int s = 0; s < S; ++s) sv[s] = landau::SolverSpeciesView{ctx->species[s].grid, ctx->f_off[s], ctx->v_off[s]};
+  if (int rc = landau::solver_create(ctx->solver, ctx->device, gv, sv, ctx->f_stride, ctx->v_stride))
+    return fail(ctx, rc, ctx->solver.err);
   return LANDAU_OK;
 }
 
@@ -468,7 +481,8 @@ void landau3v_destroy(landau3v_ctx* ctx) {
     cudaDeviceSynchronize();
   }
   for (void* p : ctx->allocs) cudaFree(p);
-  for (double* p : {ctx->F, ctx->Gs, ctx->DK, ctx->FE, ctx->EM, ctx->stage_in, ctx->stage_out})
+  landau::solver_destroy(ctx->solver);
+  for (double* p : {ctx->F, ctx->Gs, ctx->DK, ctx->FE, ctx->EM, ctx->stage_in, ctx->stage_out, ctx->st_M})
     if (p) cudaFree(p);
   for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
   delete ctx;
@@ -554,6 +568,77 @@ int landau3v_apply(landau3v_ctx* ctx, const double* batch_f_dev, int batch, doub
   return LANDAU_OK;
 }
 
+int landau3v_jacobian_apply(landau3v_ctx* ctx, const double* batch_f_dev, int batch, double dt, double* out_csr_vals_dev,
+                            double* out_rhs_dev, void* cuda_stream) {
+  if (int rc = check_call(ctx, batch_f_dev, batch, out_csr_vals_dev)) return rc;
+  if (batch > 0 && !out_rhs_dev) return fail(ctx, LANDAU_INVALID_ARG, "null buffer");
+  if (!(dt > 0)) return fail(ctx, LANDAU_INVALID_ARG, "dt must be > 0 (use +inf for the unshifted -J)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const double inv_dt = std::isinf(dt) ? 0.0 : 1.0 / dt;
+  ctx->ev_used = 0;
+  for (int b0 = 0; b0 < batch; b0 += ctx->chunk) {
+    const int nbc = std::min(ctx->chunk, batch - b0);
+    if (int rc = run_coefficients(ctx, batch_f_dev, b0, nbc, st)) return rc;
+    if (int rc = assemble_chunk(ctx, b0, nbc, inv_dt, out_csr_vals_dev, st)) return rc;
+    if (int rc = apply_chunk(ctx, batch_f_dev, b0, nbc, out_rhs_dev, st)) return rc;
+    CUDA_TRY3(ctx, cudaGetLastError());
+    mark(ctx, st);
+    ctx->last_batch = nbc;
+  }
+  ctx->last_stream = st;
+  return LANDAU_OK;
+}
+
+int landau3v_spmv(landau3v_ctx* ctx, const double* csr_vals_dev, const double* x_dev, int batch, double* y_dev,
+                  void* cuda_stream) {
+  if (int rc = check_call(ctx, csr_vals_dev, batch, y_dev)) return rc;
+  if (batch > 0 && !x_dev) return fail(ctx, LANDAU_INVALID_ARG, "null buffer");
+  if (batch == 0) return LANDAU_OK;
+  if (int rc = landau::solver_spmv(ctx->solver, csr_vals_dev, ctx->v_stride, x_dev, batch, y_dev, (cudaStream_t)cuda_stream))
+    return fail(ctx, rc, ctx->solver.err);
+  return LANDAU_OK;
+}
+
+int landau3v_solve(landau3v_ctx* ctx, const double* csr_vals_dev, const double* rhs_dev, int batch, double rtol, int max_it,
+                   double* x_dev, int* iters_dev, double* relres_dev, void* cuda_stream) {
+  if (int rc = check_call(ctx, csr_vals_dev, batch, x_dev)) return rc;
+  if (batch > 0 && !rhs_dev) return fail(ctx, LANDAU_INVALID_ARG, "null buffer");
+  if (!(rtol > 0) || max_it < 1) return fail(ctx, LANDAU_INVALID_ARG, "rtol must be > 0 and max_it >= 1");
+  if (batch == 0) return LANDAU_OK;
+  if (int rc = landau::solver_tfqmr(ctx->solver, csr_vals_dev, rhs_dev, batch, rtol, max_it, x_dev, iters_dev, relres_dev,
+                                    (cudaStream_t)cuda_stream))
+    return fail(ctx, rc, ctx->solver.err);
+  return LANDAU_OK;
+}
+
+int landau3v_step(landau3v_ctx* ctx, double* u_dev, int batch, double dt, double newton_rtol, int max_newton,
+                  double lin_rtol, int lin_max_it, double* info_host, void* cuda_stream) {
+  if (int rc = check_call(ctx, u_dev, batch, u_dev)) return rc;
+  if (!(dt > 0) || std::isinf(dt) || max_newton < 1 || !(lin_rtol > 0) || lin_max_it < 1)
+    return fail(ctx, LANDAU_INVALID_ARG, "landau3v_step: dt finite > 0, max_newton >= 1, lin_rtol > 0, lin_max_it >= 1");
+  if (info_host) info_host[0] = info_host[1] = info_host[2] = info_host[3] = 0.0;
+  if (batch == 0) return LANDAU_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // mass values (independent of f and of the entry): M = (M/1 - J[0]) since D = K = 0 for f = 0
+  if (!ctx->st_M) {
+    if (int rc = grow(ctx, &ctx->st_M, &ctx->st_M_cap, (size_t)ctx->v_stride + ctx->f_stride)) return rc;
+    double* zero_f = ctx->st_M + ctx->v_stride;
+    CUDA_TRY3(ctx, cudaMemsetAsync(zero_f, 0, sizeof(double) * ctx->f_stride, st));
+    const bool timing = ctx->timing;
+    ctx->timing = false;
+    const int rc = landau3v_jacobian(ctx, zero_f, 1, 1.0, ctx->st_M, cuda_stream);
+    ctx->timing = timing;
+    if (rc) return rc;
+  }
+  const landau::JacobianApplyFn jac = [&](const double* u, int nb, double step, double* A, double* ju) {
+    return landau3v_jacobian_apply(ctx, u, nb, step, A, ju, cuda_stream);
+  };
+  if (int rc = landau::solver_step(ctx->solver, jac, ctx->st_M, u_dev, batch, dt, newton_rtol, max_newton, lin_rtol, lin_max_it,
+                                   info_host, st))
+    return ctx->solver.err.empty() ? rc : fail(ctx, rc, ctx->solver.err);
+  return LANDAU_OK;
+}
+
 int landau3v_jacobian_host(landau3v_ctx* ctx, const double* batch_f_host, int batch, double dt, double* out_csr_vals_host,
                            void* cuda_stream) {
   if (int rc = check_call(ctx, batch_f_host, batch, out_csr_vals_host)) return rc;
@@ -600,7 +685,7 @@ int landau3v_last_stage_ms(landau3v_ctx* ctx, float* ms4) {
   return LANDAU_OK;
 }
 
-long long landau3v_launch_count(const landau3v_ctx* ctx) { return ctx ? ctx->launches : 0; }
+long long landau3v_launch_count(const landau3v_ctx* ctx) { return ctx ? ctx->launches + ctx->solver.launches : 0; }
 
 int landau3v_set_inner_kernel(landau3v_ctx* ctx, int which) {
   if (!ctx || which < 0 || which > 2) return LANDAU_INVALID_ARG;

@@ -14,7 +14,7 @@
 #include "host_setup.hpp"
 #include "landau_kernels.cuh"
 #include "k3_ring.cuh"
-#include "k4_solve.cuh"
+#include "batch_solver.hpp"
 
 using namespace landau;
 
@@ -67,16 +67,10 @@ struct landau_ctx {
   bool k3_tail_split = true;
   size_t k3_smem = 0;
   std::vector<char> k3_ring_ok;  // per species
-  // batched solve (k4_solve.cuh)
-  K4Grid* d_k4grid = nullptr;
-  K4Species* d_k4spec = nullptr;
-  int k4_max_n = 0, k4_smem_n = 0, k4_mat_nnz = 0;
-  size_t k4_smem = 0;
-  double* solve_ws = nullptr;
-  size_t solve_ws_cap = 0;
-  // landau_step scratch: A values, mass values (one entry, computed once), vectors, iteration counts
-  double *st_A = nullptr, *st_M = nullptr, *st_vec = nullptr, *st_misc = nullptr;
-  size_t st_A_cap = 0, st_M_cap = 0, st_vec_cap = 0, st_misc_cap = 0;
+  // batched solve and implicit step (batch_solver.hpp); mass values of one entry, computed at the first landau_step
+  BatchSolver solver;
+  double* st_M = nullptr;
+  size_t st_M_cap = 0;
   // scratch (grown on demand)
   double *F = nullptr, *Gp = nullptr, *DK = nullptr, *FL = nullptr, *part_buf = nullptr;
   size_t F_cap = 0, Gp_cap = 0, DK_cap = 0, FL_cap = 0, part_cap = 0;
@@ -180,7 +174,7 @@ struct NvtxRange {
 // The attribute belongs to the device's copy of the function, not to a context: keep a per-device high-water mark and
 // only ever raise it, so that two live contexts of different sizes on one GPU can be used alternately.
 constexpr int MAX_DEVICES = 64;
-size_t g_k3_smem_set[MAX_DEVICES] = {0}, g_k4_smem_set[MAX_DEVICES] = {0};
+size_t g_k3_smem_set[MAX_DEVICES] = {0};
 template <class F>
 int raise_smem_limit(landau_ctx* ctx, F func, size_t* table, size_t bytes) {
   size_t* cur = ctx->device >= 0 && ctx->device < MAX_DEVICES ? &table[ctx->device] : nullptr;
@@ -349,34 +343,12 @@ int build_device_side(landau_ctx* ctx) {
   }
   // batched solve: pattern views per grid, block offsets per species
   {
-    std::vector<K4Grid> kg(G);
-    std::vector<const int*> d_diag(G);
-    for (int g = 0; g < G; ++g) {
-      if (int rc = upload(ctx, ctx->hg[g].diag, &d_diag[g])) return rc;
-      kg[g] = K4Grid{ctx->hg[g].n_dof, ctx->hg[g].nnz, ctx->d_rowptr[g], ctx->d_colidx[g], d_diag[g]};
-      ctx->k4_max_n = std::max(ctx->k4_max_n, ctx->hg[g].n_dof);
-    }
-    std::vector<K4Species> ks(S);
-    for (int s = 0; s < S; ++s) ks[s] = K4Species{ctx->species[s].grid, ctx->f_off[s], ctx->v_off[s]};
-    const K4Grid* tg;
-    const K4Species* tsp;
-    if (int rc = upload(ctx, kg, &tg)) return rc;
-    if (int rc = upload(ctx, ks, &tsp)) return rc;
-    ctx->d_k4grid = const_cast<K4Grid*>(tg);
-    ctx->d_k4spec = const_cast<K4Species*>(tsp);
-    // Krylov vectors in shared memory when 7 n doubles fit beside the reduction scratch (227 KB per CTA on sm_100)
-    const size_t limit = 227 * 1024, fixed = 2 * (K4_THREADS / 32) * sizeof(double);
-    ctx->k4_smem_n = (int)((limit - fixed) / (K4_NVEC * sizeof(double)));
-    const int n_in_smem = std::min(ctx->k4_max_n, ctx->k4_smem_n);
-    ctx->k4_smem = fixed + (size_t)K4_NVEC * n_in_smem * sizeof(double);
-    // small systems: the pattern and one value block also go to shared memory when everything stays below 56 KB
-    // (four systems per SM)
-    int max_nnz = 0;
-    for (int g = 0; g < G; ++g) max_nnz = std::max(max_nnz, ctx->hg[g].nnz);
-    const size_t mat = (size_t)max_nnz * 12 + (size_t)(ctx->k4_max_n + 2) * 4;
-    ctx->k4_mat_nnz = (ctx->k4_max_n <= ctx->k4_smem_n && ctx->k4_smem + mat <= 56 * 1024) ? max_nnz : 0;
-    if (ctx->k4_mat_nnz) ctx->k4_smem += mat + K4_NVEC * sizeof(double);  // vectors padded to an even length
-    if (int rc = raise_smem_limit(ctx, k4_tfqmr, g_k4_smem_set, ctx->k4_smem)) return rc;
+    std::vector<SolverGridView> gv(G);
+    for (int g = 0; g < G; ++g)
+      gv[g] = SolverGridView{ctx->hg[g].n_dof, ctx->hg[g].nnz, ctx->d_rowptr[g], ctx->d_colidx[g], ctx->hg[g].diag.data()};
+    std::vector<SolverSpeciesView> sv(S);
+    for (int s = 0; s < S; ++s) sv[s] = SolverSpeciesView{ctx->species[s].grid, ctx->f_off[s], ctx->v_off[s]};
+    if (int rc = solver_create(ctx->solver, ctx->device, gv, sv, ctx->f_stride, ctx->v_stride)) return fail(ctx, rc, ctx->solver.err);
   }
   // source columns: separable nu => one group over all grids, one column per batch entry;
   // general nu => one group per grid, one column per species of the grid.
@@ -927,8 +899,8 @@ void landau_destroy(landau_ctx* ctx) {
     cudaDeviceSynchronize();
   }
   for (void* p : ctx->allocs) cudaFree(p);
-  for (double* p : {ctx->F, ctx->Gp, ctx->DK, ctx->FL, ctx->part_buf, ctx->solve_ws, ctx->stage_in, ctx->stage_out, ctx->st_A,
-                    ctx->st_M, ctx->st_vec, ctx->st_misc})
+  solver_destroy(ctx->solver);
+  for (double* p : {ctx->F, ctx->Gp, ctx->DK, ctx->FL, ctx->part_buf, ctx->stage_in, ctx->stage_out, ctx->st_M})
     if (p) cudaFree(p);
   for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
   for (cudaEvent_t e : ctx->copy_ev) cudaEventDestroy(e);
@@ -1138,10 +1110,8 @@ int landau_spmv(landau_ctx* ctx, const double* csr_vals_dev, const double* x_dev
   if (int rc = check_call(ctx, csr_vals_dev, batch, y_dev)) return rc;
   if (batch > 0 && !x_dev) return fail(ctx, LANDAU_INVALID_ARG, "null buffer");
   if (batch == 0) return LANDAU_OK;
-  k4_spmv_batch<<<batch * ctx->S, K4_THREADS, 0, (cudaStream_t)cuda_stream>>>(
-      ctx->d_k4grid, ctx->d_k4spec, ctx->S, csr_vals_dev, ctx->v_stride, x_dev, ctx->f_stride, y_dev);
-  ++ctx->launches;
-  CUDA_TRY(ctx, cudaGetLastError());
+  if (int rc = solver_spmv(ctx->solver, csr_vals_dev, ctx->v_stride, x_dev, batch, y_dev, (cudaStream_t)cuda_stream))
+    return fail(ctx, rc, ctx->solver.err);
   return LANDAU_OK;
 }
 
@@ -1151,19 +1121,9 @@ int landau_solve(landau_ctx* ctx, const double* csr_vals_dev, const double* rhs_
   if (batch > 0 && !rhs_dev) return fail(ctx, LANDAU_INVALID_ARG, "null buffer");
   if (!(rtol > 0) || max_it < 1) return fail(ctx, LANDAU_INVALID_ARG, "rtol must be > 0 and max_it >= 1");
   if (batch == 0) return LANDAU_OK;
-  long long ws_stride = 0;
-  if (ctx->k4_max_n > ctx->k4_smem_n) {  // some grid's vectors do not fit in shared memory: global workspace
-    ws_stride = (long long)K4_NVEC * ctx->k4_max_n;
-    if (int rc = grow(ctx, &ctx->solve_ws, &ctx->solve_ws_cap, (size_t)ws_stride * batch * ctx->S, false)) return rc;
-  }
-  // small systems: fewer threads per system, several systems per SM (the iteration is latency bound)
-  const int threads = ctx->k4_max_n <= 256 ? 128 : ctx->k4_max_n <= 1024 ? 256 : K4_THREADS;
-  k4_tfqmr<<<batch * ctx->S, threads, ctx->k4_smem, (cudaStream_t)cuda_stream>>>(
-      ctx->d_k4grid, ctx->d_k4spec, ctx->S, csr_vals_dev, ctx->v_stride, rhs_dev, ctx->f_stride, x_dev, rtol, max_it,
-      iters_dev, relres_dev, ctx->solve_ws, ws_stride, ctx->k4_mat_nnz ? ((ctx->k4_max_n + 1) & ~1) : ctx->k4_smem_n,
-      ctx->k4_mat_nnz);
-  ++ctx->launches;
-  CUDA_TRY(ctx, cudaGetLastError());
+  if (int rc = solver_tfqmr(ctx->solver, csr_vals_dev, rhs_dev, batch, rtol, max_it, x_dev, iters_dev, relres_dev,
+                            (cudaStream_t)cuda_stream))
+    return fail(ctx, rc, ctx->solver.err);
   return LANDAU_OK;
 }
 
@@ -1175,7 +1135,6 @@ int landau_step(landau_ctx* ctx, double* u_dev, int batch, double dt, double new
   if (info_host) info_host[0] = info_host[1] = info_host[2] = info_host[3] = 0.0;
   if (batch == 0) return LANDAU_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const size_t nf = (size_t)batch * ctx->f_stride, nsys = (size_t)batch * ctx->S;
   // mass values (independent of f and of the entry): M = (M/1 - J[0]) since D = K = 0 for f = 0
   if (!ctx->st_M) {
     if (int rc = grow(ctx, &ctx->st_M, &ctx->st_M_cap, (size_t)ctx->v_stride + ctx->f_stride, false)) return rc;
@@ -1187,51 +1146,12 @@ int landau_step(landau_ctx* ctx, double* u_dev, int batch, double dt, double new
     ctx->timing = timing;
     if (rc) return rc;
   }
-  if (int rc = grow(ctx, &ctx->st_A, &ctx->st_A_cap, (size_t)batch * ctx->v_stride, false)) return rc;
-  if (int rc = grow(ctx, &ctx->st_vec, &ctx->st_vec_cap, 4 * nf, false)) return rc;
-  if (int rc = grow(ctx, &ctx->st_misc, &ctx->st_misc_cap, nsys + 2, false)) return rc;  // iteration counts (int) + scalar
-  double *u0 = ctx->st_vec, *ju = u0 + nf, *rhs = ju + nf, *delta = rhs + nf;
-  int* iters = reinterpret_cast<int*>(ctx->st_misc);
-  unsigned long long* max_rel = reinterpret_cast<unsigned long long*>(ctx->st_misc + (nsys + 1) / 2 + 1);
-  CUDA_TRY(ctx, cudaMemcpyAsync(u0, u_dev, sizeof(double) * nf, cudaMemcpyDeviceToDevice, st));
-  const int eb = (int)std::min<size_t>((nf + 255) / 256, 65535);
-  int it = 0, worst_lin = 0, lin_failed = 0;
-  double rel = 0.0;
-  std::vector<int> h_iters(nsys);
-  for (it = 0; it < max_newton; ++it) {
-    // A = M/dt - J[u], ju = J[u] u from one inner integral
-    if (int rc = landau_jacobian_apply(ctx, u_dev, batch, dt, ctx->st_A, ju, cuda_stream)) return rc;
-    // rhs = M (u0 - u)/dt + J[u] u
-    k5_axpby<<<eb, 256, 0, st>>>((long long)nf, 1.0, u0, -1.0, u_dev, delta);
-    k4_spmv_batch<<<batch * ctx->S, K4_THREADS, 0, st>>>(ctx->d_k4grid, ctx->d_k4spec, ctx->S, ctx->st_M, 0, delta,
-                                                         ctx->f_stride, rhs);
-    k5_axpby<<<eb, 256, 0, st>>>((long long)nf, 1.0 / dt, rhs, 1.0, ju, rhs);
-    ctx->launches += 3;
-    CUDA_TRY(ctx, cudaMemsetAsync(delta, 0, sizeof(double) * nf, st));
-    if (int rc = landau_solve(ctx, ctx->st_A, rhs, batch, lin_rtol, lin_max_it, delta, iters, nullptr, cuda_stream)) return rc;
-    CUDA_TRY(ctx, cudaMemsetAsync(max_rel, 0, sizeof(unsigned long long), st));
-    k5_update<<<batch * ctx->S, 256, 0, st>>>(ctx->d_k4grid, ctx->d_k4spec, ctx->S, u_dev, delta, ctx->f_stride, max_rel);
-    ++ctx->launches;
-    unsigned long long bits = 0;
-    CUDA_TRY(ctx, cudaMemcpyAsync(&bits, max_rel, sizeof(bits), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(ctx, cudaMemcpyAsync(h_iters.data(), iters, sizeof(int) * nsys, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(ctx, cudaStreamSynchronize(st));
-    memcpy(&rel, &bits, sizeof(rel));
-    for (int v : h_iters) {
-      worst_lin = std::max(worst_lin, v < 0 ? -v - 1 : v);
-      lin_failed += v < 0;
-    }
-    if (rel <= newton_rtol) {
-      ++it;
-      break;
-    }
-  }
-  if (info_host) {
-    info_host[0] = it;
-    info_host[1] = rel;
-    info_host[2] = worst_lin;
-    info_host[3] = lin_failed;
-  }
+  const JacobianApplyFn jac = [&](const double* u, int nb, double step, double* A, double* ju) {
+    return landau_jacobian_apply(ctx, u, nb, step, A, ju, cuda_stream);
+  };
+  if (int rc = solver_step(ctx->solver, jac, ctx->st_M, u_dev, batch, dt, newton_rtol, max_newton, lin_rtol, lin_max_it,
+                           info_host, st))
+    return ctx->solver.err.empty() ? rc : fail(ctx, rc, ctx->solver.err);
   return LANDAU_OK;
 }
 
@@ -1302,7 +1222,7 @@ int landau_fp64_probe(int kind, int iters, double* tflops, void* cuda_stream) {
   return LANDAU_OK;
 }
 
-long long landau_launch_count(const landau_ctx* ctx) { return ctx ? ctx->launches : 0; }
+long long landau_launch_count(const landau_ctx* ctx) { return ctx ? ctx->launches + ctx->solver.launches : 0; }
 
 int landau_is_separable(const landau_ctx* ctx) {
   if (!ctx) return LANDAU_INVALID_ARG;
