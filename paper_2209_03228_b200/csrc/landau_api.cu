@@ -556,6 +556,24 @@ int pick_kernel(const landau_ctx* ctx, int ncols) {
   return ncols >= 8 ? 2 : 1;
 }
 
+// CTAs of the few-column kernels that fit on one SM at once (registers), per variant; queried once per device
+int small_kernel_ctas_per_sm(const landau_ctx* ctx, int kern, int ncols) {
+  static int cache[64][8] = {{0}};
+  const int v = kern == 1 ? (ncols >= 3 ? 2 : ncols == 2 ? 1 : 0) : 3 + (ncols > 32 ? 3 : ncols > 16 ? 2 : ncols > 8 ? 1 : 0);
+  int& n = cache[ctx->device & 63][v];
+  if (!n) {
+    cudaError_t e = cudaSuccess;
+    switch (v) {
+      case 0: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k2_inner_dfma<1>, 128, 0); break;
+      case 1: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k2_inner_dfma<2>, 128, 0); break;
+      case 2: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k2_inner_dfma<4>, 128, 0); break;
+      default: n = v == 3 ? 3 : v == 4 ? 2 : 1; break;  // k2_inner_dmma<1 / 2 / 4 / 8>: 82 / 126 / 164 / 255 registers x 256 threads
+    }
+    if (e != cudaSuccess || n < 1) n = 1;
+  }
+  return n;
+}
+
 // Column layout, kernel choice, j-split and scratch needs of one pass over `nbc` batch entries.
 struct ChunkPlan {
   std::vector<int> gcol0, ncols, ncols_pad, kern;
@@ -586,7 +604,10 @@ ChunkPlan plan_chunk(const landau_ctx* ctx, int nbc) {
   }
   // j-split so that small problems still fill the machine (groups whose kernel runs in stream mode cut their tiles
   // along j themselves and need none)
-  int max_blocks = 1 << 30;
+  // (the few-column kernels are latency bound: one full wave of resident CTAs, each thread with as few pairs as possible)
+  pl.nsplit = 1;
+  int min_tiles = 1 << 30;
+  for (const Group& gr : ctx->groups) min_tiles = std::min(min_tiles, gr.nj_pad / K2M_TJ);
   for (size_t q = 0; q < nq; ++q) {
     const int k = pl.kern[q];
     const Group& gr = ctx->groups[q];
@@ -596,14 +617,13 @@ ChunkPlan plan_chunk(const landau_ctx* ctx, int nbc) {
     const int blocks = k >= 3   ? ((ctx->n_i_pad + kern_ti(k) - 1) / kern_ti(k)) * (pl.ncols_pad[q] / kern_tc(k))
                        : k == 2 ? ((ctx->n_i_pad + 63) / 64) * ((pl.ncols[q] + 63) / 64)
                                 : ((ctx->n_i_pad + 127) / 128) * ((pl.ncols[q] + 3) / 4);
-    if (blocks < max_blocks) max_blocks = blocks;
+    const int want = ctx->n_sm * (k >= 3 ? 2 : std::max(2, small_kernel_ctas_per_sm(ctx, k, pl.ncols[q])));  // two short waves beat one long one
+    if (blocks < want) pl.nsplit = std::max(pl.nsplit, (want + blocks - 1) / blocks);
   }
-  const int want = 2 * ctx->n_sm;
-  if (max_blocks < want) {
-    pl.nsplit = (want + max_blocks - 1) / max_blocks;
-    int min_tiles = 1 << 30;
-    for (const Group& gr : ctx->groups) min_tiles = std::min(min_tiles, gr.nj_pad / K2M_TJ);
-    pl.nsplit = std::max(1, std::min(std::min(pl.nsplit, min_tiles), 64));
+  pl.nsplit = std::max(1, std::min(std::min(pl.nsplit, min_tiles), 64));
+  if (pl.nsplit > 1) {  // even shares: no slice of the source range without work
+    const int per = (min_tiles + pl.nsplit - 1) / pl.nsplit;
+    pl.nsplit = (min_tiles + per - 1) / per;
   }
   pl.split_stride = (long long)pl.total_cols * 5 * ctx->n_i_pad;
   for (size_t q = 0; q < nq; ++q) {
