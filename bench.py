@@ -130,7 +130,7 @@ class Problem:
             self.Bn = B3
             self.L = B3.Landau3V(cfg["grids"], cfg["species"], device=device)
             if kernel:
-                B3.landau3v_set_inner_kernel(self.L.ctx, min(kernel, 2))
+                B3.landau3v_set_inner_kernel(self.L.ctx, min(kernel, 3))
             if assembly:
                 B3.landau3v_set_assembly_kernel(self.L.ctx, 1 if assembly == 1 else 0)
             if chunk:

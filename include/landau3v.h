@@ -90,7 +90,8 @@ int landau3v_jacobian_host(landau3v_ctx* ctx, const double* batch_f_host, int ba
 /* Diagnostics (not part of the product path): frozen coefficients of the last pass, [entry][species][9][n_ip] with
  * components Dxx, Dxy, Dxz, Dyy, Dyz, Dzz, Kx, Ky, Kz (n_entries <= entries of the last pass); stage timing
  * (a1 fields, a2 inner integral, a2b combination, a3+a4 assembly or a5 apply) of the last call when enabled; kernels
- * launched so far; inner-integral kernel choice (0 auto, 1 scalar DFMA, 2 DMMA); assembly choice (0: element matrices on
+ * launched so far; inner-integral kernel choice (0 auto, 1 scalar DFMA, 2 DMMA with persistent CTAs sharing the work evenly,
+ * 3 DMMA on a grid with the source range cut into planes -- the first version, kept for A/B measurements); assembly choice (0: element matrices on
  * the MMA pipe + gather, 1: the first version, every CSR slot integrating its own entries -- kept for A/B measurements). */
 int landau3v_last_coefficients(landau3v_ctx* ctx, double* dk_host, int n_entries);
 int landau3v_set_timing(landau3v_ctx* ctx, int enabled);

@@ -47,7 +47,9 @@ struct landau3v_ctx {
   size_t EM_cap = 0;
   std::vector<long long> em_off;
   long long em_stride = 0;
-  int dmma_ctas_per_sm[5] = {0, 0, 0, 0, 0};
+  int dmma_ctas_per_sm[5] = {0, 0, 0, 0, 0}, dmma_stream_ctas_per_sm[5] = {0, 0, 0, 0, 0};
+  double* part_buf = nullptr;  // stream mode of the DMMA inner integral: accumulator parts of cut items + arrival counters
+  size_t part_cap = 0;
   int assembly_kernel = 0;  // 0: element matrices on the MMA pipe + gather, 1: per-slot quadrature (first version)
   bool k3e_configured = false;
   int k3e_ctas_per_sm = 0;
@@ -286,10 +288,24 @@ int check_call(landau3v_ctx* ctx, const void* in, int batch, const void* out) {
 // a1, a2, a2b for entries [b0, b0 + nbc): leaves D, K in ctx->DK
 int run_coefficients(landau3v_ctx* ctx, const double* batch_f, int b0, int nbc, cudaStream_t st) {
   const int G = ctx->G, S = ctx->S, NCL = ctx->n_classes;
-  const int kern = ctx->inner_kernel ? ctx->inner_kernel : (nbc >= 8 ? 2 : 1);
-  // DMMA kernel: cut the source range when (field tiles x column tiles) alone do not give four CTAs per SM
+  const int kern = ctx->inner_kernel ? std::min(ctx->inner_kernel, 2) : (nbc >= 8 ? 2 : 1);
+  // DMMA kernel, stream mode: persistent CTAs share the (item, source tile) steps evenly -- one plane of G, no wave tail
+  bool stream = false;
+  StreamPlan3 spl;
+  int stream_ctas = 0;
+  if (kern == 2 && ctx->inner_kernel != 3 && (nbc > 8 || ctx->inner_kernel == 2)) {  // 8 columns: the grid is as fast and K2b cheap
+    const int nt = inner_dmma_nt(nbc);
+    if (ctx->dmma_stream_ctas_per_sm[nt] == 0) ctx->dmma_stream_ctas_per_sm[nt] = inner_dmma_stream_ctas_per_sm(nt);
+    stream_ctas = ctx->dmma_stream_ctas_per_sm[nt] * ctx->n_sm;
+    spl = inner_dmma_stream_plan(ctx->n_pad, ctx->ranges, NCL, nbc);
+    stream = spl.step0[NCL] >= stream_ctas;
+    for (int c = 0; c < NCL; ++c) stream = stream && spl.njt[c] > 0;
+    if (stream)
+      if (int rc = grow(ctx, &ctx->part_buf, &ctx->part_cap, inner_dmma_stream_scratch(nt, stream_ctas, spl))) return rc;
+  }
+  // grid mode: cut the source range when (field tiles x column tiles) alone do not give four CTAs per SM
   int nsplit = 1;
-  if (kern == 2) {
+  if (kern == 2 && !stream) {
     const int ncol = nbc > 16 ? 32 : nbc > 8 ? 16 : 8;
     const long long items = (long long)(ctx->n_pad / (K2D_WARPS * 8)) * NCL * ((nbc + ncol - 1) / ncol);
     int min_tiles = 1 << 30;
@@ -320,7 +336,14 @@ int run_coefficients(landau3v_ctx* ctx, const double* batch_f, int b0, int nbc, 
   nvtxRangePop();
   mark(ctx, st);
   nvtxRangePushA("landau3v K2 inner integral (a2)");
-  if (kern == 2) {
+  if (kern == 2 && stream) {
+    if (launch_inner_dmma_stream(ctx->d_px, ctx->d_py, ctx->d_pz, ctx->n_pad, ctx->ranges, nbc, spl, stream_ctas, ctx->F, ctx->Gs,
+                                 ctx->part_buf, st)) {
+      nvtxRangePop();
+      return fail(ctx, LANDAU_CUDA_ERROR, "k3v_inner_dmma_stream launch failed");
+    }
+    ++ctx->launches;  // the counter memset
+  } else if (kern == 2) {
     if (int rc = launch_inner_dmma(ctx->d_px, ctx->d_py, ctx->d_pz, ctx->n_pad, ctx->ranges, NCL, nbc, nsplit, ctx->F, ctx->Gs, split_stride, st)) {
       nvtxRangePop();
       return fail(ctx, rc, "k3v_inner_dmma launch configuration failed");
@@ -482,7 +505,7 @@ void landau3v_destroy(landau3v_ctx* ctx) {
   }
   for (void* p : ctx->allocs) cudaFree(p);
   landau::solver_destroy(ctx->solver);
-  for (double* p : {ctx->F, ctx->Gs, ctx->DK, ctx->FE, ctx->EM, ctx->stage_in, ctx->stage_out, ctx->st_M})
+  for (double* p : {ctx->F, ctx->Gs, ctx->DK, ctx->FE, ctx->EM, ctx->stage_in, ctx->stage_out, ctx->st_M, ctx->part_buf})
     if (p) cudaFree(p);
   for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
   delete ctx;
@@ -688,7 +711,7 @@ int landau3v_last_stage_ms(landau3v_ctx* ctx, float* ms4) {
 long long landau3v_launch_count(const landau3v_ctx* ctx) { return ctx ? ctx->launches + ctx->solver.launches : 0; }
 
 int landau3v_set_inner_kernel(landau3v_ctx* ctx, int which) {
-  if (!ctx || which < 0 || which > 2) return LANDAU_INVALID_ARG;
+  if (!ctx || which < 0 || which > 3) return LANDAU_INVALID_ARG;
   ctx->inner_kernel = which;
   return LANDAU_OK;
 }

@@ -38,7 +38,7 @@ def _block_errors(L, got, ref, offs):
 
 
 @pytest.mark.parametrize("name", ["tiny", "tiny_uniform"])
-@pytest.mark.parametrize("kernel", [1, 2])
+@pytest.mark.parametrize("kernel", [1, 2, 3])
 @pytest.mark.parametrize("general_nu", [False, True])
 def test_tiny_parity(o3, B3, name, kernel, general_nu):
     import torch
@@ -177,7 +177,7 @@ def test_two_levels_and_general_nu_with_shared_grid(o3, B3):
     fd = torch.tensor(f, device="cuda")
     pick = [0, 8]
     ref, ref_rhs = o.jacobian_batch(f[pick], cfg["dt"]), o.apply_batch(f[pick])
-    for kernel in (1, 2):
+    for kernel in (1, 2, 3):
         B3.landau3v_set_inner_kernel(L.ctx, kernel)
         vals, rhs = L.jacobian(fd, cfg["dt"]).cpu().numpy(), L.apply(fd).cpu().numpy()
         assert _block_errors(L, vals[pick], ref, L.v_off).max() < TOL
