@@ -288,7 +288,9 @@ int check_call(landau3v_ctx* ctx, const void* in, int batch, const void* out) {
 // a1, a2, a2b for entries [b0, b0 + nbc): leaves D, K in ctx->DK
 int run_coefficients(landau3v_ctx* ctx, const double* batch_f, int b0, int nbc, cudaStream_t st) {
   const int G = ctx->G, S = ctx->S, NCL = ctx->n_classes;
-  const int kern = ctx->inner_kernel ? std::min(ctx->inner_kernel, 2) : (nbc >= 8 ? 2 : 1);
+  // the MMA kernel wins at every batch size (one entry: 0.87 against 1.36 ms on the paper's grids, its 8-column tile mostly
+  // padding); the scalar kernel stays as the plain variant for A/B and parity
+  const int kern = ctx->inner_kernel ? std::min(ctx->inner_kernel, 2) : 2;
   // DMMA kernel, stream mode: persistent CTAs share the (item, source tile) steps evenly -- one plane of G, no wave tail
   bool stream = false;
   StreamPlan3 spl;
@@ -402,8 +404,8 @@ int assemble_chunk(landau3v_ctx* ctx, int b0, int nbc, double inv_dt, double* ou
       k3v_elem_matrix<<<grid, K3E_WARPS * 32, K3E_SMEM, st>>>(ctx->d_grids, ctx->d_spec, ctx->S, nbc, ctx->max_cells, ctx->d_tab, ctx->DK,
                                                               ctx->dk_stride, inv_dt, ctx->EM, ctx->em_stride);
     }
-    k3v_gather<<<dim3((ctx->max_nnz + 255) / 256, nbc, ctx->S), 256, 0, st>>>(ctx->d_grids, ctx->d_spec, ctx->EM, ctx->em_stride, vals,
-                                                                              ctx->v_stride);
+    k3v_gather<<<dim3((ctx->max_nnz + 255) / 256, (nbc + K3G_BT - 1) / K3G_BT, ctx->S), 256, 0, st>>>(
+        ctx->d_grids, ctx->d_spec, nbc, ctx->EM, ctx->em_stride, vals, ctx->v_stride);
     ctx->launches += 2;
   }
   nvtxRangePop();

@@ -124,19 +124,41 @@ __global__ void __launch_bounds__(K3E_WARPS * 32) k3v_elem_matrix(const DevGrid3
   }
 }
 
-// grid (ceil(max nnz / 256), nbc, S): one thread per CSR slot
-__global__ void __launch_bounds__(256) k3v_gather(const DevGrid3* __restrict__ grids, const Spec3* __restrict__ spec,
+// grid (ceil(max nnz / 256), ceil(nbc / K3G_BT), S): one thread per CSR slot and K3G_BT batch entries -- the slot's list of
+// (weight, matrix entry) is read once for all of them and their loads are independent
+constexpr int K3G_BT = 8;
+__global__ void __launch_bounds__(256) k3v_gather(const DevGrid3* __restrict__ grids, const Spec3* __restrict__ spec, int nbc,
                                                   const double* __restrict__ EM, long long em_stride, double* __restrict__ vals,
                                                   long long v_stride) {
   const Spec3 sp = spec[blockIdx.z];
   const DevGrid3& g = grids[sp.grid];
-  const long long em_off = sp.em_off, v_off = sp.v_off;
-  const int n = blockIdx.x * 256 + threadIdx.x, b = blockIdx.y;
+  const int n = blockIdx.x * 256 + threadIdx.x, b0 = blockIdx.y * K3G_BT;
   if (n >= g.nnz) return;
-  const double* em = EM + (long long)b * em_stride + em_off;
-  double v = 0.0;
-  for (int p = g.as_ptr[n]; p < g.as_ptr[n + 1]; ++p) v = fma(g.as_w[p], em[g.as_code[p]], v);
-  __stcs(vals + (long long)b * v_stride + v_off + n, v);
+  const double* em = EM + (long long)b0 * em_stride + sp.em_off;
+  double v[K3G_BT];
+#pragma unroll
+  for (int k = 0; k < K3G_BT; ++k) v[k] = 0.0;
+  const int p1 = g.as_ptr[n + 1];
+  if (b0 + K3G_BT <= nbc) {
+    for (int p = g.as_ptr[n]; p < p1; ++p) {
+      const double w = g.as_w[p];
+      const double* src = em + g.as_code[p];
+#pragma unroll
+      for (int k = 0; k < K3G_BT; ++k) v[k] = fma(w, src[k * em_stride], v[k]);
+    }
+  } else {
+    for (int p = g.as_ptr[n]; p < p1; ++p) {
+      const double w = g.as_w[p];
+      const double* src = em + g.as_code[p];
+#pragma unroll
+      for (int k = 0; k < K3G_BT; ++k)
+        if (b0 + k < nbc) v[k] = fma(w, src[k * em_stride], v[k]);
+    }
+  }
+  double* dst = vals + (long long)b0 * v_stride + sp.v_off + n;
+#pragma unroll
+  for (int k = 0; k < K3G_BT; ++k)
+    if (b0 + k < nbc) __stcs(dst + k * v_stride, v[k]);
 }
 
 }  // namespace landau3v

@@ -105,7 +105,7 @@ def test_batch_edges_chunks_and_host_buffers(o3, B3):
     assert _block_errors(L, chunked, whole, L.v_off).max() < 1e-13   # summation order only (source range cut differently)
     assert _block_errors(L, chunked[[0, 7, 12]], ref, L.v_off).max() < TOL
     B3.landau3v_set_batch_chunk(L.ctx, 256)
-    one = L.jacobian(fd[3:4].contiguous(), cfg["dt"]).cpu().numpy()  # a single entry takes the scalar kernel
+    one = L.jacobian(fd[3:4].contiguous(), cfg["dt"]).cpu().numpy()  # a single entry: an 8-column tile with one column in use
     assert _block_errors(L, one, whole[3:4], L.v_off).max() < 1e-13
     # host buffers through the C ABI
     out_host = np.zeros((13, L.csr_stride))
