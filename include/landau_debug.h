@@ -57,9 +57,11 @@ int landau_last_stage_ms(landau_ctx* ctx, float* ms4);
 int landau_set_inner_kernel(landau_ctx* ctx, int which);
 
 /* Choose the element-matrix + assembly kernel: 0 auto (k3_ring: DMMA sum-factorised element matrices kept in a
- * shared-memory ring, CSR slots gathered from it; used for every grid whose ring fits in shared memory),
- * 1 force the general slot-gather kernel (k3_assemble: one thread per CSR slot, scalar FP64), 2 the ring kernel without the
- * tail cut (one CTA per (entry, species) block; for A/B measurements). */
+ * shared-memory ring, CSR slots gathered from it; used for every grid whose ring fits in shared memory -- the other grids,
+ * e.g. triangles, take k3_elem_matrix + k3_gather: element matrices to a scratch array, then one gather per CSR slot),
+ * 1 force the first general kernel (k3_assemble: one thread per CSR slot integrating its own entries, scalar FP64), 2 the ring
+ * kernel without the tail cut (one CTA per (entry, species) block), 3 element matrices + gather for every grid (1 - 3: for A/B
+ * measurements and parity tests). */
 int landau_set_assembly_kernel(landau_ctx* ctx, int which);
 
 /* Schedule of the ring assembly kernel for grid g (host query, works on host-only contexts): ring_cells = element

@@ -84,7 +84,11 @@ struct landau_ctx {
   int n_sm = 148;
   unsigned func_configured = 0;  // kernels whose dynamic shared-memory limit has been raised on this device
   bool stream_k = true;  // many-column K2: persistent CTAs sharing the steps evenly when the tiles do not fill whole waves
-  int assembly_kernel = 0;  // 0 auto (ring kernel where the grid has a schedule), 1 slot-gather kernel
+  int assembly_kernel = 0;  // 0 auto (ring kernel where the grid has a schedule, else element matrices + gather), 1 slot quadrature, 3 element matrices + gather everywhere
+  double* EM = nullptr;     // element matrices of the species without a ring schedule, [entry][species][cell][nb x nb]
+  size_t EM_cap = 0;
+  std::vector<long long> em_off;
+  long long em_stride = 0;
   int last_batch = 0;
   cudaStream_t last_stream = nullptr;
   bool timing = false;
@@ -780,16 +784,35 @@ int assemble_chunk(landau_ctx* ctx, int b0, int nbc, double inv_dt, double* out_
                                                       ctx->v_stride);
       ++ctx->launches;
     }
+    // species without a ring schedule (triangles, grids the ring does not fit): element matrices to scratch + slot gather;
+    // assembly kernel 1 keeps the first version (every slot integrating its own entries), 3 takes this path for every species
+    const auto use_ring = [&](int s) { return ctx->k3_ring_ok[s] && ctx->assembly_kernel != 1 && ctx->assembly_kernel != 3; };
+    bool need_em = false;
+    for (int s = 0; s < ctx->S; ++s) need_em = need_em || (!use_ring(s) && ctx->assembly_kernel != 1);
+    if (need_em)
+      if (int rc = grow(ctx, &ctx->EM, &ctx->EM_cap, (size_t)ctx->em_stride * nbc, false)) return rc;
     for (int s = 0; s < ctx->S; ++s) {
-      if (ctx->k3_ring_ok[s] && ctx->assembly_kernel != 1) continue;
+      if (use_ring(s)) continue;
       const int g = ctx->species[s].grid;
-      dim3 grid((ctx->hg[g].nnz + 255) / 256, nbc);
+      if (ctx->assembly_kernel == 1) {
+        dim3 grid((ctx->hg[g].nnz + 255) / 256, nbc);
 #define K3_CALL(NB_, NQ_)                                                                                                 \
   k3_assemble<NB_, NQ_><<<grid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, nbc, vals, \
                                               ctx->v_stride, ctx->v_off[s])
-      LANDAU_ELEM_DISPATCH(ctx, K3_CALL);
+        LANDAU_ELEM_DISPATCH(ctx, K3_CALL);
 #undef K3_CALL
-      ++ctx->launches;
+        ++ctx->launches;
+        continue;
+      }
+      dim3 egrid(ctx->hg[g].n_cells, (nbc + K3E_BT - 1) / K3E_BT);
+#define K3E_CALL(NB_, NQ_)                                                                                                  \
+  k3_elem_matrix<NB_, NQ_><<<egrid, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, ctx->DK, ctx->dk_stride, ctx->dk_off[s], inv_dt, nbc, ctx->EM, \
+                                                  ctx->em_stride, ctx->em_off[s])
+      LANDAU_ELEM_DISPATCH(ctx, K3E_CALL);
+#undef K3E_CALL
+      k3_gather<<<dim3((ctx->hg[g].nnz + 255) / 256, (nbc + K3G_BT - 1) / K3G_BT), 256, 0, st>>>(
+          ctx->dg[g], nbc, ctx->EM, ctx->em_stride, ctx->em_off[s], vals, ctx->v_stride, ctx->v_off[s]);
+      ctx->launches += 2;
     }
   return LANDAU_OK;
 }
@@ -857,13 +880,15 @@ int create_any(const landau_grid_desc* grids, const landau_mesh_desc* meshes, in
         ctx->nu[a * n_species + b] = nu ? nu[a * n_species + b]
                                         : species[a].charge * species[a].charge * species[b].charge * species[b].charge;
     }
-    long long fo = 0, vo = 0, dko = 0, flo = 0;
+    long long fo = 0, vo = 0, dko = 0, flo = 0, emo = 0;
     for (int a = 0; a < n_species; ++a) {
       const HostGrid& h = ctx->hg[species[a].grid];
       ctx->f_off.push_back(fo);
       ctx->v_off.push_back(vo);
       ctx->dk_off.push_back(dko);
       ctx->fl_off.push_back(flo);
+      ctx->em_off.push_back(emo);
+      emo += (long long)h.n_cells * ctx->nb * ctx->nb;
       fo += h.n_dof;
       vo += h.nnz;
       dko += 5LL * h.n_ip;
@@ -873,6 +898,7 @@ int create_any(const landau_grid_desc* grids, const landau_mesh_desc* meshes, in
     ctx->v_stride = vo;
     ctx->dk_stride = dko;
     ctx->fl_stride = flo;
+    ctx->em_stride = emo;
   } catch (const std::bad_alloc&) {
     return bail(LANDAU_OUT_OF_MEMORY, "host allocation failed");
   }
@@ -920,7 +946,7 @@ void landau_destroy(landau_ctx* ctx) {
   }
   for (void* p : ctx->allocs) cudaFree(p);
   solver_destroy(ctx->solver);
-  for (double* p : {ctx->F, ctx->Gp, ctx->DK, ctx->FL, ctx->part_buf, ctx->stage_in, ctx->stage_out, ctx->st_M})
+  for (double* p : {ctx->F, ctx->Gp, ctx->DK, ctx->FL, ctx->part_buf, ctx->stage_in, ctx->stage_out, ctx->st_M, ctx->EM})
     if (p) cudaFree(p);
   for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
   for (cudaEvent_t e : ctx->copy_ev) cudaEventDestroy(e);
@@ -1278,9 +1304,9 @@ int landau_set_inner_kernel(landau_ctx* ctx, int which) {
 }
 
 int landau_set_assembly_kernel(landau_ctx* ctx, int which) {
-  if (!ctx || which < 0 || which > 2) return LANDAU_INVALID_ARG;
+  if (!ctx || which < 0 || which > 3) return LANDAU_INVALID_ARG;
   ctx->k3_tail_split = which != 2;  // 2: ring kernel without the tail cut (one CTA per block), for A/B measurements
-  ctx->assembly_kernel = which == 1 ? 1 : 0;
+  ctx->assembly_kernel = which == 1 || which == 3 ? which : 0;
   return LANDAU_OK;
 }
 

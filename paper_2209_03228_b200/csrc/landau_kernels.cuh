@@ -6,7 +6,8 @@
 //       k2_inner_gemm    a2: (k2_gemm.cuh) tensor tile shared by the CTA, TMA-staged source tiles (many columns)
 //   K2b k2b_combine      a2: D_a, K_a = species combination of the partial sums (also sums the j-splits)
 //   K3  k3_ring          a3+a4: (k3_ring.cuh) DMMA element matrices in a shared-memory ring, gathered into batched CSR
-//       k3_assemble      a3+a4: general fallback, one thread per CSR slot
+//       k3_elem_matrix, k3_gather   a3+a4 without a ring schedule (triangles, ...): element matrices to scratch, slot gather
+//       k3_assemble      a3+a4: first version, one thread per CSR slot integrating its own entries (kept for A/B)
 //   K3' k3_elem_apply, k3_apply_gather   a5: operator application
 //   K4  k4_tfqmr         (k4_solve.cuh) batched TFQMR + Jacobi solve, the step after the path
 //
@@ -625,6 +626,85 @@ k3_assemble(DevGrid g, const DevTables* __restrict__ tab, const double* __restri
     total = fma(g.as_w[p], s, total);
   }
   vals[(long long)b * v_stride + v_off + n] = total;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// K3 for cells without a ring schedule (triangles, grids the ring does not fit): element matrices first, then a gather.
+//   k3_elem_matrix: one CTA = one cell x K3E_BT batch entries of one species; thread (a, c) forms the six products of its
+//     two basis functions per point once and applies them to the (w D, w K) of every entry (staged in shared memory, read
+//     as broadcasts):  A_e[a][c] = sum_q w_q [ phi_a phi_c / dt + grad phi_a . D grad phi_c - (grad phi_a . K) phi_c ]
+//     -> scratch EM[entry][species][cell][NB x NB]   (each D, K value is used NB^2 times instead of being re-read per slot).
+//   k3_gather: one thread per CSR slot and K3G_BT entries sums the slot's (constraint weight, matrix entry) list -- the codes
+//     of the slot lists, (cell NB + a) NB + c, are the offsets into a species' scratch block.  Written once, no atomics.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int K3E_BT = 8, K3G_BT = 8;
+
+template <int NB, int NQ = NB>
+__global__ void __launch_bounds__(256)
+k3_elem_matrix(DevGrid g, const DevTables* __restrict__ tab, const double* __restrict__ DK, long long dk_stride,
+               long long dk_off, double inv_dt, int nbatch, double* __restrict__ EM, long long em_stride, long long em_off) {
+  __shared__ double sB[NQ * NB], sX[NQ * NB], sY[NQ * NB];
+  __shared__ double sDK[K3E_BT][NQ][5];  // w Drr, w Drz, w Dzz, w Kr, w Kz
+  __shared__ double sW[NQ];
+  const int tid = threadIdx.x, cell = blockIdx.x, b0 = blockIdx.y * K3E_BT;
+  const double sr = g.cell_sr[cell], sz = g.cell_sz[cell];
+  for (int e = tid; e < NQ * NB; e += 256) {
+    sB[e] = tab->B[e];
+    sX[e] = tab->dBxi[e] * sr;
+    sY[e] = tab->dBeta[e] * sz;
+  }
+  if (tid < NQ) sW[tid] = g.ip_w[cell * NQ + tid];
+  for (int e = tid; e < K3E_BT * NQ * 5; e += 256) {
+    const int k = e % 5, q = (e / 5) % NQ, bl = e / (5 * NQ);
+    const int ip = cell * NQ + q;
+    sDK[bl][q][k] = b0 + bl < nbatch ? g.ip_w[ip] * DK[(long long)(b0 + bl) * dk_stride + dk_off + (long long)k * g.n_ip + ip] : 0.0;
+  }
+  __syncthreads();
+  if (tid >= NB * NB) return;
+  const int a = tid / NB, c = tid - a * NB;
+  double acc[K3E_BT], mass = 0.0;
+#pragma unroll
+  for (int bl = 0; bl < K3E_BT; ++bl) acc[bl] = 0.0;
+#pragma unroll 2
+  for (int q = 0; q < NQ; ++q) {
+    const double pa = sB[q * NB + a], par = sX[q * NB + a], paz = sY[q * NB + a];
+    const double pc = sB[q * NB + c], pcr = sX[q * NB + c], pcz = sY[q * NB + c];
+    const double m_rr = par * pcr, m_rz = fma(par, pcz, paz * pcr), m_zz = paz * pcz, m_r = -par * pc, m_z = -paz * pc;
+    mass = fma(sW[q], pa * pc, mass);
+#pragma unroll
+    for (int bl = 0; bl < K3E_BT; ++bl) {
+      const double* d = sDK[bl][q];
+      acc[bl] = fma(d[0], m_rr, fma(d[1], m_rz, fma(d[2], m_zz, fma(d[3], m_r, fma(d[4], m_z, acc[bl])))));
+    }
+  }
+  double* dst = EM + (long long)b0 * em_stride + em_off + (long long)cell * (NB * NB) + tid;
+#pragma unroll
+  for (int bl = 0; bl < K3E_BT; ++bl)
+    if (b0 + bl < nbatch) dst[bl * em_stride] = fma(inv_dt, mass, acc[bl]);
+}
+
+// grid (ceil(nnz / 256), ceil(nbatch / K3G_BT)) per species
+__global__ void __launch_bounds__(256)
+k3_gather(DevGrid g, int nbatch, const double* __restrict__ EM, long long em_stride, long long em_off,
+          double* __restrict__ vals, long long v_stride, long long v_off) {
+  const int n = blockIdx.x * 256 + threadIdx.x, b0 = blockIdx.y * K3G_BT;
+  if (n >= g.nnz) return;
+  const double* em = EM + (long long)b0 * em_stride + em_off;
+  double v[K3G_BT];
+#pragma unroll
+  for (int k = 0; k < K3G_BT; ++k) v[k] = 0.0;
+  const int p1 = g.as_ptr[n + 1], nb = min(K3G_BT, nbatch - b0);
+  for (int p = g.as_ptr[n]; p < p1; ++p) {
+    const double w = g.as_w[p];
+    const double* src = em + g.as_code[p];
+#pragma unroll
+    for (int k = 0; k < K3G_BT; ++k)
+      if (k < nb) v[k] = fma(w, src[k * em_stride], v[k]);
+  }
+  double* dst = vals + (long long)b0 * v_stride + v_off + n;
+#pragma unroll
+  for (int k = 0; k < K3G_BT; ++k)
+    if (k < nb) __stcs(dst + k * v_stride, v[k]);
 }
 
 // ------------------------------------------------------------------------------------------------------------

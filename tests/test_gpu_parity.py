@@ -117,6 +117,12 @@ def test_tiny_jacobian_apply_and_coefficients(orc, Bn, torch_cuda, kind, degree,
     Bn.landau_set_assembly_kernel(L.ctx, 0)
     assert _block_errors(L, vals1, ref, L.v_off).max() < TOL
     assert _block_errors(L, vals1, vals, L.v_off).max() < 1e-13
+    # and so does the element-matrix + gather path that cells without a ring schedule take (forced here: 3 entries, ragged tile)
+    Bn.landau_set_assembly_kernel(L.ctx, 3)
+    vals3 = L.jacobian(fd, cfg["dt"]).cpu().numpy()
+    Bn.landau_set_assembly_kernel(L.ctx, 0)
+    assert _block_errors(L, vals3, ref, L.v_off).max() < TOL
+    assert _block_errors(L, vals3, vals, L.v_off).max() < 1e-13
     # frozen coefficients D, K at the IPs (IP order is implementation-private: match by coordinates)
     with pytest.raises(Bn.LandauError):
         L.last_coefficients(4)                              # more entries than the last pass holds: refused, nothing copied
@@ -542,7 +548,7 @@ def test_outputs_stay_inside_their_buffers(Bn, torch_cuda):
     for cfg, B in ((W.tiny_config("quadtree", 3, batch=5), 5), (W.config(3), 300)):
         L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"])
         f = torch.tensor(W.make_batch_f(cfg, [L.dof_coords(g) for g in range(L.G)], batch=B), device="cuda")
-        for asm in (0, 1):
+        for asm in (0, 1, 3):
             Bn.landau_set_assembly_kernel(L.ctx, asm)
             vb, vals = guarded(B, L.csr_stride)
             Bn.landau_jacobian(L.ctx, f, B, cfg["dt"], vals)
