@@ -37,7 +37,7 @@ extern "C" {
 typedef enum {
   LANDAU_OK = 0,
   LANDAU_INVALID_ARG = -1,   /* NULL pointer, non-positive size, dt <= 0, species on a missing grid, ...   */
-  LANDAU_UNSUPPORTED = -2,   /* degree not in {2,3}, n_gauss_1d != degree+1, grid kind unknown, chain of
+  LANDAU_UNSUPPORTED = -2,   /* degree not in {2,3,4}, n_gauss_1d != degree+1, grid kind unknown, chain of
                                 hanging-node constraints (mesh not 2:1 balanced)                           */
   LANDAU_OUT_OF_MEMORY = -3, /* host or device allocation failed                                           */
   LANDAU_CUDA_ERROR = -4     /* any other CUDA runtime failure (no device, launch failure, ...)            */
@@ -63,7 +63,8 @@ typedef struct {
   int grid;
 } landau_species_desc;
 
-/* Element degree k (Qk) and Gauss points per direction (must be k+1; Table 13). */
+/* Element degree k (Qk, k = 2, 3, 4 -- the degrees of PAPER.md:309-313 Table 13) and Gauss points per direction (must be
+ * k+1).  Q4 cells (25 basis functions) take the general element-matrix + gather assembly, Q2 / Q3 the ring kernel. */
 typedef struct {
   int degree;
   int n_gauss_1d;
@@ -93,7 +94,7 @@ typedef struct {
   const double* vertices_rz; /* host, n_vertices x 2: (r, z) in units of v0 */
   int n_cells;
   const int* cells;          /* host, n_cells x vertices_per_cell vertex indices, counter-clockwise */
-  int vertices_per_cell;     /* 4: quadrilaterals (Qk, k = 2, 3); 3: triangles (Pk, k = 2, 3, 4; sec. 5.1) */
+  int vertices_per_cell;     /* 4: quadrilaterals (Qk, k = 2, 3, 4); 3: triangles (Pk, k = 2, 3, 4; sec. 5.1) */
 } landau_mesh_desc;
 
 /* landau_create for unstructured quadrilateral grids: meshes[n_grids] (host, read during the call) take the place of the

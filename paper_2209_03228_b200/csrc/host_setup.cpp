@@ -48,8 +48,8 @@ struct CellId {
 }  // namespace
 
 bool build_tables(int k, HostTables* t, std::string* msg) {
-  if (k != 2 && k != 3) {
-    *msg = "element degree must be 2 or 3";
+  if (k < 2 || k > 4) {
+    *msg = "element degree must be 2, 3 or 4";
     return false;
   }
   t->k = k;
@@ -61,19 +61,26 @@ bool build_tables(int k, HostTables* t, std::string* msg) {
     const double a = std::sqrt(3.0 / 5.0);
     t->gauss_x = {-a, 0.0, a};
     t->gauss_w = {5.0 / 9.0, 8.0 / 9.0, 5.0 / 9.0};
-  } else {
+  } else if (k == 3) {
     const double s = std::sqrt(6.0 / 5.0);
     const double a = std::sqrt(3.0 / 7.0 - 2.0 / 7.0 * s), b = std::sqrt(3.0 / 7.0 + 2.0 / 7.0 * s);
     const double wa = (18.0 + std::sqrt(30.0)) / 36.0, wb = (18.0 - std::sqrt(30.0)) / 36.0;
     t->gauss_x = {-b, -a, a, b};
     t->gauss_w = {wb, wa, wa, wb};
+  } else {
+    const double s = 2.0 * std::sqrt(10.0 / 7.0);
+    const double a = std::sqrt(5.0 - s) / 3.0, b = std::sqrt(5.0 + s) / 3.0;
+    const double wa = (322.0 + 13.0 * std::sqrt(70.0)) / 900.0, wb = (322.0 - 13.0 * std::sqrt(70.0)) / 900.0;
+    t->gauss_x = {-b, -a, 0.0, a, b};
+    t->gauss_w = {wb, wa, 128.0 / 225.0, wa, wb};
   }
   const int n1 = k + 1;
   std::vector<double> v(n1 * n1), d(n1 * n1);  // [q1][c]
   for (int q = 0; q < n1; ++q) equispaced_lagrange(k, t->gauss_x[q], &v[q * n1], &d[q * n1]);
   t->lag_v = v;
   t->lag_d = d;
-  {
+  t->k3_frag.assign(16 * 32, 0.0);
+  if (k <= 3) {  // the ring kernel's fragment tables hold up to 4 x 4 one-dimensional products: Q2 and Q3 only
     // 1-D product tables P[x][y][ac][q] = l^(x)_a(q) l^(y)_c(q), ac = a n1 + c  (zero outside the valid range)
     auto P = [&](int x, int y, int ac, int q) -> double {
       if (ac >= n1 * n1 || q >= n1) return 0.0;
@@ -82,7 +89,6 @@ bool build_tables(int k, HostTables* t, std::string* msg) {
     };
     // table order used by both directions: 0: P00, 1: P11, 2: P10 (derivative on the test function a), 3: P01
     const int tx[4] = {0, 1, 1, 0}, ty[4] = {0, 1, 0, 1};
-    t->k3_frag.assign(16 * 32, 0.0);
     for (int lane = 0; lane < 32; ++lane) {
       const int g = lane >> 2, tq = lane & 3;
       for (int zt = 0; zt < 4; ++zt)
@@ -437,7 +443,7 @@ int finish_grid(const HostTables& t, HostGrid* g, std::string* msg) {
     }
   }
   // ---- K3 ring schedule (tensor-product cells only: the ring kernel is sum-factorised) ----------------------------------
-  if (!t.simplex) {
+  if (!t.simplex && t.k <= 3) {
     const int nb2 = nb * nb;
     g->k3_nsteps = (g->n_cells + K3_PC - 1) / K3_PC;
     // emission step of every CSR slot = step of its last contributing cell; an element matrix stays in the ring from

@@ -146,7 +146,7 @@ int grow(landau_ctx* ctx, double** p, size_t* cap, size_t need, bool zero, cudaS
 
 int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
-// kernels templated on (basis functions, integration points) per cell: Q2, Q3 quadrilaterals, P2, P3, P4 triangles
+// kernels templated on (basis functions, integration points) per cell: Q2, Q3, Q4 quadrilaterals, P2, P3, P4 triangles
 #define LANDAU_ELEM_DISPATCH(ctx, CALL)                  \
   do {                                                   \
     const int nb_ = (ctx)->nb, nq_ = (ctx)->nq;          \
@@ -158,6 +158,8 @@ int round_up(int x, int m) { return (x + m - 1) / m * m; }
       CALL(6, 6);                                        \
     } else if (nb_ == 10 && nq_ == 12) {                 \
       CALL(10, 12);                                      \
+    } else if (nb_ == 25 && nq_ == 25) {                 \
+      CALL(25, 25);                                      \
     } else {                                             \
       CALL(15, 16);                                      \
     }                                                    \

@@ -218,9 +218,9 @@ struct DevGrid {
   const double* ap_w;
 };
 
-// basis tabulation, [q][a]; nb = nq <= 16
+// basis tabulation, [q][a]; nb, nq <= 25 (Q4)
 struct DevTables {
-  double B[256], dBxi[256], dBeta[256];
+  double B[640], dBxi[640], dBeta[640];
 };
 
 // ------------------------------------------------------------------------------------------------------------
@@ -261,7 +261,8 @@ __global__ void __launch_bounds__(256)
 k1_fields(DevGrid g, const DevTables* __restrict__ tab, MixTable mix, const double* __restrict__ batch_f,
                long long f_stride, int b0, int nbatch, double* __restrict__ F, long long nj_pad, int j_off_in_group,
                int col0, int tiled_tc) {
-  __shared__ double sT[3][NB][16];       // B, dBxi, dBeta as [a][q]
+  constexpr int NQP = (NQ + 15) / 16 * 16;
+  __shared__ double sT[3][NB][NQP];      // B, dBxi, dBeta as [a][q]
   __shared__ double sD[NB][K1T_BT], sK[NB][K1T_BT];
   const int tid = threadIdx.x, lo = tid & 15, bl = tid >> 4;
   const int cell = blockIdx.x, b = blockIdx.y * K1T_BT + bl;
@@ -272,15 +273,13 @@ k1_fields(DevGrid g, const DevTables* __restrict__ tab, MixTable mix, const doub
     sT[2][a][q] = tab->dBeta[e];
   }
   const double sr = g.cell_sr[cell], sz = g.cell_sz[cell];
-  const int j = cell * NQ + lo;
-  const double w = lo < NQ ? g.ip_w[j] : 0.0;
   const bool live = b < nbatch;
   const double* fb = batch_f + (long long)(b0 + (live ? b : 0)) * f_stride;
   for (int c = 0; c < mix.ncb; ++c) {
     __syncthreads();
-    if (lo < NB) {  // lo = basis function a
+    for (int a = lo; a < NB; a += 16) {  // basis function a (more than 16 on Q4: several per thread)
       double fD = 0.0, fK = 0.0;
-      const int p0 = g.en_ptr[cell * NB + lo], p1 = g.en_ptr[cell * NB + lo + 1];
+      const int p0 = g.en_ptr[cell * NB + a], p1 = g.en_ptr[cell * NB + a + 1];
       for (int e = mix.ptr[c]; e < mix.ptr[c + 1]; ++e) {
         const double* fs = fb + mix.species_foff[e];
         double fa = 0.0;
@@ -288,18 +287,20 @@ k1_fields(DevGrid g, const DevTables* __restrict__ tab, MixTable mix, const doub
         fD = fma(mix.wD[e], fa, fD);
         fK = fma(mix.wK[e], fa, fK);
       }
-      sD[lo][bl] = fD;
-      sK[lo][bl] = fK;
+      sD[a][bl] = fD;
+      sK[a][bl] = fK;
     }
     __syncthreads();
-    if (lo < NQ && live) {  // lo = quadrature point q
+    for (int q = lo; q < NQ && live; q += 16) {  // quadrature point q
+      const int j = cell * NQ + q;
+      const double w = g.ip_w[j];
       double v = 0.0, vx = 0.0, vy = 0.0;
 #pragma unroll
       for (int a = 0; a < NB; ++a) {
         const double fd = sD[a][bl], fk = sK[a][bl];
-        v = fma(sT[0][a][lo], fd, v);
-        vx = fma(sT[1][a][lo], fk, vx);
-        vy = fma(sT[2][a][lo], fk, vy);
+        v = fma(sT[0][a][q], fd, v);
+        vx = fma(sT[1][a][q], fk, vx);
+        vy = fma(sT[2][a][q], fk, vy);
       }
       const long long col = col0 + (long long)b * mix.ncb + c;
       double gr = vx * sr, gz = vy * sz;
@@ -660,27 +661,28 @@ k3_elem_matrix(DevGrid g, const DevTables* __restrict__ tab, const double* __res
     sDK[bl][q][k] = b0 + bl < nbatch ? g.ip_w[ip] * DK[(long long)(b0 + bl) * dk_stride + dk_off + (long long)k * g.n_ip + ip] : 0.0;
   }
   __syncthreads();
-  if (tid >= NB * NB) return;
-  const int a = tid / NB, c = tid - a * NB;
-  double acc[K3E_BT], mass = 0.0;
+  for (int e = tid; e < NB * NB; e += 256) {  // one (a, c) per thread up to Q3 / P4, three on Q4
+    const int a = e / NB, c = e - a * NB;
+    double acc[K3E_BT], mass = 0.0;
 #pragma unroll
-  for (int bl = 0; bl < K3E_BT; ++bl) acc[bl] = 0.0;
+    for (int bl = 0; bl < K3E_BT; ++bl) acc[bl] = 0.0;
 #pragma unroll 2
-  for (int q = 0; q < NQ; ++q) {
-    const double pa = sB[q * NB + a], par = sX[q * NB + a], paz = sY[q * NB + a];
-    const double pc = sB[q * NB + c], pcr = sX[q * NB + c], pcz = sY[q * NB + c];
-    const double m_rr = par * pcr, m_rz = fma(par, pcz, paz * pcr), m_zz = paz * pcz, m_r = -par * pc, m_z = -paz * pc;
-    mass = fma(sW[q], pa * pc, mass);
+    for (int q = 0; q < NQ; ++q) {
+      const double pa = sB[q * NB + a], par = sX[q * NB + a], paz = sY[q * NB + a];
+      const double pc = sB[q * NB + c], pcr = sX[q * NB + c], pcz = sY[q * NB + c];
+      const double m_rr = par * pcr, m_rz = fma(par, pcz, paz * pcr), m_zz = paz * pcz, m_r = -par * pc, m_z = -paz * pc;
+      mass = fma(sW[q], pa * pc, mass);
 #pragma unroll
-    for (int bl = 0; bl < K3E_BT; ++bl) {
-      const double* d = sDK[bl][q];
-      acc[bl] = fma(d[0], m_rr, fma(d[1], m_rz, fma(d[2], m_zz, fma(d[3], m_r, fma(d[4], m_z, acc[bl])))));
+      for (int bl = 0; bl < K3E_BT; ++bl) {
+        const double* d = sDK[bl][q];
+        acc[bl] = fma(d[0], m_rr, fma(d[1], m_rz, fma(d[2], m_zz, fma(d[3], m_r, fma(d[4], m_z, acc[bl])))));
+      }
     }
-  }
-  double* dst = EM + (long long)b0 * em_stride + em_off + (long long)cell * (NB * NB) + tid;
+    double* dst = EM + (long long)b0 * em_stride + em_off + (long long)cell * (NB * NB) + e;
 #pragma unroll
-  for (int bl = 0; bl < K3E_BT; ++bl)
-    if (b0 + bl < nbatch) dst[bl * em_stride] = fma(inv_dt, mass, acc[bl]);
+    for (int bl = 0; bl < K3E_BT; ++bl)
+      if (b0 + bl < nbatch) dst[bl * em_stride] = fma(inv_dt, mass, acc[bl]);
+  }
 }
 
 // grid (ceil(nnz / 256), ceil(nbatch / K3G_BT)) per species
@@ -720,7 +722,8 @@ __global__ void __launch_bounds__(256)
 k3_elem_apply(DevGrid g, const DevTables* __restrict__ tab, const double* __restrict__ batch_f, long long f_stride,
               long long f_off, int b0, const double* __restrict__ DK, long long dk_stride, long long dk_off, int nbatch,
               double* __restrict__ RE, long long re_stride, long long re_off) {
-  __shared__ double sT[3][NB][16];  // B, dBxi, dBeta as [a][q]
+  constexpr int NQP = (NQ + 15) / 16 * 16;
+  __shared__ double sT[3][NB][NQP];  // B, dBxi, dBeta as [a][q]
   __shared__ double sF[NB][K1T_BT], sFl[2][NQ][K1T_BT];
   const int tid = threadIdx.x, lo = tid & 15, bl = tid >> 4;
   const int cell = blockIdx.x, b = blockIdx.y * K1T_BT + bl;
@@ -732,38 +735,38 @@ k3_elem_apply(DevGrid g, const DevTables* __restrict__ tab, const double* __rest
     sT[2][a][q] = tab->dBeta[e];
   }
   const double sr = g.cell_sr[cell], sz = g.cell_sz[cell];
-  if (lo < NB) {  // lo = basis function a: constrained nodal value
+  for (int a = lo; a < NB; a += 16) {  // basis function a: constrained nodal value
     const double* fs = batch_f + (long long)(b0 + (live ? b : 0)) * f_stride + f_off;
     double fa = 0.0;
-    for (int p = g.en_ptr[cell * NB + lo]; p < g.en_ptr[cell * NB + lo + 1]; ++p) fa = fma(g.en_w[p], fs[g.en_dof[p]], fa);
-    sF[lo][bl] = fa;
+    for (int p = g.en_ptr[cell * NB + a]; p < g.en_ptr[cell * NB + a + 1]; ++p) fa = fma(g.en_w[p], fs[g.en_dof[p]], fa);
+    sF[a][bl] = fa;
   }
   __syncthreads();
-  if (lo < NQ) {  // lo = quadrature point q
+  for (int q = lo; q < NQ; q += 16) {  // quadrature point q
     double v = 0.0, vx = 0.0, vy = 0.0;
 #pragma unroll
     for (int a = 0; a < NB; ++a) {
       const double fa = sF[a][bl];
-      v = fma(sT[0][a][lo], fa, v);
-      vx = fma(sT[1][a][lo], fa, vx);
-      vy = fma(sT[2][a][lo], fa, vy);
+      v = fma(sT[0][a][q], fa, v);
+      vx = fma(sT[1][a][q], fa, vx);
+      vy = fma(sT[2][a][q], fa, vy);
     }
-    const int j = cell * NQ + lo;
+    const int j = cell * NQ + q;
     const double fr = vx * sr, fz = vy * sz, w = g.ip_w[j];
     const double* dk = DK + (long long)(live ? b : 0) * dk_stride + dk_off;
     const double Drr = dk[j], Drz = dk[g.n_ip + j], Dzz = dk[2 * g.n_ip + j], Kr = dk[3 * g.n_ip + j], Kz = dk[4 * g.n_ip + j];
-    sFl[0][lo][bl] = w * (fma(Drr, fr, Drz * fz) - Kr * v);
-    sFl[1][lo][bl] = w * (fma(Drz, fr, Dzz * fz) - Kz * v);
+    sFl[0][q][bl] = w * (fma(Drr, fr, Drz * fz) - Kr * v);
+    sFl[1][q][bl] = w * (fma(Drz, fr, Dzz * fz) - Kz * v);
   }
   __syncthreads();
-  if (lo < NB && live) {  // lo = basis function a again
+  for (int a = lo; a < NB && live; a += 16) {  // basis function a again
     double r = 0.0;
 #pragma unroll
     for (int q = 0; q < NQ; ++q) {
-      r = fma(sT[1][lo][q] * sr, sFl[0][q][bl], r);
-      r = fma(sT[2][lo][q] * sz, sFl[1][q][bl], r);
+      r = fma(sT[1][a][q] * sr, sFl[0][q][bl], r);
+      r = fma(sT[2][a][q] * sz, sFl[1][q][bl], r);
     }
-    RE[(long long)b * re_stride + re_off + cell * NB + lo] = r;
+    RE[(long long)b * re_stride + re_off + cell * NB + a] = r;
   }
 }
 

@@ -78,8 +78,8 @@ def test_create_rejects_bad_arguments(lib):
         Bn.landau_create(cfg["grids"], [dict(mass=-1.0, charge=-1.0, grid=0)], 2, cuda_device=-1)
 
 
-@pytest.mark.parametrize("cfg", [W.tiny_config("uniform", 2), W.tiny_config("quadtree", 3), W.config(1), W.config(4),
-                                 W.config(3)], ids=lambda c: c["name"])
+@pytest.mark.parametrize("cfg", [W.tiny_config("uniform", 2), W.tiny_config("quadtree", 3), W.tiny_config("uniform", 4),
+                                 W.tiny_config("quadtree", 4), W.config(1), W.config(4), W.config(3)], ids=lambda c: c["name"])
 def test_host_setup_matches_oracle(orc, lib, cfg):
     """dof numbering, CSR pattern (bit-exact), IP tables (as sets) of the product's own host set-up vs the oracle's."""
     o = orc.Oracle(cfg["grids"], cfg["species"], cfg["degree"])
@@ -138,7 +138,7 @@ def test_ring_assembly_schedule_exists_for_every_baseline_config(lib, c):
 def test_unstructured_host_setup_matches_oracle(lib, orc):
     """landau_create_meshes (topological node identification, own bilinear geometry) against the oracle's geometric
     construction: same dofs, same pattern, same integration points and weights."""
-    for k, (n, m) in ((3, (2, 2)), (2, (3, 2))):
+    for k, (n, m) in ((3, (2, 2)), (2, (3, 2)), (4, (1, 2))):
         mesh = W.semicircle_mesh(5.0, n, m)
         species = [dict(mass=1.0, charge=-1.0, grid=0)]
         L = Bn.Landau.from_meshes([mesh], species, k, device=-1)
@@ -186,5 +186,5 @@ def test_triangle_host_setup_matches_oracle(lib, orc, k, per_cell):
     quads = W.semicircle_mesh(5.0, 2, 2)
     with pytest.raises(Bn.LandauError, match="cell type"):               # one cell type per context
         Bn.Landau.from_meshes([mesh, quads], [dict(mass=1.0, charge=-1.0, grid=0), dict(mass=2.0, charge=1.0, grid=1)], 3, device=-1)
-    with pytest.raises(Bn.LandauError):                                  # Q4 quadrilaterals are not built
-        Bn.Landau.from_meshes([quads], species, 4, device=-1)
+    with pytest.raises(Bn.LandauError):                                  # Q5 quadrilaterals are not built
+        Bn.Landau.from_meshes([quads], species, 5, device=-1)

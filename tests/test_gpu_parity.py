@@ -94,7 +94,8 @@ def test_tensor_device_vs_oracle(orc, Bn, torch_cuda):
 
 
 # ------------------------------------------------------------------------------------------------ small, full batch
-@pytest.mark.parametrize("kind,degree", [("uniform", 2), ("uniform", 3), ("quadtree", 2), ("quadtree", 3)])
+@pytest.mark.parametrize("kind,degree", [("uniform", 2), ("uniform", 3), ("quadtree", 2), ("quadtree", 3), ("uniform", 4),
+                                         ("quadtree", 4)])
 @pytest.mark.parametrize("kernel", [1, 2, 3, 4, 5])
 def test_tiny_jacobian_apply_and_coefficients(orc, Bn, torch_cuda, kind, degree, kernel):
     torch = torch_cuda

@@ -49,7 +49,7 @@ def _compare(L, o, vals, rhs, f_o, dt, entries):
             assert np.linalg.norm(a - r) < TOL * np.linalg.norm(r) and np.abs(a - r).max() < TOL * np.abs(r).max()
 
 
-@pytest.mark.parametrize("degree", [2, 3])
+@pytest.mark.parametrize("degree", [2, 3, 4])
 @pytest.mark.parametrize("kernel", [0, 1])
 def test_semicircle_two_species(orc, Bn, degree, kernel):
     import torch

@@ -225,7 +225,8 @@ def _moments(o, cfg, rhs):
     return dens, mom, scale
 
 
-@pytest.mark.parametrize("kind,degree", [("uniform", 2), ("uniform", 3), ("quadtree", 2), ("quadtree", 3)])
+@pytest.mark.parametrize("kind,degree", [("uniform", 2), ("uniform", 3), ("quadtree", 2), ("quadtree", 3), ("uniform", 4),
+                                         ("quadtree", 4)])
 def test_P6_conservation_to_roundoff(orc, kind, degree):
     """Density per species, total z-momentum and total energy of J[f]f vanish to round-off."""
     cfg = W.tiny_config(kind, degree)
@@ -264,7 +265,7 @@ def _csr_bilinear(rp, ci, vals, p, q):
 @pytest.mark.parametrize("grid", [dict(kind=1, r_max=5.0, z_min=-5.0, z_max=5.0, nr=2, nz=4, levels=1),
                                   dict(kind=1, r_max=3.0, z_min=-1.0, z_max=5.0, nr=4, nz=8, levels=3)],
                          ids=["14cells", "104cells"])
-@pytest.mark.parametrize("degree", [2, 3])
+@pytest.mark.parametrize("degree", [2, 3, 4])
 def test_P6_shift_and_mass_closed_forms_on_quadtree(orc, grid, degree):
     """The shift of the output matrix (M/dt - J) - (-J) is M/dt, and M on a QUADTREE grid is pinned by closed forms (not by
     the oracle's own mass()): with nodal vectors p, q of polynomials of degree <= k per direction, p^T M q = INT p q r dr dz

@@ -43,7 +43,7 @@ def test_U1_table13_point_count_and_weights(orc):
         orc.Oracle.from_meshes([(v, c[:, ::-1].copy())], [dict(mass=1.0, charge=-1.0, grid=0)], 3)
 
 
-@pytest.mark.parametrize("k", [2, 3])
+@pytest.mark.parametrize("k", [2, 3, 4])
 def test_U2_physical_polynomials_are_reproduced(orc, k):
     o = orc.Oracle.from_meshes([W.semicircle_mesh(3.0, 2, 2)], [dict(mass=1.0, charge=-1.0, grid=0)], k)
     rz = o.dof_coords(0)
@@ -52,9 +52,12 @@ def test_U2_physical_polynomials_are_reproduced(orc, k):
     if k == 2:
         f, ex = 1 + R - 2 * Z + R * Z - 0.5 * Z * Z + 0.3 * R * R, 1 + r - 2 * z + r * z - 0.5 * z * z + 0.3 * r * r
         gr, gz = 1 + z + 0.6 * r, -2 + r - z
-    else:
+    elif k == 3:
         f, ex = R ** 3 - 2 * R * Z * Z + Z ** 3 + R * Z, r ** 3 - 2 * r * z * z + z ** 3 + r * z
         gr, gz = 3 * r * r - 2 * z * z + z, -4 * r * z + 3 * z * z + r
+    else:
+        f, ex = R ** 4 - 3 * R * R * Z * Z + Z ** 4 + R * Z, r ** 4 - 3 * r * r * z * z + z ** 4 + r * z
+        gr, gz = 4 * r ** 3 - 6 * r * z * z + z, -6 * r * r * z + 4 * z ** 3 + r
     a, b, c = o.fields(f, 0)
     scale = np.abs(ex).max()
     assert np.abs(a - ex).max() < 1e-13 * scale
