@@ -64,6 +64,13 @@ int landau_set_inner_kernel(landau_ctx* ctx, int which);
  * measurements and parity tests). */
 int landau_set_assembly_kernel(landau_ctx* ctx, int which);
 
+/* Choose the launch mode of the batched TFQMR solve: 0 / 1 one thread block per system (default), 2 ONE WARP per system
+ * where at least four systems fit in the shared memory of an SM with their values and vectors (e.g. the 142-unknown blocks
+ * of the paper's 2V throughput problem): the warps of a thread block take entries of one species and share its pattern, no
+ * block-wide barrier in the iteration.  Same iterates; measured SLOWER (1.48 against 1.31 ms for 2560 systems: six warps per
+ * SM hide less latency than sixteen), kept for A/B measurements only. */
+int landau_set_solve_kernel(landau_ctx* ctx, int which);
+
 /* Schedule of the ring assembly kernel for grid g (host query, works on host-only contexts): ring_cells = element
  * matrices kept in shared memory (0: the ring does not fit, the slot-gather kernel is used for this grid),
  * n_steps = panels of 8 cells, n_simple_slots = CSR slots fed by exactly one element-matrix entry with weight 1. */

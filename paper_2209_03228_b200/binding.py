@@ -24,7 +24,7 @@ SYMBOLS = ["landau_create", "landau_create_meshes", "landau_destroy", "landau_si
            "landau_reserve", "landau_last_error"]
 DEBUG_SYMBOLS = ["landau_last_coefficients", "landau_tensor_eval", "landau_ellip_eval", "landau_fp64_probe",
                  "landau_launch_count", "landau_is_separable", "landau_set_timing", "landau_last_stage_ms",
-                 "landau_set_inner_kernel", "landau_set_assembly_kernel", "landau_assembly_info",
+                 "landau_set_inner_kernel", "landau_set_assembly_kernel", "landau_set_solve_kernel", "landau_assembly_info",
                  "landau_set_batch_chunk"]
 
 
@@ -284,6 +284,10 @@ def landau_set_inner_kernel(ctx, which):
 
 def landau_set_assembly_kernel(ctx, which):
     _check(load().landau_set_assembly_kernel(ctx, C.c_int(which)), ctx)
+
+
+def landau_set_solve_kernel(ctx, which):
+    _check(load().landau_set_solve_kernel(ctx, C.c_int(which)), ctx)
 
 
 def landau_assembly_info(ctx, grid):

@@ -47,7 +47,7 @@ int grow(BatchSolver& s, double** p, size_t* cap, size_t need) {
 
 // The dynamic shared-memory limit belongs to the device's copy of k4_tfqmr, not to a context: keep a per-device
 // high-water mark and only ever raise it, so that live contexts of different sizes can be used alternately.
-size_t g_smem_set[64] = {0};
+size_t g_smem_set[64] = {0}, g_smem_set_warp[64] = {0};
 
 }  // namespace
 
@@ -80,10 +80,30 @@ int solver_create(BatchSolver& s, int device, const std::vector<SolverGridView>&
   const size_t mat = (size_t)max_nnz * 12 + (size_t)(s.max_n + 2) * 4;
   s.mat_nnz = (s.max_n <= s.smem_n && s.smem + mat <= 56 * 1024) ? max_nnz : 0;
   if (s.mat_nnz) s.smem += mat + K4_NVEC * sizeof(double);  // vectors padded to an even length
+  // smaller still: one WARP per system (no block-wide barrier in the iteration), the warps of a CTA on entries of one
+  // species sharing its pattern; taken when at least four systems fit in the shared memory of an SM
+  {
+    const size_t n_even = (size_t)(s.max_n + 1) & ~(size_t)1, nnz_even = (size_t)(max_nnz + 1) & ~(size_t)1;
+    const size_t pattern = ((nnz_even + n_even + 2 + 1) / 2) * sizeof(double);
+    const size_t per_warp = (K4_NVEC * n_even + nnz_even) * sizeof(double);
+    const size_t room = limit > pattern ? limit - pattern : 0;
+    const int wpc = (int)std::min<size_t>(room / per_warp, 8);
+    if (wpc >= 4) {
+      s.warp_wpc = wpc;
+      s.warp_n = (int)n_even;
+      s.warp_nnz = (int)nnz_even;
+      s.warp_smem = pattern + wpc * per_warp;
+    }
+  }
   size_t* cur = device >= 0 && device < 64 ? &g_smem_set[device] : nullptr;
   if (!cur || s.smem > *cur) {
-    SOLVER_TRY(s, cudaFuncSetAttribute(k4_tfqmr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s.smem));
+    SOLVER_TRY(s, cudaFuncSetAttribute(k4_tfqmr_t<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s.smem));
     if (cur) *cur = s.smem;
+  }
+  size_t* curw = device >= 0 && device < 64 ? &g_smem_set_warp[device] : nullptr;
+  if (s.warp_wpc && (!curw || s.warp_smem > *curw)) {
+    SOLVER_TRY(s, cudaFuncSetAttribute(k4_tfqmr_t<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s.warp_smem));
+    if (curw) *curw = s.warp_smem;
   }
   return LANDAU_OK;
 }
@@ -113,11 +133,19 @@ int solver_tfqmr(BatchSolver& s, const double* vals, const double* rhs, int batc
     ws_stride = (long long)K4_NVEC * s.max_n;
     if (int rc = grow(s, &s.ws, &s.ws_cap, (size_t)ws_stride * batch * s.S)) return rc;
   }
-  // small systems: fewer threads per system, several systems per SM (the iteration is latency bound)
-  const int threads = s.max_n <= 256 ? 128 : s.max_n <= 1024 ? 256 : K4_THREADS;
-  k4_tfqmr<<<batch * s.S, threads, s.smem, st>>>(static_cast<const K4Grid*>(s.d_grid), static_cast<const K4Species*>(s.d_spec), s.S,
-                                                 vals, s.v_stride, rhs, s.f_stride, x, rtol, max_it, iters, relres, s.ws,
-                                                 ws_stride, s.mat_nnz ? ((s.max_n + 1) & ~1) : s.smem_n, s.mat_nnz);
+  const K4Grid* kg = static_cast<const K4Grid*>(s.d_grid);
+  const K4Species* ks = static_cast<const K4Species*>(s.d_spec);
+  if (s.warp_wpc && s.use_warp) {
+    const int groups = (batch + s.warp_wpc - 1) / s.warp_wpc;
+    k4_tfqmr_t<true><<<s.S * groups, 32 * s.warp_wpc, s.warp_smem, st>>>(kg, ks, s.S, batch, vals, s.v_stride, rhs, s.f_stride, x, rtol,
+                                                                      max_it, iters, relres, nullptr, 0, s.warp_n, s.warp_nnz);
+  } else {
+    // small systems: fewer threads per system, several systems per SM (the iteration is latency bound)
+    const int threads = s.max_n <= 256 ? 128 : s.max_n <= 1024 ? 256 : K4_THREADS;
+    k4_tfqmr_t<false><<<batch * s.S, threads, s.smem, st>>>(kg, ks, s.S, batch, vals, s.v_stride, rhs, s.f_stride, x, rtol, max_it, iters,
+                                                           relres, s.ws, ws_stride, s.mat_nnz ? ((s.max_n + 1) & ~1) : s.smem_n,
+                                                           s.mat_nnz);
+  }
   ++s.launches;
   SOLVER_TRY(s, cudaGetLastError());
   return LANDAU_OK;

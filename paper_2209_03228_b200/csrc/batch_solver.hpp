@@ -27,6 +27,9 @@ struct SolverSpeciesView {
 struct BatchSolver {
   int device = -1, S = 0, max_n = 0, smem_n = 0, mat_nnz = 0;
   size_t smem = 0;
+  int warp_wpc = 0, warp_n = 0, warp_nnz = 0;  // warp-per-system mode of small systems: warps per CTA, padded sizes
+  size_t warp_smem = 0;
+  bool use_warp = false;  // opt-in (A/B): one warp per system where it applies; measured slower than one CTA per system
   long long f_stride = 0, v_stride = 0;
   void *d_grid = nullptr, *d_spec = nullptr;  // K4Grid[G], K4Species[S]
   std::vector<void*> allocs;

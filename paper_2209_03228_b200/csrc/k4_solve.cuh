@@ -65,16 +65,18 @@ __device__ __forceinline__ T k4_ld(const T* p) {
 }
 
 // LDG: pattern and values in global memory (read-only path); otherwise they may sit in shared memory (plain loads)
+// tid / nthreads: the thread's index in, and the size of, the group that owns the system (the CTA, or one warp of it)
 template <bool LDG = true, class Out>
-__device__ __forceinline__ void k4_spmv(const K4Grid& g, const double* __restrict__ vals, const double* in, Out out) {
-  const int l8 = threadIdx.x & 7, sub = (threadIdx.x & 31) >> 3;
-  const int RS = blockDim.x >> 3;  // rows per sweep of the CTA
+__device__ __forceinline__ void k4_spmv(const K4Grid& g, const double* __restrict__ vals, const double* in, Out out,
+                                        int tid = threadIdx.x, int nthreads = blockDim.x) {
+  const int l8 = tid & 7, sub = (tid & 31) >> 3;
+  const int RS = nthreads >> 3;  // rows per sweep of the group
   constexpr int U = 2;                // rows per lane group in flight
   // warp-uniform trip count (the shuffles need all 32 lanes; rows past the end contribute nothing); the row bounds of
   // the next iteration are fetched while the current rows are summed.  All value / index loads of an iteration are
   // issued before the first use: the product is bound by the latency of those loads (L2), not by their volume.
   int k0[U], k1[U];
-  const int first = (threadIdx.x >> 5) * 4;
+  const int first = (tid >> 5) * 4;
   auto bounds = [&](int row0) {
 #pragma unroll
     for (int j = 0; j < U; ++j) {
@@ -124,18 +126,70 @@ __device__ __forceinline__ void k4_spmv(const K4Grid& g, const double* __restric
   }
 }
 
+// sums of two values over one warp, result in every lane
+__device__ __forceinline__ void k4_warp_sum2(double& a, double& b) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    a += __shfl_xor_sync(0xffffffffu, a, o);
+    b += __shfl_xor_sync(0xffffffffu, b, o);
+  }
+}
+
+// WARP = false: one system per CTA (blockIdx.x = entry * n_spec + species).
+// WARP = true (small systems): one system per WARP, no block-wide barrier anywhere in the iteration -- a CTA of `wpc` warps
+// takes wpc entries of ONE species (blockIdx.x = species * ceil(batch / wpc) + entry group), so that its warps share the
+// pattern of that species' grid in shared memory; every warp keeps its own values and vectors there.
+template <bool WARP>
 __global__ void __launch_bounds__(K4_THREADS)
-k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, int n_spec, const double* __restrict__ vals,
-         long long v_stride, const double* __restrict__ rhs, long long f_stride, double* __restrict__ x, double rtol,
-         int max_it, int* __restrict__ iters, double* __restrict__ relres, double* __restrict__ ws, long long ws_stride,
-         int smem_n, int mat_nnz) {
+k4_tfqmr_t(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, int n_spec, int batch,
+           const double* __restrict__ vals, long long v_stride, const double* __restrict__ rhs, long long f_stride,
+           double* __restrict__ x, double rtol, int max_it, int* __restrict__ iters, double* __restrict__ relres,
+           double* __restrict__ ws, long long ws_stride, int smem_n, int mat_nnz) {
   extern __shared__ __align__(16) double k4_smem[];
   double* red = k4_smem;  // [2 * warps]
-  const int sidx = blockIdx.x % n_spec, b = blockIdx.x / n_spec;
+  const int wpc = blockDim.x >> 5, warp = threadIdx.x >> 5;
+  int sidx, b;
+  if (WARP) {
+    const int groups = (batch + wpc - 1) / wpc;
+    sidx = blockIdx.x / groups;
+    b = (blockIdx.x - sidx * groups) * wpc + warp;
+  } else {
+    sidx = blockIdx.x % n_spec;
+    b = blockIdx.x / n_spec;
+  }
+  const int sys = b * n_spec + sidx;  // index of the system in iters / relres / ws
   const K4Species sp = spec[sidx];
   K4Grid g = grids[sp.grid];
-  const int n = g.n, tid = threadIdx.x, nthreads = blockDim.x;
-  double* vec = n <= smem_n ? k4_smem + 2 * (K4_THREADS / 32) : ws + (long long)blockIdx.x * ws_stride;
+  const int n = g.n, tid = WARP ? (int)(threadIdx.x & 31) : (int)threadIdx.x, nthreads = WARP ? 32 : (int)blockDim.x;
+  auto sync = [&]() {
+    if (WARP)
+      __syncwarp();
+    else
+      __syncthreads();
+  };
+  auto sum2 = [&](double& p, double& q) {
+    if (WARP)
+      k4_warp_sum2(p, q);
+    else
+      k4_block_sum2(p, q, red);
+  };
+  // shared memory, WARP: [pattern of the grid: colidx (mat_nnz ints), rowptr (smem_n + 2 ints)] then per warp
+  // [7 vectors of smem_n doubles | mat_nnz values];  otherwise: [red | 7 vectors | values | colidx | rowptr]
+  double* vec;
+  if (WARP) {
+    int* scol = reinterpret_cast<int*>(k4_smem);
+    int* srow = scol + mat_nnz;
+    for (int k = threadIdx.x; k < g.nnz; k += blockDim.x) scol[k] = g.colidx[k];
+    for (int i = threadIdx.x; i <= n; i += blockDim.x) srow[i] = g.rowptr[i];
+    g.colidx = scol;
+    g.rowptr = srow;
+    double* base = k4_smem + ((mat_nnz + smem_n + 2 + 1) >> 1);
+    vec = base + (long long)warp * ((long long)K4_NVEC * smem_n + mat_nnz);
+    __syncthreads();  // the only block-wide barrier: the shared pattern is in place
+    if (b >= batch) return;
+  } else {
+    vec = n <= smem_n ? k4_smem + 2 * (K4_THREADS / 32) : ws + (long long)sys * ws_stride;
+  }
   double *rs = vec, *w = vec + n, *u = vec + 2 * n, *v = vec + 3 * n, *d = vec + 4 * n, *au = vec + 5 * n, *idg = vec + 6 * n;
   const double* a = vals + (long long)b * v_stride + sp.v_off;  // re-pointed to shared memory for small systems
   const double* bb = rhs + (long long)b * f_stride + sp.f_off;
@@ -145,7 +199,11 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
   // Small systems (mat_nnz > 0: every grid's pattern and one value block fit beside the vectors): the matrix is copied
   // to shared memory once, and the products of the iteration run from there instead of from L2.
   const bool mat_smem = mat_nnz > 0;
-  if (mat_smem) {
+  if (WARP) {
+    double* sval = vec + (long long)K4_NVEC * smem_n;
+    for (int k = tid; k < g.nnz; k += 32) sval[k] = a[k];
+    a = sval;
+  } else if (mat_smem) {
     double* sval = k4_smem + 2 * (K4_THREADS / 32) + (long long)K4_NVEC * smem_n;
     int* scol = reinterpret_cast<int*>(sval + mat_nnz);
     int* srow = scol + mat_nnz;
@@ -158,12 +216,12 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
     g.colidx = scol;
     g.rowptr = srow;
   }
-  __syncthreads();
+  sync();
   auto product = [&](const double* in, auto out) {
-    if (mat_smem)
-      k4_spmv<false>(g, a, in, out);
+    if (WARP || mat_smem)
+      k4_spmv<false>(g, a, in, out, tid, nthreads);
     else
-      k4_spmv<true>(g, a, in, out);
+      k4_spmv<true>(g, a, in, out, tid, nthreads);
   };
   // TFQMR's residual bound is updated recursively and drifts away from the true residual on ill-conditioned blocks,
   // so a converged run is CHECKED against the true (Jacobi-scaled) residual and restarted from the current x if it
@@ -181,10 +239,10 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
       u[row] = r;
       d[row] = 0.0;
     });
-    __syncthreads();
+    sync();
     double p0 = 0.0, p1 = 0.0;
     for (int i = tid; i < n; i += nthreads) p0 = fma(rs[i], rs[i], p0);
-    k4_block_sum2(p0, p1, red);
+    sum2(p0, p1);
     double rho = p0, theta = 0.0, eta = 0.0, alpha = 0.0;
     tau = sqrt(p0);
     if (restart == 0) r0norm = tau;
@@ -198,14 +256,14 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
       au[row] = t;
       v[row] = t;
     });
-    __syncthreads();
+    sync();
     bool bound_met = false;
     for (int k = 0; !bound_met && !status && m < 2 * max_it && k < K4_RUN_CAP; ++k) {  // k: half-step of this run
       const bool even = (k & 1) == 0;
       if (even) {
         double sg = 0.0, z = 0.0;
         for (int i = tid; i < n; i += nthreads) sg = fma(rs[i], v[i], sg);
-        k4_block_sum2(sg, z, red);
+        sum2(sg, z);
         if (sg == 0.0) {
           status = 2;
           break;
@@ -222,7 +280,7 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
         ww = fma(wi, wi, ww);
         rw = fma(rs[i], wi, rw);
       }
-      k4_block_sum2(ww, rw, red);
+      sum2(ww, rw);
       theta = sqrt(ww) / tau;
       const double c = 1.0 / sqrt(1.0 + theta * theta);
       tau = tau * theta * c;
@@ -233,7 +291,7 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
         bound_met = true;
       } else if (even) {
         for (int i = tid; i < n; i += nthreads) u[i] = fma(-alpha, v[i], u[i]);
-        __syncthreads();
+        sync();
         product(u, [&](int row, double s) { au[row] = idg[row] * s; });
       } else {
         if (rho == 0.0) {
@@ -243,7 +301,7 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
         const double beta = rw / rho;
         rho = rw;
         for (int i = tid; i < n; i += nthreads) u[i] = fma(beta, u[i], w[i]);
-        __syncthreads();
+        sync();
         // v = A u_new + beta (A u_old + beta v);  au = A u_new
         product(u, [&](int row, double s) {
           const double t = idg[row] * s;
@@ -251,14 +309,14 @@ k4_tfqmr(const K4Grid* __restrict__ grids, const K4Species* __restrict__ spec, i
           au[row] = t;
         });
       }
-      __syncthreads();
+      sync();
     }
     if (status == 2) break;  // breakdown
     // bound met: verify against the true residual; run cap reached: restart (a fresh shadow residual ends stagnation)
   }
   if (tid == 0) {
-    if (iters) iters[blockIdx.x] = status == 1 ? m : -m - 1;  // half-steps; negative: not converged / breakdown
-    if (relres) relres[blockIdx.x] = r0norm > 0.0 ? tau / r0norm : 0.0;  // last true residual seen (or bound)
+    if (iters) iters[sys] = status == 1 ? m : -m - 1;  // half-steps; negative: not converged / breakdown
+    if (relres) relres[sys] = r0norm > 0.0 ? tau / r0norm : 0.0;  // last true residual seen (or bound)
   }
 }
 

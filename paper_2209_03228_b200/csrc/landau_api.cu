@@ -1312,6 +1312,12 @@ int landau_set_assembly_kernel(landau_ctx* ctx, int which) {
   return LANDAU_OK;
 }
 
+int landau_set_solve_kernel(landau_ctx* ctx, int which) {
+  if (!ctx || which < 0 || which > 2) return LANDAU_INVALID_ARG;
+  ctx->solver.use_warp = which == 2;
+  return LANDAU_OK;
+}
+
 int landau_assembly_info(const landau_ctx* ctx, int grid, int* ring_cells, int* n_steps, int* n_simple_slots) {
   if (!ctx || grid < 0 || grid >= ctx->G) return LANDAU_INVALID_ARG;
   const HostGrid& h = ctx->hg[grid];

@@ -45,11 +45,13 @@ def _oracle_systems(o, f, dt):
 
 
 @pytest.mark.parametrize("kind,degree", [("uniform", 2), ("uniform", 3), ("quadtree", 2), ("quadtree", 3)])
-def test_solve_and_spmv_against_oracle(orc, Bn, torch_cuda, kind, degree):
+@pytest.mark.parametrize("solve_kernel", [0, 2])   # 0: one thread block per system; 2: these small systems take one warp each
+def test_solve_and_spmv_against_oracle(orc, Bn, torch_cuda, kind, degree, solve_kernel):
     torch = torch_cuda
     cfg = W.tiny_config(kind, degree, batch=3)
     o = orc.Oracle(cfg["grids"], cfg["species"], cfg["degree"])
     L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"])
+    Bn.landau_set_solve_kernel(L.ctx, solve_kernel)
     f = W.make_batch_f(cfg, [o.dof_coords(g) for g in range(o.G)], batch=3)
     dt = 0.7
     vals, rhs, sol = _oracle_systems(o, f, dt)
