@@ -174,6 +174,36 @@ int landau_spmv(landau_ctx* ctx, const double* csr_vals_dev, const double* x_dev
 int landau_solve(landau_ctx* ctx, const double* csr_vals_dev, const double* rhs_dev, int batch, double rtol, int max_it,
                  double* x_dev, int* iters_dev, double* relres_dev, void* cuda_stream);
 
+/* landau_solve for callers that must not allocate device memory.
+ *
+ * Who that is: a host application that has already handed the GPU's memory to its own pool -- a particle code that sizes
+ * its arrays to fill the card, a framework whose caching allocator sits at its limit -- so that a cudaMalloc from inside
+ * this library fails or eats the headroom the application counted on; and a time-step loop that cannot afford the
+ * device-wide synchronisation a cudaMalloc / cudaFree brings with it.  landau_solve is not safe for them: when a grid has
+ * more unknowns than fit in one SM's shared memory (beyond about 4,100; PAPER.md:117 discusses that case) its kernel keeps
+ * the seven Krylov vectors of every system in a global-memory workspace, which landau_solve grows with cudaMalloc.
+ *
+ * This entry point runs the same kernel with that workspace in a fixed array that is part of the library image
+ * (LANDAU_SOLVE_NOALLOC_WS_BYTES, a `static __device__` array: every GPU on which the library is used holds it from load
+ * to process exit, whether or not this function is ever called).  It calls no cudaMalloc, cudaFree or other allocating
+ * routine.  Arguments, layouts, stopping rule and results are those of landau_solve -- bit for bit, the arithmetic is
+ * the same; one system per thread block (the landau_set_solve_kernel knob of landau_debug.h is not consulted).
+ *
+ * Limit: only contexts with such a large grid use the array, 7 * (largest n_dof of the context) doubles per
+ * (entry, species) system.  A call with  7 * max n_dof * batch * n_species * 8  >  LANDAU_SOLVE_NOALLOC_WS_BYTES  is refused
+ * with LANDAU_INVALID_ARG before anything is launched (landau_last_error names the largest batch that fits): split the
+ * batch.  Contexts whose systems all fit in shared memory need no workspace and have no limit.
+ *
+ * First call on a device: the function asks the runtime once per device for the array's device address (the context's
+ * device is made current first).  Make that first call before starting any stream capture.
+ * Sharing: there is ONE array per device and process; every call on that device uses it and leaves its vectors behind.
+ * Nothing in it has to be zero on entry (the kernel writes each vector before it reads it), so calls in a row need no
+ * clearing; but two calls that can run on the GPU at the same time -- different streams, different contexts, different
+ * host threads -- overwrite each other's vectors and both results are garbage.  Order them on one stream or with events. */
+#define LANDAU_SOLVE_NOALLOC_WS_BYTES (32u << 20) /* 32 MiB = 4,194,304 doubles: 126 systems of 4,753 unknowns */
+int landau_solve_noalloc(landau_ctx* ctx, const double* csr_vals_dev, const double* rhs_dev, int batch, double rtol,
+                         int max_it, double* x_dev, int* iters_dev, double* relres_dev, void* cuda_stream);
+
 /* Jacobian and operator application from ONE evaluation of the inner integral (what a Newton iteration needs):
  * out_csr_vals_dev as landau_jacobian, out_rhs_dev as landau_apply. */
 int landau_jacobian_apply(landau_ctx* ctx, const double* batch_f_dev, int batch, double dt, double* out_csr_vals_dev,

@@ -20,7 +20,7 @@ STATUS = {0: "LANDAU_OK", -1: "LANDAU_INVALID_ARG", -2: "LANDAU_UNSUPPORTED", -3
 # declare; tests check that the headers and these lists agree and that the library exports all of them
 SYMBOLS = ["landau_create", "landau_create_meshes", "landau_destroy", "landau_sizes", "landau_dof_coords", "landau_ip_table",
            "landau_csr_pattern", "landau_csr_pattern_host", "landau_jacobian", "landau_apply", "landau_spmv",
-           "landau_solve", "landau_jacobian_apply", "landau_step", "landau_jacobian_host", "landau_apply_host",
+           "landau_solve", "landau_solve_noalloc", "landau_jacobian_apply", "landau_step", "landau_jacobian_host", "landau_apply_host",
            "landau_reserve", "landau_last_error"]
 DEBUG_SYMBOLS = ["landau_last_coefficients", "landau_tensor_eval", "landau_ellip_eval", "landau_fp64_probe",
                  "landau_launch_count", "landau_is_separable", "landau_set_timing", "landau_last_stage_ms",
@@ -195,6 +195,17 @@ def landau_solve(ctx, csr_vals, rhs, batch, rtol, max_it, x, iters=None, relres=
     rp = C.c_void_p(relres.data_ptr()) if relres is not None else None
     _check(load().landau_solve(ctx, _dev_ptr(csr_vals), _dev_ptr(rhs), C.c_int(batch), C.c_double(rtol), C.c_int(max_it),
                                _dev_ptr(x), ip, rp, _stream(stream)), ctx)
+
+
+def landau_solve_noalloc(ctx, csr_vals, rhs, batch, rtol, max_it, x, iters=None, relres=None, stream=None):
+    """landau_solve for callers whose application owns the device memory (or whose loop cannot take cudaMalloc's
+    synchronisation): the Krylov workspace of large systems is a fixed 32 MiB array inside the library, nothing is
+    allocated.  Same arguments and results as landau_solve; raises LandauError when the batch needs more than the array
+    holds.  One array per device: do not let two calls overlap on the GPU."""
+    ip = C.c_void_p(iters.data_ptr()) if iters is not None else None
+    rp = C.c_void_p(relres.data_ptr()) if relres is not None else None
+    _check(load().landau_solve_noalloc(ctx, _dev_ptr(csr_vals), _dev_ptr(rhs), C.c_int(batch), C.c_double(rtol),
+                                       C.c_int(max_it), _dev_ptr(x), ip, rp, _stream(stream)), ctx)
 
 
 def landau_jacobian_apply(ctx, batch_f, batch, dt, out_csr_vals, out_rhs, stream=None):
@@ -379,6 +390,11 @@ class Landau:
         relres = torch.zeros((B, self.S), dtype=torch.float64, device=rhs.device)
         landau_solve(self.ctx, csr_vals, rhs, B, rtol, max_it, x, iters, relres, stream)
         return x, iters, relres
+
+    def solve_noalloc(self, csr_vals, rhs, x, iters, relres, rtol=1e-10, max_it=200, stream=None):
+        """landau_solve_noalloc on buffers the CALLER owns (nothing is allocated here either): x holds the initial guess on
+        entry and the solution on return; iters [B, S] int32 and relres [B, S] float64 may be None."""
+        landau_solve_noalloc(self.ctx, csr_vals, rhs, rhs.shape[0], rtol, max_it, x, iters, relres, stream)
 
     def step(self, u, dt, newton_rtol=1e-10, max_newton=50, lin_rtol=1e-12, lin_max_it=1000, stream=None):
         """Backward-Euler step in place (u: [B, f_stride] CUDA float64)."""

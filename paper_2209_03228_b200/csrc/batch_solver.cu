@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <mutex>
 
 #include "../../include/landau.h"
 #include "k4_solve.cuh"
@@ -146,6 +147,81 @@ int solver_tfqmr(BatchSolver& s, const double* vals, const double* rhs, int batc
                                                            relres, s.ws, ws_stride, s.mat_nnz ? ((s.max_n + 1) & ~1) : s.smem_n,
                                                            s.mat_nnz);
   }
+  ++s.launches;
+  SOLVER_TRY(s, cudaGetLastError());
+  return LANDAU_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// landau_solve_noalloc: the Krylov workspace nobody allocates.
+//
+// Some users of this library cannot let it call cudaMalloc: their application owns all of the card's memory through a
+// pool of its own, or runs a time-step loop in which the device-wide synchronisation of cudaMalloc / cudaFree is not
+// acceptable.  For them the workspace of the large-system branch of k4_tfqmr (seven vectors per system in global memory)
+// is this array, which is part of the loaded library image on every device from module load to process exit.
+//
+// On the HOST side `k4_noalloc_ws` is only a handle the runtime knows the symbol by -- it is not an address on any
+// device, and a kernel handed `k4_noalloc_ws` from host code would read and write somewhere else entirely.  The address
+// each device gave to its copy has to be asked for (cudaGetSymbolAddress) with that device current; noalloc_ws_address
+// does so once per device and keeps the answer.
+// ------------------------------------------------------------------------------------------------------------
+constexpr unsigned long long K4_NOALLOC_WS_DOUBLES = LANDAU_SOLVE_NOALLOC_WS_BYTES / sizeof(double);
+static __device__ __align__(256) double k4_noalloc_ws[K4_NOALLOC_WS_DOUBLES];
+
+namespace {
+std::mutex g_noalloc_mutex;
+double* g_noalloc_addr[64] = {nullptr};  // per device ordinal: device address of that device's k4_noalloc_ws
+
+int noalloc_ws_address(BatchSolver& s, double** out) {
+  int dev = -1;
+  SOLVER_TRY(s, cudaGetDevice(&dev));
+  if (dev != s.device || dev < 0 || dev >= 64) {
+    s.err = "landau_solve_noalloc: the context's device (ordinal < 64) must be the current device";
+    return LANDAU_CUDA_ERROR;
+  }
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_addr[dev]) {
+    double* p = nullptr;
+    SOLVER_TRY(s, cudaGetSymbolAddress(reinterpret_cast<void**>(&p), k4_noalloc_ws));
+    if (!p) {
+      s.err = "landau_solve_noalloc: cudaGetSymbolAddress returned a null address for the static workspace";
+      return LANDAU_CUDA_ERROR;
+    }
+    g_noalloc_addr[dev] = p;
+  }
+  *out = g_noalloc_addr[dev];
+  return LANDAU_OK;
+}
+}  // namespace
+
+int solver_tfqmr_noalloc(BatchSolver& s, const double* vals, const double* rhs, int batch, double rtol, int max_it, double* x,
+                         int* iters, double* relres, cudaStream_t st) {
+  // the set-up of the first call on this device; later calls read the cached address
+  double* ws = nullptr;
+  if (int rc = noalloc_ws_address(s, &ws)) return rc;
+  long long ws_stride = 0;
+  if (s.max_n > s.smem_n) {  // same rule as solver_tfqmr: some grid's vectors do not fit in shared memory
+    ws_stride = (long long)K4_NVEC * s.max_n;
+    const unsigned long long need = (unsigned long long)ws_stride * (unsigned long long)batch * (unsigned long long)s.S;
+    if (need > K4_NOALLOC_WS_DOUBLES) {
+      const unsigned long long per_entry = (unsigned long long)ws_stride * (unsigned long long)s.S;
+      s.err = "landau_solve_noalloc: " + std::to_string(batch) + " entries x " + std::to_string(s.S) + " species x 7 x " +
+              std::to_string(s.max_n) + " unknowns = " + std::to_string(need * sizeof(double)) +
+              " bytes of Krylov workspace, the static array holds LANDAU_SOLVE_NOALLOC_WS_BYTES = " +
+              std::to_string(K4_NOALLOC_WS_DOUBLES * sizeof(double)) + ": at most batch = " +
+              std::to_string(K4_NOALLOC_WS_DOUBLES / per_entry) + " per call on this context (split the batch, or use landau_solve)";
+      return LANDAU_INVALID_ARG;
+    }
+  } else {
+    ws = nullptr;  // every system keeps its vectors in shared memory: the array is not touched
+  }
+  // Nothing is cleared: k4_tfqmr writes idg, then rs / w / u / d, then au / v before the first read of each, so the
+  // vectors a previous call left in the array are never seen.
+  const int threads = s.max_n <= 256 ? 128 : s.max_n <= 1024 ? 256 : K4_THREADS;
+  k4_tfqmr_t<false><<<batch * s.S, threads, s.smem, st>>>(static_cast<const K4Grid*>(s.d_grid), static_cast<const K4Species*>(s.d_spec),
+                                                         s.S, batch, vals, s.v_stride, rhs, s.f_stride, x, rtol, max_it, iters,
+                                                         relres, ws, ws_stride, s.mat_nnz ? ((s.max_n + 1) & ~1) : s.smem_n,
+                                                         s.mat_nnz);
   ++s.launches;
   SOLVER_TRY(s, cudaGetLastError());
   return LANDAU_OK;

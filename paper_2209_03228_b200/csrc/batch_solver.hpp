@@ -50,6 +50,13 @@ int solver_spmv(BatchSolver& s, const double* vals, long long vals_stride, const
 int solver_tfqmr(BatchSolver& s, const double* vals, const double* rhs, int batch, double rtol, int max_it, double* x,
                  int* iters, double* relres, cudaStream_t st);
 
+// The same solve for callers that may not allocate (landau.h: landau_solve_noalloc): the global Krylov workspace of systems
+// too large for shared memory is a fixed static __device__ array of batch_solver.cu instead of s.ws, so no cudaMalloc is
+// ever issued; LANDAU_INVALID_ARG when batch * S systems of 7 max_n doubles exceed it.  One array per device, shared by
+// every caller: overlapping calls race.  The first call on a device looks up the array's address (before any capture).
+int solver_tfqmr_noalloc(BatchSolver& s, const double* vals, const double* rhs, int batch, double rtol, int max_it, double* x,
+                         int* iters, double* relres, cudaStream_t st);
+
 // A = M/dt - J[u] (CSR values) and ju = J[u] u for `batch` entries, both from one inner integral, on the step's stream
 using JacobianApplyFn = std::function<int(const double* u, int batch, double dt, double* A, double* ju)>;
 

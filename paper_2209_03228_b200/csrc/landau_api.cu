@@ -1175,6 +1175,19 @@ int landau_solve(landau_ctx* ctx, const double* csr_vals_dev, const double* rhs_
   return LANDAU_OK;
 }
 
+// landau.h: the solve for callers that must not allocate; the workspace is the static array of batch_solver.cu
+int landau_solve_noalloc(landau_ctx* ctx, const double* csr_vals_dev, const double* rhs_dev, int batch, double rtol,
+                         int max_it, double* x_dev, int* iters_dev, double* relres_dev, void* cuda_stream) {
+  if (int rc = check_call(ctx, csr_vals_dev, batch, x_dev)) return rc;  // makes the context's device current
+  if (batch > 0 && !rhs_dev) return fail(ctx, LANDAU_INVALID_ARG, "null buffer");
+  if (!(rtol > 0) || max_it < 1) return fail(ctx, LANDAU_INVALID_ARG, "rtol must be > 0 and max_it >= 1");
+  if (batch == 0) return LANDAU_OK;
+  if (int rc = solver_tfqmr_noalloc(ctx->solver, csr_vals_dev, rhs_dev, batch, rtol, max_it, x_dev, iters_dev, relres_dev,
+                                    (cudaStream_t)cuda_stream))
+    return fail(ctx, rc, ctx->solver.err);
+  return LANDAU_OK;
+}
+
 int landau_step(landau_ctx* ctx, double* u_dev, int batch, double dt, double newton_rtol, int max_newton, double lin_rtol,
                 int lin_max_it, double* info_host, void* cuda_stream) {
   if (int rc = check_call(ctx, u_dev, batch, u_dev)) return rc;
