@@ -40,7 +40,9 @@ typedef enum {
   LANDAU_UNSUPPORTED = -2,   /* degree not in {2,3,4}, n_gauss_1d != degree+1, grid kind unknown, chain of
                                 hanging-node constraints (mesh not 2:1 balanced)                           */
   LANDAU_OUT_OF_MEMORY = -3, /* host or device allocation failed                                           */
-  LANDAU_CUDA_ERROR = -4     /* any other CUDA runtime failure (no device, launch failure, ...)            */
+  LANDAU_CUDA_ERROR = -4,    /* any other CUDA runtime failure (no device, launch failure, ...)            */
+  LANDAU_NOT_CONVERGED = -5  /* landau_step / landau3v_step only: the state was advanced to the last Newton
+                                iterate, which is not the step's solution (see landau_step)                */
 } landau_status;
 
 typedef struct landau_ctx landau_ctx; /* opaque; owns all device tables and scratch */
@@ -217,6 +219,9 @@ int landau_jacobian_apply(landau_ctx* ctx, const double* batch_f_dev, int batch,
  *   u_dev     : dev, layout of batch_f_dev; ON INPUT u^k, on output u^{k+1}
  *   info_host : host, 4 doubles or NULL: Newton iterations done, last largest relative update, most linear half-steps
  *               any system took, number of linear solves that missed lin_rtol
+ * Returns LANDAU_NOT_CONVERGED (with info_host filled and u_dev holding the last iterate) when the update is still above
+ * newton_rtol after max_newton iterations, or when a linear solve of the last iteration missed lin_rtol or broke down;
+ * linear solves that failed in earlier iterations only cost Newton iterations and are just counted in info_host[3].
  * Every operator application runs in the kernels of this library; the call synchronises cuda_stream once per Newton
  * iteration (to read the update norm).  Scratch (the batch's CSR values and four vectors) is grown on demand. */
 int landau_step(landau_ctx* ctx, double* u_dev, int batch, double dt, double newton_rtol, int max_newton, double lin_rtol,
@@ -234,6 +239,9 @@ int landau_apply_host(landau_ctx* ctx, const double* batch_f_host, int batch, do
 /* Pre-size every scratch buffer of landau_jacobian / landau_apply / landau_jacobian_apply for calls with
  * batch <= max_batch (at the current batch chunk), so that those calls neither allocate nor synchronise from the first
  * one on.  Optional: without it the scratch grows on demand (one cudaMalloc + device synchronisation per growth).
+ * Covers the element-matrix scratch of species that are not assembled by the ring kernel (under the assembly mode set at
+ * the time of the call).  Not covered: the scratch of landau_solve (large systems only; see landau_solve_noalloc), of
+ * landau_step and of the *_host variants, which still grow on first use.
  * Synchronises the device.  LANDAU_OUT_OF_MEMORY leaves the context usable. */
 int landau_reserve(landau_ctx* ctx, int max_batch);
 

@@ -75,7 +75,8 @@ int landau3v_jacobian_apply(landau3v_ctx* ctx, const double* batch_f_dev, int ba
  * preconditioned TFQMR, one system per CTA and one launch for the batch (x_dev: initial guess on input; iters_dev /
  * relres_dev: [batch][species] or NULL, negative count = tolerance missed); one backward-Euler step
  * (M/dt - J[u]) delta = M (u^k - u)/dt + J[u] u, u <- u + delta by the quasi-Newton iteration, info_host = 4 doubles or
- * NULL (Newton iterations, last largest relative update, most half-steps of any system, unconverged solves). */
+ * NULL (Newton iterations, last largest relative update, most half-steps of any system, unconverged solves);
+ * landau3v_step returns LANDAU_NOT_CONVERGED under the conditions landau_step does (u_dev then holds the last iterate). */
 int landau3v_spmv(landau3v_ctx* ctx, const double* csr_vals_dev, const double* x_dev, int batch, double* y_dev,
                   void* cuda_stream);
 int landau3v_solve(landau3v_ctx* ctx, const double* csr_vals_dev, const double* rhs_dev, int batch, double rtol, int max_it,

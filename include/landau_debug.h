@@ -71,6 +71,13 @@ int landau_set_assembly_kernel(landau_ctx* ctx, int which);
  * SM hide less latency than sixteen), kept for A/B measurements only. */
 int landau_set_solve_kernel(landau_ctx* ctx, int which);
 
+/* What landau_solve will launch on this context under the current knob: warps_per_block > 0 (4..8) when the next solve
+ * runs the warp-per-system kernel with that many systems per thread block, 0 when it runs one thread block per system
+ * (the default, and what mode 2 silently falls back to when four systems do not fit in an SM's shared memory).  Lets a
+ * test assert that the kernel it means to exercise is the one that runs.  Host query; either pointer may be NULL.
+ *   max_unknowns : largest n_dof over the context's grids (the size the shared-memory plan is made for). */
+int landau_solve_mode(const landau_ctx* ctx, int* warps_per_block, int* max_unknowns);
+
 /* Schedule of the ring assembly kernel for grid g (host query, works on host-only contexts): ring_cells = element
  * matrices kept in shared memory (0: the ring does not fit, the slot-gather kernel is used for this grid),
  * n_steps = panels of 8 cells, n_simple_slots = CSR slots fed by exactly one element-matrix entry with weight 1. */

@@ -14,7 +14,8 @@ LIB_PATH = os.path.join(_HERE, "liblandau_b200.so")
 
 LANDAU_OK = 0
 STATUS = {0: "LANDAU_OK", -1: "LANDAU_INVALID_ARG", -2: "LANDAU_UNSUPPORTED", -3: "LANDAU_OUT_OF_MEMORY",
-          -4: "LANDAU_CUDA_ERROR"}
+          -4: "LANDAU_CUDA_ERROR", -5: "LANDAU_NOT_CONVERGED"}
+LANDAU_NOT_CONVERGED = -5
 
 # every symbol include/landau.h (the product ABI) and include/landau_debug.h (diagnostics, probes, tuning knobs)
 # declare; tests check that the headers and these lists agree and that the library exports all of them
@@ -24,7 +25,7 @@ SYMBOLS = ["landau_create", "landau_create_meshes", "landau_destroy", "landau_si
            "landau_reserve", "landau_last_error"]
 DEBUG_SYMBOLS = ["landau_last_coefficients", "landau_tensor_eval", "landau_ellip_eval", "landau_fp64_probe",
                  "landau_launch_count", "landau_is_separable", "landau_set_timing", "landau_last_stage_ms",
-                 "landau_set_inner_kernel", "landau_set_assembly_kernel", "landau_set_solve_kernel", "landau_assembly_info",
+                 "landau_set_inner_kernel", "landau_set_assembly_kernel", "landau_set_solve_kernel", "landau_solve_mode", "landau_assembly_info",
                  "landau_set_batch_chunk"]
 
 
@@ -214,12 +215,15 @@ def landau_jacobian_apply(ctx, batch_f, batch, dt, out_csr_vals, out_rhs, stream
 
 
 def landau_step(ctx, u, batch, dt, newton_rtol, max_newton, lin_rtol, lin_max_it, stream=None):
-    """u: u^k in, u^{k+1} out.  Returns dict(newton_its, last_update, lin_half_steps_max, lin_failed)."""
+    """u: u^k in, u^{k+1} out.  Returns dict(newton_its, last_update, lin_half_steps_max, lin_failed, converged);
+    LANDAU_NOT_CONVERGED is reported through converged = False (u then holds the last iterate), every other failure raises."""
     info = (C.c_double * 4)()
-    _check(load().landau_step(ctx, _dev_ptr(u), C.c_int(batch), C.c_double(dt), C.c_double(newton_rtol), C.c_int(max_newton),
-                              C.c_double(lin_rtol), C.c_int(lin_max_it), info, _stream(stream)), ctx)
+    rc = load().landau_step(ctx, _dev_ptr(u), C.c_int(batch), C.c_double(dt), C.c_double(newton_rtol), C.c_int(max_newton),
+                            C.c_double(lin_rtol), C.c_int(lin_max_it), info, _stream(stream))
+    if rc != LANDAU_NOT_CONVERGED:
+        _check(rc, ctx)
     return dict(newton_its=int(info[0]), last_update=float(info[1]), lin_half_steps_max=int(info[2]),
-                lin_failed=int(info[3]))
+                lin_failed=int(info[3]), converged=rc == LANDAU_OK)
 
 
 def _host_ptr(a):
@@ -299,6 +303,13 @@ def landau_set_assembly_kernel(ctx, which):
 
 def landau_set_solve_kernel(ctx, which):
     _check(load().landau_set_solve_kernel(ctx, C.c_int(which)), ctx)
+
+
+def landau_solve_mode(ctx):
+    """(warps per block of the warp-per-system kernel, or 0 when one thread block per system runs; largest n_dof)."""
+    w, n = C.c_int(-1), C.c_int(-1)
+    _check(load().landau_solve_mode(ctx, C.byref(w), C.byref(n)), ctx)
+    return w.value, n.value
 
 
 def landau_assembly_info(ctx, grid):

@@ -123,12 +123,15 @@ def landau3v_solve(ctx, csr_vals, rhs, batch, rtol, max_it, x, iters=None, relre
 
 
 def landau3v_step(ctx, u, batch, dt, newton_rtol, max_newton, lin_rtol, lin_max_it, stream=None):
-    """u: u^k in, u^{k+1} out.  Returns dict(newton_its, last_update, lin_half_steps_max, lin_failed)."""
+    """u: u^k in, u^{k+1} out.  Returns dict(newton_its, last_update, lin_half_steps_max, lin_failed, converged);
+    LANDAU_NOT_CONVERGED is reported through converged = False (u then holds the last iterate), every other failure raises."""
     info = (C.c_double * 4)()
-    _check(load().landau3v_step(ctx, _b._dev_ptr(u), C.c_int(batch), C.c_double(dt), C.c_double(newton_rtol), C.c_int(max_newton),
-                                C.c_double(lin_rtol), C.c_int(lin_max_it), info, _b._stream(stream)), ctx)
+    rc = load().landau3v_step(ctx, _b._dev_ptr(u), C.c_int(batch), C.c_double(dt), C.c_double(newton_rtol), C.c_int(max_newton),
+                              C.c_double(lin_rtol), C.c_int(lin_max_it), info, _b._stream(stream))
+    if rc != _b.LANDAU_NOT_CONVERGED:
+        _check(rc, ctx)
     return dict(newton_its=int(info[0]), last_update=float(info[1]), lin_half_steps_max=int(info[2]),
-                lin_failed=int(info[3]))
+                lin_failed=int(info[3]), converged=rc == _b.LANDAU_OK)
 
 
 def landau3v_jacobian_host(ctx, batch_f_host, batch, dt, out_host, stream=None):

@@ -241,7 +241,7 @@ int solver_step(BatchSolver& s, const JacobianApplyFn& jacobian_apply, const dou
   const K4Species* ks = static_cast<const K4Species*>(s.d_spec);
   SOLVER_TRY(s, cudaMemcpyAsync(u0, u, sizeof(double) * nf, cudaMemcpyDeviceToDevice, st));
   const int eb = (int)std::min<size_t>((nf + 255) / 256, 65535);
-  int it = 0, worst_lin = 0, lin_failed = 0;
+  int it = 0, worst_lin = 0, lin_failed = 0, last_failed = 0;
   double rel = 0.0;
   std::vector<int> h_iters(nsys);
   for (it = 0; it < max_newton; ++it) {
@@ -262,10 +262,12 @@ int solver_step(BatchSolver& s, const JacobianApplyFn& jacobian_apply, const dou
     SOLVER_TRY(s, cudaMemcpyAsync(h_iters.data(), iters, sizeof(int) * nsys, cudaMemcpyDeviceToHost, st));
     SOLVER_TRY(s, cudaStreamSynchronize(st));
     memcpy(&rel, &bits, sizeof(rel));
+    last_failed = 0;
     for (int v : h_iters) {
       worst_lin = std::max(worst_lin, v < 0 ? -v - 1 : v);
-      lin_failed += v < 0;
+      last_failed += v < 0;
     }
+    lin_failed += last_failed;
     if (rel <= newton_rtol) {
       ++it;
       break;
@@ -276,6 +278,13 @@ int solver_step(BatchSolver& s, const JacobianApplyFn& jacobian_apply, const dou
     info_host[1] = rel;
     info_host[2] = worst_lin;
     info_host[3] = lin_failed;
+  }
+  // u holds the last iterate either way; a caller without info_host must still learn that it is not the step's solution
+  if (rel > newton_rtol || last_failed > 0) {
+    s.err = "step not converged: largest relative update " + std::to_string(rel) + " after " + std::to_string(it) +
+            " Newton iterations (newton_rtol " + std::to_string(newton_rtol) + "), " + std::to_string(last_failed) +
+            " linear solves of the last iteration missed lin_rtol";
+    return LANDAU_NOT_CONVERGED;
   }
   return LANDAU_OK;
 }

@@ -676,13 +676,31 @@ static int build_triangle_grid(const landau_mesh_desc& m, const HostTables& t, H
 }
 
 int build_mesh_grid(const landau_mesh_desc& m, const HostTables& t, HostGrid* g, std::string* msg) {
-  if (m.n_vertices < 4 || m.n_cells < 1 || !m.vertices_rz || !m.cells) {
-    *msg = "bad mesh: at least 4 vertices and 1 cell";
+  if (m.n_vertices < 3 || m.n_cells < 1 || !m.vertices_rz || !m.cells) {
+    *msg = "bad mesh: at least one cell and its vertices";
     return LANDAU_INVALID_ARG;
   }
   if ((m.vertices_per_cell == 3) != t.simplex || (m.vertices_per_cell != 3 && m.vertices_per_cell != 4)) {
     *msg = "mesh cell type does not match the context's element tables (all meshes must have the same vertices_per_cell, 3 or 4)";
     return LANDAU_UNSUPPORTED;
+  }
+  if (m.n_vertices < m.vertices_per_cell) {
+    *msg = "bad mesh: fewer vertices than one cell has";
+    return LANDAU_INVALID_ARG;
+  }
+  {  // the dof ordering divides by 2^-30 of the largest coordinate: it must be finite and non-zero
+    double extent = 0.0;
+    for (int v = 0; v < 2 * m.n_vertices; ++v) {
+      if (!std::isfinite(m.vertices_rz[v])) {
+        *msg = "bad mesh: vertex coordinate " + std::to_string(v) + " is not finite";
+        return LANDAU_INVALID_ARG;
+      }
+      extent = std::max(extent, std::fabs(m.vertices_rz[v]));
+    }
+    if (!(extent > 0.0)) {
+      *msg = "bad mesh: every vertex coordinate is zero";
+      return LANDAU_INVALID_ARG;
+    }
   }
   if (t.simplex) return build_triangle_grid(m, t, g, msg);
   const int k = t.k, n1 = k + 1, nb = t.nb, nq = t.nq, nc = m.n_cells;

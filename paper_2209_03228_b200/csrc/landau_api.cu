@@ -160,8 +160,10 @@ int round_up(int x, int m) { return (x + m - 1) / m * m; }
       CALL(10, 12);                                      \
     } else if (nb_ == 25 && nq_ == 25) {                 \
       CALL(25, 25);                                      \
-    } else {                                             \
+    } else if (nb_ == 15 && nq_ == 16) {                 \
       CALL(15, 16);                                      \
+    } else {                                             \
+      return fail((ctx), LANDAU_UNSUPPORTED, "no kernel instance for this (basis functions, points) per cell"); \
     }                                                    \
   } while (0)
 
@@ -765,7 +767,7 @@ int check_call(landau_ctx* ctx, const void* in, int batch, const void* out) {
 int assemble_chunk(landau_ctx* ctx, int b0, int nbc, double inv_dt, double* out_csr_vals_dev, cudaStream_t st) {
     NvtxRange range("landau K3 element matrices + assembly (a3+a4)");
     double* vals = out_csr_vals_dev + (long long)b0 * ctx->v_stride;
-    if (ctx->k3_nspec && ctx->assembly_kernel != 1) {
+    if (ctx->k3_nspec && ctx->assembly_kernel == 0) {  // modes 1 and 3 assemble every species below: no ring launch
       // One CTA per (entry, species) block; blocks are cut into segments of steps (each with a recomputed halo) where that
       // fills the machine: every block when the batch alone gives less than one wave of resident CTAs, otherwise just
       // enough of the LAST blocks (cut in two) to bring the CTA count up to whole waves -- 2048 blocks on 148 x 4 slots
@@ -1024,6 +1026,13 @@ int landau_reserve(landau_ctx* ctx, int max_batch) {
   if (int rc = grow(ctx, &ctx->part_buf, &ctx->part_cap, part, false)) return rc;
   if (int rc = grow(ctx, &ctx->DK, &ctx->DK_cap, (size_t)ctx->dk_stride * top, false)) return rc;
   if (int rc = grow(ctx, &ctx->FL, &ctx->FL_cap, (size_t)ctx->fl_stride * top, false)) return rc;
+  // element-matrix scratch of every species that is not assembled by the ring kernel (Q4, triangles, grids without a
+  // ring schedule, or all of them under landau_set_assembly_kernel(ctx, 3)): the rule of assemble_chunk
+  bool need_em = false;
+  for (int s = 0; s < ctx->S; ++s)
+    need_em = need_em || (ctx->assembly_kernel != 1 && !(ctx->k3_ring_ok[s] && ctx->assembly_kernel == 0));
+  if (need_em)
+    if (int rc = grow(ctx, &ctx->EM, &ctx->EM_cap, (size_t)ctx->em_stride * top, false)) return rc;
   if (!ctx->d_comb) {
     CUDA_TRY(ctx, cudaMalloc(&ctx->d_comb, sizeof(CombineTable) * ctx->S));
     ctx->allocs.push_back(ctx->d_comb);
@@ -1328,6 +1337,13 @@ int landau_set_assembly_kernel(landau_ctx* ctx, int which) {
 int landau_set_solve_kernel(landau_ctx* ctx, int which) {
   if (!ctx || which < 0 || which > 2) return LANDAU_INVALID_ARG;
   ctx->solver.use_warp = which == 2;
+  return LANDAU_OK;
+}
+
+int landau_solve_mode(const landau_ctx* ctx, int* warps_per_block, int* max_unknowns) {
+  if (!ctx) return LANDAU_INVALID_ARG;
+  if (warps_per_block) *warps_per_block = ctx->solver.use_warp ? ctx->solver.warp_wpc : 0;
+  if (max_unknowns) *max_unknowns = ctx->solver.max_n;
   return LANDAU_OK;
 }
 

@@ -188,3 +188,25 @@ def test_triangle_host_setup_matches_oracle(lib, orc, k, per_cell):
         Bn.Landau.from_meshes([mesh, quads], [dict(mass=1.0, charge=-1.0, grid=0), dict(mass=2.0, charge=1.0, grid=1)], 3, device=-1)
     with pytest.raises(Bn.LandauError):                                  # Q5 quadrilaterals are not built
         Bn.Landau.from_meshes([quads], species, 5, device=-1)
+
+
+def test_mesh_argument_checks(lib):
+    """a one-triangle mesh (3 vertices) is a valid mesh; meshes whose coordinates are all zero or not finite
+    are refused (the dof ordering divides by 2^-30 of the largest coordinate) instead of running into undefined behaviour."""
+    species = [dict(mass=1.0, charge=-1.0, grid=0)]
+    tri = (np.array([[0.0, -1.0], [1.5, -1.0], [0.0, 1.0]]), np.array([[0, 1, 2]], dtype=np.int32))
+    L = Bn.Landau.from_meshes([tri], species, 2, device=-1)
+    assert L.n_cells[0] == 1 and L.n_dof[0] == 6 and L.n_ip[0] == 6 and L.nnz[0] == 36
+    L.close()
+    quad3 = (tri[0], np.array([[0, 1, 2, 2]], dtype=np.int32))
+    with pytest.raises(Bn.LandauError, match="fewer vertices"):
+        Bn.Landau.from_meshes([quad3], species, 2, device=-1)
+    for bad_value, what in ((0.0, "zero"), (float("nan"), "not finite"), (float("inf"), "not finite")):
+        v = np.zeros((3, 2)) if bad_value == 0.0 else tri[0].copy()
+        v[1, 0] = bad_value
+        with pytest.raises(Bn.LandauError, match=what):
+            Bn.Landau.from_meshes([(v, tri[1])], species, 2, device=-1)
+        vq = np.zeros((4, 2)) if bad_value == 0.0 else np.array([[0.0, 0.0], [1.0, 0.0], [1.0, 1.0], [0.0, 1.0]])
+        vq[2, 1] = bad_value
+        with pytest.raises(Bn.LandauError, match=what):
+            Bn.Landau.from_meshes([(vq, np.array([[0, 1, 2, 3]], dtype=np.int32))], species, 2, device=-1)

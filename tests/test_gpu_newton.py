@@ -278,3 +278,33 @@ def test_two_species_anisotropic_relaxation_against_nrl(orc):
     assert abs(fd / (d1perp - d1par) - 1) < 1e-7
     assert (dperp - dpar) < fd < 0 and abs(fd / (dperp - dpar) - 1) < 0.15
     L.close()
+
+
+@pytest.mark.gpu
+def test_step_reports_missing_convergence():
+    """a step that stops at max_newton with the update above newton_rtol, or whose last linear solves missed
+    lin_rtol, returns LANDAU_NOT_CONVERGED (u holds the last iterate) -- also to a caller that passes no info_host;
+    the same step with enough iterations returns LANDAU_OK."""
+    import ctypes as C
+    import torch
+    from paper_2209_03228_b200 import binding as Bn
+    cfg = W.tiny_config("uniform", 2, batch=2)
+    L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"])
+    f0 = torch.tensor(W.make_batch_f(cfg, [L.dof_coords(g) for g in range(L.G)], batch=2), device="cuda")
+    u = f0.clone()
+    info = L.step(u, 0.1, newton_rtol=1e-12, max_newton=1, lin_rtol=1e-13, lin_max_it=500)       # one iteration is not enough
+    assert not info["converged"] and info["newton_its"] == 1 and info["last_update"] > 1e-12 and info["lin_failed"] == 0
+    assert bool(torch.isfinite(u).all()) and float((u - f0).norm()) > 0.0                          # the iterate was applied
+    assert "not converged" in Bn.landau_last_error(L.ctx)
+    u.copy_(f0)
+    st = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    rc = Bn.load().landau_step(L.ctx, C.c_void_p(u.data_ptr()), C.c_int(2), C.c_double(0.1), C.c_double(1e-12), C.c_int(1),
+                               C.c_double(1e-13), C.c_int(500), None, st)                          # no info_host
+    assert rc == Bn.LANDAU_NOT_CONVERGED == -5
+    u.copy_(f0)
+    info = L.step(u, 0.1, newton_rtol=1e-12, max_newton=60, lin_rtol=1e-13, lin_max_it=1)          # linear solves cut short
+    assert not info["converged"] and info["lin_failed"] > 0
+    u.copy_(f0)
+    info = L.step(u, 0.1, newton_rtol=1e-12, max_newton=60, lin_rtol=1e-13, lin_max_it=500)
+    assert info["converged"] and info["lin_failed"] == 0 and info["last_update"] <= 1e-12
+    L.close()

@@ -403,6 +403,35 @@ def test_two_contexts_of_different_sizes_alternate(orc, Bn, torch_cuda):
     Ls.close()
 
 
+@pytest.mark.parametrize("degree,mode", [(4, 0), (3, 3)])
+def test_reserve_covers_element_matrix_scratch(Bn, torch_cuda, degree, mode):
+    """species that are not assembled by the ring kernel (Q4; any grid under assembly mode 3) keep their
+    element matrices in a scratch buffer of their own, which landau_reserve must pre-size too: no allocation by the
+    first landau_jacobian after it, and the same values as an unreserved context."""
+    torch = torch_cuda
+    cfg = W.tiny_config("quadtree", degree, batch=12)
+
+    def make():
+        L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"])
+        Bn.landau_set_assembly_kernel(L.ctx, mode)
+        return L
+    L = make()
+    fd = torch.tensor(W.make_batch_f(cfg, [L.dof_coords(g) for g in range(L.G)], batch=12), device="cuda")
+    ref = L.jacobian(fd, cfg["dt"])                 # also loads every kernel the call takes (CUDA loads modules lazily)
+    torch.cuda.synchronize()
+    L.close()
+    L = make()
+    Bn.landau_reserve(L.ctx, 12)
+    out = torch.empty_like(ref)
+    torch.cuda.synchronize()
+    free_before = torch.cuda.mem_get_info()[0]
+    Bn.landau_jacobian(L.ctx, fd, 12, cfg["dt"], out)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free_before
+    assert float((out - ref).norm() / ref.norm()) <= 1e-13
+    L.close()
+
+
 def test_non_blocking_stream_and_reserve(orc, Bn, torch_cuda):
     """ADVICE r1 (medium): scratch zeroing must be ordered on the caller's stream (torch.cuda.Stream() is non-blocking);
     landau_reserve pre-sizes the scratch so that the compute call allocates nothing."""
