@@ -476,6 +476,15 @@ def test_config4_quadtree_bimaxwellian(orc, Bn, torch_cuda):
     _config_parity(orc, Bn, torch_cuda, W.config(4), 256, _sample_entries(256, 4)[:5])
 
 
+def test_config6_paper_throughput_problem(orc, Bn, torch_cuda):
+    """The paper's own 2V throughput problem (Table 5: ten species on three 14-cell quadtree Q3 grids,
+    142 equations per species, batch 256) in the launch configuration `bench.py --advance` and BASELINE.md's context line
+    are quoted on: Jacobian and operator application of the first, the last and seeded entries against the oracle."""
+    cfg = W.config(6)
+    assert cfg["batch"] == 256 and len(cfg["species"]) == 10 and len(cfg["grids"]) == 3
+    _config_parity(orc, Bn, torch_cuda, cfg, 256, _sample_entries(256, 6))
+
+
 def test_config5_bench_launch_configuration(orc, Bn, torch_cuda):
     """Full size of the bench workload (B = 1024, default chunking), sampled entries against the oracle."""
     _config_parity(orc, Bn, torch_cuda, W.config(5), 1024, [0, 517, 1023], check_apply=False)

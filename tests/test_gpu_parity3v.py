@@ -145,6 +145,27 @@ def test_paper_sized_grids_batch_32(o3, B3):
     L.close()
 
 
+def test_paper_problem_at_bench_launch_configuration(o3, B3):
+    """The paper's 3V throughput problem exactly as `bench.py --config 7` runs it (Table 6: ten species on three
+    120-cell Q2 grids, 1,045 equations per species, 9,720 integration points, batch 32): Jacobian and operator application
+    of the first and the last entry against the oracle (about 1e9 long-double tensor evaluations per entry)."""
+    import torch
+    cfg = W.config3v("paper")
+    assert cfg["batch"] == 32 and len(cfg["species"]) == 10
+    L = B3.Landau3V(cfg["grids"], cfg["species"])
+    o = o3.Oracle3V(cfg["grids"], cfg["species"])
+    assert list(L.n_cells) == [120] * 3 and list(L.n_dof) == [1045] * 3 and int(sum(L.n_ip)) == 9720
+    f = W.make_batch_f3v(cfg, [o.dof_coords(g) for g in range(o.G)], batch=32)
+    fd = torch.tensor(f, device="cuda")
+    vals = L.jacobian(fd, cfg["dt"])
+    rhs = L.apply(fd)
+    pick = [0, 31]
+    assert _block_errors(L, vals[pick].cpu().numpy(), o.jacobian_batch(f[pick], cfg["dt"]), L.v_off).max() < TOL
+    assert _block_errors(L, rhs[pick].cpu().numpy(), o.apply_batch(f[pick]), L.f_off).max() < TOL
+    assert bool(torch.isfinite(vals).all()) and bool(torch.isfinite(rhs).all())
+    L.close()
+
+
 def test_ten_species_three_grids(o3, B3):
     """The paper's 3V throughput problem in small: ten species on three grids (several species per grid through the mixed
     source column), batch 2, against the oracle."""

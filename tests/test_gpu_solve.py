@@ -96,6 +96,69 @@ def test_solve_and_spmv_against_oracle(orc, Bn, torch_cuda, kind, degree, solve_
     L.close()
 
 
+def test_solve_systems_too_large_for_shared_memory(orc, Bn, torch_cuda):
+    """systems whose seven Krylov vectors do not fit in an SM's shared memory (more than 4,146 unknowns) keep
+    them in a global workspace (PAPER.md:117 discusses scaling the batched solver beyond one processing element's fast
+    memory).  Electrons on a uniform 16 x 32 Q3 grid (4,753 unknowns) beside deuterium on a small grid whose vectors do fit:
+    the ORACLE's matrices and right-hand sides, CUDA TFQMR against the dense direct solve."""
+    import math
+    torch = torch_cuda
+    md = 3670.0
+    cfg = dict(W.config(5), name="eD_16x32_Q3", batch=2,
+               grids=[W._grid(0, 5.0, 16, 32), W._grid(0, 5.0 / math.sqrt(md), 4, 8)])
+    o = orc.Oracle(cfg["grids"], cfg["species"], cfg["degree"])
+    L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"])
+    _, n_max = Bn.landau_solve_mode(L.ctx)
+    assert n_max == 4753 and 7 * n_max * 8 > 227 * 1024
+    f = W.make_batch_f(cfg, [o.dof_coords(g) for g in range(o.G)], batch=2)
+    vals, rhs, sol = _oracle_systems(o, f, cfg["dt"])
+    dv, dr = torch.tensor(vals, device="cuda"), torch.tensor(rhs, device="cuda")
+    rtol = 1e-13
+    x, iters, relres = L.solve(dv, dr, rtol=rtol, max_it=20000)
+    x, iters = x.cpu().numpy(), iters.cpu().numpy()
+    assert (iters > 0).all() and float(relres.max()) <= rtol
+    for b in range(2):
+        for s in range(o.S):
+            rp, ci = o.pattern(o.sgrid[s])
+            sl = slice(o.f_off[s], o.f_off[s + 1])
+            assert SO.residual(rp, ci, vals[b, o.v_off[s]:o.v_off[s + 1]], x[b, sl], rhs[b, sl]) <= 1000 * rtol
+            err = np.linalg.norm(x[b, sl] - sol[b, sl]) / np.linalg.norm(sol[b, sl])
+            assert err <= 1e-9, (b, s, err)
+    L.close()
+
+
+def test_spmv_rows_longer_than_the_register_window(orc, Bn, torch_cuda):
+    """k4_spmv holds 48 entries of a row in registers (8 lanes x 6) and finishes longer rows -- the rows that
+    couple through hanging nodes -- in a tail loop.  Config 4's quadtree grids have such rows; seeded values on the
+    oracle's pattern, landau_spmv against the plain CSR product, every entry of a small batch."""
+    torch = torch_cuda
+    cfg = W.config(4)
+    o = orc.Oracle(cfg["grids"], cfg["species"], cfg["degree"])
+    L = Bn.Landau(cfg["grids"], cfg["species"], cfg["degree"])
+    longest = 0
+    for g in range(o.G):
+        rp, ci = o.pattern(g)
+        rp2, ci2 = L.pattern(g)
+        assert np.array_equal(rp, rp2) and np.array_equal(ci, ci2)
+        longest = max(longest, int(np.diff(rp).max()))
+    assert longest > 48, longest
+    B = 3
+    rng = np.random.default_rng(404)
+    vals = rng.standard_normal((B, L.csr_stride))
+    xs = rng.standard_normal((B, L.f_stride))
+    y = L.spmv(torch.tensor(vals, device="cuda"), torch.tensor(xs, device="cuda")).cpu().numpy()
+    for b in range(B):
+        for s in range(o.S):
+            rp, ci = o.pattern(o.sgrid[s])
+            ref = SO.csr_matvec(rp, ci, vals[b, o.v_off[s]:o.v_off[s + 1]], xs[b, o.f_off[s]:o.f_off[s + 1]])
+            got = y[b, o.f_off[s]:o.f_off[s + 1]]
+            assert np.linalg.norm(got - ref) <= 1e-13 * np.linalg.norm(ref)
+            # row by row too: a wrong tail would hide in the norm of 1,000 short rows
+            scale = SO.csr_matvec(rp, ci, np.abs(vals[b, o.v_off[s]:o.v_off[s + 1]]), np.abs(xs[b, o.f_off[s]:o.f_off[s + 1]]))
+            assert (np.abs(got - ref) <= 1e-14 * scale * np.diff(rp)).all()
+    L.close()
+
+
 @pytest.mark.parametrize("kind", ["uniform", "quadtree"])
 def test_warp_mode_with_ragged_entry_groups(Bn, torch_cuda, kind):
     """the warp-per-system kernel with more entries than warps per block and a last block that is only partly
