@@ -73,6 +73,7 @@ def parse():
                     "report the time and Newton iterations under \"advance\" (not part of value)")
     ap.add_argument("--assembly", type=int, default=0, help="assembly kernel build (landau_set_assembly_kernel; 0: default)")
     ap.add_argument("--chunk", type=int, default=0, help="batch entries per pass through the stages (0: library default)")
+    ap.add_argument("--print-csrc-hash", action="store_true", help="print the sha256 that identifies the kernel sources and exit")
     ap.add_argument("--dry-run", action="store_true", help="rank plumbing only (gloo, no GPU work): the CPU test of --gpus N")
     return ap.parse_args()
 
@@ -91,13 +92,35 @@ def workload_name(cfg, B):
     return "%s batch=%d/GPU (the paper's own problem, PAPER.md:125)" % (cfg["name"], B)
 
 
+TRAFFIC_FILE = os.path.join("profiles", "r3_traffic.json.txt")
+
+
+def csrc_sha256():
+    """sha256 over the CUDA / C++ sources of the library (file names and contents, sorted by name): the build the ncu
+    counters in TRAFFIC_FILE were captured on is identified by it (`python bench.py --print-csrc-hash`)."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2209_03228_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh", ".cpp", ".hpp", ".h")):
+            h.update(name.encode())
+            with open(os.path.join(d, name), "rb") as fh:
+                h.update(fh.read())
+    return h.hexdigest()
+
+
 def profile_data():
-    """Per-launch ncu figures of the committed `ncu --set full` captures (profiles/r2_traffic.json.txt)."""
+    """Per-launch ncu figures of the committed `ncu --set full` captures (TRAFFIC_FILE).  They describe ONE build: when the
+    sources have changed since the capture, nothing from the file is used (traffic: null, tensor FLOP: fall-back constant)
+    instead of carrying stale counters."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r2_traffic.json.txt")) as fh:
-            return json.load(fh)
+        with open(os.path.join(ROOT, TRAFFIC_FILE)) as fh:
+            prof = json.load(fh)
     except (OSError, ValueError):
-        return {}
+        return {"source": None}
+    if prof.get("csrc_sha256") != csrc_sha256():
+        return {"source": "%s is stale: captured on csrc sha256 %s" % (TRAFFIC_FILE, str(prof.get("csrc_sha256"))[:16])}
+    return prof
 
 
 def hbm_peak():
@@ -302,9 +325,9 @@ def tensor_flop(dim, prof):
     try:
         ev = float(prof[key + "_tensor_evaluations_executed"])
         return (2.0 * prof[key + "_thread_inst_dfma"] + prof[key + "_thread_inst_dmul"] + prof[key + "_thread_inst_dadd"]) / ev, \
-            "ncu (profiles/r2_traffic.json.txt)"
+            "ncu (%s)" % TRAFFIC_FILE
     except (KeyError, TypeError, ZeroDivisionError):
-        return TENSOR_FLOP_FALLBACK[dim], "fall-back constant"
+        return TENSOR_FLOP_FALLBACK[dim], "fall-back"
 
 
 def rooflines(P, B, stage_ms, fp64_peak, prof, workload):
@@ -480,15 +503,29 @@ def solve_run(P, B, f_dev0, out_dev, dev, whole):
     for s in range(L.S):
         g = L.sgrid[s]
         byts += float(half[:, s].sum()) * (12.0 * float(L.nnz[g]) + 10 * 8.0 * float(L.n_dof[g]))
+    # Denominator.  Small systems: matrix and vectors live in shared memory for the whole iteration -> all bytes go through
+    # the shared-memory crossbar, 128 B/clk per SM (B300_MICROARCH.md, LDS/STS table) x 148 SMs x the SM clock.  Larger
+    # systems: vectors in shared memory, the matrix streams from L2 in every product -> matrix bytes against the L2 read
+    # bandwidth measured by the in-process probe (the guides state no L2 figure).
+    mat_bytes = sum(float(half[:, s].sum()) * 12.0 * float(L.nnz[L.sgrid[s]]) for s in range(L.S))
+    if Bn.landau_solve_matrix_in_shared(L.ctx):
+        bound, ach = "smem", byts / (ms * 1e-3) / 1e9
+        peak = 148 * 128.0 * 1.965e9 / 1e9
+        peak_src = "148 SM x 128 B/clk (shared-memory crossbar, B300_MICROARCH.md) x 1.965 GHz"
+    else:
+        bound, ach = "l2", mat_bytes / (ms * 1e-3) / 1e9
+        peak = Bn.landau_l2_probe(32 << 20, 64)
+        peak_src = "in-process L2 read probe (landau_l2_probe: 32 MiB buffer, 16-byte ld.global.cg, all SMs)"
     return {"ms_per_batch": ms, "entries": int(nb), "systems": int(nb * L.S), "rtol": 1e-8,
             "half_steps_mean": float(half.mean()), "half_steps_max": int(half.max()),
             "not_converged": int((iters < 0).sum()),
             "max_true_relative_residual": float((res.norm(dim=1) / rhs.norm(dim=1)).max()),
             "solves_per_s": nb * L.S / (ms * 1e-3),
-            "roofline": {"kernel": "K4 batched TFQMR (k4_tfqmr)", "bound": "l2", "achieved": byts / (ms * 1e-3) / 1e9,
-                         "unit": "GB/s", "peak": None,
-                         "note": "matrix + vector bytes per half-step from L2 / shared memory; the guides state no L2 "
-                                 "bandwidth figure, ncu shows the kernel at 71 % of the L1TEX throughput (DESIGN.md K4)"}}
+            "roofline": {"kernel": "K4 batched TFQMR (k4_tfqmr)", "bound": bound, "achieved": ach, "unit": "GB/s",
+                         "peak": peak, "frac": ach / peak, "peak_source": peak_src,
+                         "bytes_model": "per half-step of a system: one product = 12 B x nnz (values + column indices)"
+                                        + (" + ~10 vector passes of 8 B x n" if bound == "smem" else
+                                           "; the ~10 vector passes per half-step stay in shared memory and are not counted")}}
 
 
 def run_dry(args):
@@ -674,6 +711,9 @@ def spawn_ranks(args):
 
 if __name__ == "__main__":
     a = parse()
+    if a.print_csrc_hash:
+        print(csrc_sha256())
+        sys.exit(0)
     if a.gpus > 1 and "WORLD_SIZE" not in os.environ:
         spawn_ranks(a)
     if a.impl == "reference":

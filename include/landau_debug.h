@@ -35,6 +35,12 @@ int landau_ellip_eval(const double* m_dev, const double* mp_dev, int n, double* 
  * (CUDA-event timed on `cuda_stream`, synchronises it). */
 int landau_fp64_probe(int kind, int iters, double* tflops, void* cuda_stream);
 
+/* L2 read-bandwidth probe, the roofline denominator of the batched solve on systems whose matrix values stream from L2 (the
+ * guides give no L2 figure): every thread block reads a buffer of `bytes` (1 MiB .. 1 GiB; choose one that stays L2-resident,
+ * e.g. 32 MiB) `iters` times with 16-byte L1-bypassing loads; *gbs receives bytes * iters / time in GB/s, best of three timed
+ * launches after one that warms the cache.  Allocates and frees its buffer; synchronises `cuda_stream`. */
+int landau_l2_probe(long long bytes, int iters, double* gbs, void* cuda_stream);
+
 /* 1 if the collision-frequency matrix was detected as rank one (nu_ab = a_a b_b: one summed source column per
  * batch entry), 0 if the general per-species-column path is used; negative on error. */
 int landau_is_separable(const landau_ctx* ctx);
@@ -75,8 +81,10 @@ int landau_set_solve_kernel(landau_ctx* ctx, int which);
  * runs the warp-per-system kernel with that many systems per thread block, 0 when it runs one thread block per system
  * (the default, and what mode 2 silently falls back to when four systems do not fit in an SM's shared memory).  Lets a
  * test assert that the kernel it means to exercise is the one that runs.  Host query; either pointer may be NULL.
- *   max_unknowns : largest n_dof over the context's grids (the size the shared-memory plan is made for). */
-int landau_solve_mode(const landau_ctx* ctx, int* warps_per_block, int* max_unknowns);
+ *   max_unknowns     : largest n_dof over the context's grids (the size the shared-memory plan is made for)
+ *   matrix_in_shared : 1 when every system's CSR values and pattern are copied to shared memory once and the products of
+ *                      the iteration run from there (small systems); 0 when they stream from L2 in every product. */
+int landau_solve_mode(const landau_ctx* ctx, int* warps_per_block, int* max_unknowns, int* matrix_in_shared);
 
 /* Schedule of the ring assembly kernel for grid g (host query, works on host-only contexts): ring_cells = element
  * matrices kept in shared memory (0: the ring does not fit, the slot-gather kernel is used for this grid),

@@ -23,7 +23,7 @@ SYMBOLS = ["landau_create", "landau_create_meshes", "landau_destroy", "landau_si
            "landau_csr_pattern", "landau_csr_pattern_host", "landau_jacobian", "landau_apply", "landau_spmv",
            "landau_solve", "landau_solve_noalloc", "landau_jacobian_apply", "landau_step", "landau_jacobian_host", "landau_apply_host",
            "landau_reserve", "landau_last_error"]
-DEBUG_SYMBOLS = ["landau_last_coefficients", "landau_tensor_eval", "landau_ellip_eval", "landau_fp64_probe",
+DEBUG_SYMBOLS = ["landau_last_coefficients", "landau_tensor_eval", "landau_ellip_eval", "landau_fp64_probe", "landau_l2_probe",
                  "landau_launch_count", "landau_is_separable", "landau_set_timing", "landau_last_stage_ms",
                  "landau_set_inner_kernel", "landau_set_assembly_kernel", "landau_set_solve_kernel", "landau_solve_mode", "landau_assembly_info",
                  "landau_set_batch_chunk"]
@@ -272,6 +272,13 @@ def landau_fp64_probe(kind, iters=20000, stream=None):
     return t.value
 
 
+def landau_l2_probe(nbytes=32 << 20, iters=64, stream=None):
+    """L2 -> SM read bandwidth in GB/s on a buffer of nbytes that stays L2-resident."""
+    t = C.c_double()
+    _check(load().landau_l2_probe(C.c_longlong(nbytes), C.c_int(iters), C.byref(t), _stream(stream)))
+    return t.value
+
+
 def landau_launch_count(ctx):
     return int(load().landau_launch_count(ctx))
 
@@ -301,14 +308,21 @@ def landau_set_assembly_kernel(ctx, which):
     _check(load().landau_set_assembly_kernel(ctx, C.c_int(which)), ctx)
 
 
+def landau_solve_matrix_in_shared(ctx):
+    """True when the solve copies every system's matrix to shared memory once (small systems); False: streamed from L2."""
+    m = C.c_int(-1)
+    _check(load().landau_solve_mode(ctx, None, None, C.byref(m)), ctx)
+    return bool(m.value)
+
+
 def landau_set_solve_kernel(ctx, which):
     _check(load().landau_set_solve_kernel(ctx, C.c_int(which)), ctx)
 
 
 def landau_solve_mode(ctx):
     """(warps per block of the warp-per-system kernel, or 0 when one thread block per system runs; largest n_dof)."""
-    w, n = C.c_int(-1), C.c_int(-1)
-    _check(load().landau_solve_mode(ctx, C.byref(w), C.byref(n)), ctx)
+    w, n, m = C.c_int(-1), C.c_int(-1), C.c_int(-1)
+    _check(load().landau_solve_mode(ctx, C.byref(w), C.byref(n), C.byref(m)), ctx)
     return w.value, n.value
 
 

@@ -62,6 +62,8 @@ struct landau_ctx {
   // K3 ring kernel: device schedule per grid, species list (only species whose grid has a ring schedule)
   K3Grid* d_k3grid = nullptr;
   K3Species* d_k3spec = nullptr;
+  const ApplySpecies* d_apply_spec = nullptr;  // K3' over all species in one launch pair
+  int apply_cells = 0, apply_dofblks = 0;
   const double* d_k3frag = nullptr;
   int k3_nspec = 0, k3_min_steps = 0, k3_ctas_per_sm = 4;
   bool k3_tail_split = true;
@@ -320,6 +322,19 @@ int build_device_side(landau_ctx* ctx) {
         d.em4 = reinterpret_cast<const uint4*>(em4);
         if (rc) return rc;
       }
+    }
+    {
+      std::vector<ApplySpecies> as(S);
+      int cells = 0, blks = 0;
+      for (int s = 0; s < S; ++s) {
+        const int g = ctx->species[s].grid;
+        cells += ctx->hg[g].n_cells;
+        blks += (ctx->hg[g].n_dof + 255) / 256;
+        as[s] = ApplySpecies{ctx->dg[g], ctx->f_off[s], ctx->dk_off[s], ctx->fl_off[s], cells, blks};
+      }
+      ctx->apply_cells = cells;
+      ctx->apply_dofblks = blks;
+      if (int rc = upload(ctx, as, &ctx->d_apply_spec)) return rc;
     }
     std::vector<K3Species> ks;
     ctx->k3_ring_ok.assign(S, 0);
@@ -825,16 +840,14 @@ int assemble_chunk(landau_ctx* ctx, int b0, int nbc, double inv_dt, double* out_
 int apply_chunk(landau_ctx* ctx, const double* batch_f_dev, int b0, int nbc, double* out_rhs_dev, cudaStream_t st) {
     NvtxRange range("landau K3' apply (a5)");
     if (int rc = grow(ctx, &ctx->FL, &ctx->FL_cap, (size_t)ctx->fl_stride * nbc, false)) return rc;
-    for (int s = 0; s < ctx->S; ++s) {
-      const int g = ctx->species[s].grid;
-      dim3 g1(ctx->hg[g].n_cells, (nbc + K1T_BT - 1) / K1T_BT), g2((ctx->hg[g].n_dof + 255) / 256, nbc);
-#define K3A_CALL(NB_, NQ_)                                                                                                \
-  k3_elem_apply<NB_, NQ_><<<g1, 256, 0, st>>>(ctx->dg[g], ctx->d_tab, batch_f_dev, ctx->f_stride, ctx->f_off[s], b0, ctx->DK,    \
-                                              ctx->dk_stride, ctx->dk_off[s], nbc, ctx->FL, ctx->fl_stride, ctx->fl_off[s]);    \
-  k3_apply_gather<NB_><<<g2, 256, 0, st>>>(ctx->dg[g], ctx->FL, ctx->fl_stride, ctx->fl_off[s], nbc, out_rhs_dev, ctx->f_stride, \
-                                           ctx->f_off[s], b0)
+    {
+      dim3 g1(ctx->apply_cells, (nbc + K1T_BT - 1) / K1T_BT), g2(ctx->apply_dofblks, nbc);
+#define K3A_CALL(NB_, NQ_)                                                                                                      \
+  k3_elem_apply_all<NB_, NQ_><<<g1, 256, 0, st>>>(ctx->d_apply_spec, ctx->S, ctx->d_tab, batch_f_dev, ctx->f_stride, b0, ctx->DK, \
+                                                  ctx->dk_stride, nbc, ctx->FL, ctx->fl_stride)
       LANDAU_ELEM_DISPATCH(ctx, K3A_CALL);
 #undef K3A_CALL
+      k3_apply_gather_all<<<g2, 256, 0, st>>>(ctx->d_apply_spec, ctx->S, ctx->FL, ctx->fl_stride, nbc, out_rhs_dev, ctx->f_stride, b0);
       ctx->launches += 2;
     }
   return LANDAU_OK;
@@ -1292,6 +1305,44 @@ int landau_fp64_probe(int kind, int iters, double* tflops, void* cuda_stream) {
   return LANDAU_OK;
 }
 
+int landau_l2_probe(long long bytes, int iters, double* gbs, void* cuda_stream) {
+  if (!gbs || iters < 1 || bytes < (1 << 20) || bytes > (1LL << 30)) return LANDAU_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0, nsm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return LANDAU_CUDA_ERROR;
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  const int nblk = nsm * 8;
+  const long long n16 = bytes / 16;
+  double2* buf = nullptr;
+  double* out = nullptr;
+  if (cudaMalloc(&buf, (size_t)n16 * 16) != cudaSuccess) return LANDAU_OUT_OF_MEMORY;
+  if (cudaMalloc(&out, sizeof(double) * nblk * 256) != cudaSuccess) {
+    cudaFree(buf);
+    return LANDAU_OUT_OF_MEMORY;
+  }
+  cudaMemsetAsync(buf, 0, (size_t)n16 * 16, st);
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  double best = 0;
+  int rc = LANDAU_OK;
+  for (int rep = 0; rep < 4 && rc == LANDAU_OK; ++rep) {  // the first repetition brings the buffer into L2 and is not counted
+    cudaEventRecord(e0, st);
+    k_probe_l2_read<<<nblk, 256, 0, st>>>(buf, n16, iters, out);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) rc = LANDAU_CUDA_ERROR;
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && rc == LANDAU_OK) best = std::max(best, (double)n16 * 16.0 * iters / (ms * 1e-3) * 1e-9);
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(buf);
+  cudaFree(out);
+  *gbs = best;
+  return rc;
+}
+
 long long landau_launch_count(const landau_ctx* ctx) { return ctx ? ctx->launches + ctx->solver.launches : 0; }
 
 int landau_is_separable(const landau_ctx* ctx) {
@@ -1340,8 +1391,9 @@ int landau_set_solve_kernel(landau_ctx* ctx, int which) {
   return LANDAU_OK;
 }
 
-int landau_solve_mode(const landau_ctx* ctx, int* warps_per_block, int* max_unknowns) {
+int landau_solve_mode(const landau_ctx* ctx, int* warps_per_block, int* max_unknowns, int* matrix_in_shared) {
   if (!ctx) return LANDAU_INVALID_ARG;
+  if (matrix_in_shared) *matrix_in_shared = (ctx->solver.use_warp && ctx->solver.warp_wpc) || ctx->solver.mat_nnz > 0;
   if (warps_per_block) *warps_per_block = ctx->solver.use_warp ? ctx->solver.warp_wpc : 0;
   if (max_unknowns) *max_unknowns = ctx->solver.max_n;
   return LANDAU_OK;

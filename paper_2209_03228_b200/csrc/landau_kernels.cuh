@@ -8,7 +8,7 @@
 //   K3  k3_ring          a3+a4: (k3_ring.cuh) DMMA element matrices in a shared-memory ring, gathered into batched CSR
 //       k3_elem_matrix, k3_gather   a3+a4 without a ring schedule (triangles, ...): element matrices to scratch, slot gather
 //       k3_assemble      a3+a4: first version, one thread per CSR slot integrating its own entries (kept for A/B)
-//   K3' k3_elem_apply, k3_apply_gather   a5: operator application
+//   K3' k3_elem_apply_all, k3_apply_gather_all   a5: operator application, one launch pair for all species
 //   K4  k4_tfqmr         (k4_solve.cuh) batched TFQMR + Jacobi solve, the step after the path
 //
 // Notation follows PAPER.md sec. 2 and DESIGN.md: i = field point, j = source point, U^D / U^K the gyro-averaged
@@ -717,16 +717,26 @@ k3_gather(DevGrid g, int nbatch, const double* __restrict__ EM, long long em_str
 //   k3_apply_gather: one thread per (dof, entry) sums its element-vector entries (constraint weights), coalesced along
 //     the dof index.
 // ------------------------------------------------------------------------------------------------------------
-template <int NB, int NQ = NB>
-__global__ void __launch_bounds__(256)
-k3_elem_apply(DevGrid g, const DevTables* __restrict__ tab, const double* __restrict__ batch_f, long long f_stride,
-              long long f_off, int b0, const double* __restrict__ DK, long long dk_stride, long long dk_off, int nbatch,
-              double* __restrict__ RE, long long re_stride, long long re_off) {
+// One launch for all species of a context (a Newton iteration applies the operator to every species: ten launch pairs on
+// the paper's ten-species problem became one pair): thread blocks are dealt to species by prefix sums of their cell /
+// dof-block counts.
+struct ApplySpecies {
+  DevGrid g;
+  long long f_off, dk_off, re_off;
+  int cell_end;    // exclusive prefix sum of n_cells over the species up to and including this one
+  int dofblk_end;  // the same for ceil(n_dof / 256)
+};
+
+template <int NB, int NQ>
+__device__ __forceinline__ void k3_elem_apply_body(const DevGrid& g, const DevTables* __restrict__ tab,
+                                                   const double* __restrict__ batch_f, long long f_stride, long long f_off, int b0,
+                                                   const double* __restrict__ DK, long long dk_stride, long long dk_off, int nbatch,
+                                                   double* __restrict__ RE, long long re_stride, long long re_off, int cell) {
   constexpr int NQP = (NQ + 15) / 16 * 16;
   __shared__ double sT[3][NB][NQP];  // B, dBxi, dBeta as [a][q]
   __shared__ double sF[NB][K1T_BT], sFl[2][NQ][K1T_BT];
   const int tid = threadIdx.x, lo = tid & 15, bl = tid >> 4;
-  const int cell = blockIdx.x, b = blockIdx.y * K1T_BT + bl;
+  const int b = blockIdx.y * K1T_BT + bl;
   const bool live = b < nbatch;
   for (int e = tid; e < NQ * NB; e += 256) {
     const int q = e / NB, a = e - q * NB;
@@ -770,17 +780,40 @@ k3_elem_apply(DevGrid g, const DevTables* __restrict__ tab, const double* __rest
   }
 }
 
-template <int NB>
+// blockIdx.x runs over the cells of all species
+template <int NB, int NQ = NB>
 __global__ void __launch_bounds__(256)
-k3_apply_gather(DevGrid g, const double* __restrict__ RE, long long re_stride, long long re_off, int nbatch,
-                double* __restrict__ rhs, long long f_stride, long long f_off, int b0) {
-  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+k3_elem_apply_all(const ApplySpecies* __restrict__ spec, int n_spec, const DevTables* __restrict__ tab,
+                  const double* __restrict__ batch_f, long long f_stride, int b0, const double* __restrict__ DK,
+                  long long dk_stride, int nbatch, double* __restrict__ RE, long long re_stride) {
+  int s = 0;
+  while (s + 1 < n_spec && (int)blockIdx.x >= spec[s].cell_end) ++s;
+  const ApplySpecies& sp = spec[s];
+  const int cell = blockIdx.x - (s ? spec[s - 1].cell_end : 0);
+  k3_elem_apply_body<NB, NQ>(sp.g, tab, batch_f, f_stride, sp.f_off, b0, DK, dk_stride, sp.dk_off, nbatch, RE, re_stride, sp.re_off,
+                             cell);
+}
+
+__device__ __forceinline__ void k3_apply_gather_body(const DevGrid& g, const double* __restrict__ RE, long long re_stride,
+                                                     long long re_off, int nbatch, double* __restrict__ rhs, long long f_stride,
+                                                     long long f_off, int b0, int n) {
   const int b = blockIdx.y;
   if (n >= g.n_dof || b >= nbatch) return;
   const double* re = RE + (long long)b * re_stride + re_off;
   double total = 0.0;
   for (int p = g.ap_ptr[n]; p < g.ap_ptr[n + 1]; ++p) total = fma(g.ap_w[p], re[g.ap_code[p]], total);
   rhs[(long long)(b0 + b) * f_stride + f_off + n] = -total;
+}
+
+// blockIdx.x runs over the 256-dof blocks of all species
+__global__ void __launch_bounds__(256)
+k3_apply_gather_all(const ApplySpecies* __restrict__ spec, int n_spec, const double* __restrict__ RE, long long re_stride,
+                    int nbatch, double* __restrict__ rhs, long long f_stride, int b0) {
+  int s = 0;
+  while (s + 1 < n_spec && (int)blockIdx.x >= spec[s].dofblk_end) ++s;
+  const ApplySpecies& sp = spec[s];
+  const int blk = blockIdx.x - (s ? spec[s - 1].dofblk_end : 0);
+  k3_apply_gather_body(sp.g, RE, re_stride, sp.re_off, nbatch, rhs, f_stride, sp.f_off, b0, blk * blockDim.x + threadIdx.x);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -820,6 +853,21 @@ __global__ void __launch_bounds__(256) k_probe_dmma(double* out, int iters, doub
 }
 
 // mixed: 8 independent DFMA chains + 4 DMMA accumulator pairs per round -- are the two pipes concurrent?
+// L2 -> SM read bandwidth (the roofline denominator of the solve on systems whose matrix values stream from L2): every
+// thread block sweeps the whole buffer `iters` times with 16-byte loads that bypass L1 (ld.global.cg)
+__global__ void __launch_bounds__(256) k_probe_l2_read(const double2* __restrict__ buf, long long n16, int iters, double* out) {
+  double acc = 0.0;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll 8
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n16; i += stride) {
+      const double2 v = __ldcg(buf + i);
+      acc += v.x + v.y;
+    }
+  }
+  out[blockIdx.x * (long long)blockDim.x + threadIdx.x] = acc;
+}
+
 __global__ void __launch_bounds__(256) k_probe_mixed(double* out, int iters, double a, double b) {
   double acc[8], c0[4], c1[4];
 #pragma unroll
